@@ -1,0 +1,139 @@
+/*
+ * pyhst.h -- C ABI of the B200-native (sm_100a) hot path of PyHST2 (arxiv/paper_1306_1392):
+ * ramp filter -> parallel-beam pixel-driven backprojection (linear detector interpolation,
+ * per-projection rotation-axis position, optional 360-degree half-acquisition field
+ * doubling) and its exactly matched adjoint forward projector.
+ *
+ * Conventions shared by every entry point
+ * ---------------------------------------
+ * - extern "C", plain pointers and sizes, int status returned, never throws, never exits.
+ * - `d_*` pointers are DEVICE pointers owned by the caller (4-byte aligned); `h_*` pointers
+ *   and the arrays inside pyhst_geom_t are HOST pointers that need only live for the duration
+ *   of the call (the library copies them).
+ * - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = default stream).
+ *   There is no implicit device synchronisation in the d_* entry points: errors detectable at
+ *   enqueue time are returned, asynchronous faults surface at the caller's next sync.
+ *   The *_host entry points synchronise `stream` before returning.
+ * - Internal workspace (filtered sinogram, filter spectra, per-projection geometry tables,
+ *   TMA tensor maps) lives in a cache keyed by shapes; pyhst_release_cache() frees it.
+ * - There is no CPU fallback: a missing/non-sm_100 device yields PYHST_ERR_UNSUPPORTED.
+ * - On any error nothing is written to the output buffers and pyhst_last_error() describes it.
+ *
+ * Geometry (paper: sec. 2.1 "rotation axis displacement and the angular position
+ * can be given in input, as a function of the projection"; L59 one sinogram per slice;
+ * readings R1-R3, R14 of DESIGN.md):
+ *   sinogram stack  q[s][p][b]   s < n_slices, p < n_angles, b < n_bins (C order, row pitch
+ *                                sino_pitch floats), float32
+ *   image stack     x[s][i][j]   i < ny (rows, y), j < nx (columns, x), C order, float32
+ *   detector coordinate of pixel (i,j) in projection p (bin centres at integers):
+ *     t_p(i,j) = axis_pos[p] + pixel_size * ((j - (nx-1)/2) cos(angles_rad[p])
+ *                                          + (i - (ny-1)/2) sin(angles_rad[p]))
+ */
+#ifndef PYHST_H_
+#define PYHST_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  PYHST_OK = 0,
+  PYHST_ERR_INVALID_ARG = 1,
+  PYHST_ERR_UNSUPPORTED = 2,
+  PYHST_ERR_NOMEM = 3,
+  PYHST_ERR_CUDA = 4
+};
+
+/* Band-limited ramp kernels, bin width 1 (reading R8; PAPER.md:L13, L63 give no formula):
+ *   Ram-Lak     h[0] = 1/4, h[n odd] = -1/(pi^2 n^2), h[n even != 0] = 0
+ *   Shepp-Logan h[n] = -2 / (pi^2 (4 n^2 - 1))                                            */
+typedef enum { PYHST_FILTER_RAMLAK = 0, PYHST_FILTER_SHEPP_LOGAN = 1 } pyhst_filter_t;
+
+/* >= 180 degrees; with 360 degrees and the axis near the detector border the
+ * detector "can be virtually doubled" (PYHST_SCAN_360_HALF, reading R10). */
+typedef enum { PYHST_SCAN_180 = 0, PYHST_SCAN_360 = 1, PYHST_SCAN_360_HALF = 2 } pyhst_scan_t;
+
+typedef struct {
+  int32_t n_slices, n_angles, n_bins; /* sinogram stack [n_slices][n_angles][n_bins], C order */
+  int64_t sino_pitch;                 /* floats between rows; 0 => n_bins (contiguous)        */
+  const double* angles_rad;           /* HOST, [n_angles]                                     */
+  const double* axis_pos;             /* HOST, [n_angles], bin coordinate of the rotation axis */
+  int32_t nx, ny;                     /* output slice size; image [n_slices][ny][nx], C order */
+  double pixel_size;                  /* in detector-bin units, > 0                            */
+} pyhst_geom_t;
+
+/* a1 -- ramp filter ("filtered back projection"; readings R8, R9).
+ * For each of n_rows rows:  out[n] = sum_{m<n_bins_in} h[n - pad_left - m] * w[m] * in[m],
+ * 0 <= n < n_bins_out: the exact LINEAR convolution of the (optionally column-weighted) row,
+ * zero-extended, with the kernel `f`; evaluated with a zero-padded FFT of length
+ * >= n_bins_in + n_bins_out.
+ *   d_in   [n_rows][n_bins_in]  float32, contiguous            (device, read)
+ *   d_out  [n_rows][out_pitch]  float32; columns >= n_bins_out are not touched
+ *                               (device, written; out_pitch 0 => n_bins_out; may not alias d_in)
+ *   d_col_weights  [n_bins_in] float32 or NULL (= all ones)    (device, read)
+ * Errors: null pointers, n_rows < 0, sizes <= 0, pad_left < 0, n_bins_out < n_bins_in +
+ * pad_left, out_pitch < n_bins_out, n_bins_in + n_bins_out > 16384 -> INVALID_ARG /
+ * UNSUPPORTED.  n_rows == 0 is a no-op. */
+int pyhst_ramp_filter(const float* d_in, float* d_out, int64_t n_rows, int32_t n_bins_in,
+                      int32_t n_bins_out, int32_t pad_left, int64_t out_pitch, pyhst_filter_t f,
+                      const float* d_col_weights, void* stream);
+
+/* a2 -- backprojection P^T ("Each tile is reconstructed by a block of threads.
+ * The values to be back-projected are read ... using ... interpolation"; L71 P^T; R4-R7):
+ *   d_img[s][i][j] = scale * sum_p lerp(q[s][p][:], t_p(i,j)),
+ *   lerp(q,t) = (1-f) qz(k) + f qz(k+1), k = floor(t), f = t - k, qz = q zero-extended
+ *   outside [0, n_bins) per tap.  FP32 FMA arithmetic, geometry bases in double.
+ *   d_sino  [n_slices][n_angles][sino_pitch] float32 (device, read)
+ *   d_img   [n_slices][ny][nx]               float32 (device, overwritten)
+ * Errors: null pointers, sizes <= 0, pixel_size <= 0 or non-finite, non-finite angle/axis,
+ * sino_pitch != 0 and < n_bins -> INVALID_ARG. */
+int pyhst_backproject(const float* d_sino, float* d_img, const pyhst_geom_t* g, float scale,
+                      void* stream);
+
+/* a3 -- forward projection P, the exact transpose of a2 (eq. 1; L211
+ * Alg. 1 "Fp"; reading R13):
+ *   d_sino[s][p][b] = scale * sum_{i,j} Lambda(t_p(i,j) - b) * x[s][i][j],
+ *   Lambda(u) = max(0, 1 - |u|).  Computed as a gather over detector bins (no atomics), so
+ *   <P x, y> = <x, P^T y> holds up to FP32 rounding for the same `g`.
+ *   d_img   [n_slices][ny][nx]               float32 (device, read)
+ *   d_sino  [n_slices][n_angles][sino_pitch] float32 (device, columns < n_bins overwritten) */
+int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t* g, float scale,
+                          void* stream);
+
+/* a4 -- FBP = a1 then a2 (readings R8-R10):
+ *   PYHST_SCAN_180 / PYHST_SCAN_360 : rows filtered onto n_bins, scale = pi / n_angles.
+ *   PYHST_SCAN_360_HALF: rows weighted by the overlap ramp w (R10; cbar = mean axis position),
+ *     filtered onto the virtually doubled row of pyhst_halfacq_extent(), axis shifted by
+ *     pad_left, all projections backprojected with scale = 2 pi / n_angles.
+ *   d_sino_raw [n_slices][n_angles][sino_pitch] float32 (device, read)
+ *   d_img      [n_slices][ny][nx] float32 (device, overwritten)                            */
+int pyhst_fbp(const float* d_sino_raw, float* d_img, const pyhst_geom_t* g, pyhst_filter_t f,
+              pyhst_scan_t mode, void* stream);
+
+/* Same as pyhst_fbp with HOST buffers (pinned or pageable): the stack is processed in slice
+ * chunks, host->device copy of chunk n+1 and device->host copy of chunk n-1 overlapping the
+ * kernels of chunk n (three internal streams, ordered after `stream`).  Synchronises before
+ * returning.  max_slices_per_chunk <= 0 lets the library choose. */
+int pyhst_fbp_host(const float* h_sino_raw, float* h_img, const pyhst_geom_t* g,
+                   pyhst_filter_t f, pyhst_scan_t mode, int32_t max_slices_per_chunk,
+                   void* stream);
+
+/* Extended row length / left padding of the virtually doubled detector (R10):
+ * far = max(cbar, n_bins-1-cbar); *n_bins_ext = ceil(2 far) + 1 rounded up to a multiple of
+ * 64; *pad_left = 0 if the axis is right of the detector centre else n_bins_ext - n_bins. */
+int pyhst_halfacq_extent(int32_t n_bins, double cbar, int32_t* n_bins_ext, int32_t* pad_left);
+
+/* Selects the backprojection kernel: 0 = automatic (default), 1 = reference one-thread-per-
+ * pixel kernel (global loads; kept for cross-checks), 2 = tiled shared-memory kernel.
+ * Returns the previous value.  Test/bench hook; results agree within FP32 rounding. */
+int pyhst_set_backproject_variant(int variant);
+
+const char* pyhst_last_error(void); /* thread-local, static storage; "" if none */
+void pyhst_release_cache(void);     /* frees cached plans / workspace (synchronises the device) */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PYHST_H_ */

@@ -1,0 +1,13 @@
+"""paper_1306_1392_b200 -- B200-native (sm_100a) projector pair, ramp filter and FBP of PyHST2.
+
+The product is the C-ABI library declared in ``include/pyhst.h`` (hand-written CUDA under
+``csrc/``); ``binding`` is a thin ctypes marshalling layer with the same names and
+``workloads`` makes the seeded synthetic inputs.  There is no CPU fallback: every entry
+point raises if the CUDA library is missing or no sm_100 device is present.
+"""
+from . import workloads  # noqa: F401
+from .binding import (  # noqa: F401
+    FILTER_RAMLAK, FILTER_SHEPP_LOGAN, SCAN_180, SCAN_360, SCAN_360_HALF, PyhstError,
+    backproject, fbp, fbp_host, forward_project, halfacq_extent, last_error, library_path,
+    ramp_filter, release_cache, set_backproject_variant,
+)

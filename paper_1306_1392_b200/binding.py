@@ -1,0 +1,199 @@
+"""Thin ctypes binding of ``include/pyhst.h`` -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA library (``csrc/`` -> ``libpyhst_b200.so``).
+PyTorch is used for device memory and streams only.  There is no CPU fallback: if the
+library cannot be loaded, or a call fails, ``PyhstError`` is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, c_char_p, c_double, c_float, c_int, c_int32, c_int64, c_void_p
+
+import numpy as np
+
+FILTER_RAMLAK = 0
+FILTER_SHEPP_LOGAN = 1
+SCAN_180 = 0
+SCAN_360 = 1
+SCAN_360_HALF = 2
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBNAME = "libpyhst_b200.so"
+
+# every symbol include/pyhst.h declares
+EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
+           "pyhst_fbp_host", "pyhst_halfacq_extent", "pyhst_set_backproject_variant",
+           "pyhst_last_error", "pyhst_release_cache")
+
+
+class PyhstError(RuntimeError):
+    pass
+
+
+class Geom(ctypes.Structure):
+    _fields_ = [("n_slices", c_int32), ("n_angles", c_int32), ("n_bins", c_int32),
+                ("sino_pitch", c_int64), ("angles_rad", POINTER(c_double)),
+                ("axis_pos", POINTER(c_double)), ("nx", c_int32), ("ny", c_int32),
+                ("pixel_size", c_double)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return os.path.join(_HERE, _LIBNAME)
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if not os.path.exists(path):
+        raise PyhstError("%s is not built (run `python -c 'import __graft_entry__ as g; g.build()'`); "
+                         "there is no CPU fallback" % path)
+    lib = ctypes.CDLL(path)
+    lib.pyhst_ramp_filter.argtypes = [c_void_p, c_void_p, c_int64, c_int32, c_int32, c_int32, c_int64,
+                                      c_int, c_void_p, c_void_p]
+    lib.pyhst_backproject.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_void_p]
+    lib.pyhst_forward_project.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_void_p]
+    lib.pyhst_fbp.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_int, c_int, c_void_p]
+    lib.pyhst_fbp_host.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_int, c_int, c_int32, c_void_p]
+    lib.pyhst_halfacq_extent.argtypes = [c_int32, c_double, POINTER(c_int32), POINTER(c_int32)]
+    lib.pyhst_set_backproject_variant.argtypes = [c_int]
+    lib.pyhst_last_error.restype = c_char_p
+    lib.pyhst_release_cache.restype = None
+    _lib = lib
+    return lib
+
+
+def last_error() -> str:
+    return _load().pyhst_last_error().decode()
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise PyhstError("%s failed (status %d): %s" % (what, rc, last_error()))
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return c_void_p(torch.cuda.current_stream().cuda_stream)
+    return c_void_p(int(getattr(stream, "cuda_stream", stream)))
+
+
+def _dev(t, name):
+    """Device pointer of a contiguous float32 CUDA tensor."""
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise PyhstError("%s must be a contiguous float32 CUDA tensor" % name)
+    return c_void_p(t.data_ptr())
+
+
+def _geom(n_slices, n_angles, n_bins, angles, axis, nx, ny, pixel_size, sino_pitch=0):
+    angles = np.ascontiguousarray(angles, dtype=np.float64)
+    axis = np.ascontiguousarray(axis, dtype=np.float64)
+    if angles.shape != (n_angles,) or axis.shape != (n_angles,):
+        raise PyhstError("angles and axis must both have shape [n_angles]")
+    g = Geom(n_slices, n_angles, n_bins, sino_pitch, angles.ctypes.data_as(POINTER(c_double)),
+             axis.ctypes.data_as(POINTER(c_double)), nx, ny, float(pixel_size))
+    g._keep = (angles, axis)
+    return g
+
+
+def ramp_filter(d_in, n_bins_out=None, pad_left=0, filter=FILTER_RAMLAK, col_weights=None, out=None,
+                stream=None):
+    """pyhst_ramp_filter: float32 CUDA [..., n_bins_in] -> [..., n_bins_out] (contiguous)."""
+    import torch
+    lib = _load()
+    b_in = d_in.shape[-1]
+    b_out = b_in if n_bins_out is None else int(n_bins_out)
+    n_rows = d_in.numel() // b_in if b_in else 0
+    if out is None:
+        out = torch.empty(d_in.shape[:-1] + (b_out,), dtype=torch.float32, device=d_in.device)
+    w = None if col_weights is None else _dev(col_weights, "col_weights")
+    _check(lib.pyhst_ramp_filter(_dev(d_in, "d_in"), _dev(out, "out"), n_rows, b_in, b_out, pad_left,
+                                 out.shape[-1], filter, w, _stream(stream)), "pyhst_ramp_filter")
+    return out
+
+
+def backproject(d_sino, angles, axis, nx, ny, pixel_size=1.0, scale=1.0, out=None, stream=None):
+    """pyhst_backproject: float32 CUDA [S,P,B] -> [S,ny,nx]."""
+    import torch
+    lib = _load()
+    s, p, b = d_sino.shape
+    if out is None:
+        out = torch.empty((s, ny, nx), dtype=torch.float32, device=d_sino.device)
+    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size)
+    _check(lib.pyhst_backproject(_dev(d_sino, "d_sino"), _dev(out, "out"), ctypes.byref(g), scale,
+                                 _stream(stream)), "pyhst_backproject")
+    return out
+
+
+def forward_project(d_img, angles, axis, n_bins, pixel_size=1.0, scale=1.0, out=None, stream=None):
+    """pyhst_forward_project: float32 CUDA [S,ny,nx] -> [S,P,B]."""
+    import torch
+    lib = _load()
+    s, ny, nx = d_img.shape
+    p = len(angles)
+    if out is None:
+        out = torch.empty((s, p, n_bins), dtype=torch.float32, device=d_img.device)
+    g = _geom(s, p, n_bins, angles, axis, nx, ny, pixel_size)
+    _check(lib.pyhst_forward_project(_dev(d_img, "d_img"), _dev(out, "out"), ctypes.byref(g), scale,
+                                     _stream(stream)), "pyhst_forward_project")
+    return out
+
+
+def fbp(d_sino_raw, angles, axis, nx, ny, pixel_size=1.0, filter=FILTER_RAMLAK, mode=SCAN_180, out=None,
+        stream=None):
+    """pyhst_fbp: float32 CUDA [S,P,B] -> [S,ny,nx]."""
+    import torch
+    lib = _load()
+    s, p, b = d_sino_raw.shape
+    if out is None:
+        out = torch.empty((s, ny, nx), dtype=torch.float32, device=d_sino_raw.device)
+    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size)
+    _check(lib.pyhst_fbp(_dev(d_sino_raw, "d_sino_raw"), _dev(out, "out"), ctypes.byref(g), filter, mode,
+                         _stream(stream)), "pyhst_fbp")
+    return out
+
+
+def _host_ptr(a, name):
+    import torch
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != torch.float32 or not a.is_contiguous():
+            raise PyhstError("%s must be a contiguous float32 host tensor" % name)
+        return c_void_p(a.data_ptr())
+    if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags.c_contiguous):
+        raise PyhstError("%s must be a contiguous float32 host array" % name)
+    return c_void_p(a.ctypes.data)
+
+
+def fbp_host(h_sino_raw, angles, axis, nx, ny, pixel_size=1.0, filter=FILTER_RAMLAK, mode=SCAN_180,
+             out=None, max_slices_per_chunk=0, stream=None):
+    """pyhst_fbp_host: HOST float32 [S,P,B] (numpy or pinned torch) -> HOST [S,ny,nx]."""
+    lib = _load()
+    s, p, b = h_sino_raw.shape
+    if out is None:
+        out = np.empty((s, ny, nx), dtype=np.float32)
+    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size)
+    _check(lib.pyhst_fbp_host(_host_ptr(h_sino_raw, "h_sino_raw"), _host_ptr(out, "out"), ctypes.byref(g),
+                              filter, mode, max_slices_per_chunk, _stream(stream)), "pyhst_fbp_host")
+    return out
+
+
+def halfacq_extent(n_bins, cbar):
+    ext, pad = c_int32(0), c_int32(0)
+    _check(_load().pyhst_halfacq_extent(n_bins, float(cbar), ctypes.byref(ext), ctypes.byref(pad)),
+           "pyhst_halfacq_extent")
+    return int(ext.value), int(pad.value)
+
+
+def set_backproject_variant(variant: int) -> int:
+    return int(_load().pyhst_set_backproject_variant(int(variant)))
+
+
+def release_cache():
+    _load().pyhst_release_cache()

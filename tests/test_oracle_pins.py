@@ -1,0 +1,411 @@
+"""Pins of the oracle (K1-K12 of SURVEY.md sec. 8(c)) -- CPU only.
+
+Each pin fixes the oracle against something other than itself: closed forms, invariants,
+dense brute force built entry by entry in this file, numpy's FFT, scipy quadrature, the
+phantom itself.  A dropped term, wrong sign/index or transposed operand in
+oracle/pyhst_oracle.c fails at least one of them.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import integrate
+
+from paper_1306_1392_b200 import workloads as wl
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _geom(rng, P, B, span=math.pi, jitter=0.3, drift=1.5):
+    angles = np.sort(rng.uniform(0, span, size=P)) if jitter else np.arange(P) * span / P
+    axis = (B - 1) / 2.0 + rng.uniform(-drift, drift, size=P)
+    return angles, axis
+
+
+def _coords(angles, axis, nx, ny, h):
+    """t[p,i,j] typed out from reading R1-R3, independently of the oracle."""
+    j = np.arange(nx) - (nx - 1) / 2.0
+    i = np.arange(ny) - (ny - 1) / 2.0
+    return (axis[:, None, None] + h * (j[None, None, :] * np.cos(angles)[:, None, None]
+                                       + i[None, :, None] * np.sin(angles)[:, None, None]))
+
+
+def _dense_matrix(angles, axis, nx, ny, B, h):
+    """A[(p,b),(i,j)] = Lambda(t_p(i,j) - b), entry by entry (K4)."""
+    t = _coords(angles, axis, nx, ny, h)
+    P = len(angles)
+    A = np.zeros((P, B, ny, nx))
+    for p in range(P):
+        for b in range(B):
+            A[p, b] = np.maximum(0.0, 1.0 - np.abs(t[p] - b))
+    return A.reshape(P * B, ny * nx)
+
+
+# --------------------------------------------------------------------------- K1
+def test_k1_affine_rows_backproject_exactly(oracle):
+    rng = np.random.default_rng(1)
+    S, P, B, nx, ny, h = 2, 9, 64, 20, 17, 0.9
+    angles, axis = _geom(rng, P, B)
+    alpha, beta = rng.normal(size=(S, P)), rng.normal(size=(S, P))
+    # rows exactly representable in float32: small dyadic rationals
+    alpha, beta = np.round(alpha * 64) / 64, np.round(beta * 64) / 64
+    sino = (alpha[..., None] + beta[..., None] * np.arange(B)).astype(np.float32)
+    assert np.array_equal(sino.astype(np.float64), alpha[..., None] + beta[..., None] * np.arange(B))
+    t = _coords(angles, axis, nx, ny, h)
+    assert t.min() >= 0 and t.max() <= B - 1, "all taps must be on the detector for K1"
+    want = 0.37 * np.einsum("sp,pij->sij", alpha, np.ones_like(t)) + 0.37 * np.einsum("sp,pij->sij", beta, t)
+    got = oracle.backproject(sino, angles, axis, nx, ny, pixel_size=h, scale=0.37)
+    np.testing.assert_allclose(got, want, rtol=1e-13, atol=1e-12)
+
+
+# --------------------------------------------------------------------------- K2
+def test_k2_forward_projection_mass_and_first_moment(oracle):
+    rng = np.random.default_rng(2)
+    S, P, B, nx, ny, h = 2, 11, 80, 24, 30, 1.1
+    angles, axis = _geom(rng, P, B)
+    x = rng.normal(size=(S, ny, nx)).astype(np.float32)
+    t = _coords(angles, axis, nx, ny, h)
+    assert t.min() >= 0 and t.max() <= B - 1
+    y = oracle.forward_project(x, angles, axis, B, pixel_size=h, scale=1.7)
+    mass = 1.7 * x.astype(np.float64).sum(axis=(1, 2))
+    np.testing.assert_allclose(y.sum(axis=2), np.repeat(mass[:, None], P, 1), rtol=1e-12, atol=1e-11)
+    mom = 1.7 * np.einsum("pij,sij->sp", t, x.astype(np.float64))
+    np.testing.assert_allclose((y * np.arange(B)).sum(axis=2), mom, rtol=1e-12, atol=1e-9)
+
+
+# --------------------------------------------------------------------------- K3
+@pytest.mark.parametrize("B,axis_off", [(70, 0.0), (40, 9.3)])   # second: pixels fall off the detector
+def test_k3_adjoint_identity(oracle, B, axis_off):
+    rng = np.random.default_rng(3)
+    S, P, nx, ny, h = 2, 13, 37, 29, 1.0
+    angles, axis = _geom(rng, P, B)
+    axis = axis + axis_off
+    x = rng.normal(size=(S, ny, nx)).astype(np.float32)
+    y = rng.normal(size=(S, P, B)).astype(np.float32)
+    Ax = oracle.forward_project(x, angles, axis, B, pixel_size=h)
+    ATy = oracle.backproject(y, angles, axis, nx, ny, pixel_size=h)
+    lhs, rhs = np.vdot(Ax, y.astype(np.float64)), np.vdot(x.astype(np.float64), ATy)
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(Ax) * np.linalg.norm(y)
+
+
+# --------------------------------------------------------------------------- K4
+@pytest.mark.parametrize("P", [1, 7, 16])
+def test_k4_dense_brute_force(oracle, P):
+    rng = np.random.default_rng(40 + P)
+    B, nx, ny = 25, 16, 16
+    h = rng.uniform(0.7, 1.3)
+    angles = rng.uniform(0, 2 * math.pi, size=P)
+    axis = 12.0 + rng.uniform(-3, 3, size=P)          # some pixels leave the detector
+    A = _dense_matrix(angles, axis, nx, ny, B, h)
+    x = rng.normal(size=(1, ny, nx)).astype(np.float32)
+    y = rng.normal(size=(1, P, B)).astype(np.float32)
+    fp = oracle.forward_project(x, angles, axis, B, pixel_size=h, scale=0.5)
+    bp = oracle.backproject(y, angles, axis, nx, ny, pixel_size=h, scale=2.0)
+    np.testing.assert_allclose(fp.ravel(), 0.5 * A @ x.astype(np.float64).ravel(), rtol=0, atol=1e-13 * 50)
+    np.testing.assert_allclose(bp.ravel(), 2.0 * A.T @ y.astype(np.float64).ravel(), rtol=0, atol=1e-13 * 50)
+
+
+def test_k4_forward_projection_approximates_line_integrals(oracle):
+    """Sanity bound only: the pixel-driven FP is a binning projector, so FP*h ~ the
+    Lambda-smoothed line integral of the piecewise-constant image, to O(1/N)."""
+    N, B, h = 16, 25, 1.0
+    x = np.zeros((1, N, N), dtype=np.float32)
+    x[0, 4:12, 5:11] = 1.0
+    angles = np.array([0.3, 1.1, 2.0])
+    axis = np.full(3, 12.0)
+    fp = oracle.forward_project(x, angles, axis, B, pixel_size=h)[0]
+    # brute force: integrate the indicator image over a fine grid, bin with the hat function
+    sub = 64
+    g = (np.arange(N * sub) + 0.5) / sub - 0.5 - (N - 1) / 2.0
+    X, Y = np.meshgrid(g, g)
+    fine = np.repeat(np.repeat(x[0].astype(np.float64), sub, 0), sub, 1) / sub ** 2
+    for p in range(3):
+        t = axis[p] + X * math.cos(angles[p]) + Y * math.sin(angles[p])
+        ref = np.array([(np.maximum(0, 1 - np.abs(t - b)) * fine).sum() for b in range(B)])
+        assert np.abs(fp[p] - ref).max() <= 0.08 * ref.max()
+
+
+# --------------------------------------------------------------------------- K5
+def test_k5_zero_extension_per_tap(oracle):
+    B, N, h = 6, 9, 1.0
+    angles = np.array([0.0, math.pi / 2, 0.7])
+    axis = np.full(3, 3.4)
+    # a delta sinogram back-projects to the hat function of the detector coordinate
+    for b0 in (0, 3, 5):
+        y = np.zeros((1, 3, B), dtype=np.float32)
+        y[0, :, b0] = 1.0
+        bp = oracle.backproject(y, angles, axis, N, N, pixel_size=h)
+        t = _coords(angles, axis, N, N, h)
+        np.testing.assert_allclose(bp[0], np.maximum(0, 1 - np.abs(t - b0)).sum(0), atol=1e-14)
+    # a corner pixel whose coordinate lies in (-1,0) still feeds bin 0 with weight f
+    x = np.zeros((1, N, N), dtype=np.float32)
+    x[0, 0, 0] = 1.0
+    t00 = _coords(angles, axis, N, N, h)[:, 0, 0]
+    fp = oracle.forward_project(x, angles, axis, B, pixel_size=h)[0]
+    for p in range(3):
+        want = np.maximum(0, 1 - np.abs(t00[p] - np.arange(B)))
+        np.testing.assert_allclose(fp[p], want, atol=1e-14)
+    assert -1 < t00[0] < 0 and fp[0, 0] > 0          # the k = -1 case really occurs
+
+
+# --------------------------------------------------------------------------- K6
+def test_k6_kernel_values_match_closed_forms(oracle):
+    rows = np.loadtxt(os.path.join(GOLDEN, "ramp_kernel_closed_form.txt"))
+    for f, n, h in rows:
+        assert oracle.ramp_kernel(int(f), [int(n)])[0] == pytest.approx(h, rel=1e-15, abs=1e-18)
+
+
+def test_k6_kernel_sums_and_spectrum(oracle):
+    N = 20000
+    n = np.arange(-N, N + 1)
+    # sum over all lags is 0; the tails beyond N have closed forms
+    rl = oracle.ramp_kernel(0, n)
+    tail_rl = -2.0 / math.pi ** 2 * (math.pi ** 2 / 8 - np.sum(1.0 / np.arange(1, N + 1, 2) ** 2.0))
+    assert abs(rl.sum() + tail_rl) < 1e-15
+    sl = oracle.ramp_kernel(1, n)
+    # sum_{n>N} 1/(4n^2-1) telescopes to 1/(2(2N+1))
+    tail_sl = -2.0 / math.pi ** 2 * 2 * (1.0 / (2 * (2 * N + 1)))
+    assert abs(sl.sum() + tail_sl) < 1e-14
+    # DFT of the truncated kernels ~ |k|/M (Ram-Lak), |sin(pi k/M)|/pi (Shepp-Logan)
+    M = 1024
+    lag = np.fft.fftfreq(M, 1.0 / M).astype(np.int64)
+    k = np.abs(np.fft.fftfreq(M, 1.0 / M))
+    H0 = np.fft.fft(oracle.ramp_kernel(0, lag)).real
+    H1 = np.fft.fft(oracle.ramp_kernel(1, lag)).real
+    assert np.abs(H0 - k / M).max() < 2.0 / M
+    assert np.abs(H1 - np.abs(np.sin(math.pi * k / M)) / math.pi).max() < 2.0 / M
+
+
+def test_k6_filter_of_delta_returns_kernel(oracle):
+    B = 33
+    for f in (0, 1):
+        q = np.zeros((1, B), dtype=np.float32)
+        q[0, 10] = 1.0
+        g = oracle.ramp_filter(q, n_bins_out=B + 7, pad_left=4, filter=f)[0]
+        np.testing.assert_allclose(g, oracle.ramp_kernel(f, np.arange(B + 7) - 4 - 10), atol=1e-16)
+
+
+# --------------------------------------------------------------------------- K7
+@pytest.mark.parametrize("f", [0, 1])
+def test_k7_direct_convolution_equals_fft_convolution(oracle, f):
+    rng = np.random.default_rng(7)
+    B_in, B_out, pad = 61, 90, 13
+    q = rng.normal(size=(5, B_in)).astype(np.float32)
+    w = rng.uniform(0, 1, size=B_in).astype(np.float32)
+    g = oracle.ramp_filter(q, n_bins_out=B_out, pad_left=pad, filter=f, col_weights=w)
+    M = 256
+    lag = np.fft.fftfreq(M, 1.0 / M).astype(np.int64)
+    H = np.fft.fft(oracle.ramp_kernel(f, lag))
+    z = np.zeros((5, M))
+    z[:, pad:pad + B_in] = q.astype(np.float64) * w.astype(np.float64)
+    ref = np.fft.ifft(np.fft.fft(z, axis=1) * H, axis=1).real[:, :B_out]
+    np.testing.assert_allclose(g, ref, atol=1e-12)
+
+
+# --------------------------------------------------------------------------- K8
+def test_k8_analytic_radon_against_quadrature_and_symmetry():
+    import torch
+    ell = np.array([[3.0, -2.0, 7.0, 4.0, 0.6, 1.5]])
+    angles = np.array([0.2, 1.3, 2.9])
+    s = torch.tensor(np.tile(np.linspace(-12, 12, 9), (3, 1)))
+    got = wl.ellipse_radon(ell, angles, s).numpy()
+    x0, y0, a, b, phi, rho = ell[0]
+
+    def inside(u, th, sv):
+        x = sv * math.cos(th) - u * math.sin(th)
+        y = sv * math.sin(th) + u * math.cos(th)
+        xr = (x - x0) * math.cos(phi) + (y - y0) * math.sin(phi)
+        yr = -(x - x0) * math.sin(phi) + (y - y0) * math.cos(phi)
+        return rho * float((xr / a) ** 2 + (yr / b) ** 2 <= 1.0)
+    for p, th in enumerate(angles):
+        for n, sv in enumerate(s[p].numpy()):
+            u = np.linspace(-20, 20, 100001)
+            ref = np.trapezoid([inside(v, th, sv) for v in u[::50]], u[::50])
+            assert abs(got[p, n] - ref) < 0.05
+    # p(theta + pi, -s) = p(theta, s), exactly
+    got2 = wl.ellipse_radon(ell, angles + math.pi, -s).numpy()
+    np.testing.assert_allclose(got2, got, rtol=1e-12, atol=1e-12)
+    # a disc gives the chord 2 rho sqrt(R^2 - s^2)
+    disc = np.array([[0.0, 0.0, 5.0, 5.0, 0.0, 2.0]])
+    sv = torch.tensor([[0.0, 3.0, 4.0, 5.0, 6.0]])
+    np.testing.assert_allclose(wl.ellipse_radon(disc, np.array([0.77]), sv).numpy()[0],
+                               [20.0, 16.0, 12.0, 0.0, 0.0], atol=1e-12)
+    # polygon chords: a unit square seen along an axis and along its diagonal
+    sq = [np.array([[-1, -1], [1, -1], [1, 1], [-1, 1]], dtype=float)]
+    ch = wl.polygon_radon(sq, [1.0], np.array([0.0, math.pi / 4]), torch.tensor([[0.0, 0.5, 1.5], [0.0, 0.5, 1.5]]))
+    np.testing.assert_allclose(ch.numpy(), [[2, 2, 0], [2 * math.sqrt(2), 2 * (math.sqrt(2) - 0.5), 0]], atol=1e-12)
+
+
+# --------------------------------------------------------------------------- K9
+def test_k9_forward_projection_of_gaussian_blob(oracle):
+    """(approx.) FP * h^2 of a sampled Gaussian blob -> (sqrt(2 pi) sigma exp(-u^2/2 sigma^2) * Lambda)
+    evaluated at b - c - s0, as the pixel size h -> 0 (a Riemann sum of Gaussian x hat; the hat is
+    only C0, so convergence is O(h^2), not spectral).  Pins the sign of s0, the roles of cos/sin,
+    the h scaling and the per-projection axis."""
+    B, sig = 96, 3.5
+    x0, y0 = 2.3, -4.1                               # blob centre in bin units about the axis
+    angles = np.array([0.0, 0.4, 1.9, 2.8])
+    axis = np.array([47.5, 47.9, 46.3, 48.0])
+    peak = math.sqrt(2 * math.pi) * sig
+    refs = {}
+    for p, th in enumerate(angles):
+        s0 = x0 * math.cos(th) + y0 * math.sin(th)
+        for b in range(30, 66, 3):
+            ctr = b - axis[p] - s0
+            refs[p, b], _ = integrate.quad(
+                lambda u: max(0.0, 1 - abs(u - ctr)) * peak * math.exp(-u * u / (2 * sig * sig)),
+                ctr - 1, ctr + 1, points=[ctr], epsabs=1e-13, epsrel=1e-13)
+    errs = []
+    for h in (0.5, 0.25, 0.125):
+        N = int(48 / h)
+        j = (np.arange(N) - (N - 1) / 2.0) * h
+        X, Y = np.meshgrid(j, j)
+        img = np.exp(-((X - x0) ** 2 + (Y - y0) ** 2) / (2 * sig ** 2))[None].astype(np.float32)
+        fp = oracle.forward_project(img, angles, axis, B, pixel_size=h, scale=h * h)[0]
+        errs.append(max(abs(fp[p, b] - r) for (p, b), r in refs.items()) / peak)
+    assert errs[0] > 3 * errs[1] > 9 * errs[2]
+    assert errs[2] < 1e-4
+
+
+def test_k9_axis_aligned_projections_are_row_and_column_sums(oracle):
+    """theta = 0, pi/2, pi with h = 1 and integer axis: every pixel lands on a bin centre, so the
+    projector reduces to plain column / row sums (pins orientation R2: t grows with j at theta=0
+    and with i at theta=pi/2) and BP reduces to smearing the row back."""
+    rng = np.random.default_rng(9)
+    nx, ny, B = 12, 9, 21
+    x = rng.integers(-4, 5, size=(1, ny, nx)).astype(np.float32)
+    angles = np.array([0.0, math.pi / 2, math.pi])
+    axis = np.array([10.0, 8.0, 10.0])
+    j0, i0 = (nx - 1) / 2.0, (ny - 1) / 2.0
+    # shift so that pixel centres fall on integers: nx even -> half-integer offsets, fix via axis
+    axis = axis + np.array([0.5, 0.0, 0.5])
+    fp = oracle.forward_project(x, angles, axis, B)[0]
+    col, row = x[0].sum(0).astype(np.float64), x[0].sum(1).astype(np.float64)
+    want0 = np.zeros(B); want0[(axis[0] + np.arange(nx) - j0).astype(int)] = col
+    want1 = np.zeros(B); want1[(axis[1] + np.arange(ny) - i0).astype(int)] = row
+    want2 = np.zeros(B); want2[(axis[2] - (np.arange(nx) - j0)).astype(int)] = col
+    np.testing.assert_allclose(fp[0], want0, atol=1e-12)
+    np.testing.assert_allclose(fp[1], want1, atol=1e-12)
+    np.testing.assert_allclose(fp[2], want2, atol=1e-12)
+    y = rng.integers(-4, 5, size=(1, 3, B)).astype(np.float32)
+    bp = oracle.backproject(y, angles, axis, nx, ny)[0]
+    want = (y[0, 0][(axis[0] + np.arange(nx) - j0).astype(int)][None, :]
+            + y[0, 1][(axis[1] + np.arange(ny) - i0).astype(int)][:, None]
+            + y[0, 2][(axis[2] - (np.arange(nx) - j0)).astype(int)][None, :])
+    np.testing.assert_allclose(bp, want, atol=1e-12)
+
+
+# --------------------------------------------------------------------------- K10
+def test_k10_fbp_converges_to_the_phantom(oracle):
+    import torch
+    errs, means = [], []
+    for N in (32, 64, 128):
+        B = N + 1 if N % 2 == 0 else N
+        P = int(math.ceil(math.pi * N / 2))
+        R = 0.35 * N
+        ell = np.array([[0.05 * N, -0.03 * N, R, 0.7 * R, 0.5, 1.0],
+                        [-0.1 * N, 0.08 * N, 0.3 * R, 0.25 * R, 1.2, -0.4]])
+        angles = np.arange(P) * math.pi / P
+        axis = np.full(P, (B - 1) / 2.0)
+        s = torch.arange(B, dtype=torch.float64)[None, :] - torch.tensor(axis)[:, None]
+        sino = wl.ellipse_radon(ell, angles, s).numpy()[None].astype(np.float32)
+        rec = oracle.fbp(sino, angles, axis, N, N, filter=oracle.FILTER_RAMLAK, mode=oracle.SCAN_180)[0]
+        truth = wl.rasterize_ellipses(ell, N, N)
+        # pixels at least 2 px from any edge: erode by comparing with shifted copies
+        core = np.ones_like(truth, dtype=bool)
+        for di in range(-2, 3):
+            for dj in range(-2, 3):
+                core &= np.roll(np.roll(truth, di, 0), dj, 1) == truth
+        jj = np.arange(N) - (N - 1) / 2.0                # and inside the detector's field of view
+        core &= (jj[None, :] ** 2 + jj[:, None] ** 2) < (N / 2 - 2) ** 2
+        errs.append(np.sqrt(np.mean((rec - truth)[core] ** 2)))
+        means.append((rec[np.isclose(truth, 0.6) & core].mean() if N >= 64 else None,   # 1.0 - 0.4
+                      rec[np.isclose(truth, 1.0) & core].mean(), rec[(truth == 0) & core].mean()))
+    # thresholds: the paper gives no number; these bound the oracle's first run (0.0242, 0.0188,
+    # 0.0141; interior means 0.60024, 1.00009, -8e-5 at N = 128) with ~15 % slack
+    assert errs[0] > errs[1] > errs[2]
+    assert errs[2] < 0.0165
+    assert abs(means[2][0] - 0.6) < 1e-3 and abs(means[2][1] - 1.0) < 5e-4 and abs(means[2][2]) < 5e-4
+
+
+# --------------------------------------------------------------------------- K11
+def test_k11_half_acquisition_equals_full_detector_scan(oracle):
+    import torch
+    B, c, P = 128, 118.0, 360
+    N = 2 * int(c)
+    ell = np.array([[10.0, -20.0, 60.0, 45.0, 0.3, 1.0], [-40.0, 30.0, 25.0, 18.0, 1.0, 0.5]])
+    angles = np.arange(P) * 2 * math.pi / P
+    axis = np.full(P, c)
+    s_half = torch.arange(B, dtype=torch.float64)[None, :] - torch.tensor(axis)[:, None]
+    half = wl.ellipse_radon(ell, angles, s_half).numpy()[None].astype(np.float32)
+    Bf = 2 * int(c) + 1
+    s_full = torch.arange(Bf, dtype=torch.float64)[None, :] - torch.tensor(axis)[:, None]
+    full = wl.ellipse_radon(ell, angles, s_full).numpy()[None].astype(np.float32)
+    r_half = oracle.fbp(half, angles, axis, N, N, mode=oracle.SCAN_360_HALF)[0]
+    r_full = oracle.fbp(full, angles, axis, N, N, mode=oracle.SCAN_360)[0]
+    jj = np.arange(N) - (N - 1) / 2.0
+    disc = (jj[None, :] ** 2 + jj[:, None] ** 2) < (c - 4) ** 2
+    assert np.abs(r_half - r_full)[disc].max() < 5e-3 * np.abs(r_full).max()
+    # weights: w(s) + w(-s) = 1 on the overlap, exactly; 1 beyond it; both axis sides
+    for cbar in (118.0, 9.0, 100.25):
+        w = oracle.halfacq_weights(B, cbar)
+        right = cbar >= (B - 1) / 2
+        omega = (B - 1 - cbar) if right else cbar
+        for b in range(B):
+            sv = b - cbar
+            mirror = cbar - sv
+            if abs(sv) <= omega and float(mirror).is_integer() and 0 <= mirror < B:
+                assert w[b] + w[int(mirror)] == pytest.approx(1.0, abs=1e-15)
+            if (sv < -omega and right) or (sv > omega and not right):
+                assert w[b] == 1.0
+    ext, pad = oracle.halfacq_extent(2048, 1900.0)
+    assert (ext, pad) == (3840, 0)
+    ext, pad = oracle.halfacq_extent(2048, 147.0)
+    assert (ext, pad) == (3840, 3840 - 2048)
+
+
+def test_k11_fbp_modes_scale(oracle):
+    """SCAN_360 over a doubled angle list equals SCAN_180 (each ray measured twice, scale pi/P)."""
+    w = wl.custom(1, 40, 48, 32, 32, noise=0.0, seed=3)
+    sino = w.sinogram()
+    r180 = oracle.fbp(sino, w.angles, w.axis, 32, 32, mode=oracle.SCAN_180)
+    ang2 = np.concatenate([w.angles, w.angles])
+    ax2 = np.concatenate([w.axis, w.axis])
+    r360 = oracle.fbp(np.concatenate([sino, sino], 1), ang2, ax2, 32, 32, mode=oracle.SCAN_360)
+    np.testing.assert_allclose(r360, r180, rtol=1e-12, atol=1e-14)
+
+
+# --------------------------------------------------------------------------- K12
+def test_k12_batch_independence_and_point_variants(oracle):
+    w = wl.custom(3, 21, 50, 31, 27, pixel_size=1.2, drift=1.0, seed=5)
+    sino = w.sinogram()
+    full = oracle.backproject(sino, w.angles, w.axis, w.nx, w.ny, w.pixel_size, 0.5)
+    for s in range(3):
+        one = oracle.backproject(sino[s:s + 1], w.angles, w.axis, w.nx, w.ny, w.pixel_size, 0.5)
+        assert np.array_equal(one[0], full[s])
+    pts = np.array([[0, 0, 0], [2, 26, 30], [1, 13, 7]])
+    got = oracle.backproject_points(sino, w.angles, w.axis, w.nx, w.ny, pts, w.pixel_size, 0.5)
+    assert np.array_equal(got, full[pts[:, 0], pts[:, 1], pts[:, 2]])
+    x = wl.random_image(3, w.ny, w.nx, seed=1)
+    fpf = oracle.forward_project(x, w.angles, w.axis, w.n_bins, w.pixel_size, 2.0)
+    rows = np.array([[0, 0], [2, 20], [1, 11]])
+    fpr = oracle.forward_project_rows(x, w.angles, w.axis, w.n_bins, rows, w.pixel_size, 2.0)
+    assert np.array_equal(fpr, fpf[rows[:, 0], rows[:, 1]])
+    rec = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, w.pixel_size, filter=1, mode=0)
+    recp = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, w.pixel_size, filter=1, mode=0, pts=pts)
+    assert np.array_equal(recp, rec[pts[:, 0], pts[:, 1], pts[:, 2]])
+    # fbp = filter then backproject with scale pi/P
+    filt = oracle.ramp_filter(sino, filter=1)
+    rec2 = oracle.backproject(filt, w.angles, w.axis, w.nx, w.ny, w.pixel_size, math.pi / w.n_angles)
+    assert np.array_equal(rec2, rec)
+
+
+def test_oracle_rejects_bad_arguments(oracle):
+    q = np.zeros((1, 4, 8), dtype=np.float32)
+    with pytest.raises(ValueError):
+        oracle.backproject(q, np.zeros(4), np.array([0, 0, np.nan, 0.0]), 4, 4)
+    with pytest.raises(ValueError):
+        oracle.backproject(q, np.zeros(4), np.zeros(4), 4, 4, pixel_size=0.0)
+    with pytest.raises(ValueError):
+        oracle.ramp_filter(q[0], n_bins_out=4)
