@@ -1,0 +1,417 @@
+// C ABI of libpyhst_b200 (include/pyhst.h): argument validation, plan / workspace caches and the
+// sequencing of the kernels.  Every step of the hot path runs on the device; there is no CPU
+// fallback (a missing or non-sm_100 device yields PYHST_ERR_UNSUPPORTED).
+#include <cmath>
+#include <cstring>
+#include <list>
+#include <mutex>
+
+#include "common.h"
+
+namespace pyhst {
+
+// ---- errors ------------------------------------------------------------------------------
+char* last_error_buf() {
+  static thread_local char buf[512] = {0};
+  return buf;
+}
+
+int set_error(int status, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(last_error_buf(), 512, fmt, ap);
+  va_end(ap);
+  return status;
+}
+
+int require_sm100(int* n_sm) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return set_error(PYHST_ERR_UNSUPPORTED, "no CUDA device (%s); there is no CPU fallback",
+                     cudaGetErrorString(e));
+  }
+  static int cached_dev = -1, cached_major = 0, cached_sms = 0;
+  if (dev != cached_dev) {
+    int major = 0, sms = 0;
+    PYHST_CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    PYHST_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    cached_dev = dev;
+    cached_major = major;
+    cached_sms = sms;
+  }
+  if (cached_major != 10)
+    return set_error(PYHST_ERR_UNSUPPORTED,
+                     "device has compute capability %d.x; this library is built for sm_100a only",
+                     cached_major);
+  if (n_sm) *n_sm = cached_sms;
+  return PYHST_OK;
+}
+
+// ---- caches ------------------------------------------------------------------------------
+namespace {
+std::mutex g_mu;
+std::list<GeomPlan> g_geom;
+uint64_t g_tick = 0;
+struct Ws { void* p = nullptr; size_t bytes = 0; };
+Ws g_ws[WS_COUNT];
+int g_bp_variant = 0;
+cudaStream_t g_streams[3] = {nullptr, nullptr, nullptr};
+cudaEvent_t g_events[8] = {nullptr};
+}  // namespace
+
+int get_geom_plan(const pyhst_geom_t* g, double axis_shift, cudaStream_t stream,
+                  const GeomPlan** out) {
+  std::lock_guard<std::mutex> lock(g_mu);
+  const size_t n = (size_t)g->n_angles;
+  for (auto& pl : g_geom) {
+    if (pl.n_angles == g->n_angles && pl.pixel_size == g->pixel_size && pl.axis_shift == axis_shift &&
+        std::memcmp(pl.angles.data(), g->angles_rad, n * sizeof(double)) == 0 &&
+        std::memcmp(pl.axis.data(), g->axis_pos, n * sizeof(double)) == 0) {
+      pl.last_use = ++g_tick;
+      *out = &pl;
+      return PYHST_OK;
+    }
+  }
+  if (g_geom.size() >= 16) {  // evict the least recently used plan
+    auto lru = g_geom.begin();
+    for (auto it = g_geom.begin(); it != g_geom.end(); ++it)
+      if (it->last_use < lru->last_use) lru = it;
+    cudaFree(lru->d_proj);  // synchronises: no kernel can still be reading it
+    cudaFreeHost(lru->h_pinned);
+    g_geom.erase(lru);
+  }
+  GeomPlan pl;
+  pl.n_angles = g->n_angles;
+  pl.pixel_size = g->pixel_size;
+  pl.axis_shift = axis_shift;
+  pl.angles.assign(g->angles_rad, g->angles_rad + n);
+  pl.axis.assign(g->axis_pos, g->axis_pos + n);
+  PYHST_CUDA_TRY(cudaMallocHost(&pl.h_pinned, n * sizeof(ProjGeom)));
+  cudaError_t e = cudaMalloc(&pl.d_proj, n * sizeof(ProjGeom));
+  if (e != cudaSuccess) {
+    cudaFreeHost(pl.h_pinned);
+    return set_error(PYHST_ERR_NOMEM, "cudaMalloc of the geometry table failed: %s",
+                     cudaGetErrorString(e));
+  }
+  for (size_t p = 0; p < n; ++p) {  // cos/sin in double (R11)
+    pl.h_pinned[p].ch = g->pixel_size * std::cos(g->angles_rad[p]);
+    pl.h_pinned[p].sh = g->pixel_size * std::sin(g->angles_rad[p]);
+    pl.h_pinned[p].c = g->axis_pos[p] + axis_shift;
+  }
+  PYHST_CUDA_TRY(cudaMemcpyAsync(pl.d_proj, pl.h_pinned, n * sizeof(ProjGeom), cudaMemcpyHostToDevice,
+                                 stream));
+  pl.last_use = ++g_tick;
+  g_geom.push_back(std::move(pl));
+  *out = &g_geom.back();
+  return PYHST_OK;
+}
+
+int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr) {
+  std::lock_guard<std::mutex> lock(g_mu);
+  Ws& w = g_ws[slot];
+  if (w.bytes < bytes) {
+    if (w.p) {
+      cudaFree(w.p);  // synchronises the device: nothing can still be using the old block
+      w.p = nullptr;
+      w.bytes = 0;
+    }
+    cudaError_t e = cudaMalloc(&w.p, bytes);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      w.p = nullptr;
+      return set_error(PYHST_ERR_NOMEM, "workspace allocation of %zu bytes failed: %s", bytes,
+                       cudaGetErrorString(e));
+    }
+    w.bytes = bytes;
+  }
+  *ptr = w.p;
+  return PYHST_OK;
+}
+
+// ---- validation --------------------------------------------------------------------------
+static int check_geom(const pyhst_geom_t* g, int64_t* pitch) {
+  if (!g) return set_error(PYHST_ERR_INVALID_ARG, "geometry is NULL");
+  if (g->n_slices <= 0 || g->n_angles <= 0 || g->n_bins <= 0 || g->nx <= 0 || g->ny <= 0)
+    return set_error(PYHST_ERR_INVALID_ARG, "sizes must be positive (S=%d P=%d B=%d nx=%d ny=%d)",
+                     g->n_slices, g->n_angles, g->n_bins, g->nx, g->ny);
+  if (!g->angles_rad || !g->axis_pos)
+    return set_error(PYHST_ERR_INVALID_ARG, "angles_rad / axis_pos is NULL");
+  if (!(g->pixel_size > 0.0) || !std::isfinite(g->pixel_size))
+    return set_error(PYHST_ERR_INVALID_ARG, "pixel_size must be positive and finite");
+  if (g->sino_pitch != 0 && g->sino_pitch < g->n_bins)
+    return set_error(PYHST_ERR_INVALID_ARG, "sino_pitch %lld < n_bins %d", (long long)g->sino_pitch,
+                     g->n_bins);
+  for (int32_t p = 0; p < g->n_angles; ++p)
+    if (!std::isfinite(g->angles_rad[p]) || !std::isfinite(g->axis_pos[p]))
+      return set_error(PYHST_ERR_INVALID_ARG, "angle / axis position %d is not finite", p);
+  if (g->n_angles > 65535)
+    return set_error(PYHST_ERR_UNSUPPORTED, "more than 65535 projections");
+  *pitch = g->sino_pitch ? g->sino_pitch : g->n_bins;
+  return PYHST_OK;
+}
+
+static int check_ptr(const void* p, const char* name) {
+  if (!p) return set_error(PYHST_ERR_INVALID_ARG, "%s is NULL", name);
+  if (reinterpret_cast<uintptr_t>(p) & 3)
+    return set_error(PYHST_ERR_INVALID_ARG, "%s is not 4-byte aligned", name);
+  return PYHST_OK;
+}
+
+static QiLayout qi_layout(int32_t n_slices, int32_t n_angles, int32_t n_bins, double pixel_size) {
+  QiLayout L;
+  L.n_groups = (n_slices + 3) / 4;
+  L.n_angles = n_angles;
+  L.n_bins = n_bins;
+  const int W = backproject_tiled_window(pixel_size);
+  L.zpad = W > 0 ? W : 16;
+  return L;
+}
+
+static bool use_tiled(double pixel_size) {
+  if (g_bp_variant == 1) return false;
+  return backproject_tiled_window(pixel_size) > 0;
+}
+
+}  // namespace pyhst
+
+using namespace pyhst;
+
+extern "C" {
+
+const char* pyhst_last_error(void) { return last_error_buf(); }
+
+int pyhst_set_backproject_variant(int variant) {
+  const int prev = g_bp_variant;
+  if (variant >= 0 && variant <= 2) g_bp_variant = variant;
+  return prev;
+}
+
+void pyhst_release_cache(void) {
+  cudaDeviceSynchronize();
+  release_filter_plans();
+  std::lock_guard<std::mutex> lock(g_mu);
+  for (auto& pl : g_geom) {
+    cudaFree(pl.d_proj);
+    cudaFreeHost(pl.h_pinned);
+  }
+  g_geom.clear();
+  for (int i = 0; i < WS_COUNT; ++i) {
+    if (g_ws[i].p) cudaFree(g_ws[i].p);
+    g_ws[i] = Ws();
+  }
+  for (auto& s : g_streams) if (s) { cudaStreamDestroy(s); s = nullptr; }
+  for (auto& e : g_events) if (e) { cudaEventDestroy(e); e = nullptr; }
+}
+
+int pyhst_halfacq_extent(int32_t n_bins, double cbar, int32_t* n_bins_ext, int32_t* pad_left) {
+  if (n_bins <= 0 || !n_bins_ext || !pad_left || !std::isfinite(cbar))
+    return set_error(PYHST_ERR_INVALID_ARG, "pyhst_halfacq_extent: bad argument");
+  const double mid = 0.5 * (double)(n_bins - 1);
+  const double far = cbar >= mid ? cbar : (double)(n_bins - 1) - cbar;
+  int64_t need = (int64_t)std::ceil(2.0 * far) + 1;
+  if (need < n_bins) need = n_bins;
+  const int64_t ext = ((need + 63) / 64) * 64;
+  if (ext > (1 << 20)) return set_error(PYHST_ERR_INVALID_ARG, "axis too far off the detector");
+  *n_bins_ext = (int32_t)ext;
+  *pad_left = cbar >= mid ? 0 : (int32_t)(ext - n_bins);
+  return PYHST_OK;
+}
+
+int pyhst_ramp_filter(const float* d_in, float* d_out, int64_t n_rows, int32_t n_bins_in,
+                      int32_t n_bins_out, int32_t pad_left, int64_t out_pitch, pyhst_filter_t f,
+                      const float* d_col_weights, void* stream) {
+  PYHST_TRY(check_ptr(d_in, "d_in"));
+  PYHST_TRY(check_ptr(d_out, "d_out"));
+  if (d_col_weights) PYHST_TRY(check_ptr(d_col_weights, "d_col_weights"));
+  if (n_rows < 0 || n_bins_in <= 0 || n_bins_out <= 0 || pad_left < 0)
+    return set_error(PYHST_ERR_INVALID_ARG, "pyhst_ramp_filter: sizes must be positive");
+  if (n_bins_out < n_bins_in + pad_left)
+    return set_error(PYHST_ERR_INVALID_ARG, "n_bins_out %d < n_bins_in %d + pad_left %d", n_bins_out,
+                     n_bins_in, pad_left);
+  if (out_pitch == 0) out_pitch = n_bins_out;
+  if (out_pitch < n_bins_out)
+    return set_error(PYHST_ERR_INVALID_ARG, "out_pitch %lld < n_bins_out %d", (long long)out_pitch,
+                     n_bins_out);
+  if (f != PYHST_FILTER_RAMLAK && f != PYHST_FILTER_SHEPP_LOGAN)
+    return set_error(PYHST_ERR_INVALID_ARG, "unknown filter %d", (int)f);
+  if ((int64_t)n_bins_in + n_bins_out > 16384)
+    return set_error(PYHST_ERR_UNSUPPORTED, "n_bins_in + n_bins_out > 16384");
+  PYHST_TRY(require_sm100(nullptr));
+  return launch_ramp_filter(d_in, n_bins_in, n_rows, n_bins_in, n_bins_out, pad_left, (int)f,
+                            d_col_weights, d_out, out_pitch, nullptr, nullptr, 0,
+                            static_cast<cudaStream_t>(stream));
+}
+
+int pyhst_backproject(const float* d_sino, float* d_img, const pyhst_geom_t* g, float scale,
+                      void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  int64_t pitch = 0;
+  PYHST_TRY(check_ptr(d_sino, "d_sino"));
+  PYHST_TRY(check_ptr(d_img, "d_img"));
+  PYHST_TRY(check_geom(g, &pitch));
+  PYHST_TRY(require_sm100(nullptr));
+  const GeomPlan* plan = nullptr;
+  PYHST_TRY(get_geom_plan(g, 0.0, stream, &plan));
+  BpArgs a{d_img, g->n_slices, g->n_angles, g->n_bins, g->nx, g->ny, scale, plan->d_proj,
+           g->pixel_size};
+  if (!use_tiled(g->pixel_size)) {
+    if (g_bp_variant == 2)
+      return set_error(PYHST_ERR_UNSUPPORTED, "tiled backprojector does not cover pixel_size %g",
+                       g->pixel_size);
+    return launch_backproject_reference(d_sino, pitch, a, stream);
+  }
+  const QiLayout L = qi_layout(g->n_slices, g->n_angles, g->n_bins, g->pixel_size);
+  void* qi = nullptr;
+  PYHST_TRY(get_workspace(WS_QI, L.bytes(), &qi));
+  PYHST_TRY(launch_repack_to_qi(d_sino, pitch, g->n_slices, static_cast<float4*>(qi), L, stream));
+  return launch_backproject_tiled(static_cast<const float4*>(qi), L, a, stream);
+}
+
+int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t* g, float scale,
+                          void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  int64_t pitch = 0;
+  PYHST_TRY(check_ptr(d_img, "d_img"));
+  PYHST_TRY(check_ptr(d_sino, "d_sino"));
+  PYHST_TRY(check_geom(g, &pitch));
+  PYHST_TRY(require_sm100(nullptr));
+  const GeomPlan* plan = nullptr;
+  PYHST_TRY(get_geom_plan(g, 0.0, stream, &plan));
+  void* img_t = nullptr;
+  PYHST_TRY(get_workspace(WS_IMG_T, (size_t)g->n_slices * g->nx * g->ny * 4, &img_t));
+  PYHST_TRY(launch_transpose_images(d_img, static_cast<float*>(img_t), g->n_slices, g->ny, g->nx,
+                                    stream));
+  FpArgs a{d_img, static_cast<const float*>(img_t), d_sino, pitch, g->n_slices, g->n_angles,
+           g->n_bins, g->nx, g->ny, scale, plan->d_proj};
+  return launch_forward_project(a, stream);
+}
+
+// FBP of slices [s0, s0 + ns) of a device stack; d_img points at slice s0's image.
+static int fbp_device(const float* d_sino_raw, int64_t pitch, float* d_img, const pyhst_geom_t* g,
+                      int32_t ns, pyhst_filter_t f, pyhst_scan_t mode, cudaStream_t stream) {
+  const double PI = 3.14159265358979323846264338327950288;
+  int32_t b_out = g->n_bins, pad_left = 0;
+  const float* d_w = nullptr;
+  double scale = PI / (double)g->n_angles;
+  if (mode == PYHST_SCAN_360_HALF) {
+    double cbar = 0.0;
+    for (int32_t p = 0; p < g->n_angles; ++p) cbar += g->axis_pos[p];
+    cbar /= (double)g->n_angles;
+    const double mid = 0.5 * (double)(g->n_bins - 1);
+    const double omega = cbar >= mid ? (double)(g->n_bins - 1) - cbar : cbar;
+    if (!(omega > 0.0))
+      return set_error(PYHST_ERR_INVALID_ARG, "half acquisition: mean axis %g is off the detector", cbar);
+    PYHST_TRY(pyhst_halfacq_extent(g->n_bins, cbar, &b_out, &pad_left));
+    void* w = nullptr;
+    PYHST_TRY(get_workspace(WS_WEIGHTS, (size_t)g->n_bins * 4, &w));
+    PYHST_TRY(launch_halfacq_weights(static_cast<float*>(w), g->n_bins, cbar, stream));
+    d_w = static_cast<const float*>(w);
+    scale = 2.0 * PI / (double)g->n_angles;
+  }
+  if ((int64_t)g->n_bins + b_out > 16384)
+    return set_error(PYHST_ERR_UNSUPPORTED, "n_bins + filtered row length > 16384");
+  const GeomPlan* plan = nullptr;
+  PYHST_TRY(get_geom_plan(g, (double)pad_left, stream, &plan));
+  BpArgs a{d_img, ns, g->n_angles, b_out, g->nx, g->ny, (float)scale, plan->d_proj, g->pixel_size};
+  const int64_t P = g->n_angles;
+  if (!use_tiled(g->pixel_size)) {
+    if (g_bp_variant == 2)
+      return set_error(PYHST_ERR_UNSUPPORTED, "tiled backprojector does not cover pixel_size %g",
+                       g->pixel_size);
+    void* rows = nullptr;
+    PYHST_TRY(get_workspace(WS_ROWS, (size_t)ns * P * b_out * 4, &rows));
+    for (int32_t s = 0; s < ns; ++s)
+      PYHST_TRY(launch_ramp_filter(d_sino_raw + (int64_t)s * P * pitch, pitch, P, g->n_bins, b_out,
+                                   pad_left, (int)f, d_w, static_cast<float*>(rows) + (int64_t)s * P * b_out,
+                                   b_out, nullptr, nullptr, 0, stream));
+    return launch_backproject_reference(static_cast<const float*>(rows), b_out, a, stream);
+  }
+  const QiLayout L = qi_layout(ns, g->n_angles, b_out, g->pixel_size);
+  void* qi = nullptr;
+  PYHST_TRY(get_workspace(WS_QI, L.bytes(), &qi));
+  for (int32_t grp = 0; grp < L.n_groups; ++grp) {
+    const int32_t n_in = std::min(4, ns - grp * 4);
+    PYHST_TRY(launch_ramp_filter(d_sino_raw + (int64_t)grp * 4 * P * pitch, pitch, (int64_t)n_in * P,
+                                 g->n_bins, b_out, pad_left, (int)f, d_w, nullptr, 0,
+                                 static_cast<float4*>(qi) + (int64_t)grp * L.group_f4(), &L, n_in,
+                                 stream));
+  }
+  return launch_backproject_tiled(static_cast<const float4*>(qi), L, a, stream);
+}
+
+static int check_fbp(const pyhst_geom_t* g, pyhst_filter_t f, pyhst_scan_t mode, int64_t* pitch) {
+  PYHST_TRY(check_geom(g, pitch));
+  if (f != PYHST_FILTER_RAMLAK && f != PYHST_FILTER_SHEPP_LOGAN)
+    return set_error(PYHST_ERR_INVALID_ARG, "unknown filter %d", (int)f);
+  if (mode != PYHST_SCAN_180 && mode != PYHST_SCAN_360 && mode != PYHST_SCAN_360_HALF)
+    return set_error(PYHST_ERR_INVALID_ARG, "unknown scan mode %d", (int)mode);
+  return require_sm100(nullptr);
+}
+
+int pyhst_fbp(const float* d_sino_raw, float* d_img, const pyhst_geom_t* g, pyhst_filter_t f,
+              pyhst_scan_t mode, void* stream) {
+  int64_t pitch = 0;
+  PYHST_TRY(check_ptr(d_sino_raw, "d_sino_raw"));
+  PYHST_TRY(check_ptr(d_img, "d_img"));
+  PYHST_TRY(check_fbp(g, f, mode, &pitch));
+  return fbp_device(d_sino_raw, pitch, d_img, g, g->n_slices, f, mode, static_cast<cudaStream_t>(stream));
+}
+
+int pyhst_fbp_host(const float* h_sino_raw, float* h_img, const pyhst_geom_t* g, pyhst_filter_t f,
+                   pyhst_scan_t mode, int32_t max_slices_per_chunk, void* stream_) {
+  cudaStream_t user = static_cast<cudaStream_t>(stream_);
+  int64_t pitch = 0;
+  PYHST_TRY(check_ptr(h_sino_raw, "h_sino_raw"));
+  PYHST_TRY(check_ptr(h_img, "h_img"));
+  PYHST_TRY(check_fbp(g, f, mode, &pitch));
+  // chunk = a multiple of 4 slices (one slice group of the interleaved layout)
+  int32_t chunk = max_slices_per_chunk > 0 ? max_slices_per_chunk : 8;
+  chunk = std::max(4, (chunk / 4) * 4);
+  chunk = std::min(chunk, ((g->n_slices + 3) / 4) * 4);
+  const int64_t P = g->n_angles;
+  const size_t in_bytes = (size_t)chunk * P * pitch * 4, out_bytes = (size_t)chunk * g->nx * g->ny * 4;
+  for (int i = 0; i < 3; ++i)
+    if (!g_streams[i]) PYHST_CUDA_TRY(cudaStreamCreateWithFlags(&g_streams[i], cudaStreamNonBlocking));
+  for (int i = 0; i < 8; ++i)
+    if (!g_events[i]) PYHST_CUDA_TRY(cudaEventCreateWithFlags(&g_events[i], cudaEventDisableTiming));
+  cudaStream_t s_in = g_streams[0], s_k = g_streams[1], s_out = g_streams[2];
+  void *d_in[2], *d_out[2];  // device double buffers
+  void* blk = nullptr;
+  PYHST_TRY(get_workspace(WS_CHUNKS, 2 * in_bytes + 2 * out_bytes, &blk));
+  d_in[0] = blk;
+  d_in[1] = static_cast<char*>(blk) + in_bytes;
+  d_out[0] = static_cast<char*>(blk) + 2 * in_bytes;
+  d_out[1] = static_cast<char*>(blk) + 2 * in_bytes + out_bytes;
+  cudaEvent_t ev_start = g_events[0];
+  cudaEvent_t ev_in[2] = {g_events[1], g_events[2]}, ev_k[2] = {g_events[3], g_events[4]},
+              ev_out[2] = {g_events[5], g_events[6]};
+  PYHST_CUDA_TRY(cudaEventRecord(ev_start, user));
+  for (int i = 0; i < 3; ++i) PYHST_CUDA_TRY(cudaStreamWaitEvent(g_streams[i], ev_start, 0));
+  int n = 0;
+  for (int32_t s0 = 0; s0 < g->n_slices; s0 += chunk, ++n) {
+    const int32_t ns = std::min(chunk, g->n_slices - s0);
+    const int b = n & 1;
+    if (n >= 2) PYHST_CUDA_TRY(cudaStreamWaitEvent(s_in, ev_k[b], 0));    // kernels of chunk n-2 read d_in[b]
+    PYHST_CUDA_TRY(cudaMemcpyAsync(d_in[b], h_sino_raw + (int64_t)s0 * P * pitch, (size_t)ns * P * pitch * 4,
+                                   cudaMemcpyHostToDevice, s_in));
+    PYHST_CUDA_TRY(cudaEventRecord(ev_in[b], s_in));
+    PYHST_CUDA_TRY(cudaStreamWaitEvent(s_k, ev_in[b], 0));
+    if (n >= 2) PYHST_CUDA_TRY(cudaStreamWaitEvent(s_k, ev_out[b], 0));   // D2H of chunk n-2 read d_out[b]
+    pyhst_geom_t gc = *g;
+    gc.n_slices = ns;
+    PYHST_TRY(fbp_device(static_cast<const float*>(d_in[b]), pitch, static_cast<float*>(d_out[b]), &gc,
+                         ns, f, mode, s_k));
+    PYHST_CUDA_TRY(cudaEventRecord(ev_k[b], s_k));
+    PYHST_CUDA_TRY(cudaStreamWaitEvent(s_out, ev_k[b], 0));
+    PYHST_CUDA_TRY(cudaMemcpyAsync(h_img + (int64_t)s0 * g->nx * g->ny, d_out[b],
+                                   (size_t)ns * g->nx * g->ny * 4, cudaMemcpyDeviceToHost, s_out));
+    PYHST_CUDA_TRY(cudaEventRecord(ev_out[b], s_out));
+  }
+  for (int i = 0; i < 3; ++i) PYHST_CUDA_TRY(cudaStreamSynchronize(g_streams[i]));
+  PYHST_CUDA_TRY(cudaStreamSynchronize(user));
+  return PYHST_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,118 @@
+// Internal helpers of libpyhst_b200 (not part of the C ABI; see include/pyhst.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <vector>
+
+#include "../../include/pyhst.h"
+
+namespace pyhst {
+
+// ---- thread-local last error ------------------------------------------------------------
+char* last_error_buf();
+int set_error(int status, const char* fmt, ...);
+
+#define PYHST_CUDA_TRY(expr)                                                                   \
+  do {                                                                                         \
+    cudaError_t _e = (expr);                                                                   \
+    if (_e != cudaSuccess)                                                                     \
+      return ::pyhst::set_error(_e == cudaErrorMemoryAllocation ? PYHST_ERR_NOMEM              \
+                                                                : PYHST_ERR_CUDA,              \
+                                "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e),        \
+                                __FILE__, __LINE__);                                           \
+  } while (0)
+
+#define PYHST_TRY(expr)            \
+  do {                             \
+    int _s = (expr);               \
+    if (_s != PYHST_OK) return _s; \
+  } while (0)
+
+// sm_100 device present and current?  (no CPU fallback: anything else is UNSUPPORTED)
+int require_sm100(int* n_sm);
+
+// ---- per-projection geometry, built in double on the host (reading R11) -----------------
+// t_p(i,j) = c + ch * (j - j0) + sh * (i - i0),  ch = h cos(theta_p), sh = h sin(theta_p)
+struct ProjGeom {
+  double ch, sh, c;
+};
+
+struct GeomPlan {
+  // key
+  int32_t n_angles = 0;
+  double pixel_size = 0, axis_shift = 0;
+  std::vector<double> angles, axis;
+  // device table [n_angles]
+  ProjGeom* d_proj = nullptr;
+  ProjGeom* h_pinned = nullptr;
+  uint64_t last_use = 0;
+};
+
+// Returns a cached (or new) device geometry table for g (axis shifted by axis_shift bins).
+int get_geom_plan(const pyhst_geom_t* g, double axis_shift, cudaStream_t stream,
+                  const GeomPlan** out);
+
+// Grow-only device workspace slots owned by the library (freed by pyhst_release_cache).
+enum WorkspaceSlot { WS_QI = 0, WS_FFT = 1, WS_WEIGHTS = 2, WS_IMG_T = 3, WS_ROWS = 4,
+                     WS_CHUNKS = 5, WS_COUNT = 6 };
+int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr);
+
+// ---- interleaved sinogram layout consumed by the tiled backprojector ---------------------
+// QI[g][p][zpad + b][sl]: slice group g = s / 4, sl = s % 4, one float4 per (g, p, bin);
+// every row carries `zpad` zero bins on both sides so that a tile's detector window is one
+// contiguous, 16-byte aligned run of float4 that never leaves the row (reading R6).
+struct QiLayout {
+  int32_t n_groups, n_angles, n_bins, zpad;
+  int64_t row_f4() const { return (int64_t)n_bins + 2 * (int64_t)zpad; }          // float4 per row
+  int64_t group_f4() const { return row_f4() * n_angles; }                        // float4 per group
+  size_t bytes() const { return (size_t)group_f4() * (size_t)n_groups * 16; }
+};
+
+// ---- kernels' host launchers (each validates nothing; api.cu did) -------------------------
+struct BpArgs {
+  float* d_img;          // [S][ny][nx]
+  int32_t n_slices, n_angles, n_bins, nx, ny;
+  float scale;
+  const ProjGeom* d_proj;
+  double pixel_size;
+};
+int launch_backproject_reference(const float* d_sino, int64_t pitch, const BpArgs& a,
+                                 cudaStream_t stream);
+// window width (bins) the tiled kernel needs for this pixel size; 0 if unsupported
+int backproject_tiled_window(double pixel_size);
+int launch_backproject_tiled(const float4* d_qi, const QiLayout& L, const BpArgs& a,
+                             cudaStream_t stream);
+// [S][P][pitch] -> QI (zero pads and missing slices written as zeros)
+int launch_repack_to_qi(const float* d_sino, int64_t pitch, int32_t n_slices, float4* d_qi,
+                        const QiLayout& L, cudaStream_t stream);
+
+struct FpArgs {
+  const float* d_img;    // [S][ny][nx]
+  const float* d_img_t;  // [S][nx][ny] (transposed copy, made by launch_transpose_images)
+  float* d_sino;         // [S][P][pitch]
+  int64_t pitch;
+  int32_t n_slices, n_angles, n_bins, nx, ny;
+  float scale;
+  const ProjGeom* d_proj;
+};
+int launch_transpose_images(const float* d_img, float* d_img_t, int32_t n_slices, int32_t ny,
+                            int32_t nx, cudaStream_t stream);
+int launch_forward_project(const FpArgs& a, cudaStream_t stream);
+
+// Ramp filter of `n_rows` rows.  Exactly one of the two outputs is used:
+//   d_out != nullptr : plain rows [n_rows][out_pitch]
+//   d_qi  != nullptr : rows are [n_slices_in <= 4][n_angles] of ONE slice group, written
+//                      interleaved into d_qi (already offset to that group), pads zeroed.
+int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int32_t n_bins_in,
+                       int32_t n_bins_out, int32_t pad_left, int filter,
+                       const float* d_col_weights, float* d_out, int64_t out_pitch,
+                       float4* d_qi, const QiLayout* L, int32_t n_slices_in,
+                       cudaStream_t stream);
+int launch_halfacq_weights(float* d_w, int32_t n_bins, double cbar, cudaStream_t stream);
+void release_filter_plans();
+
+}  // namespace pyhst

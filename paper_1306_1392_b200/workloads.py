@@ -37,8 +37,20 @@ def _rng(cfg: int, slice_idx: int) -> np.random.Generator:
     return np.random.Generator(np.random.PCG64(SEED_BASE + 1000 * cfg + slice_idx))
 
 
+# Device on which the sinograms are synthesised.  "cpu" (default) is what the parity tests use:
+# the arrays are bit-reproducible across machines.  bench.py sets it to "cuda" so that a full
+# 16-slice stack is made in seconds; the noise stream then comes from the device generator.
+_DEVICE = "cpu"
+
+
+def set_device(device: str) -> str:
+    global _DEVICE
+    prev, _DEVICE = _DEVICE, str(device)
+    return prev
+
+
 def _torch_gen(cfg: int, slice_idx: int) -> torch.Generator:
-    g = torch.Generator(device="cpu")
+    g = torch.Generator(device=_DEVICE)
     g.manual_seed(SEED_BASE + 1000 * cfg + slice_idx + 500)
     return g
 
@@ -54,7 +66,7 @@ def ellipse_radon(ell: np.ndarray, angles: np.ndarray, s: torch.Tensor) -> torch
     (a disc of radius R reduces to the chord 2 rho sqrt(R^2 - s^2)).
     """
     out = torch.zeros_like(s)
-    th = torch.as_tensor(np.asarray(angles, dtype=np.float64))
+    th = torch.as_tensor(np.asarray(angles, dtype=np.float64)).to(s.device)
     for x0, y0, a, b, phi, rho in np.asarray(ell, dtype=np.float64).reshape(-1, 6):
         r2 = (a * torch.cos(th - phi)) ** 2 + (b * torch.sin(th - phi)) ** 2
         s0 = x0 * torch.cos(th) + y0 * torch.sin(th)
@@ -70,7 +82,7 @@ def polygon_radon(polys: Sequence[np.ndarray], rhos: Sequence[float], angles: np
     The line {x cos + y sin = s} is parametrised by u along (-sin, cos); each edge is a
     half-plane that clips the interval of u; the chord is the length left."""
     out = torch.zeros_like(s)
-    th = torch.as_tensor(np.asarray(angles, dtype=np.float64))
+    th = torch.as_tensor(np.asarray(angles, dtype=np.float64)).to(s.device)
     ct, st = torch.cos(th)[:, None], torch.sin(th)[:, None]
     for verts, rho in zip(polys, rhos):
         verts = np.asarray(verts, dtype=np.float64)
@@ -161,11 +173,16 @@ class Workload:
 
     def bin_offsets(self) -> torch.Tensor:
         """s[p,b] = b - c_p (float64 [P,B])."""
-        b = torch.arange(self.n_bins, dtype=torch.float64)
-        return b[None, :] - torch.as_tensor(self.axis)[:, None]
+        b = torch.arange(self.n_bins, dtype=torch.float64, device=_DEVICE)
+        return b[None, :] - torch.as_tensor(self.axis).to(_DEVICE)[:, None]
 
     def sinogram_slice(self, s: int) -> np.ndarray:
-        return self._slice_fn(self, s).to(torch.float32).numpy()
+        return self._slice_fn(self, s).to(torch.float32).cpu().numpy()
+
+    def sinogram_tensor(self, slices: Optional[Sequence[int]] = None) -> torch.Tensor:
+        """float32 [S,P,B] torch tensor left on the synthesis device (see set_device)."""
+        idx = range(self.n_slices) if slices is None else slices
+        return torch.stack([self._slice_fn(self, s).to(torch.float32) for s in idx], dim=0)
 
     def sinogram(self, slices: Optional[Sequence[int]] = None) -> np.ndarray:
         """float32 [S,P,B] (C order) for the requested slices (default: all)."""
@@ -179,7 +196,7 @@ class Workload:
 
 def _gauss(p: torch.Tensor, rel_sigma: float, gen: torch.Generator) -> torch.Tensor:
     sigma = rel_sigma * float(p.abs().max())
-    return p + sigma * torch.randn(p.shape, dtype=torch.float64, generator=gen)
+    return p + sigma * torch.randn(p.shape, dtype=torch.float64, generator=gen, device=p.device)
 
 
 def _poisson_log(p: torch.Tensor, photons: float, gen: torch.Generator) -> torch.Tensor:

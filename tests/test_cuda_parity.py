@@ -1,0 +1,278 @@
+"""GPU-vs-oracle parity of the four C-ABI entry points (run on a B200 with ``-m gpu``).
+
+Both sides get the same seeded float32 inputs from ``paper_1306_1392_b200.workloads``; the CUDA
+path is called through the C ABI (ctypes binding) and compared element by element with the
+double-precision oracle.  The bar is BASELINE.json's: relative L2 error <= 1e-5 and max-abs error
+<= 1e-4 * max|oracle|.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+REL_L2 = 1e-5
+MAX_ABS = 1e-4
+
+
+@pytest.fixture(scope="module")
+def lib():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device; there is no CPU fallback")
+    import paper_1306_1392_b200 as P
+    P.binding._load()          # fail loudly if libpyhst_b200.so is missing
+    yield P
+    P.release_cache()
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def assert_parity(got, want, what, rel=REL_L2, mabs=MAX_ABS):
+    got = np.asarray(got, dtype=np.float64)
+    want = np.asarray(want, dtype=np.float64)
+    assert got.shape == want.shape, what
+    assert np.isfinite(got).all(), what + ": non-finite output"
+    num = np.linalg.norm((got - want).ravel())
+    den = np.linalg.norm(want.ravel())
+    peak = np.abs(want).max()
+    err_max = np.abs(got - want).max()
+    assert num <= rel * den + 1e-30, "%s: rel-L2 %.3e > %.1e" % (what, num / max(den, 1e-300), rel)
+    assert err_max <= mabs * peak + 1e-30, "%s: max-abs %.3e > %.1e * %.3e" % (what, err_max, mabs, peak)
+    return num / max(den, 1e-300)
+
+
+# ------------------------------------------------------------------------------ backprojection
+BP_CASES = [
+    # S, P, B, nx, ny, h, axis, drift  -- ragged slice group, ragged chunk of projections, several tiles
+    (1, 1, 40, 33, 21, 1.0, None, 0.0),
+    (5, 37, 211, 150, 70, 1.0, None, 1.5),
+    (3, 50, 97, 130, 131, 0.8, 30.2, 0.7),      # axis off centre: many pixels leave the detector
+    (2, 19, 64, 200, 90, 1.3, None, 0.0),       # pixel larger than a bin: image wider than detector
+    (4, 16, 300, 64, 64, 0.5, None, 2.0),       # exactly one tile and one chunk
+    (9, 33, 180, 70, 129, 1.0, 179.0, 0.0),     # axis at the detector border
+]
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("case", BP_CASES)
+def test_backproject_matches_oracle(lib, oracle, case, variant):
+    S, P, B, nx, ny, h, axis, drift = case
+    wl = lib.workloads
+    w = wl.custom(S, P, B, nx, ny, pixel_size=h, axis=axis, drift=drift, jitter_angles=0.01, seed=P)
+    sino = wl.random_sinogram(S, P, B, seed=B)
+    want = oracle.backproject(sino, w.angles, w.axis, nx, ny, pixel_size=h, scale=0.37)
+    prev = lib.set_backproject_variant(variant)
+    try:
+        got = lib.backproject(_dev(sino), w.angles, w.axis, nx, ny, pixel_size=h, scale=0.37).cpu().numpy()
+    finally:
+        lib.set_backproject_variant(prev)
+    assert_parity(got, want, "backproject variant %d %r" % (variant, case))
+
+
+def test_backproject_config1_full(lib, oracle):
+    w = lib.workloads.config(1)
+    sino = lib.workloads.random_sinogram(1, w.n_angles, w.n_bins, seed=1)
+    want = oracle.backproject(sino, w.angles, w.axis, w.nx, w.ny)
+    got = lib.backproject(_dev(sino), w.angles, w.axis, w.nx, w.ny).cpu().numpy()
+    assert_parity(got, want, "backproject cfg1")
+
+
+def test_backproject_batch_independence(lib):
+    """K12 on the device: a slice's result does not depend on the stack it is computed in."""
+    wl = lib.workloads
+    w = wl.custom(6, 40, 120, 90, 80, drift=1.0)
+    sino = _dev(wl.random_sinogram(6, 40, 120, seed=5))
+    full = lib.backproject(sino, w.angles, w.axis, 90, 80)
+    one = lib.backproject(sino[2:3].contiguous(), w.angles, w.axis, 90, 80)
+    assert (full[2] == one[0]).all()
+
+
+def test_backproject_affine_rows(lib):
+    """K1 on the device: rows linear in the bin index back-project to scale * sum_p(alpha + beta t)."""
+    rng = np.random.default_rng(11)
+    S, P, B, nx, ny, h = 2, 23, 400, 140, 100, 1.0
+    angles = np.sort(rng.uniform(0, math.pi, P))
+    axis = (B - 1) / 2 + rng.uniform(-1, 1, P)
+    alpha = np.round(rng.normal(size=(S, P)) * 64) / 64
+    beta = np.round(rng.normal(size=(S, P)) * 64) / 1024
+    sino = (alpha[..., None] + beta[..., None] * np.arange(B)).astype(np.float32)
+    j = np.arange(nx) - (nx - 1) / 2
+    i = np.arange(ny) - (ny - 1) / 2
+    t = axis[:, None, None] + h * (j[None, None, :] * np.cos(angles)[:, None, None]
+                                   + i[None, :, None] * np.sin(angles)[:, None, None])
+    assert t.min() >= 0 and t.max() <= B - 1
+    want = np.einsum("sp,pij->sij", alpha, np.ones_like(t)) + np.einsum("sp,pij->sij", beta, t)
+    got = lib.backproject(_dev(sino), angles, axis, nx, ny, pixel_size=h).cpu().numpy()
+    assert_parity(got, want, "affine rows")
+
+
+# ------------------------------------------------------------------------------ forward projection
+FP_CASES = [
+    (1, 1, 40, 33, 21, 1.0, None, 0.0),
+    (3, 37, 211, 150, 70, 1.0, None, 1.5),
+    (2, 50, 97, 130, 131, 0.8, 30.2, 0.7),
+    (2, 19, 64, 200, 90, 1.3, None, 0.0),
+    (2, 24, 300, 64, 64, 0.5, None, 2.0),       # pixel smaller than a bin: > 3 pixels per line in a strip
+]
+
+
+@pytest.mark.parametrize("case", FP_CASES)
+def test_forward_project_matches_oracle(lib, oracle, case):
+    S, P, B, nx, ny, h, axis, drift = case
+    wl = lib.workloads
+    w = wl.custom(S, P, B, nx, ny, pixel_size=h, axis=axis, drift=drift, jitter_angles=0.01, seed=P,
+                  span=2 * math.pi)
+    x = wl.random_image(S, ny, nx, seed=nx)
+    want = oracle.forward_project(x, w.angles, w.axis, B, pixel_size=h, scale=1.7)
+    got = lib.forward_project(_dev(x), w.angles, w.axis, B, pixel_size=h, scale=1.7).cpu().numpy()
+    assert_parity(got, want, "forward_project %r" % (case,))
+
+
+def test_forward_project_axis_aligned_angles(lib, oracle):
+    """theta = 0, pi/2, pi, 3pi/2 exactly: the strip degenerates onto pixel rows / columns."""
+    wl = lib.workloads
+    S, B, nx, ny = 2, 90, 60, 50
+    angles = np.array([0.0, math.pi / 2, math.pi, 1.5 * math.pi, math.pi / 4, 3 * math.pi / 4])
+    axis = np.array([44.5, 44.5, 44.0, 45.25, 44.5, 44.5])
+    x = wl.random_image(S, ny, nx, seed=3)
+    want = oracle.forward_project(x, angles, axis, B)
+    got = lib.forward_project(_dev(x), angles, axis, B).cpu().numpy()
+    assert_parity(got, want, "forward_project axis-aligned")
+
+
+@pytest.mark.parametrize("B,axis", [(260, None), (120, 75.3)])
+def test_adjoint_identity_on_device(lib, B, axis):
+    """K3 in FP32: |<P x, y> - <x, P^T y>| <= 1e-5 ||P x|| ||y||."""
+    import torch
+    wl = lib.workloads
+    S, P, nx, ny = 3, 61, 170, 150
+    w = wl.custom(S, P, B, nx, ny, axis=axis, drift=1.0, jitter_angles=0.02)
+    x = _dev(wl.random_image(S, ny, nx, seed=1))
+    y = _dev(wl.random_sinogram(S, P, B, seed=2))
+    Px = lib.forward_project(x, w.angles, w.axis, B)
+    Pty = lib.backproject(y, w.angles, w.axis, nx, ny)
+    lhs = torch.dot(Px.double().ravel(), y.double().ravel()).item()
+    rhs = torch.dot(x.double().ravel(), Pty.double().ravel()).item()
+    bound = 1e-5 * Px.double().norm().item() * y.double().norm().item()
+    assert abs(lhs - rhs) <= bound, (lhs, rhs, bound)
+
+
+# ------------------------------------------------------------------------------ ramp filter
+@pytest.mark.parametrize("f", [0, 1])
+@pytest.mark.parametrize("b_in,b_out,pad,weights", [(367, 367, 0, False), (128, 256, 0, True),
+                                                    (100, 192, 92, True), (64, 64, 0, False),
+                                                    (2048, 2048, 0, False)])
+def test_ramp_filter_matches_oracle(lib, oracle, f, b_in, b_out, pad, weights):
+    rng = np.random.default_rng(b_in + f)
+    rows = rng.normal(size=(7, b_in)).astype(np.float32)
+    w = rng.uniform(0, 1, b_in).astype(np.float32) if weights else None
+    want = oracle.ramp_filter(rows, n_bins_out=b_out, pad_left=pad, filter=f, col_weights=w)
+    got = lib.ramp_filter(_dev(rows), n_bins_out=b_out, pad_left=pad, filter=f,
+                          col_weights=None if w is None else _dev(w)).cpu().numpy()
+    assert_parity(got, want, "ramp_filter")
+
+
+def test_ramp_filter_zero_rows_is_a_noop(lib):
+    import torch
+    out = lib.ramp_filter(torch.empty((0, 64), dtype=torch.float32, device="cuda"))
+    assert out.shape == (0, 64)
+
+
+# ------------------------------------------------------------------------------ FBP, the five configs
+def test_fbp_config1_full(lib, oracle):
+    w = lib.workloads.config(1)
+    sino = w.sinogram()
+    want = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode)
+    got = lib.fbp(_dev(sino), w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode).cpu().numpy()
+    assert_parity(got, want, "fbp cfg1")
+    # host-buffer entry point: same result through chunked copies
+    got_h = lib.fbp_host(sino, w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode)
+    assert np.array_equal(got_h, got)
+
+
+@pytest.mark.parametrize("cfg,shrink,n_slices", [(2, 8, 6), (3, 8, 4), (4, 4, 3), (5, 8, 9)])
+def test_fbp_shrunken_configs(lib, oracle, cfg, shrink, n_slices):
+    """Configs 2-5 with every length divided by `shrink` (same structure: drift, half acquisition,
+    noise model), whole images compared."""
+    w = lib.workloads.config(cfg, shrink=shrink, n_slices=n_slices)
+    sino = w.sinogram()
+    want = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode)
+    got = lib.fbp(_dev(sino), w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode).cpu().numpy()
+    assert_parity(got, want, "fbp cfg%d/%d" % (cfg, shrink))
+    got_h = lib.fbp_host(sino, w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode,
+                         max_slices_per_chunk=4)
+    assert np.array_equal(got_h, got)
+
+
+def _sample_points(rng, n, slices, ny, nx):
+    pts = np.stack([rng.choice(slices, n), rng.integers(0, ny, n), rng.integers(0, nx, n)], axis=1)
+    corners = [(slices[0], 0, 0), (slices[0], ny - 1, nx - 1), (slices[-1], 0, nx - 1), (slices[-1], ny - 1, 0),
+               (slices[0], ny // 2, nx // 2)]
+    return np.concatenate([pts, np.array(corners)], axis=0).astype(np.int32)
+
+
+@pytest.mark.parametrize("cfg,n_slices", [(2, 16), (3, 4), (5, 8)])
+def test_fbp_full_size_sampled(lib, oracle, cfg, n_slices):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (config 5 with 8 of its
+    64 slices): the oracle evaluates sampled pixels one by one."""
+    w = lib.workloads.config(cfg, n_slices=n_slices)
+    rng = np.random.default_rng(cfg)
+    check = [0, n_slices - 1] if cfg != 5 else [n_slices - 3]
+    sino = w.sinogram()
+    got = lib.fbp(_dev(sino), w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode).cpu().numpy()
+    pts = _sample_points(rng, 400, check, w.ny, w.nx)
+    want = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode, pts=pts)
+    g = got[pts[:, 0], pts[:, 1], pts[:, 2]]
+    assert_parity(g, want, "fbp cfg%d full size (sampled)" % cfg)
+
+
+def test_projector_pair_config4_full(lib, oracle):
+    """Config 4 (iterative): the pair P, P^T at full size on sampled rows / pixels + the K3 identity."""
+    import torch
+    w = lib.workloads.config(4)
+    rng = np.random.default_rng(4)
+    y0 = w.sinogram()
+    x0 = lib.fbp(_dev(y0), w.angles, w.axis, w.nx, w.ny).contiguous()
+    x0h = x0.cpu().numpy()
+    Px = lib.forward_project(x0, w.angles, w.axis, w.n_bins)
+    rows = np.stack([rng.integers(0, w.n_slices, 24), rng.integers(0, w.n_angles, 24)], axis=1)
+    want = oracle.forward_project_rows(x0h, w.angles, w.axis, w.n_bins, rows)
+    assert_parity(Px.cpu().numpy()[rows[:, 0], rows[:, 1]], want, "forward_project cfg4 rows")
+    Pty = lib.backproject(_dev(y0), w.angles, w.axis, w.nx, w.ny)
+    pts = _sample_points(rng, 2000, [0, w.n_slices - 1], w.ny, w.nx)
+    want = oracle.backproject_points(y0, w.angles, w.axis, w.nx, w.ny, pts)
+    assert_parity(Pty.cpu().numpy()[pts[:, 0], pts[:, 1], pts[:, 2]], want, "backproject cfg4 points")
+    yd = _dev(y0)
+    lhs = torch.dot(Px.double().ravel(), yd.double().ravel()).item()
+    rhs = torch.dot(x0.double().ravel(), Pty.double().ravel()).item()
+    assert abs(lhs - rhs) <= 1e-5 * Px.double().norm().item() * yd.double().norm().item()
+
+
+# ------------------------------------------------------------------------------ errors
+def test_invalid_arguments_are_rejected(lib):
+    import torch
+    wl = lib.workloads
+    w = wl.custom(1, 8, 32, 16, 16)
+    sino = _dev(wl.random_sinogram(1, 8, 32))
+    with pytest.raises(lib.PyhstError):
+        lib.backproject(sino, w.angles, w.axis, 16, 16, pixel_size=0.0)
+    bad = w.angles.copy()
+    bad[3] = np.nan
+    with pytest.raises(lib.PyhstError):
+        lib.backproject(sino, bad, w.axis, 16, 16)
+    with pytest.raises(lib.PyhstError):
+        lib.ramp_filter(sino.reshape(8, 32), n_bins_out=16)
+    with pytest.raises(lib.PyhstError):
+        lib.fbp(sino, w.angles, w.axis, 16, 16, filter=7)
+    with pytest.raises(lib.PyhstError):
+        lib.backproject(sino.double(), w.angles, w.axis, 16, 16)
+    assert "filter" in lib.last_error() or lib.last_error() != ""
+    out = torch.full((1, 16, 16), 5.0, device="cuda")
+    with pytest.raises(lib.PyhstError):
+        lib.backproject(sino, w.angles, w.axis, 16, 16, pixel_size=-1.0, out=out)
+    assert (out == 5.0).all()          # nothing written on error
