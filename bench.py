@@ -1,0 +1,370 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path on BASELINE.json's config 2, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference] [--config C]
+
+A *step* is one pass of the whole hot path over one synthetic batch:
+pyhst_fbp (a1 ramp filter -> a2 backprojection = a4) followed by pyhst_forward_project (a3) of the
+reconstructed stack.  `value` counts the pixel*projection*slice updates of BOTH projector calls per
+second of step time (GUPS); `metrics` breaks the step down per stage (CUDA events recorded by the
+library on the launching stream): backprojection GUPS, forward-projection GUPS, FBP slices/s.
+
+N > 1 (torchrun, one rank per GPU): slices are independent, every rank runs the
+same per-GPU stack (weak scaling, no data-path collective); time = max over ranks.
+
+--impl reference times the oracle (oracle/, fp64 CPU) on the host cores on a bounded sample of the
+same workload.  The product path never touches oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "projector updates/s over one hot-path step (ramp filter + backprojection + forward projection)"
+UNIT = "GUPS"
+FP32_LANES_PER_SM = 128          # FP32 FMA lanes per SM per clock (4 SMSP x 32)
+LANE_OPS_PER_UPDATE = 2          # lerp FMA + accumulate FMA
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return json.load(fh), "measured"
+    except OSError:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        fd, self.path = tempfile.mkstemp(suffix=".csv")
+        os.close(fd)
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        with open(self.path) as fh:
+            for line in fh:
+                f = [x.strip() for x in line.split(",")]
+                if len(f) < 7:
+                    continue
+                try:
+                    sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+                except ValueError:
+                    continue
+                for n, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+        os.unlink(self.path)
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), power_w_max=max(pw),
+                       reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def _workload(P, args):
+    w = P.workloads.config(args.config, n_slices=args.slices or None)
+    return w
+
+
+def _config_dict(w, world, extra=None):
+    d = {"workload": "BASELINE.json configs[%d] (%s): %d slices x %dx%d, %d projections x %d bins per GPU"
+                     % (w.cfg - 1, w.name, w.n_slices, w.ny, w.nx, w.n_angles, w.n_bins),
+         "slices_per_gpu": w.n_slices, "n_angles": w.n_angles, "n_bins": w.n_bins, "nx": w.nx, "ny": w.ny,
+         "filter": ["ram-lak", "shepp-logan"][w.filter], "scan": ["180", "360", "360-half"][w.mode],
+         "parallelism": "slices sharded over %d GPU(s), no collective" % world,
+         "step": "pyhst_fbp (ramp filter + backprojection) then pyhst_forward_project of the result",
+         "l2": "inputs larger than L2 (sinogram stack %.0f MB, image stack %.0f MB vs 126 MB L2)"
+               % (w.n_slices * w.n_angles * w.n_bins * 4 / 1e6, w.n_slices * w.nx * w.ny * 4 / 1e6)}
+    if extra:
+        d.update(extra)
+    return d
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+
+    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    if world != args.gpus:
+        if world == 1 and args.gpus > 1:
+            raise SystemExit("--gpus %d needs torchrun with --nproc-per-node %d" % (args.gpus, args.gpus))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference "
+                         "for the oracle baseline)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_1306_1392_b200 as P
+    from paper_1306_1392_b200 import sharding
+
+    P.binding._load()
+    w = _workload(P, args)
+    S, NP, B, nx, ny = w.n_slices, w.n_angles, w.n_bins, w.nx, w.ny
+    # weak scaling: rank r reconstructs slices [r*S, (r+1)*S) of a world*S-slice scan
+    first = sharding.slice_range(S * world, world, rank)[0]
+    P.workloads.set_device("cuda")
+    sino = w.sinogram_tensor(range(first, first + S)).contiguous()
+    P.workloads.set_device("cpu")
+    img = torch.empty((S, ny, nx), dtype=torch.float32, device="cuda")
+    proj = torch.empty((S, NP, B), dtype=torch.float32, device="cuda")
+    updates = S * nx * ny * NP                      # per projector call, per GPU
+
+    def step():
+        P.fbp(sino, w.angles, w.axis, nx, ny, w.pixel_size, filter=w.filter, mode=w.mode, out=img)
+        P.forward_project(img, w.angles, w.axis, B, w.pixel_size, out=proj)
+
+    for _ in range(max(args.warmup, 1)):
+        step()
+    torch.cuda.synchronize()
+    P.profile_read(reset=True)
+    P.profile_enable(True)
+    sampler = ClockSampler(local)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+    ev1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop()
+    ms_total = sharding.max_over_ranks(ev0.elapsed_time(ev1), dist if world > 1 else None)
+    stages = P.profile_read(reset=True)
+    P.profile_enable(False)
+    ms_step = ms_total / args.steps
+
+    # ---- end to end: host (pinned) buffers through the *_host entry points
+    e2e = None
+    if not args.no_e2e:
+        h_sino = torch.empty(sino.shape, dtype=torch.float32, pin_memory=True)
+        h_sino.copy_(sino)
+        h_img = torch.empty((S, ny, nx), dtype=torch.float32, pin_memory=True)
+        h_proj = torch.empty((S, NP, B), dtype=torch.float32, pin_memory=True)
+
+        def e2e_step():
+            P.fbp_host(h_sino, w.angles, w.axis, nx, ny, w.pixel_size, filter=w.filter, mode=w.mode,
+                       out=h_img, max_slices_per_chunk=4)
+            P.forward_project_host(h_img, w.angles, w.axis, B, w.pixel_size, out=h_proj,
+                                   max_slices_per_chunk=4)
+
+        for _ in range(min(args.warmup, 2) or 1):
+            e2e_step()
+        n_e2e = max(1, min(args.steps, 5))
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            e2e_step()
+        torch.cuda.synchronize()
+        ms_e2e = sharding.max_over_ranks((time.perf_counter() - t0) * 1e3, dist if world > 1 else None) / n_e2e
+        e2e = {"value": 2 * updates * world / (ms_e2e * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms_e2e,
+               "steps": n_e2e,
+               "h2d_bytes_per_step": int(h_sino.numel() * 4 + h_img.numel() * 4),
+               "d2h_bytes_per_step": int(h_img.numel() * 4 + h_proj.numel() * 4),
+               "api": "pyhst_fbp_host + pyhst_forward_project_host (pinned host buffers, 4-slice chunks, "
+                      "copies overlapped with kernels)"}
+        P.profile_read(reset=True)
+        del h_sino, h_img, h_proj
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks, peaks_kind = _peaks()
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+    peak_tflops = n_sm * FP32_LANES_PER_SM * 2 * f_max / 1e12   # FP32 FMA issue peak at max clock
+
+    def kernel_roofline(stage, name):
+        ms, launches, _ = stages[stage]
+        if launches == 0:
+            return None
+        avg_ms = ms / launches
+        ach = updates * LANE_OPS_PER_UPDATE * 2 / (avg_ms * 1e-3) / 1e12
+        r = {"kernel": name, "bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s",
+             "frac": ach / peak_tflops, "traffic": None, "avg_ms": avg_ms, "launches": launches,
+             "updates_per_launch": updates, "flop_per_update": 2 * LANE_OPS_PER_UPDATE,
+             "gups": updates / (avg_ms * 1e-3) / 1e9,
+             "peak_note": "%d SMs x 128 FP32 lanes x 2 flop x %.0f MHz (sm_max_mhz, %s peaks file); "
+                          "algorithmic work = 2 FMA per (pixel, projection, slice)"
+                          % (n_sm, f_max / 1e6, peaks_kind)}
+        if clocks.get("sm_mhz"):
+            r["frac_at_sampled_clock"] = r["frac"] * (f_max / 1e6) / clocks["sm_mhz"]
+        tr = _traffic().get(stage)
+        if tr is not None:
+            r["traffic"] = tr
+        return r
+
+    roofs = [x for x in (kernel_roofline("backproject", "bp_tiled_kernel"),
+                         kernel_roofline("forward_project", "fp_gather_kernel")) if x]
+    roofs.sort(key=lambda r: -r["avg_ms"] * r["launches"])
+    ms_bp = stages["backproject"][0] / args.steps
+    ms_fp = (stages["forward_project"][0] + stages["transpose"][0]) / args.steps
+    ms_filter = stages["ramp_filter"][0] / args.steps
+    own = sum(v[1] for v in stages.values())
+    line = {
+        "metric": METRIC, "value": 2 * updates * world / (ms_step * 1e-3) / 1e9, "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "impl": "b200",
+        "config": _config_dict(w, world),
+        "metrics": {"backprojection_gups": updates * world / (ms_bp * 1e-3) / 1e9 if ms_bp else None,
+                    "forward_projection_gups": updates * world / (ms_fp * 1e-3) / 1e9 if ms_fp else None,
+                    "fbp_slices_per_s": S * world / ((ms_filter + ms_bp) * 1e-3) if ms_bp else None,
+                    "ms_ramp_filter": ms_filter, "ms_backproject": ms_bp, "ms_forward_project": ms_fp,
+                    "note": "per-stage device ms of rank 0 (CUDA events recorded by the library on the "
+                            "launching stream, inside the timed region)"},
+        "clocks": clocks, "e2e": e2e,
+        "gpu_launches": own, "gpu_launches_per_step": own / args.steps,
+        "library_launches": {"cufft_execs": sum(v[2] for v in stages.values())},
+        "roofline": roofs[0] if roofs else None, "roofline_other": roofs[1:],
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(P.workloads, args)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _traffic():
+    """dram bytes per launch from the committed ncu --set full capture (profiles/traffic.json)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            return json.load(fh)
+    except (OSError, ValueError):
+        return {}
+
+
+def _oracle_sample(wl_mod, args):
+    """One bounded sample of the workload for the oracle: the first `cpu_slices` slices (default 1) at
+    full size -- all projections, bins and pixels, so every inner loop has the workload's own length."""
+    w = wl_mod.config(args.config, n_slices=max(1, args.cpu_slices))
+    sino = w.sinogram()
+    return w, sino
+
+
+def _time_oracle_step(oracle, w, sino):
+    """One hot-path step in the oracle, as it stands: FBP (direct-convolution filter + BP, fp64) then
+    forward projection of the float32-rounded result."""
+    import numpy as np
+    t0 = time.perf_counter()
+    img = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, pixel_size=w.pixel_size, filter=w.filter, mode=w.mode)
+    oracle.forward_project(img.astype(np.float32), w.angles, w.axis, w.n_bins, pixel_size=w.pixel_size)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(wl_mod, args):
+    import oracle
+    oracle.build()
+    w, sino = _oracle_sample(wl_mod, args)
+    sec = _time_oracle_step(oracle, w, sino)
+    upd = w.n_slices * w.nx * w.ny * w.n_angles
+    return {"value": 2 * upd / sec / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "seconds": sec,
+            "sample": "%d of the config's slices at full size (%dx%d, %d projections x %d bins): oracle FBP "
+                      "(direct O(B^2) ramp convolution + backprojection, fp64, OpenMP) + oracle forward "
+                      "projection, one pass" % (w.n_slices, w.ny, w.nx, w.n_angles, w.n_bins)}
+
+
+def run_reference(args):
+    rank, world = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1)
+    if rank != 0:
+        return
+    from paper_1306_1392_b200 import workloads as wl_mod
+    import oracle
+    oracle.build()
+    w, sino = _oracle_sample(wl_mod, args)
+    full = wl_mod.config(args.config, n_slices=args.slices or None)
+    for _ in range(args.warmup_ref):
+        _time_oracle_step(oracle, w, sino)
+    steps = max(1, min(args.steps, args.max_ref_steps))
+    secs = [_time_oracle_step(oracle, w, sino) for _ in range(steps)]
+    sec = sum(secs) / len(secs)
+    upd = w.n_slices * w.nx * w.ny * w.n_angles
+    val = 2 * upd / sec / 1e9
+    sample = ("each step = %d of %d slices of the config at full size, oracle FBP + forward projection"
+              % (w.n_slices, full.n_slices))
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": steps, "warmup": args.warmup_ref, "ms_per_step": sec * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": _config_dict(full, 1, {"reference": "oracle/ (fp64 CPU, OpenMP) on the host cores; " + sample}),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default 2)")
+    ap.add_argument("--slices", type=int, default=0, help="override slices per GPU")
+    ap.add_argument("--cpu-slices", type=int, default=1, help="slices in the oracle's bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--warmup-ref", type=int, default=0)
+    ap.add_argument("--max-ref-steps", type=int, default=2)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        sys.stderr.write("note: fewer than 3 warm-up steps; the number is not a valid bench value\n")
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

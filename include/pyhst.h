@@ -120,6 +120,14 @@ int pyhst_fbp_host(const float* h_sino_raw, float* h_img, const pyhst_geom_t* g,
                    pyhst_filter_t f, pyhst_scan_t mode, int32_t max_slices_per_chunk,
                    void* stream);
 
+/* a2 / a3 with HOST buffers, same chunked pipeline and synchronisation as pyhst_fbp_host.
+ * With sino_pitch > n_bins the padding columns of h_sino travel too (forward projection leaves
+ * them unspecified). */
+int pyhst_backproject_host(const float* h_sino, float* h_img, const pyhst_geom_t* g, float scale,
+                           int32_t max_slices_per_chunk, void* stream);
+int pyhst_forward_project_host(const float* h_img, float* h_sino, const pyhst_geom_t* g, float scale,
+                               int32_t max_slices_per_chunk, void* stream);
+
 /* Extended row length / left padding of the virtually doubled detector (R10):
  * far = max(cbar, n_bins-1-cbar); *n_bins_ext = ceil(2 far) + 1 rounded up to a multiple of
  * 64; *pad_left = 0 if the axis is right of the detector centre else n_bins_ext - n_bins. */
@@ -129,6 +137,24 @@ int pyhst_halfacq_extent(int32_t n_bins, double cbar, int32_t* n_bins_ext, int32
  * pixel kernel (global loads; kept for cross-checks), 2 = tiled shared-memory kernel.
  * Returns the previous value.  Test/bench hook; results agree within FP32 rounding. */
 int pyhst_set_backproject_variant(int variant);
+
+/* Stage accounting for bench.py / tests.  Stages of the hot path, in call order: */
+enum {
+  PYHST_STAGE_FILTER = 0,      /* a1: pad/weight + cuFFT R2C + x H + cuFFT C2R + crop/interleave */
+  PYHST_STAGE_REPACK = 1,      /* a2: [S][P][B] -> slice-interleaved layout (pyhst_backproject only) */
+  PYHST_STAGE_BACKPROJECT = 2, /* a2: the backprojection kernel                                  */
+  PYHST_STAGE_TRANSPOSE = 3,   /* a3: image transpose for the column walk                        */
+  PYHST_STAGE_FORWARD = 4,     /* a3: the forward-projection kernel                              */
+  PYHST_N_STAGES = 5
+};
+/* pyhst_profile_enable(1): from now on every stage is bracketed by a pair of CUDA events recorded
+ * on the stream the stage is launched on (no synchronisation is added).  Returns the previous
+ * setting.  pyhst_profile_read() synchronises the recorded events and returns, accumulated since
+ * the last reset, per stage: device milliseconds (ms, nullable), number of the library's own
+ * kernel launches (kernels, nullable; counted whether or not profiling is enabled) and number of
+ * cuFFT executions (fft_execs, nullable).  Arrays are HOST, [PYHST_N_STAGES]. */
+int pyhst_profile_enable(int enable);
+int pyhst_profile_read(double* ms, int64_t* kernels, int64_t* fft_execs, int32_t reset);
 
 const char* pyhst_last_error(void); /* thread-local, static storage; "" if none */
 void pyhst_release_cache(void);     /* frees cached plans / workspace (synchronises the device) */

@@ -23,7 +23,7 @@ _LIBNAME = "libpyhst_b200.so"
 
 # every symbol include/pyhst.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
-           "pyhst_fbp_host", "pyhst_halfacq_extent", "pyhst_set_backproject_variant",
+           "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant",
            "pyhst_last_error", "pyhst_release_cache")
 
 
@@ -60,8 +60,12 @@ def _load():
     lib.pyhst_forward_project.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_void_p]
     lib.pyhst_fbp.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_int, c_int, c_void_p]
     lib.pyhst_fbp_host.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_int, c_int, c_int32, c_void_p]
+    lib.pyhst_backproject_host.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_int32, c_void_p]
+    lib.pyhst_forward_project_host.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_int32, c_void_p]
     lib.pyhst_halfacq_extent.argtypes = [c_int32, c_double, POINTER(c_int32), POINTER(c_int32)]
     lib.pyhst_set_backproject_variant.argtypes = [c_int]
+    lib.pyhst_profile_enable.argtypes = [c_int]
+    lib.pyhst_profile_read.argtypes = [POINTER(c_double), POINTER(c_int64), POINTER(c_int64), c_int32]
     lib.pyhst_last_error.restype = c_char_p
     lib.pyhst_release_cache.restype = None
     _lib = lib
@@ -184,6 +188,34 @@ def fbp_host(h_sino_raw, angles, axis, nx, ny, pixel_size=1.0, filter=FILTER_RAM
     return out
 
 
+def backproject_host(h_sino, angles, axis, nx, ny, pixel_size=1.0, scale=1.0, out=None,
+                     max_slices_per_chunk=0, stream=None):
+    """pyhst_backproject_host: HOST float32 [S,P,B] -> HOST [S,ny,nx]."""
+    lib = _load()
+    s, p, b = h_sino.shape
+    if out is None:
+        out = np.empty((s, ny, nx), dtype=np.float32)
+    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size)
+    _check(lib.pyhst_backproject_host(_host_ptr(h_sino, "h_sino"), _host_ptr(out, "out"), ctypes.byref(g),
+                                      scale, max_slices_per_chunk, _stream(stream)), "pyhst_backproject_host")
+    return out
+
+
+def forward_project_host(h_img, angles, axis, n_bins, pixel_size=1.0, scale=1.0, out=None,
+                         max_slices_per_chunk=0, stream=None):
+    """pyhst_forward_project_host: HOST float32 [S,ny,nx] -> HOST [S,P,B]."""
+    lib = _load()
+    s, ny, nx = h_img.shape
+    p = len(angles)
+    if out is None:
+        out = np.empty((s, p, n_bins), dtype=np.float32)
+    g = _geom(s, p, n_bins, angles, axis, nx, ny, pixel_size)
+    _check(lib.pyhst_forward_project_host(_host_ptr(h_img, "h_img"), _host_ptr(out, "out"), ctypes.byref(g),
+                                          scale, max_slices_per_chunk, _stream(stream)),
+           "pyhst_forward_project_host")
+    return out
+
+
 def halfacq_extent(n_bins, cbar):
     ext, pad = c_int32(0), c_int32(0)
     _check(_load().pyhst_halfacq_extent(n_bins, float(cbar), ctypes.byref(ext), ctypes.byref(pad)),
@@ -193,6 +225,21 @@ def halfacq_extent(n_bins, cbar):
 
 def set_backproject_variant(variant: int) -> int:
     return int(_load().pyhst_set_backproject_variant(int(variant)))
+
+
+STAGES = ("ramp_filter", "repack", "backproject", "transpose", "forward_project")
+
+
+def profile_enable(enable: bool) -> bool:
+    return bool(_load().pyhst_profile_enable(1 if enable else 0))
+
+
+def profile_read(reset: bool = True):
+    """{stage: (device ms, own kernel launches, cuFFT executions)} accumulated since the last reset."""
+    n = len(STAGES)
+    ms, k, f = (c_double * n)(), (c_int64 * n)(), (c_int64 * n)()
+    _check(_load().pyhst_profile_read(ms, k, f, 1 if reset else 0), "pyhst_profile_read")
+    return {STAGES[i]: (float(ms[i]), int(k[i]), int(f[i])) for i in range(n)}
 
 
 def release_cache():

@@ -61,6 +61,51 @@ cudaStream_t g_streams[3] = {nullptr, nullptr, nullptr};
 cudaEvent_t g_events[8] = {nullptr};
 }  // namespace
 
+// ---- stage accounting --------------------------------------------------------------------
+namespace {
+struct StageEvents { Stage st; cudaEvent_t a, b; };
+std::mutex g_prof_mu;
+bool g_prof_on = false;
+std::vector<StageEvents> g_prof_pending;
+std::vector<cudaEvent_t> g_prof_pool;
+double g_prof_ms[ST_COUNT] = {0};
+int64_t g_prof_kernels[ST_COUNT] = {0}, g_prof_fft[ST_COUNT] = {0};
+
+cudaEvent_t prof_event() {
+  if (!g_prof_pool.empty()) {
+    cudaEvent_t e = g_prof_pool.back();
+    g_prof_pool.pop_back();
+    return e;
+  }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+}  // namespace
+
+StageScope::StageScope(Stage st_, cudaStream_t stream_) : st(st_), stream(stream_), slot(-1) {
+  std::lock_guard<std::mutex> lock(g_prof_mu);
+  if (!g_prof_on) return;
+  StageEvents ev{st, prof_event(), prof_event()};
+  if (!ev.a || !ev.b) return;
+  cudaEventRecord(ev.a, stream);
+  slot = (int)g_prof_pending.size();
+  g_prof_pending.push_back(ev);
+}
+StageScope::~StageScope() {
+  if (slot < 0) return;
+  std::lock_guard<std::mutex> lock(g_prof_mu);
+  if (slot < (int)g_prof_pending.size()) cudaEventRecord(g_prof_pending[slot].b, stream);
+}
+void StageScope::kernels(int n) {
+  std::lock_guard<std::mutex> lock(g_prof_mu);
+  g_prof_kernels[st] += n;
+}
+void StageScope::library(int n) {
+  std::lock_guard<std::mutex> lock(g_prof_mu);
+  g_prof_fft[st] += n;
+}
+
 int get_geom_plan(const pyhst_geom_t* g, double axis_shift, cudaStream_t stream,
                   const GeomPlan** out) {
   std::lock_guard<std::mutex> lock(g_mu);
@@ -182,6 +227,33 @@ extern "C" {
 
 const char* pyhst_last_error(void) { return last_error_buf(); }
 
+int pyhst_profile_enable(int enable) {
+  std::lock_guard<std::mutex> lock(g_prof_mu);
+  const int prev = g_prof_on ? 1 : 0;
+  g_prof_on = enable != 0;
+  return prev;
+}
+
+int pyhst_profile_read(double* ms, int64_t* kernels, int64_t* fft_execs, int32_t reset) {
+  std::lock_guard<std::mutex> lock(g_prof_mu);
+  for (auto& ev : g_prof_pending) {
+    PYHST_CUDA_TRY(cudaEventSynchronize(ev.b));
+    float t = 0.f;
+    PYHST_CUDA_TRY(cudaEventElapsedTime(&t, ev.a, ev.b));
+    g_prof_ms[ev.st] += (double)t;
+    g_prof_pool.push_back(ev.a);
+    g_prof_pool.push_back(ev.b);
+  }
+  g_prof_pending.clear();
+  for (int i = 0; i < ST_COUNT; ++i) {
+    if (ms) ms[i] = g_prof_ms[i];
+    if (kernels) kernels[i] = g_prof_kernels[i];
+    if (fft_execs) fft_execs[i] = g_prof_fft[i];
+    if (reset) { g_prof_ms[i] = 0; g_prof_kernels[i] = 0; g_prof_fft[i] = 0; }
+  }
+  return PYHST_OK;
+}
+
 int pyhst_set_backproject_variant(int variant) {
   const int prev = g_bp_variant;
   if (variant >= 0 && variant <= 2) g_bp_variant = variant;
@@ -222,6 +294,8 @@ int pyhst_halfacq_extent(int32_t n_bins, double cbar, int32_t* n_bins_ext, int32
 int pyhst_ramp_filter(const float* d_in, float* d_out, int64_t n_rows, int32_t n_bins_in,
                       int32_t n_bins_out, int32_t pad_left, int64_t out_pitch, pyhst_filter_t f,
                       const float* d_col_weights, void* stream) {
+  if (n_rows == 0 && n_bins_in > 0 && n_bins_out >= n_bins_in + pad_left && pad_left >= 0)
+    return PYHST_OK;  // empty stack: nothing to read or write (pointers may be NULL)
   PYHST_TRY(check_ptr(d_in, "d_in"));
   PYHST_TRY(check_ptr(d_out, "d_out"));
   if (d_col_weights) PYHST_TRY(check_ptr(d_col_weights, "d_col_weights"));
@@ -359,25 +433,23 @@ int pyhst_fbp(const float* d_sino_raw, float* d_img, const pyhst_geom_t* g, pyhs
   return fbp_device(d_sino_raw, pitch, d_img, g, g->n_slices, f, mode, static_cast<cudaStream_t>(stream));
 }
 
-int pyhst_fbp_host(const float* h_sino_raw, float* h_img, const pyhst_geom_t* g, pyhst_filter_t f,
-                   pyhst_scan_t mode, int32_t max_slices_per_chunk, void* stream_) {
-  cudaStream_t user = static_cast<cudaStream_t>(stream_);
-  int64_t pitch = 0;
-  PYHST_TRY(check_ptr(h_sino_raw, "h_sino_raw"));
-  PYHST_TRY(check_ptr(h_img, "h_img"));
-  PYHST_TRY(check_fbp(g, f, mode, &pitch));
-  // chunk = a multiple of 4 slices (one slice group of the interleaved layout)
-  int32_t chunk = max_slices_per_chunk > 0 ? max_slices_per_chunk : 8;
-  chunk = std::max(4, (chunk / 4) * 4);
-  chunk = std::min(chunk, ((g->n_slices + 3) / 4) * 4);
-  const int64_t P = g->n_angles;
-  const size_t in_bytes = (size_t)chunk * P * pitch * 4, out_bytes = (size_t)chunk * g->nx * g->ny * 4;
+}  // extern "C"
+
+// Host-buffer pipeline shared by the *_host entry points: the stack is cut into chunks of
+// `chunk` slices; H2D of chunk n+1 and D2H of chunk n-1 overlap the kernels of chunk n
+// (three internal streams ordered after `user`, double-buffered device blocks).
+template <class Body>
+static int host_pipeline(const float* h_in, size_t in_floats_per_slice, float* h_out,
+                         size_t out_floats_per_slice, int32_t n_slices, int32_t chunk,
+                         cudaStream_t user, Body body) {
+  const size_t in_bytes = (size_t)chunk * in_floats_per_slice * 4;
+  const size_t out_bytes = (size_t)chunk * out_floats_per_slice * 4;
   for (int i = 0; i < 3; ++i)
     if (!g_streams[i]) PYHST_CUDA_TRY(cudaStreamCreateWithFlags(&g_streams[i], cudaStreamNonBlocking));
   for (int i = 0; i < 8; ++i)
     if (!g_events[i]) PYHST_CUDA_TRY(cudaEventCreateWithFlags(&g_events[i], cudaEventDisableTiming));
   cudaStream_t s_in = g_streams[0], s_k = g_streams[1], s_out = g_streams[2];
-  void *d_in[2], *d_out[2];  // device double buffers
+  void *d_in[2], *d_out[2];
   void* blk = nullptr;
   PYHST_TRY(get_workspace(WS_CHUNKS, 2 * in_bytes + 2 * out_bytes, &blk));
   d_in[0] = blk;
@@ -390,28 +462,84 @@ int pyhst_fbp_host(const float* h_sino_raw, float* h_img, const pyhst_geom_t* g,
   PYHST_CUDA_TRY(cudaEventRecord(ev_start, user));
   for (int i = 0; i < 3; ++i) PYHST_CUDA_TRY(cudaStreamWaitEvent(g_streams[i], ev_start, 0));
   int n = 0;
-  for (int32_t s0 = 0; s0 < g->n_slices; s0 += chunk, ++n) {
-    const int32_t ns = std::min(chunk, g->n_slices - s0);
+  for (int32_t s0 = 0; s0 < n_slices; s0 += chunk, ++n) {
+    const int32_t ns = std::min(chunk, n_slices - s0);
     const int b = n & 1;
-    if (n >= 2) PYHST_CUDA_TRY(cudaStreamWaitEvent(s_in, ev_k[b], 0));    // kernels of chunk n-2 read d_in[b]
-    PYHST_CUDA_TRY(cudaMemcpyAsync(d_in[b], h_sino_raw + (int64_t)s0 * P * pitch, (size_t)ns * P * pitch * 4,
-                                   cudaMemcpyHostToDevice, s_in));
+    if (n >= 2) PYHST_CUDA_TRY(cudaStreamWaitEvent(s_in, ev_k[b], 0));   // kernels of chunk n-2 read d_in[b]
+    PYHST_CUDA_TRY(cudaMemcpyAsync(d_in[b], h_in + (size_t)s0 * in_floats_per_slice,
+                                   (size_t)ns * in_floats_per_slice * 4, cudaMemcpyHostToDevice, s_in));
     PYHST_CUDA_TRY(cudaEventRecord(ev_in[b], s_in));
     PYHST_CUDA_TRY(cudaStreamWaitEvent(s_k, ev_in[b], 0));
-    if (n >= 2) PYHST_CUDA_TRY(cudaStreamWaitEvent(s_k, ev_out[b], 0));   // D2H of chunk n-2 read d_out[b]
-    pyhst_geom_t gc = *g;
-    gc.n_slices = ns;
-    PYHST_TRY(fbp_device(static_cast<const float*>(d_in[b]), pitch, static_cast<float*>(d_out[b]), &gc,
-                         ns, f, mode, s_k));
+    if (n >= 2) PYHST_CUDA_TRY(cudaStreamWaitEvent(s_k, ev_out[b], 0));  // D2H of chunk n-2 reads d_out[b]
+    PYHST_TRY(body(static_cast<const float*>(d_in[b]), static_cast<float*>(d_out[b]), ns, s_k));
     PYHST_CUDA_TRY(cudaEventRecord(ev_k[b], s_k));
     PYHST_CUDA_TRY(cudaStreamWaitEvent(s_out, ev_k[b], 0));
-    PYHST_CUDA_TRY(cudaMemcpyAsync(h_img + (int64_t)s0 * g->nx * g->ny, d_out[b],
-                                   (size_t)ns * g->nx * g->ny * 4, cudaMemcpyDeviceToHost, s_out));
+    PYHST_CUDA_TRY(cudaMemcpyAsync(h_out + (size_t)s0 * out_floats_per_slice, d_out[b],
+                                   (size_t)ns * out_floats_per_slice * 4, cudaMemcpyDeviceToHost, s_out));
     PYHST_CUDA_TRY(cudaEventRecord(ev_out[b], s_out));
   }
   for (int i = 0; i < 3; ++i) PYHST_CUDA_TRY(cudaStreamSynchronize(g_streams[i]));
   PYHST_CUDA_TRY(cudaStreamSynchronize(user));
   return PYHST_OK;
+}
+
+// chunk = a multiple of 4 slices (one slice group of the interleaved layout)
+static int32_t host_chunk(int32_t requested, int32_t n_slices) {
+  int32_t chunk = requested > 0 ? requested : 8;
+  chunk = std::max(4, (chunk / 4) * 4);
+  return std::min(chunk, ((n_slices + 3) / 4) * 4);
+}
+
+extern "C" {
+
+int pyhst_fbp_host(const float* h_sino_raw, float* h_img, const pyhst_geom_t* g, pyhst_filter_t f,
+                   pyhst_scan_t mode, int32_t max_slices_per_chunk, void* stream_) {
+  int64_t pitch = 0;
+  PYHST_TRY(check_ptr(h_sino_raw, "h_sino_raw"));
+  PYHST_TRY(check_ptr(h_img, "h_img"));
+  PYHST_TRY(check_fbp(g, f, mode, &pitch));
+  return host_pipeline(
+      h_sino_raw, (size_t)g->n_angles * pitch, h_img, (size_t)g->nx * g->ny, g->n_slices,
+      host_chunk(max_slices_per_chunk, g->n_slices), static_cast<cudaStream_t>(stream_),
+      [&](const float* d_in, float* d_out, int32_t ns, cudaStream_t s) {
+        pyhst_geom_t gc = *g;
+        gc.n_slices = ns;
+        return fbp_device(d_in, pitch, d_out, &gc, ns, f, mode, s);
+      });
+}
+
+int pyhst_backproject_host(const float* h_sino, float* h_img, const pyhst_geom_t* g, float scale,
+                           int32_t max_slices_per_chunk, void* stream_) {
+  int64_t pitch = 0;
+  PYHST_TRY(check_ptr(h_sino, "h_sino"));
+  PYHST_TRY(check_ptr(h_img, "h_img"));
+  PYHST_TRY(check_geom(g, &pitch));
+  PYHST_TRY(require_sm100(nullptr));
+  return host_pipeline(
+      h_sino, (size_t)g->n_angles * pitch, h_img, (size_t)g->nx * g->ny, g->n_slices,
+      host_chunk(max_slices_per_chunk, g->n_slices), static_cast<cudaStream_t>(stream_),
+      [&](const float* d_in, float* d_out, int32_t ns, cudaStream_t s) {
+        pyhst_geom_t gc = *g;
+        gc.n_slices = ns;
+        return pyhst_backproject(d_in, d_out, &gc, scale, s);
+      });
+}
+
+int pyhst_forward_project_host(const float* h_img, float* h_sino, const pyhst_geom_t* g, float scale,
+                               int32_t max_slices_per_chunk, void* stream_) {
+  int64_t pitch = 0;
+  PYHST_TRY(check_ptr(h_img, "h_img"));
+  PYHST_TRY(check_ptr(h_sino, "h_sino"));
+  PYHST_TRY(check_geom(g, &pitch));
+  PYHST_TRY(require_sm100(nullptr));
+  return host_pipeline(
+      h_img, (size_t)g->nx * g->ny, h_sino, (size_t)g->n_angles * pitch, g->n_slices,
+      host_chunk(max_slices_per_chunk, g->n_slices), static_cast<cudaStream_t>(stream_),
+      [&](const float* d_in, float* d_out, int32_t ns, cudaStream_t s) {
+        pyhst_geom_t gc = *g;
+        gc.n_slices = ns;
+        return pyhst_forward_project(d_in, d_out, &gc, scale, s);
+      });
 }
 
 }  // extern "C"

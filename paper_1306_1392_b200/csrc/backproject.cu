@@ -50,6 +50,8 @@ int launch_backproject_reference(const float* d_sino, int64_t pitch, const BpArg
   dim3 grid((a.nx + 31) / 32, (a.ny + 7) / 8, a.n_slices);
   if (grid.y > 65535 || grid.z > 65535)
     return set_error(PYHST_ERR_UNSUPPORTED, "reference backprojector: grid too large");
+  StageScope scope(ST_BACKPROJECT, stream);
+  scope.kernels();
   bp_reference_kernel<<<grid, block, 0, stream>>>(d_sino, pitch, a.d_img, a.n_angles, a.n_bins,
                                                   a.nx, a.ny, a.scale, a.d_proj);
   PYHST_CUDA_TRY(cudaGetLastError());
@@ -83,6 +85,8 @@ int launch_repack_to_qi(const float* d_sino, int64_t pitch, int32_t n_slices, fl
   dim3 grid((unsigned)((L.row_f4() + 255) / 256), L.n_angles, L.n_groups);
   if (grid.y > 65535 || grid.z > 65535)
     return set_error(PYHST_ERR_UNSUPPORTED, "repack: more than 65535 projections or slice groups");
+  StageScope scope(ST_REPACK, stream);
+  scope.kernels();
   repack_to_qi_kernel<<<grid, block, 0, stream>>>(d_sino, pitch, n_slices, L.n_angles, L.n_bins,
                                                   L.zpad, d_qi);
   PYHST_CUDA_TRY(cudaGetLastError());
@@ -286,6 +290,8 @@ int launch_backproject_tiled(const float4* d_qi, const QiLayout& L, const BpArgs
   dim3 grid((a.nx + TX - 1) / TX, (a.ny + TY - 1) / TY, L.n_groups);
   if (grid.y > 65535 || grid.z > 65535)
     return set_error(PYHST_ERR_UNSUPPORTED, "tiled backprojector: grid too large");
+  StageScope scope(ST_BACKPROJECT, stream);
+  scope.kernels();
   bp_tiled_kernel<<<grid, NT, smem, stream>>>(d_qi, L.row_f4(), L.zpad, a.d_img, a.n_slices,
                                               a.n_angles, a.n_bins, a.nx, a.ny, a.scale, a.d_proj,
                                               W);

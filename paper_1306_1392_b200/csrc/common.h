@@ -32,6 +32,23 @@ int set_error(int status, const char* fmt, ...);
     if (_s != PYHST_OK) return _s; \
   } while (0)
 
+// ---- stage accounting (pyhst_profile_*, include/pyhst.h) ----------------------------------
+// Every launcher opens a StageScope: it always counts the library's own kernel launches and the
+// cuFFT executions of the stage, and -- only while profiling is enabled -- brackets the stage
+// with CUDA events on the launching stream.
+enum Stage { ST_FILTER = PYHST_STAGE_FILTER, ST_REPACK = PYHST_STAGE_REPACK,
+             ST_BACKPROJECT = PYHST_STAGE_BACKPROJECT, ST_TRANSPOSE = PYHST_STAGE_TRANSPOSE,
+             ST_FORWARD = PYHST_STAGE_FORWARD, ST_COUNT = PYHST_N_STAGES };
+struct StageScope {
+  StageScope(Stage st, cudaStream_t stream);
+  ~StageScope();
+  void kernels(int n = 1);   // own kernels launched
+  void library(int n = 1);   // cuFFT executions
+  Stage st;
+  cudaStream_t stream;
+  int slot;
+};
+
 // sm_100 device present and current?  (no CPU fallback: anything else is UNSUPPORTED)
 int require_sm100(int* n_sm);
 

@@ -205,6 +205,7 @@ int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int3
   void* ws = nullptr;
   PYHST_TRY(get_workspace(WS_FFT, (size_t)batch_rows * Mp * 4, &ws));
   float* buf = static_cast<float*>(ws);
+  StageScope scope(ST_FILTER, stream);
 
   for (int64_t r0 = 0; r0 < n_rows; r0 += batch_rows) {
     const int nb = (int)std::min<int64_t>(batch_rows, n_rows - r0);
@@ -215,24 +216,29 @@ int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int3
     // gridDim.y <= 65535: split the row range of the elementwise kernels
     for (int y0 = 0; y0 < nb; y0 += 65535) {
       const int ny = std::min(65535, nb - y0);
+      scope.kernels();
       pad_weight_kernel<<<dim3((Mp + 255) / 256, ny), 256, 0, stream>>>(
           d_in + (r0 + y0) * in_pitch, in_pitch, d_col_weights, buf + (int64_t)y0 * Mp, Mp,
           n_bins_in, pad_left);
     }
+    scope.library(2);
     PYHST_CUFFT_TRY(cufftExecR2C(pl.r2c, buf, reinterpret_cast<cufftComplex*>(buf)));
     for (int y0 = 0; y0 < nb; y0 += 65535) {
       const int ny = std::min(65535, nb - y0);
+      scope.kernels();
       multiply_spectrum_kernel<<<dim3((nk + 255) / 256, ny), 256, 0, stream>>>(
           reinterpret_cast<float2*>(buf) + (int64_t)y0 * nk, d_H, nk);
     }
     PYHST_CUFFT_TRY(cufftExecC2R(pl.c2r, reinterpret_cast<cufftComplex*>(buf), buf));
     if (d_qi) {
       const int64_t row_f4 = L->row_f4();
+      scope.kernels();
       crop_interleave_kernel<<<dim3((unsigned)((row_f4 + 255) / 256), L->n_angles), 256, 0, stream>>>(
           buf, Mp, d_qi, L->n_angles, n_bins_out, L->zpad, n_slices_in);
     } else {
       for (int y0 = 0; y0 < nb; y0 += 65535) {
         const int ny = std::min(65535, nb - y0);
+        scope.kernels();
         crop_rows_kernel<<<dim3((n_bins_out + 255) / 256, ny), 256, 0, stream>>>(
             buf + (int64_t)y0 * Mp, Mp, d_out + (r0 + y0) * out_pitch, out_pitch, n_bins_out);
       }

@@ -40,6 +40,8 @@ int launch_transpose_images(const float* d_img, float* d_img_t, int32_t n_slices
   dim3 grid((nx + 31) / 32, (ny + 31) / 32, n_slices);
   if (grid.y > 65535 || grid.z > 65535)
     return set_error(PYHST_ERR_UNSUPPORTED, "transpose: grid too large");
+  StageScope scope(ST_TRANSPOSE, stream);
+  scope.kernels();
   transpose_images_kernel<<<grid, block, 0, stream>>>(d_img, d_img_t, ny, nx);
   PYHST_CUDA_TRY(cudaGetLastError());
   return PYHST_OK;
@@ -97,6 +99,8 @@ int launch_forward_project(const FpArgs& a, cudaStream_t stream) {
   dim3 grid((a.n_bins + FP_NT - 1) / FP_NT, a.n_angles, a.n_slices);
   if (grid.y > 65535 || grid.z > 65535)
     return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: grid too large");
+  StageScope scope(ST_FORWARD, stream);
+  scope.kernels();
   fp_gather_kernel<<<grid, FP_NT, 0, stream>>>(a.d_img, a.d_img_t, a.d_sino, a.pitch, a.n_angles,
                                                a.n_bins, a.nx, a.ny, a.scale, a.d_proj);
   PYHST_CUDA_TRY(cudaGetLastError());

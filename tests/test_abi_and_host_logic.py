@@ -1,0 +1,168 @@
+"""CPU-side checks (-m "not gpu"): the C-ABI library loads and exports every symbol that
+include/pyhst.h declares, errors that are detectable without a device are reported, and the
+multi-GPU plumbing (slice sharding, max-over-ranks, gather) works under gloo with world_size 2.
+No compute call is made without a GPU.
+"""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def cuda_lib():
+    from paper_1306_1392_b200 import build
+    return ctypes.CDLL(build.build())
+
+
+def _declared_symbols():
+    src = open(os.path.join(ROOT, "include", "pyhst.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(pyhst_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_symbols_are_exported(cuda_lib):
+    names = _declared_symbols()
+    assert {"pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp"} <= set(names)
+    for n in names:
+        assert hasattr(cuda_lib, n), "libpyhst_b200.so does not export %s" % n
+
+
+def test_binding_lists_every_header_symbol():
+    from paper_1306_1392_b200 import binding
+    assert sorted(binding.EXPORTS) == _declared_symbols()
+
+
+def test_library_has_sm100a_code_and_tma():
+    """The shipped library carries sm_100a SASS with the TMA bulk copy (UBLKCP) in the projectors."""
+    from paper_1306_1392_b200 import build
+    lib = build.build()
+    out = subprocess.run(["cuobjdump", "-lelf", lib], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+    sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True).stdout
+    assert "UBLKCP" in sass
+
+
+def test_halfacq_extent_host_logic(cuda_lib, oracle):
+    """Pure host function: no device needed; must agree with the oracle's reading R10."""
+    cuda_lib.pyhst_halfacq_extent.argtypes = [ctypes.c_int32, ctypes.c_double,
+                                              ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32)]
+    for n_bins, cbar in [(2048, 1900.0), (2048, 147.0), (128, 118.0), (128, 63.5), (367, 10.25), (64, 60.0)]:
+        ext, pad = ctypes.c_int32(), ctypes.c_int32()
+        assert cuda_lib.pyhst_halfacq_extent(n_bins, cbar, ctypes.byref(ext), ctypes.byref(pad)) == 0
+        assert (ext.value, pad.value) == oracle.halfacq_extent(n_bins, cbar)
+        assert ext.value % 64 == 0 and ext.value >= 2 * max(cbar, n_bins - 1 - cbar) + 1
+    assert cuda_lib.pyhst_halfacq_extent(0, 1.0, None, None) != 0
+
+
+def test_argument_errors_without_device(cuda_lib):
+    """Validation happens before any CUDA call: NULL pointers / bad sizes -> INVALID_ARG + message."""
+    cuda_lib.pyhst_last_error.restype = ctypes.c_char_p
+    cuda_lib.pyhst_ramp_filter.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32,
+                                           ctypes.c_int32, ctypes.c_int32, ctypes.c_int64, ctypes.c_int,
+                                           ctypes.c_void_p, ctypes.c_void_p]
+    assert cuda_lib.pyhst_ramp_filter(None, None, 4, 64, 64, 0, 0, 0, None, None) == 1
+    assert b"NULL" in cuda_lib.pyhst_last_error()
+    assert cuda_lib.pyhst_ramp_filter(None, None, 0, 64, 64, 0, 0, 0, None, None) == 0      # empty stack: no-op
+    assert cuda_lib.pyhst_ramp_filter(None, None, 0, 64, 32, 0, 0, 0, None, None) == 1      # still validated
+    cuda_lib.pyhst_backproject.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_float,
+                                           ctypes.c_void_p]
+    assert cuda_lib.pyhst_backproject(None, None, None, 1.0, None) == 1
+
+
+def test_no_cpu_fallback_without_device():
+    """On a box without a GPU the product path must fail loudly, not route through the oracle."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    import paper_1306_1392_b200 as P
+    x = torch.zeros((1, 8, 32), dtype=torch.float32)
+    with pytest.raises(P.PyhstError):
+        P.backproject(x, np.zeros(8), np.full(8, 15.5), 16, 16)
+    # a raw call with fake non-NULL pointers still stops at the device check (UNSUPPORTED = 2)
+    lib = P.binding._load()
+    ang = (ctypes.c_double * 8)(*([0.0] * 8))
+    g = P.binding.Geom(1, 8, 32, 0, ang, ang, 16, 16, 1.0)
+    assert lib.pyhst_backproject(ctypes.c_void_p(4096), ctypes.c_void_p(8192), ctypes.byref(g), 1.0, None) == 2
+    assert "no CPU fallback" in P.last_error()
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_1306_1392_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cuh", ".cpp")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
+                assert "pyhst_oracle" not in text, f
+    text = (open(os.path.join(ROOT, "oracle", "pyhst_oracle.c")).read()
+            + open(os.path.join(ROOT, "oracle", "__init__.py")).read())
+    assert not re.search(r"^\s*(import|from)\s+paper_1306_1392_b200\b", text, flags=re.M)
+    assert "#include \"../paper" not in text and "pyhst.h" not in text
+
+
+# ------------------------------------------------------------------ sharding (single process)
+def test_slice_range_partitions_exactly():
+    from paper_1306_1392_b200.sharding import slice_range
+    for n in [0, 1, 5, 16, 64, 67]:
+        for world in [1, 2, 3, 8]:
+            spans = [slice_range(n, world, r) for r in range(world)]
+            assert spans[0][0] == 0 and spans[-1][1] == n
+            assert all(a[1] == b[0] for a, b in zip(spans, spans[1:]))
+            sizes = [b - a for a, b in spans]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        slice_range(4, 2, 2)
+
+
+# ------------------------------------------------------------------ sharding under gloo, world_size 2
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, %(root)r)
+import numpy as np, torch, torch.distributed as dist
+from paper_1306_1392_b200 import sharding, workloads
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+S = 5
+a, b = sharding.slice_range(S, world, rank)
+w = workloads.config(1, shrink=8, n_slices=S)
+local = torch.from_numpy(w.sinogram(range(a, b)))           # each rank synthesises only its slices
+full = sharding.gather_slices(local, S, dist)
+t = sharding.max_over_ranks(10.0 + rank, dist)
+assert t == 10.0 + world - 1, t
+if rank == 0:
+    want = torch.from_numpy(w.sinogram())
+    assert full.shape == want.shape and torch.equal(full, want)
+    print("OK", flush=True)
+dist.destroy_process_group()
+"""
+
+
+def test_gloo_world2_sharding(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER % {"root": ROOT})
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", OMP_NUM_THREADS="1")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+                        "--master-addr", "127.0.0.1", "--master-port", "29613", str(script)],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "OK" in r.stdout
+
+
+def test_bench_reference_arm_runs_on_cpu():
+    """bench.py --impl reference prints one JSON line with the contract's keys (tiny config 1)."""
+    import json
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1",
+                        "--steps", "1"], capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    for k in ("impl", "metric", "value", "unit", "n_gpus", "steps", "ms_per_step", "higher_is_better",
+              "cpu_baseline", "e2e", "config"):
+        assert k in line
+    assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
