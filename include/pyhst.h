@@ -138,6 +138,11 @@ int pyhst_halfacq_extent(int32_t n_bins, double cbar, int32_t* n_bins_ext, int32
  * Returns the previous value.  Test/bench hook; results agree within FP32 rounding. */
 int pyhst_set_backproject_variant(int variant);
 
+/* Selects the forward-projection kernel: 0 = automatic (default), 1 = generic gather kernel (one
+ * thread per bin and slice, global loads; kept for cross-checks and for pixel sizes the banded
+ * kernel does not cover), 2 = banded shared-memory kernel.  Returns the previous value. */
+int pyhst_set_forward_project_variant(int variant);
+
 /* Stage accounting for bench.py / tests.  Stages of the hot path, in call order: */
 enum {
   PYHST_STAGE_FILTER = 0,      /* a1: pad/weight + cuFFT R2C + x H + cuFFT C2R + crop/interleave */

@@ -23,7 +23,7 @@ _LIBNAME = "libpyhst_b200.so"
 
 # every symbol include/pyhst.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
-           "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant",
+           "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant",
            "pyhst_last_error", "pyhst_release_cache")
 
 
@@ -64,6 +64,7 @@ def _load():
     lib.pyhst_forward_project_host.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_int32, c_void_p]
     lib.pyhst_halfacq_extent.argtypes = [c_int32, c_double, POINTER(c_int32), POINTER(c_int32)]
     lib.pyhst_set_backproject_variant.argtypes = [c_int]
+    lib.pyhst_set_forward_project_variant.argtypes = [c_int]
     lib.pyhst_profile_enable.argtypes = [c_int]
     lib.pyhst_profile_read.argtypes = [POINTER(c_double), POINTER(c_int64), POINTER(c_int64), c_int32]
     lib.pyhst_last_error.restype = c_char_p
@@ -225,6 +226,10 @@ def halfacq_extent(n_bins, cbar):
 
 def set_backproject_variant(variant: int) -> int:
     return int(_load().pyhst_set_backproject_variant(int(variant)))
+
+
+def set_forward_project_variant(variant: int) -> int:
+    return int(_load().pyhst_set_forward_project_variant(int(variant)))
 
 
 STAGES = ("ramp_filter", "repack", "backproject", "transpose", "forward_project")

@@ -2,6 +2,7 @@
 // sequencing of the kernels.  Every step of the hot path runs on the device; there is no CPU
 // fallback (a missing or non-sm_100 device yields PYHST_ERR_UNSUPPORTED).
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <list>
 #include <mutex>
@@ -57,6 +58,8 @@ uint64_t g_tick = 0;
 struct Ws { void* p = nullptr; size_t bytes = 0; };
 Ws g_ws[WS_COUNT];
 int g_bp_variant = 0;
+int g_fp_variant = 0;
+std::list<FpPlan> g_fp_plans;
 cudaStream_t g_streams[3] = {nullptr, nullptr, nullptr};
 cudaEvent_t g_events[8] = {nullptr};
 }  // namespace
@@ -151,6 +154,66 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, cudaStream_t stream,
   g_geom.push_back(std::move(pl));
   *out = &g_geom.back();
   return PYHST_OK;
+}
+
+int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out) {
+  std::lock_guard<std::mutex> lock(g_mu);
+  const size_t n = (size_t)g->n_angles;
+  for (auto& pl : g_fp_plans) {
+    if (pl.n_angles == g->n_angles && pl.n_bins == g->n_bins && pl.nx == g->nx && pl.ny == g->ny &&
+        pl.pixel_size == g->pixel_size &&
+        std::memcmp(pl.angles.data(), g->angles_rad, n * sizeof(double)) == 0 &&
+        std::memcmp(pl.axis.data(), g->axis_pos, n * sizeof(double)) == 0) {
+      pl.last_use = ++g_tick;
+      *out = &pl;
+      return PYHST_OK;
+    }
+  }
+  if (g_fp_plans.size() >= 8) {
+    auto lru = g_fp_plans.begin();
+    for (auto it = g_fp_plans.begin(); it != g_fp_plans.end(); ++it)
+      if (it->last_use < lru->last_use) lru = it;
+    cudaFree(lru->d_projs);  // synchronises: no kernel can still be reading them
+    cudaFree(lru->d_chunks);
+    g_fp_plans.erase(lru);
+  }
+  FpPlan pl;
+  pl.n_angles = g->n_angles;
+  pl.n_bins = g->n_bins;
+  pl.nx = g->nx;
+  pl.ny = g->ny;
+  pl.pixel_size = g->pixel_size;
+  pl.angles.assign(g->angles_rad, g->angles_rad + n);
+  pl.axis.assign(g->axis_pos, g->axis_pos + n);
+  std::vector<FpProjD> projs;
+  std::vector<FpChunk> chunks;
+  if (build_fp_tables(g, &pl, &projs, &chunks)) {
+    PYHST_CUDA_TRY(cudaMalloc(&pl.d_projs, projs.size() * sizeof(FpProjD)));
+    PYHST_CUDA_TRY(cudaMalloc(&pl.d_chunks, chunks.size() * sizeof(FpChunk)));
+    // pageable sources: the copies are complete (staged) when the calls return
+    PYHST_CUDA_TRY(cudaMemcpyAsync(pl.d_projs, projs.data(), projs.size() * sizeof(FpProjD),
+                                   cudaMemcpyHostToDevice, stream));
+    PYHST_CUDA_TRY(cudaMemcpyAsync(pl.d_chunks, chunks.data(), chunks.size() * sizeof(FpChunk),
+                                   cudaMemcpyHostToDevice, stream));
+    if (std::getenv("PYHST_DEBUG"))
+      fprintf(stderr, "[pyhst] fp plan: P=%d B=%d %dx%d h=%g -> W=%d nc=%d chunks=%d (rows %d cols %d)\n",
+              g->n_angles, g->n_bins, g->nx, g->ny, g->pixel_size, pl.W, pl.nc, pl.n_chunks,
+              (int)pl.any_rows, (int)pl.any_cols);
+  } else {
+    pl.n_chunks = 0;  // geometry not covered by the banded kernel: the generic gather kernel runs
+  }
+  pl.last_use = ++g_tick;
+  g_fp_plans.push_back(std::move(pl));
+  *out = &g_fp_plans.back();
+  return PYHST_OK;
+}
+
+void release_fp_plans() {
+  for (auto& pl : g_fp_plans) {
+    cudaFree(pl.d_projs);
+    cudaFree(pl.d_chunks);
+  }
+  g_fp_plans.clear();
 }
 
 int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr) {
@@ -260,10 +323,17 @@ int pyhst_set_backproject_variant(int variant) {
   return prev;
 }
 
+int pyhst_set_forward_project_variant(int variant) {
+  const int prev = g_fp_variant;
+  if (variant >= 0 && variant <= 2) g_fp_variant = variant;
+  return prev;
+}
+
 void pyhst_release_cache(void) {
   cudaDeviceSynchronize();
   release_filter_plans();
   std::lock_guard<std::mutex> lock(g_mu);
+  release_fp_plans();
   for (auto& pl : g_geom) {
     cudaFree(pl.d_proj);
     cudaFreeHost(pl.h_pinned);
@@ -353,6 +423,15 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
   PYHST_TRY(require_sm100(nullptr));
   const GeomPlan* plan = nullptr;
   PYHST_TRY(get_geom_plan(g, 0.0, stream, &plan));
+  if (g_fp_variant != 1) {
+    const FpPlan* fplan = nullptr;
+    PYHST_TRY(get_fp_plan(g, stream, &fplan));
+    if (fplan->n_chunks > 0)
+      return launch_forward_project_banded(d_img, d_sino, pitch, g, scale, *fplan, stream);
+    if (g_fp_variant == 2)
+      return set_error(PYHST_ERR_UNSUPPORTED, "banded forward projector does not cover pixel_size %g",
+                       g->pixel_size);
+  }
   void* img_t = nullptr;
   PYHST_TRY(get_workspace(WS_IMG_T, (size_t)g->n_slices * g->nx * g->ny * 4, &img_t));
   PYHST_TRY(launch_transpose_images(d_img, static_cast<float*>(img_t), g->n_slices, g->ny, g->nx,

@@ -75,7 +75,7 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, cudaStream_t stream,
 
 // Grow-only device workspace slots owned by the library (freed by pyhst_release_cache).
 enum WorkspaceSlot { WS_QI = 0, WS_FFT = 1, WS_WEIGHTS = 2, WS_IMG_T = 3, WS_ROWS = 4,
-                     WS_CHUNKS = 5, WS_COUNT = 6 };
+                     WS_CHUNKS = 5, WS_XI = 6, WS_COUNT = 7 };
 int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr);
 
 // ---- interleaved sinogram layout consumed by the tiled backprojector ---------------------
@@ -107,6 +107,50 @@ int launch_backproject_tiled(const float4* d_qi, const QiLayout& L, const BpArgs
 int launch_repack_to_qi(const float* d_sino, int64_t pitch, int32_t n_slices, float4* d_qi,
                         const QiLayout& L, cudaStream_t stream);
 
+// ---- interleaved, zero-padded image layout consumed by the banded forward projector -------
+// XI[g][v][zpad + u][sl]: slice group g = s / 4, one float4 per (g, line v, position u); every
+// line carries `zpad` zero float4 on both sides.  Two copies: lines = image rows (u = j, v = i)
+// for projections walked along rows, lines = image columns (u = i, v = j) for the others.
+struct XiLayout {
+  int32_t n_groups, nv, nu, zpad;
+  int64_t line_f4() const { return (int64_t)nu + 2 * (int64_t)zpad; }
+  int64_t group_f4() const { return line_f4() * nv; }
+  size_t bytes() const { return (size_t)group_f4() * (size_t)n_groups * 16; }
+};
+
+// Per-projection constants of the banded forward projector (line walk, |cu| >= |cv|):
+//   strip centre on line v for bin b:  u*(b, v) = b inv_cu + k0 + sD v   (double, R11)
+struct FpProjD {
+  double inv_cu, k0, sD;
+  float s, hw, cuabs;  // (float)sD, |1/cu| = half-width of the strip in pixels, |cu|
+  int32_t p;           // projection index in the caller's order
+};
+struct FpChunk {
+  int32_t first, count;  // range in the permuted FpProjD table
+  int32_t cls;           // 0: lines are image rows, 1: lines are image columns
+  int32_t pad_;
+};
+struct FpPlan {
+  // key
+  int32_t n_angles = 0, n_bins = 0, nx = 0, ny = 0;
+  double pixel_size = 0;
+  std::vector<double> angles, axis;
+  // product
+  int32_t npj = 0, W = 0, nc = 0, n_chunks = 0;
+  bool any_rows = false, any_cols = false;
+  FpProjD* d_projs = nullptr;
+  FpChunk* d_chunks = nullptr;
+  uint64_t last_use = 0;
+};
+int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out);  // api.cu
+// fills the host tables of a plan; returns false if the banded kernel cannot cover the geometry
+bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* projs,
+                     std::vector<FpChunk>* chunks);  // forward_project.cu
+void release_fp_plans();
+int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pitch,
+                                  const pyhst_geom_t* g, float scale, const FpPlan& plan,
+                                  cudaStream_t stream);
+
 struct FpArgs {
   const float* d_img;    // [S][ny][nx]
   const float* d_img_t;  // [S][nx][ny] (transposed copy, made by launch_transpose_images)
@@ -131,5 +175,43 @@ int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int3
                        cudaStream_t stream);
 int launch_halfacq_weights(float* d_w, int32_t n_bins, double cbar, cudaStream_t stream);
 void release_filter_plans();
+
+// ---- device helpers: mbarrier + TMA bulk copy (inline PTX) -----------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+               "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+// TMA bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+
+#endif  // __CUDACC__
 
 }  // namespace pyhst

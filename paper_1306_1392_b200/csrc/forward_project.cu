@@ -11,6 +11,10 @@
 // The position of the strip centre on each line is evaluated in double and only the small
 // offset (pixel - centre) is carried in FP32 (R11), so the weights are the same function of
 // (pixel, bin) as the backprojector's.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
 #include "common.h"
 
 namespace pyhst {
@@ -103,6 +107,372 @@ int launch_forward_project(const FpArgs& a, cudaStream_t stream) {
   scope.kernels();
   fp_gather_kernel<<<grid, FP_NT, 0, stream>>>(a.d_img, a.d_img_t, a.d_sino, a.pitch, a.n_angles,
                                                a.n_bins, a.nx, a.ny, a.scale, a.d_proj);
+  PYHST_CUDA_TRY(cudaGetLastError());
+  return PYHST_OK;
+}
+
+
+// ==========================================================================================
+// Banded forward projector (the product path).
+//
+// A block owns NB consecutive detector bins of up to NPJ projections of one walk class and one
+// slice group (4 slices interleaved as float4).  It walks the image lines in bands of RB lines:
+// per band the window of the interleaved image that the block's strips cross is staged into
+// shared memory with one TMA bulk copy per line (mbarrier-signalled, double-buffered); every
+// thread then gathers, for each of its (bin, projection) pairs and each line of the band, the NC
+// pixels that can lie inside the strip |t - b| < 1, with weights 1 - |cu| |u - u*| (FP32 FMA),
+// and accumulates 4 slices in registers.  No atomics: each output is written once.
+// The strip centre u* is evaluated in double once per (pair, band) relative to the window and
+// split into an integer and a fraction in [-1/2, 1/2]; only the fraction is carried in FP32 (R11).
+// ==========================================================================================
+namespace {
+
+constexpr int FB_NB = 128;    // bins per block
+constexpr int FB_NPJ = 16;    // projections per block (at most)
+constexpr int FB_RB = 8;      // lines per band
+constexpr int FB_NT = 256;    // threads: 128 bin lanes x 2 projection parities, 8 pairs per thread
+constexpr int FB_PAIRS = FB_NB * FB_NPJ / FB_NT;
+constexpr int FB_HDR = 1024;  // 2 mbarriers, 2 origins, NPJ x FpProjD
+constexpr int FB_WMAX = 416;  // window capacity (float4 per line): 2 x 8 x 416 x 16 B = 104 KB
+
+struct XiDims { int32_t nv, nu, zpad; };
+
+template <int NC>
+__global__ void __launch_bounds__(FB_NT, 2)
+fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_cols, XiDims dr,
+               XiDims dc, float* __restrict__ sino, int64_t pitch, int S, int P, int B, float scale,
+               const FpProjD* __restrict__ projs, const FpChunk* __restrict__ chunks, int W) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);        // [2]
+  int* sorigin = reinterpret_cast<int*>(smem + 16);          // [2]
+  FpProjD* sproj = reinterpret_cast<FpProjD*>(smem + 64);    // [FB_NPJ]
+  float4* buf = reinterpret_cast<float4*>(smem + FB_HDR);    // [2][FB_RB][W]
+
+  const int tid = threadIdx.x, lane = tid & 31;
+  const FpChunk ck = chunks[blockIdx.y];
+  const int g = blockIdx.z;
+  const int b0 = blockIdx.x * FB_NB;
+  const XiDims d = ck.cls ? dc : dr;
+  const int64_t line_f4 = (int64_t)d.nu + 2 * d.zpad;
+  const float4* xi = (ck.cls ? xi_cols : xi_rows) + (int64_t)g * d.nv * line_f4;
+  const int n_bands = (d.nv + FB_RB - 1) / FB_RB;
+  const uint32_t row_bytes = (uint32_t)W * 16u;
+
+  if (tid < ck.count) sproj[tid] = projs[ck.first + tid];
+  if (tid == 0) {
+    mbar_init(&full[0], FB_RB);
+    mbar_init(&full[1], FB_RB);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  // warp 0: window origin of band k (min over the chunk's strips at the band's four corners, in
+  // double), then one bulk copy per line of the band
+  auto produce = [&](int k) {
+    const int vb = k * FB_RB;
+    const int rows = min(FB_RB, d.nv - vb);
+    double lo = 1e300;
+    if (lane < ck.count) {
+      const FpProjD pj = sproj[lane];
+      const double ua = fma((double)b0, pj.inv_cu, pj.k0);
+      const double ub = fma((double)(b0 + FB_NB - 1), pj.inv_cu, pj.k0);
+      const double va = pj.sD * (double)vb, vz = pj.sD * (double)(vb + rows - 1);
+      lo = fmin(fmin(ua, ub) + fmin(va, vz), lo) - (double)pj.hw;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    double of = floor(lo) - 1.0;
+    of = fmax(of, -(double)d.zpad);
+    of = fmin(of, (double)(d.nu + d.zpad - W));
+    const int origin = (int)of;
+    uint64_t* bar = &full[k & 1];
+    if (lane == 0) sorigin[k & 1] = origin;
+    if (lane < FB_RB) {
+      if (lane < rows) {
+        mbar_arrive_expect_tx(bar, row_bytes);
+        bulk_g2s(buf + ((k & 1) * FB_RB + lane) * W,
+                 xi + (int64_t)(vb + lane) * line_f4 + (origin + d.zpad), row_bytes, bar);
+      } else {
+        mbar_arrive(bar);
+      }
+    }
+  };
+
+  if (tid < 32) produce(0);
+
+  float acc[FB_PAIRS][4];
+#pragma unroll
+  for (int m = 0; m < FB_PAIRS; ++m)
+#pragma unroll
+    for (int sl = 0; sl < 4; ++sl) acc[m][sl] = 0.f;
+
+  const int bl = tid & (FB_NB - 1);
+  const int par = tid >> 7;
+  const double bd = (double)(b0 + bl);
+  const int idx_hi = W - NC;
+
+  for (int k = 0; k < n_bands; ++k) {
+    __syncthreads();  // everyone is done with band k-1: its stage may be overwritten
+    if (k + 1 < n_bands && tid < 32) produce(k + 1);
+    mbar_wait(&full[k & 1], (uint32_t)((k >> 1) & 1));
+    const int origin = sorigin[k & 1];
+    const int vb = k * FB_RB;
+    const int rows = min(FB_RB, d.nv - vb);
+    const float4* stage = buf + (k & 1) * FB_RB * W;
+#pragma unroll
+    for (int m = 0; m < FB_PAIRS; ++m) {
+      const int pj = par + 2 * m;
+      if (pj >= ck.count) break;
+      const FpProjD* sp = &sproj[pj];
+      // strip centre on the band's first line, relative to the window (double), split (R11)
+      const double A = fma(sp->sD, (double)vb, fma(bd, sp->inv_cu, sp->k0)) - (double)origin;
+      const int ai = __double2int_rn(A);
+      const float afr = (float)(A - (double)ai);
+      const float s = sp->s, hw = sp->hw, cuabs = sp->cuabs;
+#pragma unroll 2
+      for (int r = 0; r < rows; ++r) {
+        const float dfr = fmaf(s, (float)r, afr);
+        const float jf = ceilf(dfr - hw);        // first pixel that can lie inside the strip
+        const float d0 = jf - dfr;               // in [-hw, -hw + 1)
+        int idx = ai + (int)jf;
+        idx = min(max(idx, 0), idx_hi);          // only acts where the strip is off the image
+        const float4* wp = stage + r * W + idx;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+          const float w = fmaxf(0.f, fmaf(-cuabs, fabsf(d0 + (float)c), 1.f));
+          const float4 v = wp[c];
+          acc[m][0] = fmaf(w, v.x, acc[m][0]);
+          acc[m][1] = fmaf(w, v.y, acc[m][1]);
+          acc[m][2] = fmaf(w, v.z, acc[m][2]);
+          acc[m][3] = fmaf(w, v.w, acc[m][3]);
+        }
+      }
+    }
+  }
+
+  const int b = b0 + bl;
+  if (b < B) {
+#pragma unroll
+    for (int m = 0; m < FB_PAIRS; ++m) {
+      const int pj = par + 2 * m;
+      if (pj >= ck.count) break;
+      const int p = sproj[pj].p;
+#pragma unroll
+      for (int sl = 0; sl < 4; ++sl) {
+        const int s = g * 4 + sl;
+        if (s < S) sino[((int64_t)s * P + p) * pitch + b] = scale * acc[m][sl];
+      }
+    }
+  }
+}
+
+// [S][ny][nx] -> XI rows copy [g][ny][zr + nx + zr] and XI columns copy [g][nx][zc + ny + zc]
+__global__ void repack_image_kernel(const float* __restrict__ img, int S, int ny, int nx,
+                                    float4* __restrict__ xi_rows, int zr, float4* __restrict__ xi_cols,
+                                    int zc) {
+  __shared__ float tile[4][32][33];
+  const int g = blockIdx.z;
+  const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+#pragma unroll
+  for (int sl = 0; sl < 4; ++sl) {
+    const int s = g * 4 + sl;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+      const int y = by + r, x = bx + threadIdx.x;
+      tile[sl][r][threadIdx.x] = (s < S && y < ny && x < nx) ? img[((int64_t)s * ny + y) * nx + x] : 0.f;
+    }
+  }
+  __syncthreads();
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    if (xi_rows) {
+      const int y = by + r, x = bx + threadIdx.x;
+      if (y < ny && x < nx)
+        xi_rows[((int64_t)g * ny + y) * (nx + 2 * zr) + zr + x] =
+            make_float4(tile[0][r][threadIdx.x], tile[1][r][threadIdx.x], tile[2][r][threadIdx.x],
+                        tile[3][r][threadIdx.x]);
+    }
+    if (xi_cols) {
+      const int x = bx + r, y = by + threadIdx.x;
+      if (y < ny && x < nx)
+        xi_cols[((int64_t)g * nx + x) * (ny + 2 * zc) + zc + y] =
+            make_float4(tile[0][threadIdx.x][r], tile[1][threadIdx.x][r], tile[2][threadIdx.x][r],
+                        tile[3][threadIdx.x][r]);
+    }
+  }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// host: walk classes, chunks of projections and the window width (all in double)
+// ------------------------------------------------------------------------------------------
+namespace {
+
+struct Extent { double lo[4], hi[4]; };  // of u* - hw over a block's corners, at the 4 extreme (segment, band) places
+
+// u*(b, v) - hw is affine in (b, v): over a block (NB bins x RB lines) its extremes sit at the
+// block's corners; the window width max - min is convex in the block position, so its maximum
+// over all blocks is attained at the four extreme (segment, band) positions.
+Extent proj_extent(const FpProjD& pj, int n_bins, int nv) {
+  Extent e;
+  const int seg_last = ((n_bins + FB_NB - 1) / FB_NB - 1) * FB_NB;
+  const int band_last = ((nv + FB_RB - 1) / FB_RB - 1) * FB_RB;
+  int q = 0;
+  for (int b0 : {0, seg_last})
+    for (int vb : {0, band_last}) {
+      const int rows = std::min(FB_RB, nv - vb);
+      double lo = 1e300, hi = -1e300;
+      for (int b : {b0, b0 + FB_NB - 1})
+        for (int v : {vb, vb + rows - 1}) {
+          const double u = (double)b * pj.inv_cu + pj.k0 + pj.sD * (double)v - (double)pj.hw;
+          lo = std::min(lo, u);
+          hi = std::max(hi, u);
+        }
+      e.lo[q] = lo;
+      e.hi[q] = hi;
+      ++q;
+    }
+  return e;
+}
+
+int width_of(const Extent& e, int nc) {
+  int w = 0;
+  for (int q = 0; q < 4; ++q) {
+    const double origin = std::floor(e.lo[q]) - 1.0;
+    w = std::max(w, (int)(std::ceil(e.hi[q]) - origin) + nc + 2);  // + 2: slack for the convexity bound
+  }
+  return w;
+}
+
+Extent merge(const Extent& a, const Extent& b) {
+  Extent e;
+  for (int q = 0; q < 4; ++q) {
+    e.lo[q] = std::min(a.lo[q], b.lo[q]);
+    e.hi[q] = std::max(a.hi[q], b.hi[q]);
+  }
+  return e;
+}
+
+}  // namespace
+
+bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* projs,
+                     std::vector<FpChunk>* chunks) {
+  const int P = g->n_angles;
+  const double h = g->pixel_size;
+  // candidates per line: the open strip of width 2 / |cu| <= 2 sqrt(2) / h holds at most nc pixels
+  const int nc = (int)std::ceil(2.0 * std::sqrt(2.0) / h - 1e-9);
+  if (nc > 6) return false;
+  plan->nc = nc <= 3 ? 3 : (nc <= 4 ? 4 : 6);
+  std::vector<int> order[2];
+  std::vector<FpProjD> all(P);
+  for (int p = 0; p < P; ++p) {
+    const double ch = h * std::cos(g->angles_rad[p]), sh = h * std::sin(g->angles_rad[p]);
+    const int cls = std::fabs(ch) >= std::fabs(sh) ? 0 : 1;
+    const double cu = cls ? sh : ch, cv = cls ? ch : sh;
+    const int nu = cls ? g->ny : g->nx, nv = cls ? g->nx : g->ny;
+    const double u0 = 0.5 * (double)(nu - 1), v0 = 0.5 * (double)(nv - 1);
+    FpProjD& d = all[p];
+    d.inv_cu = 1.0 / cu;
+    d.k0 = u0 + (cv * v0 - g->axis_pos[p]) * d.inv_cu;
+    d.sD = -cv * d.inv_cu;
+    d.s = (float)d.sD;
+    d.hw = (float)std::fabs(d.inv_cu);
+    d.cuabs = (float)std::fabs(cu);
+    d.p = p;
+    order[cls].push_back(p);
+  }
+  projs->clear();
+  chunks->clear();
+  plan->any_rows = !order[0].empty();
+  plan->any_cols = !order[1].empty();
+  // neighbours in angle have neighbouring strips: sort each class by angle (stable: the caller's
+  // order is kept for the usual monotone lists)
+  for (int cls = 0; cls < 2; ++cls)
+    std::stable_sort(order[cls].begin(), order[cls].end(),
+                     [&](int a, int b) { return g->angles_rad[a] < g->angles_rad[b]; });
+  // window width: that of full chunks of FB_NPJ neighbours if it fits, else the capacity
+  int w_full = 0;
+  std::vector<Extent> ext(P);
+  for (int cls = 0; cls < 2; ++cls) {
+    const int nv = cls ? g->nx : g->ny;
+    for (int p : order[cls]) ext[p] = proj_extent(all[p], g->n_bins, nv);
+    for (size_t i = 0; i < order[cls].size(); i += FB_NPJ) {
+      Extent e = ext[order[cls][i]];
+      for (size_t j = i + 1; j < std::min(order[cls].size(), i + FB_NPJ); ++j) e = merge(e, ext[order[cls][j]]);
+      w_full = std::max(w_full, width_of(e, plan->nc));
+    }
+  }
+  const int W = std::min(std::max(w_full, plan->nc + 4), FB_WMAX);
+  plan->W = W;
+  plan->npj = FB_NPJ;
+  // greedy chunks: add neighbours while the window still fits
+  for (int cls = 0; cls < 2; ++cls) {
+    size_t i = 0;
+    while (i < order[cls].size()) {
+      Extent e = ext[order[cls][i]];
+      if (width_of(e, plan->nc) > W) return false;  // one projection alone does not fit
+      FpChunk ck{(int32_t)projs->size(), 1, cls, 0};
+      projs->push_back(all[order[cls][i]]);
+      size_t j = i + 1;
+      for (; j < order[cls].size() && ck.count < FB_NPJ; ++j) {
+        const Extent m = merge(e, ext[order[cls][j]]);
+        if (width_of(m, plan->nc) > W) break;
+        e = m;
+        projs->push_back(all[order[cls][j]]);
+        ++ck.count;
+      }
+      chunks->push_back(ck);
+      i = j;
+    }
+  }
+  plan->n_chunks = (int32_t)chunks->size();
+  return plan->n_chunks <= 65535;
+}
+
+int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pitch,
+                                  const pyhst_geom_t* g, float scale, const FpPlan& plan,
+                                  cudaStream_t stream) {
+  const int n_groups = (g->n_slices + 3) / 4;
+  const int W = plan.W;
+  XiLayout Lr{n_groups, g->ny, g->nx, W}, Lc{n_groups, g->nx, g->ny, W};
+  const size_t bytes_r = plan.any_rows ? Lr.bytes() : 0, bytes_c = plan.any_cols ? Lc.bytes() : 0;
+  void* ws = nullptr;
+  PYHST_TRY(get_workspace(WS_XI, bytes_r + bytes_c, &ws));
+  float4* xi_r = plan.any_rows ? static_cast<float4*>(ws) : nullptr;
+  float4* xi_c = plan.any_cols ? reinterpret_cast<float4*>(static_cast<char*>(ws) + bytes_r) : nullptr;
+  // the zero pads are written once per (block, layout); the repack only touches the interior
+  static const void* pads_ptr = nullptr;
+  static size_t pads_key[6] = {0};
+  const size_t key[6] = {bytes_r, bytes_c, (size_t)g->nx, (size_t)g->ny, (size_t)W, (size_t)n_groups};
+  {
+    StageScope scope(ST_TRANSPOSE, stream);
+    if (pads_ptr != ws || std::memcmp(pads_key, key, sizeof(key)) != 0) {
+      PYHST_CUDA_TRY(cudaMemsetAsync(ws, 0, bytes_r + bytes_c, stream));
+      pads_ptr = ws;
+      std::memcpy(pads_key, key, sizeof(key));
+    }
+    dim3 block(32, 8, 1);
+    dim3 grid((g->nx + 31) / 32, (g->ny + 31) / 32, n_groups);
+    if (grid.y > 65535 || grid.z > 65535)
+      return set_error(PYHST_ERR_UNSUPPORTED, "image repack: grid too large");
+    scope.kernels();
+    repack_image_kernel<<<grid, block, 0, stream>>>(d_img, g->n_slices, g->ny, g->nx, xi_r, W, xi_c, W);
+    PYHST_CUDA_TRY(cudaGetLastError());
+  }
+  const size_t smem = FB_HDR + (size_t)2 * FB_RB * W * 16;
+  static size_t configured[3] = {0, 0, 0};
+  const int vi = plan.nc == 3 ? 0 : (plan.nc == 4 ? 1 : 2);
+  auto kern = plan.nc == 3 ? fp_band_kernel<3> : (plan.nc == 4 ? fp_band_kernel<4> : fp_band_kernel<6>);
+  if (smem > configured[vi]) {
+    PYHST_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured[vi] = smem;
+  }
+  dim3 grid((g->n_bins + FB_NB - 1) / FB_NB, plan.n_chunks, n_groups);
+  if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
+  StageScope scope(ST_FORWARD, stream);
+  scope.kernels();
+  const XiDims dr{g->ny, g->nx, W}, dc{g->nx, g->ny, W};
+  kern<<<grid, FB_NT, smem, stream>>>(xi_r, xi_c, dr, dc, d_sino, pitch, g->n_slices, g->n_angles,
+                                      g->n_bins, scale, plan.d_projs, plan.d_chunks, W);
   PYHST_CUDA_TRY(cudaGetLastError());
   return PYHST_OK;
 }

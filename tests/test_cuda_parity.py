@@ -114,6 +114,9 @@ def test_backproject_affine_rows(lib):
 # ------------------------------------------------------------------------------ forward projection
 FP_CASES = [
     (1, 1, 40, 33, 21, 1.0, None, 0.0),
+    (5, 45, 300, 260, 270, 1.0, None, 1.0),     # several bin segments, bands and chunks, ragged slice group
+    (2, 21, 150, 100, 90, 0.72, None, 0.5),     # 4 candidate pixels per line
+    (1, 9, 400, 80, 60, 2.5, None, 0.0),        # detector much longer than the image: strips off the image
     (3, 37, 211, 150, 70, 1.0, None, 1.5),
     (2, 50, 97, 130, 131, 0.8, 30.2, 0.7),
     (2, 19, 64, 200, 90, 1.3, None, 0.0),
@@ -121,16 +124,21 @@ FP_CASES = [
 ]
 
 
+@pytest.mark.parametrize("variant", [1, 2])
 @pytest.mark.parametrize("case", FP_CASES)
-def test_forward_project_matches_oracle(lib, oracle, case):
+def test_forward_project_matches_oracle(lib, oracle, case, variant):
     S, P, B, nx, ny, h, axis, drift = case
     wl = lib.workloads
     w = wl.custom(S, P, B, nx, ny, pixel_size=h, axis=axis, drift=drift, jitter_angles=0.01, seed=P,
                   span=2 * math.pi)
     x = wl.random_image(S, ny, nx, seed=nx)
     want = oracle.forward_project(x, w.angles, w.axis, B, pixel_size=h, scale=1.7)
-    got = lib.forward_project(_dev(x), w.angles, w.axis, B, pixel_size=h, scale=1.7).cpu().numpy()
-    assert_parity(got, want, "forward_project %r" % (case,))
+    prev = lib.set_forward_project_variant(variant)
+    try:
+        got = lib.forward_project(_dev(x), w.angles, w.axis, B, pixel_size=h, scale=1.7).cpu().numpy()
+    finally:
+        lib.set_forward_project_variant(prev)
+    assert_parity(got, want, "forward_project variant %d %r" % (variant, case))
 
 
 def test_forward_project_axis_aligned_angles(lib, oracle):
