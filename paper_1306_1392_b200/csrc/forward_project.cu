@@ -130,7 +130,7 @@ namespace {
 constexpr int FB_NB = 128;    // bins per block
 constexpr int FB_NPJ = 16;    // projections per block (at most)
 constexpr int FB_RB = 8;      // lines per band
-constexpr int FB_NT = 256;    // threads: 128 bin lanes x 2 projection parities, 8 pairs per thread
+constexpr int FB_NT = 256;    // threads: 8 warps x (16 bins x 2 projection parities), 8 pairs per thread
 constexpr int FB_PAIRS = FB_NB * FB_NPJ / FB_NT;
 constexpr int FB_HDR = 1024;  // 2 mbarriers, 2 origins, NPJ x FpProjD
 constexpr int FB_WMAX = 416;  // window capacity (float4 per line): 2 x 8 x 416 x 16 B = 104 KB
@@ -206,8 +206,11 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
 #pragma unroll
     for (int sl = 0; sl < 4; ++sl) acc[m][sl] = 0.f;
 
-  const int bl = tid & (FB_NB - 1);
-  const int par = tid >> 7;
+  // lane pairs hold the same bin of two neighbouring projections: a quarter-warp (the unit of a
+  // 128-bit shared load) then spans 4 bins x 2 projections, i.e. < 8 consecutive float4 -> no
+  // bank conflict, where 8 consecutive bins at 45 degrees would span 10
+  const int bl = (tid >> 5) * 16 + (lane >> 1);
+  const int par = lane & 1;
   const double bd = (double)(b0 + bl);
   const int idx_hi = W - NC;
 
