@@ -109,12 +109,13 @@ void StageScope::library(int n) {
   g_prof_fft[st] += n;
 }
 
-int get_geom_plan(const pyhst_geom_t* g, double axis_shift, cudaStream_t stream,
+int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cudaStream_t stream,
                   const GeomPlan** out) {
   std::lock_guard<std::mutex> lock(g_mu);
   const size_t n = (size_t)g->n_angles;
   for (auto& pl : g_geom) {
-    if (pl.n_angles == g->n_angles && pl.pixel_size == g->pixel_size && pl.axis_shift == axis_shift &&
+    if (pl.n_angles == g->n_angles && pl.n_bins == n_bins && pl.pixel_size == g->pixel_size &&
+        pl.axis_shift == axis_shift &&
         std::memcmp(pl.angles.data(), g->angles_rad, n * sizeof(double)) == 0 &&
         std::memcmp(pl.axis.data(), g->axis_pos, n * sizeof(double)) == 0) {
       pl.last_use = ++g_tick;
@@ -127,11 +128,14 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, cudaStream_t stream,
     for (auto it = g_geom.begin(); it != g_geom.end(); ++it)
       if (it->last_use < lru->last_use) lru = it;
     cudaFree(lru->d_proj);  // synchronises: no kernel can still be reading it
+    cudaFree(lru->d_run);
+    cudaFree(lru->d_flip);
     cudaFreeHost(lru->h_pinned);
     g_geom.erase(lru);
   }
   GeomPlan pl;
   pl.n_angles = g->n_angles;
+  pl.n_bins = n_bins;
   pl.pixel_size = g->pixel_size;
   pl.axis_shift = axis_shift;
   pl.angles.assign(g->angles_rad, g->angles_rad + n);
@@ -150,6 +154,34 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, cudaStream_t stream,
   }
   PYHST_CUDA_TRY(cudaMemcpyAsync(pl.d_proj, pl.h_pinned, n * sizeof(ProjGeom), cudaMemcpyHostToDevice,
                                  stream));
+  // run backprojector: class A (|sh| <= |ch|, runs along y) first, then class B (runs along x);
+  // a row is stored reversed (t -> n_bins-1-t: ch, sh change sign) when its run step is negative
+  {
+    std::vector<RunProj> run;
+    std::vector<uint8_t> flip(n, 0);
+    run.reserve(n);
+    for (int cls = 0; cls < 2; ++cls)
+      for (size_t p = 0; p < n; ++p) {
+        const ProjGeom& pg = pl.h_pinned[p];
+        const int c = std::fabs(pg.sh) <= std::fabs(pg.ch) ? 0 : 1;
+        if (c != cls) continue;
+        const double step = cls ? pg.ch : pg.sh;
+        RunProj r{pg.ch, pg.sh, pg.c, (int32_t)p, cls};
+        if (step < 0.0) {
+          r.ch = -pg.ch;
+          r.sh = -pg.sh;
+          r.c = (double)(n_bins - 1) - pg.c;
+          flip[p] = 1;
+        }
+        run.push_back(r);
+        (cls ? pl.n_b : pl.n_a)++;
+      }
+    PYHST_CUDA_TRY(cudaMalloc(&pl.d_run, n * sizeof(RunProj)));
+    PYHST_CUDA_TRY(cudaMalloc(&pl.d_flip, n));
+    // pageable sources: staged before the calls return
+    PYHST_CUDA_TRY(cudaMemcpyAsync(pl.d_run, run.data(), n * sizeof(RunProj), cudaMemcpyHostToDevice, stream));
+    PYHST_CUDA_TRY(cudaMemcpyAsync(pl.d_flip, flip.data(), n, cudaMemcpyHostToDevice, stream));
+  }
   pl.last_use = ++g_tick;
   g_geom.push_back(std::move(pl));
   *out = &g_geom.back();
@@ -273,13 +305,20 @@ static QiLayout qi_layout(int32_t n_slices, int32_t n_angles, int32_t n_bins, do
   L.n_angles = n_angles;
   L.n_bins = n_bins;
   const int W = backproject_tiled_window(pixel_size);
-  L.zpad = W > 0 ? W : 16;
+  L.zpad = W > 0 ? W + 4 : 16;
   return L;
 }
 
-static bool use_tiled(double pixel_size) {
-  if (g_bp_variant == 1) return false;
-  return backproject_tiled_window(pixel_size) > 0;
+// 1 = reference, 2 = tiled, 3 = run; -1 = the requested variant does not cover the geometry
+static int pick_bp_kernel(double pixel_size) {
+  const bool tiled_ok = backproject_tiled_window(pixel_size) > 0;
+  const bool run_ok = backproject_run_window(pixel_size) > 0;
+  switch (g_bp_variant) {
+    case 1: return 1;
+    case 2: return tiled_ok ? 2 : -1;
+    case 3: return run_ok ? 3 : -1;
+    default: return run_ok ? 3 : (tiled_ok ? 2 : 1);
+  }
 }
 
 }  // namespace pyhst
@@ -319,7 +358,7 @@ int pyhst_profile_read(double* ms, int64_t* kernels, int64_t* fft_execs, int32_t
 
 int pyhst_set_backproject_variant(int variant) {
   const int prev = g_bp_variant;
-  if (variant >= 0 && variant <= 2) g_bp_variant = variant;
+  if (variant >= 0 && variant <= 3) g_bp_variant = variant;
   return prev;
 }
 
@@ -336,6 +375,8 @@ void pyhst_release_cache(void) {
   release_fp_plans();
   for (auto& pl : g_geom) {
     cudaFree(pl.d_proj);
+    cudaFree(pl.d_run);
+    cudaFree(pl.d_flip);
     cudaFreeHost(pl.h_pinned);
   }
   g_geom.clear();
@@ -384,7 +425,7 @@ int pyhst_ramp_filter(const float* d_in, float* d_out, int64_t n_rows, int32_t n
     return set_error(PYHST_ERR_UNSUPPORTED, "n_bins_in + n_bins_out > 16384");
   PYHST_TRY(require_sm100(nullptr));
   return launch_ramp_filter(d_in, n_bins_in, n_rows, n_bins_in, n_bins_out, pad_left, (int)f,
-                            d_col_weights, d_out, out_pitch, nullptr, nullptr, 0,
+                            d_col_weights, d_out, out_pitch, nullptr, nullptr, 0, nullptr,
                             static_cast<cudaStream_t>(stream));
 }
 
@@ -397,19 +438,22 @@ int pyhst_backproject(const float* d_sino, float* d_img, const pyhst_geom_t* g, 
   PYHST_TRY(check_geom(g, &pitch));
   PYHST_TRY(require_sm100(nullptr));
   const GeomPlan* plan = nullptr;
-  PYHST_TRY(get_geom_plan(g, 0.0, stream, &plan));
+  PYHST_TRY(get_geom_plan(g, 0.0, g->n_bins, stream, &plan));
   BpArgs a{d_img, g->n_slices, g->n_angles, g->n_bins, g->nx, g->ny, scale, plan->d_proj,
            g->pixel_size};
-  if (!use_tiled(g->pixel_size)) {
-    if (g_bp_variant == 2)
-      return set_error(PYHST_ERR_UNSUPPORTED, "tiled backprojector does not cover pixel_size %g",
-                       g->pixel_size);
-    return launch_backproject_reference(d_sino, pitch, a, stream);
-  }
+  const int kern = pick_bp_kernel(g->pixel_size);
+  if (kern < 0)
+    return set_error(PYHST_ERR_UNSUPPORTED, "backprojector variant %d does not cover pixel_size %g",
+                     g_bp_variant, g->pixel_size);
+  if (kern == 1) return launch_backproject_reference(d_sino, pitch, a, stream);
   const QiLayout L = qi_layout(g->n_slices, g->n_angles, g->n_bins, g->pixel_size);
   void* qi = nullptr;
   PYHST_TRY(get_workspace(WS_QI, L.bytes(), &qi));
-  PYHST_TRY(launch_repack_to_qi(d_sino, pitch, g->n_slices, static_cast<float4*>(qi), L, stream));
+  PYHST_TRY(launch_repack_to_qi(d_sino, pitch, g->n_slices, static_cast<float4*>(qi), L,
+                                kern == 3 ? plan->d_flip : nullptr, stream));
+  if (kern == 3)
+    return launch_backproject_run(static_cast<const float4*>(qi), L, a, plan->d_run, plan->n_a, plan->n_b,
+                                  stream);
   return launch_backproject_tiled(static_cast<const float4*>(qi), L, a, stream);
 }
 
@@ -422,7 +466,7 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
   PYHST_TRY(check_geom(g, &pitch));
   PYHST_TRY(require_sm100(nullptr));
   const GeomPlan* plan = nullptr;
-  PYHST_TRY(get_geom_plan(g, 0.0, stream, &plan));
+  PYHST_TRY(get_geom_plan(g, 0.0, g->n_bins, stream, &plan));
   if (g_fp_variant != 1) {
     const FpPlan* fplan = nullptr;
     PYHST_TRY(get_fp_plan(g, stream, &fplan));
@@ -466,19 +510,20 @@ static int fbp_device(const float* d_sino_raw, int64_t pitch, float* d_img, cons
   if ((int64_t)g->n_bins + b_out > 16384)
     return set_error(PYHST_ERR_UNSUPPORTED, "n_bins + filtered row length > 16384");
   const GeomPlan* plan = nullptr;
-  PYHST_TRY(get_geom_plan(g, (double)pad_left, stream, &plan));
+  PYHST_TRY(get_geom_plan(g, (double)pad_left, b_out, stream, &plan));
   BpArgs a{d_img, ns, g->n_angles, b_out, g->nx, g->ny, (float)scale, plan->d_proj, g->pixel_size};
   const int64_t P = g->n_angles;
-  if (!use_tiled(g->pixel_size)) {
-    if (g_bp_variant == 2)
-      return set_error(PYHST_ERR_UNSUPPORTED, "tiled backprojector does not cover pixel_size %g",
-                       g->pixel_size);
+  const int kern = pick_bp_kernel(g->pixel_size);
+  if (kern < 0)
+    return set_error(PYHST_ERR_UNSUPPORTED, "backprojector variant %d does not cover pixel_size %g",
+                     g_bp_variant, g->pixel_size);
+  if (kern == 1) {
     void* rows = nullptr;
     PYHST_TRY(get_workspace(WS_ROWS, (size_t)ns * P * b_out * 4, &rows));
     for (int32_t s = 0; s < ns; ++s)
       PYHST_TRY(launch_ramp_filter(d_sino_raw + (int64_t)s * P * pitch, pitch, P, g->n_bins, b_out,
                                    pad_left, (int)f, d_w, static_cast<float*>(rows) + (int64_t)s * P * b_out,
-                                   b_out, nullptr, nullptr, 0, stream));
+                                   b_out, nullptr, nullptr, 0, nullptr, stream));
     return launch_backproject_reference(static_cast<const float*>(rows), b_out, a, stream);
   }
   const QiLayout L = qi_layout(ns, g->n_angles, b_out, g->pixel_size);
@@ -489,8 +534,11 @@ static int fbp_device(const float* d_sino_raw, int64_t pitch, float* d_img, cons
     PYHST_TRY(launch_ramp_filter(d_sino_raw + (int64_t)grp * 4 * P * pitch, pitch, (int64_t)n_in * P,
                                  g->n_bins, b_out, pad_left, (int)f, d_w, nullptr, 0,
                                  static_cast<float4*>(qi) + (int64_t)grp * L.group_f4(), &L, n_in,
-                                 stream));
+                                 kern == 3 ? plan->d_flip : nullptr, stream));
   }
+  if (kern == 3)
+    return launch_backproject_run(static_cast<const float4*>(qi), L, a, plan->d_run, plan->n_a, plan->n_b,
+                                  stream);
   return launch_backproject_tiled(static_cast<const float4*>(qi), L, a, stream);
 }
 

@@ -58,19 +58,33 @@ struct ProjGeom {
   double ch, sh, c;
 };
 
+// Per-projection entry of the run backprojector, in processing order (class A first):
+//   class A: |sh| <= |ch|, runs along y;  class B: |ch| < |sh|, runs along x.
+// ch/sh/c are those of the (possibly reversed) stored row, so that the run step is >= 0.
+struct RunProj {
+  double ch, sh, c;
+  int32_t p;     // row of the interleaved sinogram
+  int32_t cls;   // 0 = A, 1 = B
+};
+
 struct GeomPlan {
   // key
-  int32_t n_angles = 0;
+  int32_t n_angles = 0, n_bins = 0;
   double pixel_size = 0, axis_shift = 0;
   std::vector<double> angles, axis;
   // device table [n_angles]
   ProjGeom* d_proj = nullptr;
   ProjGeom* h_pinned = nullptr;
+  // run backprojector: permuted / sign-normalised table and the per-row reversal flags
+  RunProj* d_run = nullptr;
+  uint8_t* d_flip = nullptr;
+  int32_t n_a = 0, n_b = 0;
   uint64_t last_use = 0;
 };
 
 // Returns a cached (or new) device geometry table for g (axis shifted by axis_shift bins).
-int get_geom_plan(const pyhst_geom_t* g, double axis_shift, cudaStream_t stream,
+// n_bins = length of the rows the backprojector reads (the filtered length inside pyhst_fbp)
+int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cudaStream_t stream,
                   const GeomPlan** out);
 
 // Grow-only device workspace slots owned by the library (freed by pyhst_release_cache).
@@ -105,7 +119,12 @@ int launch_backproject_tiled(const float4* d_qi, const QiLayout& L, const BpArgs
                              cudaStream_t stream);
 // [S][P][pitch] -> QI (zero pads and missing slices written as zeros)
 int launch_repack_to_qi(const float* d_sino, int64_t pitch, int32_t n_slices, float4* d_qi,
-                        const QiLayout& L, cudaStream_t stream);
+                        const QiLayout& L, const uint8_t* d_flip, cudaStream_t stream);
+// run kernel (product path): window width it needs, 0 if the geometry is not covered
+int backproject_run_window(double pixel_size);
+struct RunProj;
+int launch_backproject_run(const float4* d_qi, const QiLayout& L, const BpArgs& a,
+                           const RunProj* d_run, int32_t n_a, int32_t n_b, cudaStream_t stream);
 
 // ---- interleaved, zero-padded image layout consumed by the banded forward projector -------
 // XI[g][v][zpad + u][sl]: slice group g = s / 4, one float4 per (g, line v, position u); every
@@ -171,7 +190,7 @@ int launch_forward_project(const FpArgs& a, cudaStream_t stream);
 int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int32_t n_bins_in,
                        int32_t n_bins_out, int32_t pad_left, int filter,
                        const float* d_col_weights, float* d_out, int64_t out_pitch,
-                       float4* d_qi, const QiLayout* L, int32_t n_slices_in,
+                       float4* d_qi, const QiLayout* L, int32_t n_slices_in, const uint8_t* d_flip,
                        cudaStream_t stream);
 int launch_halfacq_weights(float* d_w, int32_t n_bins, double cbar, cudaStream_t stream);
 void release_filter_plans();

@@ -142,14 +142,16 @@ __global__ void crop_rows_kernel(const float* __restrict__ buf, int Mp, float* _
 
 // rows r = sl * P + p of one slice group -> QI[p][zpad + b][sl], pads and missing slices zero
 __global__ void crop_interleave_kernel(const float* __restrict__ buf, int Mp, float4* __restrict__ qi,
-                                       int P, int n_bins_out, int zpad, int n_slices_in) {
+                                       int P, int n_bins_out, int zpad, int n_slices_in,
+                                       const uint8_t* __restrict__ flip) {
   const int64_t row_f4 = (int64_t)n_bins_out + 2 * zpad;
   const int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int p = blockIdx.y;
   if (x >= row_f4) return;
-  const int64_t b = x - zpad;
+  int64_t b = x - zpad;
   float v[4] = {0.f, 0.f, 0.f, 0.f};
   if (b >= 0 && b < n_bins_out) {
+    if (flip && flip[p]) b = n_bins_out - 1 - b;  // reversed row, see bp_run_kernel
 #pragma unroll
     for (int sl = 0; sl < 4; ++sl)
       if (sl < n_slices_in) v[sl] = buf[((int64_t)sl * P + p) * Mp + b];
@@ -185,7 +187,7 @@ int launch_halfacq_weights(float* d_w, int32_t n_bins, double cbar, cudaStream_t
 int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int32_t n_bins_in,
                        int32_t n_bins_out, int32_t pad_left, int filter,
                        const float* d_col_weights, float* d_out, int64_t out_pitch,
-                       float4* d_qi, const QiLayout* L, int32_t n_slices_in,
+                       float4* d_qi, const QiLayout* L, int32_t n_slices_in, const uint8_t* d_flip,
                        cudaStream_t stream) {
   if (n_rows == 0) return PYHST_OK;
   std::lock_guard<std::mutex> lock(g_mu);
@@ -234,7 +236,7 @@ int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int3
       const int64_t row_f4 = L->row_f4();
       scope.kernels();
       crop_interleave_kernel<<<dim3((unsigned)((row_f4 + 255) / 256), L->n_angles), 256, 0, stream>>>(
-          buf, Mp, d_qi, L->n_angles, n_bins_out, L->zpad, n_slices_in);
+          buf, Mp, d_qi, L->n_angles, n_bins_out, L->zpad, n_slices_in, d_flip);
     } else {
       for (int y0 = 0; y0 < nb; y0 += 65535) {
         const int ny = std::min(65535, nb - y0);

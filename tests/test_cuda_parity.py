@@ -55,15 +55,18 @@ BP_CASES = [
     (2, 19, 64, 200, 90, 1.3, None, 0.0),       # pixel larger than a bin: image wider than detector
     (4, 16, 300, 64, 64, 0.5, None, 2.0),       # exactly one tile and one chunk
     (9, 33, 180, 70, 129, 1.0, 179.0, 0.0),     # axis at the detector border
+    (6, 70, 260, 200, 190, 1.0, None, 1.0),     # 360-degree angles: every class / row-reversal combination
+    (2, 40, 64, 300, 40, 1.2, None, 0.0),       # image far wider than the detector: windows clamped on the pads
 ]
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 @pytest.mark.parametrize("case", BP_CASES)
 def test_backproject_matches_oracle(lib, oracle, case, variant):
     S, P, B, nx, ny, h, axis, drift = case
     wl = lib.workloads
-    w = wl.custom(S, P, B, nx, ny, pixel_size=h, axis=axis, drift=drift, jitter_angles=0.01, seed=P)
+    w = wl.custom(S, P, B, nx, ny, pixel_size=h, axis=axis, drift=drift, jitter_angles=0.01, seed=P,
+                  span=2 * math.pi if P == 70 else math.pi)
     sino = wl.random_sinogram(S, P, B, seed=B)
     want = oracle.backproject(sino, w.angles, w.axis, nx, ny, pixel_size=h, scale=0.37)
     prev = lib.set_backproject_variant(variant)
