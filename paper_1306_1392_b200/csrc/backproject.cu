@@ -297,7 +297,6 @@ __device__ __forceinline__ void bp_run_pass(const float4* __restrict__ qg, int64
   const uint32_t win_bytes = (uint32_t)W * 16u;
   const double dx0 = (double)x0 - 0.5 * (double)(nx - 1);
   const double dy0 = (double)y0 - 0.5 * (double)(ny - 1);
-  const unsigned long long one2 = pack2(1.f, 1.f), mone2 = pack2(-1.f, -1.f);
   const int n_chunks = (ne + NA - 1) / NA;
 
   // thread a < NA owns entry c*NA + a of chunk c: window origin and local base in double (R11)
@@ -354,41 +353,42 @@ __device__ __forceinline__ void bp_run_pass(const float4* __restrict__ qg, int64
       const int k = __float_as_int(tm) - RMAGIC_I;
       const float f0 = t - (tm - 8388608.f);
       uint32_t addr = wb + (uint32_t)(a * W + k) * 16u;
-      float4 qa, qb;
+      float4 qa, qb;  // lower / upper tap of 4 slices
       asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
                    : "=f"(qa.x), "=f"(qa.y), "=f"(qa.z), "=f"(qa.w) : "r"(addr));
       asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+16];"
                    : "=f"(qb.x), "=f"(qb.y), "=f"(qb.z), "=f"(qb.w) : "r"(addr));
-      unsigned long long f2 = pack2(f0, f0);
-      const unsigned long long dl2 = pack2(gg.y, gg.y);
+      float f = f0;
+      const float dl = gg.y;
 #pragma unroll
       for (int n = 0; n < RN; ++n) {
-        const unsigned long long w2 = fma2(f2, mone2, one2);  // 1 - f
+        const float w = 1.f - f;
+        const unsigned long long w2 = pack2(w, w), f2 = pack2(f, f);  // scalar-broadcast operands
         ffma2(acc[n][0], pack2(qa.x, qa.y), w2);
         ffma2(acc[n][1], pack2(qa.z, qa.w), w2);
         ffma2(acc[n][0], pack2(qb.x, qb.y), f2);
         ffma2(acc[n][1], pack2(qb.z, qb.w), f2);
         if (n + 1 < RN) {
           // f += dl; if f >= 1 the run moved on by one bin: f -= 1, the upper tap becomes the
-          // lower one and one new float4 is loaded -- all predicated, registers updated in place
+          // lower one and one new float4 is loaded -- all predicated, registers updated in place.
+          // Two of the four register moves are written as x + (-0) so that they issue on the FMA
+          // pipe instead of the half-rate ALU pipe that FSEL/MOV use.
           asm volatile(
               "{\n\t"
               ".reg .pred p;\n\t"
-              ".reg .f32 lo, hi;\n\t"
-              "add.rn.f32x2 %9, %9, %10;\n\t"
-              "mov.b64 {lo, hi}, %9;\n\t"
-              "setp.ge.f32 p, lo, 0f3F800000;\n\t"
-              "@p add.rn.f32x2 %9, %9, %11;\n\t"
+              "add.rn.f32 %9, %9, %10;\n\t"
+              "setp.ge.f32 p, %9, 0f3F800000;\n\t"
+              "@p add.rn.f32 %9, %9, 0fBF800000;\n\t"
               "@p mov.f32 %0, %4;\n\t"
-              "@p mov.f32 %1, %5;\n\t"
+              "@p add.rn.f32 %1, %5, 0f80000000;\n\t"
               "@p mov.f32 %2, %6;\n\t"
-              "@p mov.f32 %3, %7;\n\t"
+              "@p add.rn.f32 %3, %7, 0f80000000;\n\t"
               "@p add.u32 %8, %8, 16;\n\t"
               "@p ld.shared.v4.f32 {%4, %5, %6, %7}, [%8+16];\n\t"
               "}"
               : "+f"(qa.x), "+f"(qa.y), "+f"(qa.z), "+f"(qa.w), "+f"(qb.x), "+f"(qb.y), "+f"(qb.z),
-                "+f"(qb.w), "+r"(addr), "+l"(f2)
-              : "l"(dl2), "l"(mone2));
+                "+f"(qb.w), "+r"(addr), "+f"(f)
+              : "f"(dl));
         }
       }
     }
