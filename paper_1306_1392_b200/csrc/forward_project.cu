@@ -138,7 +138,7 @@ constexpr int FB_WMAX = 416;  // window capacity (float4 per line): 2 x 8 x 416 
 struct XiDims { int32_t nv, nu, zpad; };
 
 template <int NC>
-__global__ void __launch_bounds__(FB_NT, 2)
+__global__ void __launch_bounds__(FB_NT, 3)
 fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_cols, XiDims dr,
                XiDims dc, float* __restrict__ sino, int64_t pitch, int S, int P, int B, float scale,
                const FpProjD* __restrict__ projs, const FpChunk* __restrict__ chunks, int W) {
@@ -235,9 +235,12 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
 #pragma unroll 2
       for (int r = 0; r < rows; ++r) {
         const float dfr = fmaf(s, (float)r, afr);
-        const float jf = ceilf(dfr - hw);        // first pixel that can lie inside the strip
+        // first pixel that can lie inside the strip: ceil(dfr - hw) by a round-up add of
+        // 1.5 * 2^23 (|dfr - hw| < 2^22), integer part read from the mantissa -- no XU-pipe F2I
+        const float jm = __fadd_ru(dfr - hw, 12582912.f);
+        const float jf = jm - 12582912.f;
         const float d0 = jf - dfr;               // in [-hw, -hw + 1)
-        int idx = ai + (int)jf;
+        int idx = ai + (__float_as_int(jm) - 0x4b400000);
         idx = min(max(idx, 0), idx_hi);          // only acts where the strip is off the image
         const float4* wp = stage + r * W + idx;
 #pragma unroll
@@ -392,19 +395,27 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
   for (int cls = 0; cls < 2; ++cls)
     std::stable_sort(order[cls].begin(), order[cls].end(),
                      [&](int a, int b) { return g->angles_rad[a] < g->angles_rad[b]; });
-  // window width: that of full chunks of FB_NPJ neighbours if it fits, else the capacity
-  int w_full = 0;
+  // window width: wide enough for ~all chunks of FB_NPJ neighbours (the 90th percentile of their
+  // widths: a chunk that straddles a jump in angle, e.g. 45 -> 135 degrees inside a walk class, is
+  // simply split below) and for every single projection; at most the capacity
   std::vector<Extent> ext(P);
+  std::vector<int> widths;
+  int w_single = 0;
   for (int cls = 0; cls < 2; ++cls) {
     const int nv = cls ? g->nx : g->ny;
-    for (int p : order[cls]) ext[p] = proj_extent(all[p], g->n_bins, nv);
+    for (int p : order[cls]) {
+      ext[p] = proj_extent(all[p], g->n_bins, nv);
+      w_single = std::max(w_single, width_of(ext[p], plan->nc));
+    }
     for (size_t i = 0; i < order[cls].size(); i += FB_NPJ) {
       Extent e = ext[order[cls][i]];
       for (size_t j = i + 1; j < std::min(order[cls].size(), i + FB_NPJ); ++j) e = merge(e, ext[order[cls][j]]);
-      w_full = std::max(w_full, width_of(e, plan->nc));
+      widths.push_back(width_of(e, plan->nc));
     }
   }
-  const int W = std::min(std::max(w_full, plan->nc + 4), FB_WMAX);
+  std::sort(widths.begin(), widths.end());
+  const int w_most = widths.empty() ? 0 : widths[(widths.size() - 1) * 9 / 10];
+  const int W = std::min(std::max(std::max(w_most, w_single), plan->nc + 4), FB_WMAX);
   plan->W = W;
   plan->npj = FB_NPJ;
   // greedy chunks: add neighbours while the window still fits
