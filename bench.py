@@ -244,8 +244,8 @@ def run_b200(args):
             r["traffic"] = tr
         return r
 
-    roofs = [x for x in (kernel_roofline("backproject", "bp_tiled_kernel"),
-                         kernel_roofline("forward_project", "fp_gather_kernel")) if x]
+    roofs = [x for x in (kernel_roofline("backproject", "bp_run_kernel"),
+                         kernel_roofline("forward_project", "fp_band_kernel")) if x]
     roofs.sort(key=lambda r: -r["avg_ms"] * r["launches"])
     ms_bp = stages["backproject"][0] / args.steps
     ms_fp = (stages["forward_project"][0] + stages["transpose"][0]) / args.steps
