@@ -309,15 +309,18 @@ static QiLayout qi_layout(int32_t n_slices, int32_t n_angles, int32_t n_bins, do
   return L;
 }
 
-// 1 = reference, 2 = tiled, 3 = run; -1 = the requested variant does not cover the geometry
+// 1 = reference, 2 = tiled, 3 = run (4 slices per thread), 4 = run8 (8 slices per thread, the
+// product path); -1 = the requested variant does not cover the geometry
 static int pick_bp_kernel(double pixel_size) {
   const bool tiled_ok = backproject_tiled_window(pixel_size) > 0;
   const bool run_ok = backproject_run_window(pixel_size) > 0;
+  const bool run8_ok = run_ok && backproject_run8_window(pixel_size) > 0;
   switch (g_bp_variant) {
     case 1: return 1;
     case 2: return tiled_ok ? 2 : -1;
     case 3: return run_ok ? 3 : -1;
-    default: return run_ok ? 3 : (tiled_ok ? 2 : 1);
+    case 4: return run8_ok ? 4 : -1;
+    default: return run8_ok ? 4 : (run_ok ? 3 : (tiled_ok ? 2 : 1));
   }
 }
 
@@ -358,7 +361,7 @@ int pyhst_profile_read(double* ms, int64_t* kernels, int64_t* fft_execs, int32_t
 
 int pyhst_set_backproject_variant(int variant) {
   const int prev = g_bp_variant;
-  if (variant >= 0 && variant <= 3) g_bp_variant = variant;
+  if (variant >= 0 && variant <= 4) g_bp_variant = variant;
   return prev;
 }
 
@@ -450,7 +453,10 @@ int pyhst_backproject(const float* d_sino, float* d_img, const pyhst_geom_t* g, 
   void* qi = nullptr;
   PYHST_TRY(get_workspace(WS_QI, L.bytes(), &qi));
   PYHST_TRY(launch_repack_to_qi(d_sino, pitch, g->n_slices, static_cast<float4*>(qi), L,
-                                kern == 3 ? plan->d_flip : nullptr, stream));
+                                kern >= 3 ? plan->d_flip : nullptr, stream));
+  if (kern == 4)
+    return launch_backproject_run8(static_cast<const float4*>(qi), L, a, plan->d_run, plan->n_a, plan->n_b,
+                                   stream);
   if (kern == 3)
     return launch_backproject_run(static_cast<const float4*>(qi), L, a, plan->d_run, plan->n_a, plan->n_b,
                                   stream);
@@ -534,8 +540,11 @@ static int fbp_device(const float* d_sino_raw, int64_t pitch, float* d_img, cons
     PYHST_TRY(launch_ramp_filter(d_sino_raw + (int64_t)grp * 4 * P * pitch, pitch, (int64_t)n_in * P,
                                  g->n_bins, b_out, pad_left, (int)f, d_w, nullptr, 0,
                                  static_cast<float4*>(qi) + (int64_t)grp * L.group_f4(), &L, n_in,
-                                 kern == 3 ? plan->d_flip : nullptr, stream));
+                                 kern >= 3 ? plan->d_flip : nullptr, stream));
   }
+  if (kern == 4)
+    return launch_backproject_run8(static_cast<const float4*>(qi), L, a, plan->d_run, plan->n_a, plan->n_b,
+                                   stream);
   if (kern == 3)
     return launch_backproject_run(static_cast<const float4*>(qi), L, a, plan->d_run, plan->n_a, plan->n_b,
                                   stream);

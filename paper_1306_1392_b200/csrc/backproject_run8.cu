@@ -1,0 +1,323 @@
+// Backprojection P^T, the product kernel (include/pyhst.h a2; readings R1-R7,
+// R11 of DESIGN.md):   img[s,i,j] = scale * sum_p lerp(q[s,p,:], c_p + ch_p (j-j0) + sh_p (i-i0))
+//
+// bp_run8_kernel<PASS>: the run scheme of bp_run_kernel (backproject.cu) with the measured cost
+// model of sm_100a applied.  On B200 an FFMA2 occupies the issue port for two cycles, so every
+// instruction of the run loop costs as much as one FFMA: a warp-step (32 lanes x 4 slices x one
+// pixel x one projection = 128 updates) is 8 slots of algorithmic FMA work plus one slot per
+// overhead instruction.  Hence:
+//   * a thread owns EIGHT slices (two interleaved slice groups): the weight logic (f += dl, wrap,
+//     w = 1 - f, predicate, address) is shared by twice the FMA work;
+//   * runs are 8 pixels long (64 accumulator registers), four independent projections are kept in
+//     flight per thread (the loop is latency-sensitive at 4 warps per scheduler);
+//   * the producer role rotates over the warps: the producing warp computes the window geometry
+//     in double (R11) and issues the TMA bulk copies two chunks ahead; warps meet only through
+//     full/empty mbarriers -- no block-wide barrier in the projection loop;
+//   * class A (|sh| <= |ch|, lanes along x, runs along y) and class B (lanes along y, runs along
+//     x) are two launches: pass 0 writes the image, pass 1 adds to it.
+#include "common.h"
+
+namespace pyhst {
+
+namespace {
+
+constexpr int R8_LANES = 64;   // tile extent along the fast axis of the class (one lane each)
+constexpr int R8_RN = 8;       // pixels per run
+constexpr int R8_RG = 4;       // runs per lane column: extent along the slow axis = RG * RN = 32
+constexpr int R8_SLOW = R8_RG * R8_RN;
+constexpr int R8_NC = 256;     // consumer threads (8 warps)
+constexpr int R8_NT = R8_NC;
+constexpr int R8_NA = 8;       // projections per staged chunk
+constexpr int R8_NS = 4;       // stages
+constexpr int R8_AHEAD = 2;    // chunks in flight ahead of the one being consumed (<= NS - 2:
+                               // the producer warp may then run two chunks ahead of the slowest warp)
+constexpr int R8_HDR = 1024;   // mbarriers + geometry ring; keeps the windows 128-B aligned
+
+__device__ __forceinline__ unsigned long long r8_pack2(float lo, float hi) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void r8_unpack2(unsigned long long v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ void r8_ffma2(unsigned long long& d, unsigned long long a,
+                                         unsigned long long b) {
+  asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
+}
+
+#define R8_LD4(q, a)                                                                      \
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"                                 \
+               : "=f"(q.x), "=f"(q.y), "=f"(q.z), "=f"(q.w)                               \
+               : "r"(a))
+
+}  // namespace
+
+namespace {
+
+// One run of R8_RN pixels of one projection, 8 slices: (qa, qb) / (ra, rb) are the lower / upper
+// taps of the two slice groups, kept in registers.  f += dl; when f >= 1 the run has moved on by
+// one bin: f -= 1, the upper taps become the lower ones and one new float4 per group is loaded --
+// all predicated, registers updated in place.  Half of the register moves are written as x + (-0)
+// (FMA pipe), half as FSEL (ALU pipe).
+__device__ __forceinline__ void r8_run(unsigned long long (&acc)[R8_RN][4], uint32_t addr,
+                                       uint32_t addr2, float f, const float dl) {
+  float4 qa, qb, ra, rb;
+  R8_LD4(qa, addr);
+  R8_LD4(qb, addr + 16);
+  R8_LD4(ra, addr2);
+  R8_LD4(rb, addr2 + 16);
+#pragma unroll
+  for (int n = 0; n < R8_RN; ++n) {
+    const float w = 1.f - f;
+    const unsigned long long w2 = r8_pack2(w, w), f2 = r8_pack2(f, f);  // scalar-broadcast operands
+    r8_ffma2(acc[n][0], r8_pack2(qa.x, qa.y), w2);
+    r8_ffma2(acc[n][1], r8_pack2(qa.z, qa.w), w2);
+    r8_ffma2(acc[n][2], r8_pack2(ra.x, ra.y), w2);
+    r8_ffma2(acc[n][3], r8_pack2(ra.z, ra.w), w2);
+    r8_ffma2(acc[n][0], r8_pack2(qb.x, qb.y), f2);
+    r8_ffma2(acc[n][1], r8_pack2(qb.z, qb.w), f2);
+    r8_ffma2(acc[n][2], r8_pack2(rb.x, rb.y), f2);
+    r8_ffma2(acc[n][3], r8_pack2(rb.z, rb.w), f2);
+    if (n + 1 < R8_RN) {
+      asm volatile(
+          "{\n\t"
+          ".reg .pred p;\n\t"
+          "add.rn.f32 %18, %18, %19;\n\t"
+          "setp.ge.f32 p, %18, 0f3F800000;\n\t"
+          "@p add.rn.f32 %18, %18, 0fBF800000;\n\t"
+          "@p mov.f32 %0, %4;\n\t"
+          "@p add.rn.f32 %1, %5, 0f80000000;\n\t"
+          "@p mov.f32 %2, %6;\n\t"
+          "@p add.rn.f32 %3, %7, 0f80000000;\n\t"
+          "@p mov.f32 %8, %12;\n\t"
+          "@p add.rn.f32 %9, %13, 0f80000000;\n\t"
+          "@p mov.f32 %10, %14;\n\t"
+          "@p add.rn.f32 %11, %15, 0f80000000;\n\t"
+          "@p add.u32 %16, %16, 16;\n\t"
+          "@p add.u32 %17, %17, 16;\n\t"
+          "@p ld.shared.v4.f32 {%4, %5, %6, %7}, [%16+16];\n\t"
+          "@p ld.shared.v4.f32 {%12, %13, %14, %15}, [%17+16];\n\t"
+          "}"
+          : "+f"(qa.x), "+f"(qa.y), "+f"(qa.z), "+f"(qa.w), "+f"(qb.x), "+f"(qb.y), "+f"(qb.z),
+            "+f"(qb.w), "+f"(ra.x), "+f"(ra.y), "+f"(ra.z), "+f"(ra.w), "+f"(rb.x), "+f"(rb.y),
+            "+f"(rb.z), "+f"(rb.w), "+r"(addr), "+r"(addr2), "+f"(f)
+          : "f"(dl));
+    }
+  }
+}
+
+}  // namespace
+
+// PASS 0: entries [e0, e0 + ne) are class A (lanes along x, runs along y), tile 64 (x) x 32 (y).
+// PASS 1: class B (lanes along y, runs along x), tile 32 (x) x 64 (y).
+// add != 0: the tile is added to what is already in img (pass 1 after pass 0).
+template <int PASS>
+__global__ void __launch_bounds__(R8_NT, 2)
+bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* img, int S,
+               int n_groups, int P, int B, int nx, int ny, float scale,
+               const RunProj* __restrict__ run, int e0, int ne, int add, int W) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);         // [NS]
+  uint64_t* empty = reinterpret_cast<uint64_t*>(smem + 64);   // [NS]
+  float4* geo = reinterpret_cast<float4*>(smem + 128);        // [NS][NA] (c_fast, dl, base, t_hi)
+  float4* buf = reinterpret_cast<float4*>(smem + R8_HDR);     // [NS][NA][2][W]
+
+  constexpr int EX = PASS ? R8_SLOW : R8_LANES, EY = PASS ? R8_LANES : R8_SLOW;
+  const int tid = threadIdx.x;
+  const int x0 = blockIdx.x * EX, y0 = blockIdx.y * EY;
+  const int gA = blockIdx.z * 2, gB = min(gA + 1, n_groups - 1);
+  const int n_chunks = (ne + R8_NA - 1) / R8_NA;
+  const uint32_t win_bytes = (uint32_t)W * 16u;
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < R8_NS; ++s) {
+      mbar_init(&full[s], R8_NA);
+      mbar_init(&empty[s], R8_NC / 32);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  // ---------------- producer role (one warp, lanes < NA): window geometry in double (R11) + TMA
+  // bulk copies of chunk c into stage c % NS; the stage was last read as chunk c - NS
+  const double dx0 = (double)x0 - 0.5 * (double)(nx - 1);
+  const double dy0 = (double)y0 - 0.5 * (double)(ny - 1);
+  const float4* qA = qi + (int64_t)gA * P * row_f4;
+  const float4* qB = qi + (int64_t)gB * P * row_f4;
+  auto produce = [&](int c) {
+    const int st = c % R8_NS;
+    if (c >= R8_NS) mbar_wait(&empty[st], (uint32_t)(((c / R8_NS) - 1) & 1));
+    const int pl = tid & 31;
+    if (pl < R8_NA) {
+      const int e = c * R8_NA + pl;
+      uint64_t* bar = &full[st];
+      if (e < ne) {
+        const RunProj pg = run[e0 + e];
+        const double base = pg.c + pg.ch * dx0 + pg.sh * dy0;  // t of the tile's pixel (0,0)
+        const double tmin = base + fmin(0.0, pg.ch * (EX - 1)) + fmin(0.0, pg.sh * (EY - 1));
+        double o = floor(tmin) - 1.0;                           // one bin of slack for FP32 rounding
+        o = fmax(o, -(double)zpad);
+        o = fmin(o, (double)(B + zpad - W));
+        const float cf = (float)(PASS ? pg.sh : pg.ch), dl = (float)(PASS ? pg.ch : pg.sh);
+        // runs that would leave the window (only possible where the window is clamped onto the
+        // zero pads, i.e. where every tap is zero) are moved inside it
+        geo[st * R8_NA + pl] =
+            make_float4(cf, dl, (float)(base - o), (float)(W - 3) - (float)(R8_RN - 1) * dl);
+        const int64_t src = (int64_t)pg.p * row_f4 + (int64_t)o + zpad;
+        float4* dst = buf + (size_t)(st * R8_NA + pl) * 2 * W;
+        mbar_arrive_expect_tx(bar, 2 * win_bytes);
+        bulk_g2s(dst, qA + src, win_bytes, bar);
+        bulk_g2s(dst + W, qB + src, win_bytes, bar);
+      } else {
+        mbar_arrive(bar);
+      }
+    }
+    __syncwarp();
+  };
+  if (tid < 32) {
+#pragma unroll 1
+    for (int c = 0; c < R8_AHEAD && c < n_chunks; ++c) produce(c);
+  }
+
+  // ---------------- consumers
+  const int fl = tid & (R8_LANES - 1);       // position along the fast axis of the class
+  const int rn = (tid >> 6) * R8_RN;         // first pixel of the run along the slow axis
+  const float ffl = (float)fl, frn = (float)rn;
+  const uint32_t wb = smem_u32(buf);
+  const uint32_t goff = win_bytes;
+
+  unsigned long long acc[R8_RN][4];
+#pragma unroll
+  for (int n = 0; n < R8_RN; ++n)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[n][j] = 0ull;
+
+  for (int c = 0; c < n_chunks; ++c) {
+    // the producer role rotates over the warps, so that no warp is the slowest one
+    if ((tid >> 5) == ((c + R8_AHEAD) & 7) && c + R8_AHEAD < n_chunks) produce(c + R8_AHEAD);
+    const int st = c % R8_NS;
+    mbar_wait(&full[st], (uint32_t)((c / R8_NS) & 1));
+    const int na = min(R8_NA, ne - c * R8_NA);
+    const float4* gch = geo + st * R8_NA;
+    const uint32_t sb = wb + (uint32_t)(st * R8_NA) * 2u * win_bytes;
+#pragma unroll 4
+    for (int a = 0; a < na; ++a) {
+      const float4 gg = gch[a];
+      float t = fmaf(ffl, gg.x, fmaf(frn, gg.y, gg.z));
+      t = fminf(fmaxf(t, 0.f), gg.w);
+      const float tm = __fadd_rd(t, 8388608.f);
+      const int k = __float_as_int(tm) - 0x4b000000;
+      const float f0 = t - (tm - 8388608.f);
+      const uint32_t addr = sb + (uint32_t)a * 2u * win_bytes + (uint32_t)k * 16u;
+      r8_run(acc, addr, addr + goff, f0, gg.y);
+    }
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(&empty[st]);
+  }
+
+  // ---------------- write the tile: acc[n][0..1] = slices of group gA, acc[n][2..3] = group gA + 1
+  if (PASS == 0) {  // pixel (x0 + fl, y0 + rn + n): lanes along x, coalesced
+    const int x = x0 + fl;
+    if (x < nx) {
+#pragma unroll
+      for (int n = 0; n < R8_RN; ++n) {
+        const int y = y0 + rn + n;
+        if (y >= ny) continue;
+        float v[8];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) r8_unpack2(acc[n][j], v[2 * j], v[2 * j + 1]);
+#pragma unroll
+        for (int sl = 0; sl < 8; ++sl) {
+          const int s = gA * 4 + sl;
+          if (s < S) {
+            float* dst = img + ((int64_t)s * ny + y) * nx + x;
+            *dst = add ? fmaf(scale, v[sl], *dst) : scale * v[sl];
+          }
+        }
+      }
+    }
+  } else {  // pixel (x0 + rn + n, y0 + fl): 8 consecutive x per thread
+    const int y = y0 + fl;
+    if (y < ny) {
+      float v[R8_RN][8];
+#pragma unroll
+      for (int n = 0; n < R8_RN; ++n)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) r8_unpack2(acc[n][j], v[n][2 * j], v[n][2 * j + 1]);
+#pragma unroll
+      for (int sl = 0; sl < 8; ++sl) {
+        const int s = gA * 4 + sl;
+        if (s >= S) continue;
+        float* row = img + ((int64_t)s * ny + y) * nx + x0 + rn;
+        const bool vec = ((reinterpret_cast<uintptr_t>(row) & 15) == 0) && (x0 + rn + R8_RN <= nx);
+#pragma unroll
+        for (int n4 = 0; n4 < R8_RN; n4 += 4) {
+          if (vec) {
+            float4 o = add ? *reinterpret_cast<const float4*>(row + n4) : make_float4(0.f, 0.f, 0.f, 0.f);
+            o.x = fmaf(scale, v[n4][sl], o.x);
+            o.y = fmaf(scale, v[n4 + 1][sl], o.y);
+            o.z = fmaf(scale, v[n4 + 2][sl], o.z);
+            o.w = fmaf(scale, v[n4 + 3][sl], o.w);
+            *reinterpret_cast<float4*>(row + n4) = o;
+          } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              if (x0 + rn + n4 + j < nx)
+                row[n4 + j] = fmaf(scale, v[n4 + j][sl], add ? row[n4 + j] : 0.f);
+          }
+        }
+      }
+    }
+  }
+}
+
+// window (bins) a 64 x 32 tile touches: span <= h sqrt(63^2 + 31^2), + floor, second tap, slack
+int backproject_run8_window(double pixel_size) {
+  if (!(pixel_size * 0.70710678118654757 < 0.999)) return 0;  // run step must stay below one bin
+  const double span = pixel_size * sqrt((double)((R8_LANES - 1) * (R8_LANES - 1) +
+                                                 (R8_SLOW - 1) * (R8_SLOW - 1)));
+  const double w = ceil(span) + 5.0;
+  if (w > 256.0) return 0;
+  return ((int)w + 3) & ~3;
+}
+
+int launch_backproject_run8(const float4* d_qi, const QiLayout& L, const BpArgs& a,
+                            const RunProj* d_run, int32_t n_a, int32_t n_b, cudaStream_t stream) {
+  const int W = backproject_run8_window(a.pixel_size);
+  if (W == 0 || W > L.n_bins + 2 * L.zpad || L.zpad < W + 2)
+    return set_error(PYHST_ERR_UNSUPPORTED, "run8 backprojector: window %d does not fit", W);
+  const size_t smem = R8_HDR + (size_t)R8_NS * R8_NA * 2 * W * 16;
+  if (smem > 110 * 1024)
+    return set_error(PYHST_ERR_UNSUPPORTED, "run8 backprojector: pixel size too large");
+  static size_t configured = 0;
+  if (smem > configured) {
+    PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = smem;
+  }
+  const unsigned gz = (unsigned)((L.n_groups + 1) / 2);
+  dim3 grid_a((a.nx + R8_LANES - 1) / R8_LANES, (a.ny + R8_SLOW - 1) / R8_SLOW, gz);
+  dim3 grid_b((a.nx + R8_SLOW - 1) / R8_SLOW, (a.ny + R8_LANES - 1) / R8_LANES, gz);
+  if (grid_a.y > 65535 || grid_b.y > 65535 || gz > 65535)
+    return set_error(PYHST_ERR_UNSUPPORTED, "run8 backprojector: grid too large");
+  StageScope scope(ST_BACKPROJECT, stream);
+  if (n_a > 0 || n_b == 0) {  // n_a == n_b == 0 cannot happen (n_angles > 0); pass 0 also zero-fills
+    scope.kernels();
+    bp_run8_kernel<0><<<grid_a, R8_NT, smem, stream>>>(d_qi, L.row_f4(), L.zpad, a.d_img, a.n_slices,
+                                                       L.n_groups, L.n_angles, a.n_bins, a.nx, a.ny,
+                                                       a.scale, d_run, 0, n_a, 0, W);
+    PYHST_CUDA_TRY(cudaGetLastError());
+  }
+  if (n_b > 0) {
+    scope.kernels();
+    bp_run8_kernel<1><<<grid_b, R8_NT, smem, stream>>>(d_qi, L.row_f4(), L.zpad, a.d_img, a.n_slices,
+                                                       L.n_groups, L.n_angles, a.n_bins, a.nx, a.ny,
+                                                       a.scale, d_run, n_a, n_b, n_a > 0 ? 1 : 0, W);
+    PYHST_CUDA_TRY(cudaGetLastError());
+  }
+  return PYHST_OK;
+}
+
+}  // namespace pyhst

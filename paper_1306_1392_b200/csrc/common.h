@@ -126,6 +126,11 @@ struct RunProj;
 int launch_backproject_run(const float4* d_qi, const QiLayout& L, const BpArgs& a,
                            const RunProj* d_run, int32_t n_a, int32_t n_b, cudaStream_t stream);
 
+// run8 kernel (8 slices per thread, producer warp; backproject_run8.cu)
+int backproject_run8_window(double pixel_size);
+int launch_backproject_run8(const float4* d_qi, const QiLayout& L, const BpArgs& a,
+                            const RunProj* d_run, int32_t n_a, int32_t n_b, cudaStream_t stream);
+
 // ---- interleaved, zero-padded image layout consumed by the banded forward projector -------
 // XI[g][v][zpad + u][sl]: slice group g = s / 4, one float4 per (g, line v, position u); every
 // line carries `zpad` zero float4 on both sides.  Two copies: lines = image rows (u = j, v = i)

@@ -60,7 +60,7 @@ BP_CASES = [
 ]
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 @pytest.mark.parametrize("case", BP_CASES)
 def test_backproject_matches_oracle(lib, oracle, case, variant):
     S, P, B, nx, ny, h, axis, drift = case
