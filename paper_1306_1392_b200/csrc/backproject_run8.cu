@@ -28,23 +28,7 @@ constexpr int R8_SLOW = R8_RG * R8_RN;
 constexpr int R8_NC = 256;     // consumer threads (8 warps)
 constexpr int R8_NT = R8_NC;
 constexpr int R8_NA = 8;       // projections per staged chunk
-constexpr int R8_NS = 4;       // stages
-constexpr int R8_AHEAD = 2;    // chunks in flight ahead of the one being consumed (<= NS - 2:
-                               // the producer warp may then run two chunks ahead of the slowest warp)
 constexpr int R8_HDR = 1024;   // mbarriers + geometry ring; keeps the windows 128-B aligned
-
-__device__ __forceinline__ unsigned long long r8_pack2(float lo, float hi) {
-  unsigned long long r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-  return r;
-}
-__device__ __forceinline__ void r8_unpack2(unsigned long long v, float& lo, float& hi) {
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ void r8_ffma2(unsigned long long& d, unsigned long long a,
-                                         unsigned long long b) {
-  asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
-}
 
 #define R8_LD4(q, a)                                                                      \
   asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"                                 \
@@ -59,33 +43,35 @@ namespace {
 // taps of the two slice groups, kept in registers.  f += dl; when f >= 1 the run has moved on by
 // one bin: f -= 1, the upper taps become the lower ones and one new float4 per group is loaded --
 // all predicated, registers updated in place.  Half of the register moves are written as x + (-0)
-// (FMA pipe), half as FSEL (ALU pipe).
-__device__ __forceinline__ void r8_run(unsigned long long (&acc)[R8_RN][4], uint32_t addr,
-                                       uint32_t addr2, float f, const float dl) {
+// (FMA pipe), half as FSEL (ALU pipe).  The interpolation is scalar FFMA: an FFMA2 holds the issue
+// port for two cycles on sm_100a, so packing saves nothing and costs pair-alignment MOVs.
+// GOFF = byte offset of the second group's window (compile-time: one address register).
+template <int GOFF>
+__device__ __forceinline__ void r8_run(float (&acc)[R8_RN][8], uint32_t addr, float f,
+                                       const float dl) {
   float4 qa, qb, ra, rb;
   R8_LD4(qa, addr);
   R8_LD4(qb, addr + 16);
-  R8_LD4(ra, addr2);
-  R8_LD4(rb, addr2 + 16);
+  R8_LD4(ra, addr + GOFF);
+  R8_LD4(rb, addr + GOFF + 16);
 #pragma unroll
   for (int n = 0; n < R8_RN; ++n) {
     const float w = 1.f - f;
-    const unsigned long long w2 = r8_pack2(w, w), f2 = r8_pack2(f, f);  // scalar-broadcast operands
-    r8_ffma2(acc[n][0], r8_pack2(qa.x, qa.y), w2);
-    r8_ffma2(acc[n][1], r8_pack2(qa.z, qa.w), w2);
-    r8_ffma2(acc[n][2], r8_pack2(ra.x, ra.y), w2);
-    r8_ffma2(acc[n][3], r8_pack2(ra.z, ra.w), w2);
-    r8_ffma2(acc[n][0], r8_pack2(qb.x, qb.y), f2);
-    r8_ffma2(acc[n][1], r8_pack2(qb.z, qb.w), f2);
-    r8_ffma2(acc[n][2], r8_pack2(rb.x, rb.y), f2);
-    r8_ffma2(acc[n][3], r8_pack2(rb.z, rb.w), f2);
+    acc[n][0] = fmaf(qb.x, f, fmaf(qa.x, w, acc[n][0]));
+    acc[n][1] = fmaf(qb.y, f, fmaf(qa.y, w, acc[n][1]));
+    acc[n][2] = fmaf(qb.z, f, fmaf(qa.z, w, acc[n][2]));
+    acc[n][3] = fmaf(qb.w, f, fmaf(qa.w, w, acc[n][3]));
+    acc[n][4] = fmaf(rb.x, f, fmaf(ra.x, w, acc[n][4]));
+    acc[n][5] = fmaf(rb.y, f, fmaf(ra.y, w, acc[n][5]));
+    acc[n][6] = fmaf(rb.z, f, fmaf(ra.z, w, acc[n][6]));
+    acc[n][7] = fmaf(rb.w, f, fmaf(ra.w, w, acc[n][7]));
     if (n + 1 < R8_RN) {
       asm volatile(
           "{\n\t"
           ".reg .pred p;\n\t"
-          "add.rn.f32 %18, %18, %19;\n\t"
-          "setp.ge.f32 p, %18, 0f3F800000;\n\t"
-          "@p add.rn.f32 %18, %18, 0fBF800000;\n\t"
+          "add.rn.f32 %17, %17, %18;\n\t"
+          "setp.ge.f32 p, %17, 0f3F800000;\n\t"
+          "@p add.rn.f32 %17, %17, 0fBF800000;\n\t"
           "@p mov.f32 %0, %4;\n\t"
           "@p add.rn.f32 %1, %5, 0f80000000;\n\t"
           "@p mov.f32 %2, %6;\n\t"
@@ -95,14 +81,13 @@ __device__ __forceinline__ void r8_run(unsigned long long (&acc)[R8_RN][4], uint
           "@p mov.f32 %10, %14;\n\t"
           "@p add.rn.f32 %11, %15, 0f80000000;\n\t"
           "@p add.u32 %16, %16, 16;\n\t"
-          "@p add.u32 %17, %17, 16;\n\t"
           "@p ld.shared.v4.f32 {%4, %5, %6, %7}, [%16+16];\n\t"
-          "@p ld.shared.v4.f32 {%12, %13, %14, %15}, [%17+16];\n\t"
+          "@p ld.shared.v4.f32 {%12, %13, %14, %15}, [%16+%19];\n\t"
           "}"
           : "+f"(qa.x), "+f"(qa.y), "+f"(qa.z), "+f"(qa.w), "+f"(qb.x), "+f"(qb.y), "+f"(qb.z),
             "+f"(qb.w), "+f"(ra.x), "+f"(ra.y), "+f"(ra.z), "+f"(ra.w), "+f"(rb.x), "+f"(rb.y),
-            "+f"(rb.z), "+f"(rb.w), "+r"(addr), "+r"(addr2), "+f"(f)
-          : "f"(dl));
+            "+f"(rb.z), "+f"(rb.w), "+r"(addr), "+f"(f)
+          : "f"(dl), "n"(GOFF + 16));
     }
   }
 }
@@ -112,7 +97,11 @@ __device__ __forceinline__ void r8_run(unsigned long long (&acc)[R8_RN][4], uint
 // PASS 0: entries [e0, e0 + ne) are class A (lanes along x, runs along y), tile 64 (x) x 32 (y).
 // PASS 1: class B (lanes along y, runs along x), tile 32 (x) x 64 (y).
 // add != 0: the tile is added to what is already in img (pass 1 after pass 0).
-template <int PASS>
+// WS = window slot stride in float4 (compile-time, so that the second slice group's taps sit at a
+// constant offset from the first one's); W <= WS bins are staged.  NS = stages; chunks are issued
+// NS - 2 ahead of the one being consumed (the producing warp may then run ahead of the slowest
+// warp by up to two chunks without waiting).
+template <int PASS, int WS, int NS>
 __global__ void __launch_bounds__(R8_NT, 2)
 bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* img, int S,
                int n_groups, int P, int B, int nx, int ny, float scale,
@@ -121,7 +110,7 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);         // [NS]
   uint64_t* empty = reinterpret_cast<uint64_t*>(smem + 64);   // [NS]
   float4* geo = reinterpret_cast<float4*>(smem + 128);        // [NS][NA] (c_fast, dl, base, t_hi)
-  float4* buf = reinterpret_cast<float4*>(smem + R8_HDR);     // [NS][NA][2][W]
+  float4* buf = reinterpret_cast<float4*>(smem + R8_HDR);     // [NS][NA][2][WS]
 
   constexpr int EX = PASS ? R8_SLOW : R8_LANES, EY = PASS ? R8_LANES : R8_SLOW;
   const int tid = threadIdx.x;
@@ -132,7 +121,7 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
 
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < R8_NS; ++s) {
+    for (int s = 0; s < NS; ++s) {
       mbar_init(&full[s], R8_NA);
       mbar_init(&empty[s], R8_NC / 32);
     }
@@ -147,8 +136,8 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
   const float4* qA = qi + (int64_t)gA * P * row_f4;
   const float4* qB = qi + (int64_t)gB * P * row_f4;
   auto produce = [&](int c) {
-    const int st = c % R8_NS;
-    if (c >= R8_NS) mbar_wait(&empty[st], (uint32_t)(((c / R8_NS) - 1) & 1));
+    const int st = c % NS;
+    if (c >= NS) mbar_wait(&empty[st], (uint32_t)(((c / NS) - 1) & 1));
     const int pl = tid & 31;
     if (pl < R8_NA) {
       const int e = c * R8_NA + pl;
@@ -166,10 +155,10 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
         geo[st * R8_NA + pl] =
             make_float4(cf, dl, (float)(base - o), (float)(W - 3) - (float)(R8_RN - 1) * dl);
         const int64_t src = (int64_t)pg.p * row_f4 + (int64_t)o + zpad;
-        float4* dst = buf + (size_t)(st * R8_NA + pl) * 2 * W;
+        float4* dst = buf + (size_t)(st * R8_NA + pl) * 2 * WS;
         mbar_arrive_expect_tx(bar, 2 * win_bytes);
         bulk_g2s(dst, qA + src, win_bytes, bar);
-        bulk_g2s(dst + W, qB + src, win_bytes, bar);
+        bulk_g2s(dst + WS, qB + src, win_bytes, bar);
       } else {
         mbar_arrive(bar);
       }
@@ -178,7 +167,7 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
   };
   if (tid < 32) {
 #pragma unroll 1
-    for (int c = 0; c < R8_AHEAD && c < n_chunks; ++c) produce(c);
+    for (int c = 0; c < (NS - 2) && c < n_chunks; ++c) produce(c);
   }
 
   // ---------------- consumers
@@ -186,22 +175,21 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
   const int rn = (tid >> 6) * R8_RN;         // first pixel of the run along the slow axis
   const float ffl = (float)fl, frn = (float)rn;
   const uint32_t wb = smem_u32(buf);
-  const uint32_t goff = win_bytes;
 
-  unsigned long long acc[R8_RN][4];
+  float acc[R8_RN][8];
 #pragma unroll
   for (int n = 0; n < R8_RN; ++n)
 #pragma unroll
-    for (int j = 0; j < 4; ++j) acc[n][j] = 0ull;
+    for (int j = 0; j < 8; ++j) acc[n][j] = 0.f;
 
   for (int c = 0; c < n_chunks; ++c) {
     // the producer role rotates over the warps, so that no warp is the slowest one
-    if ((tid >> 5) == ((c + R8_AHEAD) & 7) && c + R8_AHEAD < n_chunks) produce(c + R8_AHEAD);
-    const int st = c % R8_NS;
-    mbar_wait(&full[st], (uint32_t)((c / R8_NS) & 1));
+    if ((tid >> 5) == ((c + (NS - 2)) & 7) && c + (NS - 2) < n_chunks) produce(c + (NS - 2));
+    const int st = c % NS;
+    mbar_wait(&full[st], (uint32_t)((c / NS) & 1));
     const int na = min(R8_NA, ne - c * R8_NA);
     const float4* gch = geo + st * R8_NA;
-    const uint32_t sb = wb + (uint32_t)(st * R8_NA) * 2u * win_bytes;
+    const uint32_t sb = wb + (uint32_t)(st * R8_NA) * (2u * WS * 16u);
 #pragma unroll 4
     for (int a = 0; a < na; ++a) {
       const float4 gg = gch[a];
@@ -210,8 +198,8 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
       const float tm = __fadd_rd(t, 8388608.f);
       const int k = __float_as_int(tm) - 0x4b000000;
       const float f0 = t - (tm - 8388608.f);
-      const uint32_t addr = sb + (uint32_t)a * 2u * win_bytes + (uint32_t)k * 16u;
-      r8_run(acc, addr, addr + goff, f0, gg.y);
+      const uint32_t addr = sb + (uint32_t)a * (2u * WS * 16u) + (uint32_t)k * 16u;
+      r8_run<WS * 16>(acc, addr, f0, gg.y);
     }
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(&empty[st]);
@@ -227,7 +215,7 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
         if (y >= ny) continue;
         float v[8];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) r8_unpack2(acc[n][j], v[2 * j], v[2 * j + 1]);
+        for (int j = 0; j < 8; ++j) v[j] = acc[n][j];
 #pragma unroll
         for (int sl = 0; sl < 8; ++sl) {
           const int s = gA * 4 + sl;
@@ -245,7 +233,7 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
 #pragma unroll
       for (int n = 0; n < R8_RN; ++n)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) r8_unpack2(acc[n][j], v[n][2 * j], v[n][2 * j + 1]);
+        for (int j = 0; j < 8; ++j) v[n][j] = acc[n][j];
 #pragma unroll
       for (int sl = 0; sl < 8; ++sl) {
         const int s = gA * 4 + sl;
@@ -279,23 +267,23 @@ int backproject_run8_window(double pixel_size) {
   const double span = pixel_size * sqrt((double)((R8_LANES - 1) * (R8_LANES - 1) +
                                                  (R8_SLOW - 1) * (R8_SLOW - 1)));
   const double w = ceil(span) + 5.0;
-  if (w > 256.0) return 0;
+  if (w > 112.0) return 0;
   return ((int)w + 3) & ~3;
 }
 
-int launch_backproject_run8(const float4* d_qi, const QiLayout& L, const BpArgs& a,
-                            const RunProj* d_run, int32_t n_a, int32_t n_b, cudaStream_t stream) {
-  const int W = backproject_run8_window(a.pixel_size);
-  if (W == 0 || W > L.n_bins + 2 * L.zpad || L.zpad < W + 2)
-    return set_error(PYHST_ERR_UNSUPPORTED, "run8 backprojector: window %d does not fit", W);
-  const size_t smem = R8_HDR + (size_t)R8_NS * R8_NA * 2 * W * 16;
-  if (smem > 110 * 1024)
-    return set_error(PYHST_ERR_UNSUPPORTED, "run8 backprojector: pixel size too large");
-  static size_t configured = 0;
-  if (smem > configured) {
-    PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = smem;
+namespace {
+
+template <int WS, int NS>
+int launch_run8(const float4* d_qi, const QiLayout& L, const BpArgs& a, const RunProj* d_run,
+                int32_t n_a, int32_t n_b, int W, cudaStream_t stream) {
+  const size_t smem = R8_HDR + (size_t)NS * R8_NA * 2 * WS * 16;
+  static bool configured = false;
+  if (!configured) {
+    PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<0, WS, NS>,
+                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<1, WS, NS>,
+                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = true;
   }
   const unsigned gz = (unsigned)((L.n_groups + 1) / 2);
   dim3 grid_a((a.nx + R8_LANES - 1) / R8_LANES, (a.ny + R8_SLOW - 1) / R8_SLOW, gz);
@@ -303,21 +291,33 @@ int launch_backproject_run8(const float4* d_qi, const QiLayout& L, const BpArgs&
   if (grid_a.y > 65535 || grid_b.y > 65535 || gz > 65535)
     return set_error(PYHST_ERR_UNSUPPORTED, "run8 backprojector: grid too large");
   StageScope scope(ST_BACKPROJECT, stream);
-  if (n_a > 0 || n_b == 0) {  // n_a == n_b == 0 cannot happen (n_angles > 0); pass 0 also zero-fills
+  if (n_a > 0 || n_b == 0) {  // n_a == n_b == 0 cannot happen (n_angles > 0)
     scope.kernels();
-    bp_run8_kernel<0><<<grid_a, R8_NT, smem, stream>>>(d_qi, L.row_f4(), L.zpad, a.d_img, a.n_slices,
-                                                       L.n_groups, L.n_angles, a.n_bins, a.nx, a.ny,
-                                                       a.scale, d_run, 0, n_a, 0, W);
+    bp_run8_kernel<0, WS, NS><<<grid_a, R8_NT, smem, stream>>>(
+        d_qi, L.row_f4(), L.zpad, a.d_img, a.n_slices, L.n_groups, L.n_angles, a.n_bins, a.nx, a.ny,
+        a.scale, d_run, 0, n_a, 0, W);
     PYHST_CUDA_TRY(cudaGetLastError());
   }
   if (n_b > 0) {
     scope.kernels();
-    bp_run8_kernel<1><<<grid_b, R8_NT, smem, stream>>>(d_qi, L.row_f4(), L.zpad, a.d_img, a.n_slices,
-                                                       L.n_groups, L.n_angles, a.n_bins, a.nx, a.ny,
-                                                       a.scale, d_run, n_a, n_b, n_a > 0 ? 1 : 0, W);
+    bp_run8_kernel<1, WS, NS><<<grid_b, R8_NT, smem, stream>>>(
+        d_qi, L.row_f4(), L.zpad, a.d_img, a.n_slices, L.n_groups, L.n_angles, a.n_bins, a.nx, a.ny,
+        a.scale, d_run, n_a, n_b, n_a > 0 ? 1 : 0, W);
     PYHST_CUDA_TRY(cudaGetLastError());
   }
   return PYHST_OK;
+}
+
+}  // namespace
+
+int launch_backproject_run8(const float4* d_qi, const QiLayout& L, const BpArgs& a,
+                            const RunProj* d_run, int32_t n_a, int32_t n_b, cudaStream_t stream) {
+  const int W = backproject_run8_window(a.pixel_size);
+  if (W == 0 || W > L.n_bins + 2 * L.zpad || L.zpad < W + 2)
+    return set_error(PYHST_ERR_UNSUPPORTED, "run8 backprojector: window %d does not fit", W);
+  // two instantiations: slots of 80 bins, 4 stages (pixel size <= 1.03), or 112 bins, 3 stages
+  if (W <= 80) return launch_run8<80, 4>(d_qi, L, a, d_run, n_a, n_b, W, stream);
+  return launch_run8<112, 3>(d_qi, L, a, d_run, n_a, n_b, W, stream);
 }
 
 }  // namespace pyhst
