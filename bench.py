@@ -225,13 +225,18 @@ def run_b200(args):
     peak_tflops = n_sm * FP32_LANES_PER_SM * 2 * f_max / 1e12   # FP32 FMA issue peak at max clock
 
     def kernel_roofline(stage, name):
+        # one "launch" of the roofline = one call of the stage (all S*nx*ny*P updates); the run8
+        # backprojector covers it with two kernel launches (class A, then class B projections)
         ms, launches, _ = stages[stage]
         if launches == 0:
             return None
+        kernels_per_call = max(1, round(launches / args.steps))
+        launches = args.steps
         avg_ms = ms / launches
         ach = updates * LANE_OPS_PER_UPDATE * 2 / (avg_ms * 1e-3) / 1e12
         r = {"kernel": name, "bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s",
              "frac": ach / peak_tflops, "traffic": None, "avg_ms": avg_ms, "launches": launches,
+             "kernels_per_launch": kernels_per_call,
              "updates_per_launch": updates, "flop_per_update": 2 * LANE_OPS_PER_UPDATE,
              "gups": updates / (avg_ms * 1e-3) / 1e9,
              "peak_note": "%d SMs x 128 FP32 lanes x 2 flop x %.0f MHz (sm_max_mhz, %s peaks file); "
@@ -244,7 +249,7 @@ def run_b200(args):
             r["traffic"] = tr
         return r
 
-    roofs = [x for x in (kernel_roofline("backproject", "bp_run_kernel"),
+    roofs = [x for x in (kernel_roofline("backproject", "bp_run8_kernel<0> + bp_run8_kernel<1>"),
                          kernel_roofline("forward_project", "fp_band_kernel")) if x]
     roofs.sort(key=lambda r: -r["avg_ms"] * r["launches"])
     ms_bp = stages["backproject"][0] / args.steps
