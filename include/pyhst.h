@@ -134,8 +134,11 @@ int pyhst_forward_project_host(const float* h_img, float* h_sino, const pyhst_ge
 int pyhst_halfacq_extent(int32_t n_bins, double cbar, int32_t* n_bins_ext, int32_t* pad_left);
 
 /* Selects the backprojection kernel: 0 = automatic (default), 1 = reference one-thread-per-
- * pixel kernel (global loads; kept for cross-checks), 2 = tiled shared-memory kernel.
- * Returns the previous value.  Test/bench hook; results agree within FP32 rounding. */
+ * pixel kernel (global loads; kept for cross-checks), 2 = tiled shared-memory kernel, 3 = run
+ * kernel with 4 slices per thread, 4 = run kernel with 8 slices per thread (what 0 picks for
+ * pixel sizes below sqrt(2) bins).  A variant that does not cover the geometry makes the next
+ * call return PYHST_ERR_UNSUPPORTED.  Returns the previous value.  Test/bench hook; results
+ * agree within FP32 rounding. */
 int pyhst_set_backproject_variant(int variant);
 
 /* Selects the forward-projection kernel: 0 = automatic (default), 1 = generic gather kernel (one
