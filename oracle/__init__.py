@@ -210,3 +210,64 @@ def fbp(sino_raw, angles, axis, nx, ny, pixel_size=1.0, filter=FILTER_RAMLAK, mo
     _check(lib.oracle_fbp(*common, None, *tail, c_int64(len(pts)), _p(ps, c_int32),
                           _p(pi, c_int32), _p(pj, c_int32), _p(out, c_double)), "fbp(points)")
     return out
+
+
+# ---- NEXT row N1: TV-regularised FISTA (eq. 1-3; readings R17-R20) ----------
+def forward_project_f64(img, angles, axis, n_bins, pixel_size=1.0, scale=1.0):
+    """img float64 [S,ny,nx] -> float64 [S,P,B]; the input is not rounded to float32."""
+    lib = _load()
+    img = _f64(img)
+    s, ny, nx = img.shape
+    angles, axis = _f64(angles), _f64(axis)
+    p = angles.shape[0]
+    sino = np.empty((s, p, n_bins), dtype=np.float64)
+    _check(lib.oracle_forward_project_f64(
+        _p(img, c_double), _p(sino, c_double), c_int32(s), c_int32(p), c_int32(n_bins),
+        _p(angles, c_double), _p(axis, c_double), c_int32(nx), c_int32(ny), c_double(pixel_size),
+        c_double(scale)), "forward_project_f64")
+    return sino
+
+
+def tv(x) -> float:
+    """Isotropic total variation (eq. 2) of a stack [S,ny,nx], summed over slices."""
+    lib = _load()
+    lib.oracle_tv.restype = c_double
+    x = _f64(x)
+    s, ny, nx = x.shape
+    return float(lib.oracle_tv(_p(x, c_double), c_int32(s), c_int32(ny), c_int32(nx)))
+
+
+def prox_tv(z, tau, n_inner):
+    """argmin_x 1/2 ||x - z||^2 + tau TV(x) per slice, n_inner dual projected-gradient steps."""
+    lib = _load()
+    z = _f64(z)
+    s, ny, nx = z.shape
+    x = np.empty_like(z)
+    _check(lib.oracle_prox_tv(_p(z, c_double), _p(x, c_double), c_int32(s), c_int32(ny), c_int32(nx),
+                              c_double(tau), c_int32(n_inner)), "prox_tv")
+    return x
+
+
+def lipschitz(angles, axis, n_bins, nx, ny, pixel_size=1.0, n_power=8) -> float:
+    """1.1 x the power-iteration estimate of lambda_max(P^T P) (R17)."""
+    lib = _load()
+    angles, axis = _f64(angles), _f64(axis)
+    out = c_double(0.0)
+    _check(lib.oracle_lipschitz(c_int32(angles.shape[0]), c_int32(n_bins), _p(angles, c_double),
+                                _p(axis, c_double), c_int32(nx), c_int32(ny), c_double(pixel_size),
+                                c_int32(n_power), ctypes.byref(out)), "lipschitz")
+    return float(out.value)
+
+
+def fista_tv(data, angles, axis, nx, ny, beta, L, n_iter, n_inner=20, pixel_size=1.0):
+    """data float32 [S,P,B] -> (x float64 [S,ny,nx], energy float64 [n_iter])."""
+    lib = _load()
+    data = _f32(data)
+    s, p, b, angles, axis = _geom(data.shape, angles, axis)
+    x = np.empty((s, ny, nx), dtype=np.float64)
+    energy = np.zeros(max(n_iter, 1), dtype=np.float64)
+    _check(lib.oracle_fista_tv(_p(data, c_float), c_int64(b), _p(x, c_double), c_int32(s), c_int32(p),
+                               c_int32(b), _p(angles, c_double), _p(axis, c_double), c_int32(nx),
+                               c_int32(ny), c_double(pixel_size), c_double(beta), c_double(L),
+                               c_int32(n_iter), c_int32(n_inner), _p(energy, c_double)), "fista_tv")
+    return x, energy[:n_iter]

@@ -24,7 +24,11 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): K1 affine rows, K2 mass /
  * first moment, K3 adjoint identity, K4 dense brute force, K5 zero extension,
  * K6 kernel sums / DFT, K7 FFT vs direct sum, K9 Gaussian blob, K10 FBP ->
- * phantom, K11 half acquisition, K12 batch independence.
+ * phantom, K11 half acquisition, K12 batch independence; for the TV-FISTA
+ * part at the end of this file (tests/test_oracle_pins_fista.py): K13 TV closed
+ * forms, K14 proximal step (limits, two-plateau closed form, optimality), K15
+ * Lipschitz constant vs dense eigenvalue, K16 first iterates vs a dense matrix
+ * and the O(1/k^2) bound, K17 energy value / regularisation / batch.
  * NOT pinned: the orientation conventions R1/R2 against PyHST2's own (no
  * reference output exists): "PyHST convention parity unpinned".
  *
@@ -356,5 +360,208 @@ int oracle_fbp(const float* sino_raw, int64_t pitch, double* img, int32_t n_slic
                                          nx, ny, h, scale, n_pts, ps, pi, pj, out);
   }
   free(axis_out); free(filt); free(wf);
+  return rc;
+}
+
+/* ============================================================================
+ * NEXT row N1: TV-regularised FISTA
+ * (sec. 3.1, eq. 1-3):  x = argmin 1/2 ||y - P x||^2 + beta TV(x),
+ * TV(x) = sum_pixels sqrt((d1 x)^2 + (d2 x)^2)  (isotropic, eq. 2), solved by
+ * FISTA (L84, ref. [18]); "the value of the energy in (3) is displayed" (L86).
+ * The paper gives neither the discrete gradient, the inner solver of the TV
+ * proximal step, the step size nor the starting point: readings R17-R20 of
+ * DESIGN.md, quoted where used.  Everything below is double precision, index
+ * order, no blocking; slices are independent (the operator is the same).
+ * Pins: tests/test_oracle_pins.py K13-K17.
+ * ========================================================================== */
+
+/* FP of a double image (same scatter as fp_row; input not rounded to float). */
+static void fp_row_f64(const double* x, double* y, int32_t n_bins, double c, double h, double ct,
+                       double st, int32_t nx, int32_t ny, double scale) {
+  const double j0 = 0.5 * (double)(nx - 1), i0 = 0.5 * (double)(ny - 1);
+  for (int32_t b = 0; b < n_bins; ++b) y[b] = 0.0;
+  for (int32_t i = 0; i < ny; ++i)
+    for (int32_t j = 0; j < nx; ++j) {
+      double t = detector_coord(c, h, ct, st, (double)j - j0, (double)i - i0);
+      double kf = floor(t);
+      double f = t - kf;
+      double v = x[(int64_t)i * nx + j];
+      if (kf >= 0.0 && kf < (double)n_bins) y[(int64_t)kf] += (1.0 - f) * v;
+      if (kf + 1.0 >= 0.0 && kf + 1.0 < (double)n_bins) y[(int64_t)kf + 1] += f * v;
+    }
+  for (int32_t b = 0; b < n_bins; ++b) y[b] *= scale;
+}
+
+int oracle_forward_project_f64(const double* img, double* sino, int32_t n_slices, int32_t n_angles,
+                               int32_t n_bins, const double* angles, const double* axis,
+                               int32_t nx, int32_t ny, double h, double scale) {
+  int rc = check_geom(n_slices, n_angles, n_bins, angles, axis, nx, ny, h);
+  if (rc || !img || !sino) return rc ? rc : ORACLE_ERR_INVALID_ARG;
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int32_t s = 0; s < n_slices; ++s)
+    for (int32_t p = 0; p < n_angles; ++p)
+      fp_row_f64(img + (int64_t)s * ny * nx, sino + ((int64_t)s * n_angles + p) * n_bins, n_bins,
+                 axis[p], h, cos(angles[p]), sin(angles[p]), nx, ny, scale);
+  return ORACLE_OK;
+}
+
+/* Discrete gradient (R18): forward differences, zero at the last column / row.
+ *   (d1 x)[i,j] = x[i,j+1] - x[i,j] (j < nx-1), (d2 x)[i,j] = x[i+1,j] - x[i,j] (i < ny-1). */
+static inline double d1_at(const double* x, int32_t nx, int32_t i, int32_t j) {
+  return j + 1 < nx ? x[(int64_t)i * nx + j + 1] - x[(int64_t)i * nx + j] : 0.0;
+}
+static inline double d2_at(const double* x, int32_t nx, int32_t ny, int32_t i, int32_t j) {
+  return i + 1 < ny ? x[(int64_t)(i + 1) * nx + j] - x[(int64_t)i * nx + j] : 0.0;
+}
+
+/* TV(x) of eq. 2, summed over all slices of the stack. */
+double oracle_tv(const double* x, int32_t n_slices, int32_t ny, int32_t nx) {
+  double tv = 0.0;
+  for (int32_t s = 0; s < n_slices; ++s) {
+    const double* xs = x + (int64_t)s * ny * nx;
+    for (int32_t i = 0; i < ny; ++i)
+      for (int32_t j = 0; j < nx; ++j) {
+        double a = d1_at(xs, nx, i, j), b = d2_at(xs, nx, ny, i, j);
+        tv += sqrt(a * a + b * b);
+      }
+  }
+  return tv;
+}
+
+/* Adjoint of the gradient: (G^T p)[i,j] = p1[i,j-1] - p1[i,j] + p2[i-1,j] - p2[i,j]
+ * with p1[i,-1] = p2[-1,j] = 0 and p1[i,nx-1] = p2[ny-1,j] = 0 (those components of
+ * the gradient are identically zero). */
+static inline double gt_at(const double* p1, const double* p2, int32_t nx, int32_t ny, int32_t i,
+                           int32_t j) {
+  double v = 0.0;
+  if (j > 0) v += p1[(int64_t)i * nx + j - 1];
+  if (j + 1 < nx) v -= p1[(int64_t)i * nx + j];
+  if (i > 0) v += p2[(int64_t)(i - 1) * nx + j];
+  if (i + 1 < ny) v -= p2[(int64_t)i * nx + j];
+  return v;
+}
+
+/* Proximal operator of tau * TV (R18):  x = argmin_x 1/2 ||x - z||^2 + tau TV(x), per slice.
+ * Dual form: x = z - tau G^T p with |p[i,j]| <= 1 (isotropic: the pair (p1, p2) of a pixel lies
+ * in the unit disc).  n_inner projected-gradient steps on the dual (Chambolle 2004), step
+ * 1 / (8 tau) (||G||^2 <= 8), started from p = 0:
+ *     u = z - tau G^T p ;  q = p + G u / (8 tau) ;  p = q / max(1, |q|).
+ * tau <= 0 or n_inner == 0 returns x = z. */
+int oracle_prox_tv(const double* z, double* x, int32_t n_slices, int32_t ny, int32_t nx, double tau,
+                   int32_t n_inner) {
+  if (!z || !x || n_slices <= 0 || ny <= 0 || nx <= 0 || n_inner < 0) return ORACLE_ERR_INVALID_ARG;
+  const int64_t n = (int64_t)ny * nx;
+  if (!(tau > 0.0) || n_inner == 0) {
+    memcpy(x, z, sizeof(double) * (size_t)(n * n_slices));
+    return ORACLE_OK;
+  }
+  int rc = ORACLE_OK;
+#pragma omp parallel for schedule(static)
+  for (int32_t s = 0; s < n_slices; ++s) {
+    const double* zs = z + s * n;
+    double* u = x + s * n; /* the output doubles as u */
+    double* p1 = (double*)calloc((size_t)(2 * n), sizeof(double));
+    if (!p1) { rc = ORACLE_ERR_NOMEM; continue; }
+    double* p2 = p1 + n;
+    for (int32_t it = 0; it <= n_inner; ++it) {
+      for (int32_t i = 0; i < ny; ++i)
+        for (int32_t j = 0; j < nx; ++j)
+          u[(int64_t)i * nx + j] = zs[(int64_t)i * nx + j] - tau * gt_at(p1, p2, nx, ny, i, j);
+      if (it == n_inner) break; /* u = z - tau G^T p of the last dual iterate is the result */
+      for (int32_t i = 0; i < ny; ++i)
+        for (int32_t j = 0; j < nx; ++j) {
+          double q1 = p1[(int64_t)i * nx + j] + d1_at(u, nx, i, j) / (8.0 * tau);
+          double q2 = p2[(int64_t)i * nx + j] + d2_at(u, nx, ny, i, j) / (8.0 * tau);
+          double m = sqrt(q1 * q1 + q2 * q2);
+          if (m < 1.0) m = 1.0;
+          p1[(int64_t)i * nx + j] = q1 / m;
+          p2[(int64_t)i * nx + j] = q2 / m;
+        }
+    }
+    free(p1);
+  }
+  return rc;
+}
+
+/* Lipschitz constant of the data term (R17): n_power iterations v <- P^T P v from v = 1 on ONE
+ * slice (the operator is the same for every slice); returns 1.1 * ||v_n|| / ||v_{n-1}||
+ * (the power iteration approaches lambda_max(P^T P) from below; FISTA needs L >= lambda_max). */
+int oracle_lipschitz(int32_t n_angles, int32_t n_bins, const double* angles, const double* axis,
+                     int32_t nx, int32_t ny, double h, int32_t n_power, double* L) {
+  int rc = check_geom(1, n_angles, n_bins, angles, axis, nx, ny, h);
+  if (rc || !L || n_power <= 0) return rc ? rc : ORACLE_ERR_INVALID_ARG;
+  const int64_t n = (int64_t)ny * nx, m = (int64_t)n_angles * n_bins;
+  double* v = (double*)malloc(sizeof(double) * (size_t)(2 * n + m));
+  if (!v) return ORACLE_ERR_NOMEM;
+  double* w = v + n;
+  double* y = w + n;
+  for (int64_t k = 0; k < n; ++k) v[k] = 1.0;
+  double ratio = 0.0;
+  for (int32_t it = 0; it < n_power && rc == ORACLE_OK; ++it) {
+    double nv = 0.0, nw = 0.0;
+    rc = oracle_forward_project_f64(v, y, 1, n_angles, n_bins, angles, axis, nx, ny, h, 1.0);
+    if (!rc) rc = oracle_backproject_f64(y, n_bins, w, 1, n_angles, n_bins, angles, axis, nx, ny, h, 1.0);
+    for (int64_t k = 0; k < n; ++k) { nv += v[k] * v[k]; nw += w[k] * w[k]; }
+    ratio = sqrt(nw) / sqrt(nv);
+    for (int64_t k = 0; k < n; ++k) v[k] = w[k] / sqrt(nw); /* normalised: no overflow */
+  }
+  *L = 1.1 * ratio;
+  free(v);
+  return rc;
+}
+
+/* FISTA for eq. 3 (Beck & Teboulle's scheme, ref. [18]; R19, R20):
+ *   x_0 = y_0 = 0, t_0 = 1;   for k = 0 .. n_iter-1:
+ *     r = P y_k - data ;  energy[k] = 1/2 ||r||^2 + beta TV(y_k)     (eq. 3 at the point where the
+ *                                                                     gradient is taken: one P, P^T
+ *                                                                     pair per iteration, R19)
+ *     z = y_k - P^T r / L                                             (gradient of eq. 9's sign, R16)
+ *     x_{k+1} = prox_{(beta/L) TV}(z)                                 (oracle_prox_tv, n_inner steps)
+ *     t_{k+1} = (1 + sqrt(1 + 4 t_k^2)) / 2 ;  y_{k+1} = x_{k+1} + (t_k - 1)/t_{k+1} (x_{k+1} - x_k)
+ * data: float32 [S][P][pitch] widened exactly; x_out = x_{n_iter} [S][ny][nx] in double; energy
+ * (nullable) [n_iter], summed over the slices of the stack. */
+int oracle_fista_tv(const float* data, int64_t pitch, double* x_out, int32_t n_slices,
+                    int32_t n_angles, int32_t n_bins, const double* angles, const double* axis,
+                    int32_t nx, int32_t ny, double h, double beta, double L, int32_t n_iter,
+                    int32_t n_inner, double* energy) {
+  int rc = check_geom(n_slices, n_angles, n_bins, angles, axis, nx, ny, h);
+  if (rc || !data || !x_out || !(L > 0.0) || !(beta >= 0.0) || n_iter < 0 || n_inner < 0)
+    return rc ? rc : ORACLE_ERR_INVALID_ARG;
+  if (pitch == 0) pitch = n_bins;
+  const int64_t n = (int64_t)n_slices * ny * nx, m = (int64_t)n_slices * n_angles * n_bins;
+  double* xk = (double*)calloc((size_t)(4 * n + m), sizeof(double));
+  if (!xk) return ORACLE_ERR_NOMEM;
+  double* yk = xk + n;
+  double* z = yk + n;
+  double* g = z + n;
+  double* r = g + n;
+  double t = 1.0;
+  for (int32_t k = 0; k < n_iter && rc == ORACLE_OK; ++k) {
+    rc = oracle_forward_project_f64(yk, r, n_slices, n_angles, n_bins, angles, axis, nx, ny, h, 1.0);
+    if (rc) break;
+    double half = 0.0;
+    for (int32_t s = 0; s < n_slices; ++s)
+      for (int32_t p = 0; p < n_angles; ++p)
+        for (int32_t b = 0; b < n_bins; ++b) {
+          int64_t o = ((int64_t)s * n_angles + p) * n_bins + b;
+          r[o] -= (double)data[((int64_t)s * n_angles + p) * pitch + b];
+          half += r[o] * r[o];
+        }
+    if (energy) energy[k] = 0.5 * half + beta * oracle_tv(yk, n_slices, ny, nx);
+    rc = oracle_backproject_f64(r, n_bins, g, n_slices, n_angles, n_bins, angles, axis, nx, ny, h, 1.0);
+    if (rc) break;
+    for (int64_t i = 0; i < n; ++i) z[i] = yk[i] - g[i] / L;
+    rc = oracle_prox_tv(z, g, n_slices, ny, nx, beta / L, n_inner); /* g := x_{k+1} */
+    if (rc) break;
+    const double tn = 0.5 * (1.0 + sqrt(1.0 + 4.0 * t * t));
+    const double mom = (t - 1.0) / tn;
+    for (int64_t i = 0; i < n; ++i) {
+      yk[i] = g[i] + mom * (g[i] - xk[i]);
+      xk[i] = g[i];
+    }
+    t = tn;
+  }
+  memcpy(x_out, xk, sizeof(double) * (size_t)n);
+  free(xk);
   return rc;
 }
