@@ -128,6 +128,26 @@ int pyhst_backproject_host(const float* h_sino, float* h_img, const pyhst_geom_t
 int pyhst_forward_project_host(const float* h_img, float* h_sino, const pyhst_geom_t* g, float scale,
                                int32_t max_slices_per_chunk, void* stream);
 
+/* NEXT row N1: TV-regularised FISTA, PAPER.md L73-L86 (sec. 3.1, eq. 1-3):
+ *     x = argmin 1/2 ||data - P x||^2 + beta TV(x),  TV = isotropic total variation (eq. 2),
+ * solved by FISTA (L84, ref. [18]) with P = pyhst_forward_project and P^T = pyhst_backproject
+ * (scale 1), one pair per iteration.  Readings R16-R20 of DESIGN.md: gradient P^T (P y - data);
+ * step 1/L with L = 1.1 x the estimate of lambda_max(P^T P) after n_power power iterations from
+ * v = 1 on one slice; TV proximal step by n_inner projected-gradient steps on the dual (forward
+ * differences, zero at the last row / column, step 1/8, dual restarted at zero every outer
+ * iteration); x0 = 0; energy[k] = eq. 3 evaluated at the point y_k where the gradient of
+ * iteration k is taken, summed over the slices of the stack.
+ *   d_data   DEVICE [n_slices][n_angles][sino_pitch] f32, read only
+ *   d_img    DEVICE [n_slices][ny][nx] f32, overwritten with x after n_iter iterations
+ *   energy   HOST [n_iter] or NULL;  lipschitz HOST scalar or NULL.  If either is given the call
+ *            copies them back and synchronises `stream` before returning; otherwise it only enqueues.
+ * Errors: null pointers, beta < 0 or not finite, n_iter < 0, n_inner < 0, n_power <= 0 ->
+ * PYHST_ERR_INVALID_ARG; no sm_100 device -> PYHST_ERR_UNSUPPORTED.  Workspace (7 image stacks +
+ * one sinogram stack) is owned by the library and freed by pyhst_release_cache(). */
+int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geom_t* g, float beta,
+                   int32_t n_iter, int32_t n_inner, int32_t n_power, double* energy,
+                   double* lipschitz, void* stream);
+
 /* Extended row length / left padding of the virtually doubled detector (R10):
  * far = max(cbar, n_bins-1-cbar); *n_bins_ext = ceil(2 far) + 1 rounded up to a multiple of
  * 64; *pad_left = 0 if the axis is right of the detector centre else n_bins_ext - n_bins. */

@@ -23,7 +23,7 @@ _LIBNAME = "libpyhst_b200.so"
 
 # every symbol include/pyhst.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
-           "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant",
+           "pyhst_fista_tv", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant",
            "pyhst_last_error", "pyhst_release_cache")
 
 
@@ -62,6 +62,8 @@ def _load():
     lib.pyhst_fbp_host.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_int, c_int, c_int32, c_void_p]
     lib.pyhst_backproject_host.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_int32, c_void_p]
     lib.pyhst_forward_project_host.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_int32, c_void_p]
+    lib.pyhst_fista_tv.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_int32, c_int32, c_int32,
+                                   POINTER(c_double), POINTER(c_double), c_void_p]
     lib.pyhst_halfacq_extent.argtypes = [c_int32, c_double, POINTER(c_int32), POINTER(c_int32)]
     lib.pyhst_set_backproject_variant.argtypes = [c_int]
     lib.pyhst_set_forward_project_variant.argtypes = [c_int]
@@ -163,6 +165,26 @@ def fbp(d_sino_raw, angles, axis, nx, ny, pixel_size=1.0, filter=FILTER_RAMLAK, 
     _check(lib.pyhst_fbp(_dev(d_sino_raw, "d_sino_raw"), _dev(out, "out"), ctypes.byref(g), filter, mode,
                          _stream(stream)), "pyhst_fbp")
     return out
+
+
+def fista_tv(d_data, angles, axis, nx, ny, beta, n_iter, n_inner=20, n_power=8, pixel_size=1.0, out=None,
+             want_energy=True, stream=None):
+    """pyhst_fista_tv: float32 CUDA data [S,P,B] -> (x [S,ny,nx] CUDA, energy float64 [n_iter], L).
+    With want_energy=False nothing is copied back and the call does not synchronise."""
+    import torch
+    lib = _load()
+    s, p, b = d_data.shape
+    if out is None:
+        out = torch.empty((s, ny, nx), dtype=torch.float32, device=d_data.device)
+    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size)
+    energy = np.zeros(max(int(n_iter), 1), dtype=np.float64)
+    lip = c_double(0.0)
+    _check(lib.pyhst_fista_tv(_dev(d_data, "d_data"), _dev(out, "out"), ctypes.byref(g), float(beta),
+                              int(n_iter), int(n_inner), int(n_power),
+                              energy.ctypes.data_as(POINTER(c_double)) if want_energy else None,
+                              ctypes.byref(lip) if want_energy else None, _stream(stream)),
+           "pyhst_fista_tv")
+    return out, energy[:int(n_iter)], float(lip.value)
 
 
 def _host_ptr(a, name):

@@ -1,0 +1,247 @@
+// TV-regularised FISTA (include/pyhst.h pyhst_fista_tv; NEXT row N1 of SURVEY.md sec. 8(f);
+// PAPER.md L73-L86, sec. 3.1, eq. 1-3; readings R16-R20 of DESIGN.md):
+//
+//   x = argmin 1/2 ||data - P x||^2 + beta TV(x),  TV(x) = sum_pixels sqrt((d1 x)^2 + (d2 x)^2)
+//
+// Every iteration calls the projector pair once (pyhst_forward_project, pyhst_backproject of this
+// library) and a handful of element-wise / 5-point-stencil kernels over the image stack:
+//   r = P y - data, 1/2 ||r||^2            ftv_residual_kernel
+//   z = y - P^T r / L, TV(y)               ftv_step_kernel
+//   n_inner dual projected-gradient steps  ftv_dual_kernel   (p ping-pongs between two buffers)
+//   x+ = z - tau G^T p, momentum           ftv_finish_kernel
+// All scalars (L, the energies) stay on the device: the loop enqueues without a host sync.
+#include <algorithm>
+#include <cmath>
+#include <vector>
+
+#include "common.h"
+
+namespace pyhst {
+
+namespace {
+
+constexpr int FT_BX = 32, FT_BY = 8;
+
+// block-wide sum of a float into a double accumulator in global memory
+__device__ __forceinline__ void block_sum_to(double v, double* dst) {
+  __shared__ double part[FT_BX * FT_BY / 32];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  const int t = threadIdx.y * blockDim.x + threadIdx.x;
+  if ((t & 31) == 0) part[t >> 5] = v;
+  __syncthreads();
+  if (t == 0) {
+    double s = 0.0;
+    for (int w = 0; w < (int)(blockDim.x * blockDim.y) / 32; ++w) s += part[w];
+    atomicAdd(dst, s);
+  }
+}
+
+// forward differences, zero at the last column / row (R18)
+__device__ __forceinline__ float d1f(const float* x, int nx, int i, int j) {
+  return j + 1 < nx ? x[(int64_t)i * nx + j + 1] - x[(int64_t)i * nx + j] : 0.f;
+}
+__device__ __forceinline__ float d2f(const float* x, int nx, int ny, int i, int j) {
+  return i + 1 < ny ? x[(int64_t)(i + 1) * nx + j] - x[(int64_t)i * nx + j] : 0.f;
+}
+// (G^T p)[i,j] = p1[i,j-1] - p1[i,j] + p2[i-1,j] - p2[i,j]; p1 of the last column and p2 of the
+// last row are identically zero (they are never made non-zero by ftv_dual_kernel)
+__device__ __forceinline__ float gtf(const float* p1, const float* p2, int nx, int ny, int i, int j) {
+  float v = 0.f;
+  if (j > 0) v += p1[(int64_t)i * nx + j - 1];
+  if (j + 1 < nx) v -= p1[(int64_t)i * nx + j];
+  if (i > 0) v += p2[(int64_t)(i - 1) * nx + j];
+  if (i + 1 < ny) v -= p2[(int64_t)i * nx + j];
+  return v;
+}
+
+// r[s,p,b] -= data[s,p,b] (r contiguous, data pitched); *half_acc += 1/2 sum r^2
+__global__ void ftv_residual_kernel(float* __restrict__ r, const float* __restrict__ data,
+                                    int64_t data_pitch, int n_bins, int64_t n_rows, double* half_acc) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  double acc = 0.0;
+  for (int64_t row = (int64_t)blockIdx.y * blockDim.y + threadIdx.y; row < n_rows;
+       row += (int64_t)gridDim.y * blockDim.y) {
+    if (b < n_bins) {
+      const float v = r[row * n_bins + b] - data[row * data_pitch + b];
+      r[row * n_bins + b] = v;
+      acc += 0.5 * (double)v * (double)v;
+    }
+  }
+  block_sum_to(acc, half_acc);
+}
+
+// z = y - g * (1/L);  *tv_acc += beta * TV(y)   (energy of eq. 3 at y, R19)
+__global__ void ftv_step_kernel(const float* __restrict__ y, const float* __restrict__ g,
+                                float* __restrict__ z, int nx, int ny, const double* L, double beta,
+                                double* tv_acc) {
+  const int j = blockIdx.x * FT_BX + threadIdx.x, i = blockIdx.y * FT_BY + threadIdx.y;
+  const int64_t o = (int64_t)blockIdx.z * ny * nx;
+  double tv = 0.0;
+  if (i < ny && j < nx) {
+    const float inv_l = (float)(1.0 / *L);
+    const int64_t k = o + (int64_t)i * nx + j;
+    z[k] = fmaf(-g[k], inv_l, y[k]);
+    const float a = d1f(y + o, nx, i, j), b = d2f(y + o, nx, ny, i, j);
+    tv = beta * (double)sqrtf(a * a + b * b);
+  }
+  if (tv_acc) block_sum_to(tv, tv_acc);
+}
+
+// one dual projected-gradient step (R18):  u = z - tau G^T p ;  q = p + G u / (8 tau) ;
+// p' = q / max(1, |q|)  -- p is read from (p1, p2) and written to (q1, q2) (Jacobi: ping-pong)
+__global__ void ftv_dual_kernel(const float* __restrict__ z, const float* __restrict__ p1,
+                                const float* __restrict__ p2, float* __restrict__ q1,
+                                float* __restrict__ q2, int nx, int ny, const double* L, double beta) {
+  const int j = blockIdx.x * FT_BX + threadIdx.x, i = blockIdx.y * FT_BY + threadIdx.y;
+  if (i >= ny || j >= nx) return;
+  const int64_t o = (int64_t)blockIdx.z * ny * nx;
+  z += o; p1 += o; p2 += o;
+  const float tau = (float)(beta / *L);
+  const float step = 1.f / (8.f * tau);
+  const int64_t k = (int64_t)i * nx + j;
+  const float u = fmaf(-tau, gtf(p1, p2, nx, ny, i, j), z[k]);
+  float a = 0.f, b = 0.f;
+  if (j + 1 < nx) a = fmaf(-tau, gtf(p1, p2, nx, ny, i, j + 1), z[k + 1]) - u;
+  if (i + 1 < ny) b = fmaf(-tau, gtf(p1, p2, nx, ny, i + 1, j), z[k + nx]) - u;
+  const float n1 = fmaf(a, step, p1[k]), n2 = fmaf(b, step, p2[k]);
+  const float m = fmaxf(1.f, sqrtf(n1 * n1 + n2 * n2));
+  q1[o + k] = n1 / m;
+  q2[o + k] = n2 / m;
+}
+
+// x+ = z - tau G^T p (tau = 0: x+ = z);  y = x+ + mom (x+ - x);  x = x+
+__global__ void ftv_finish_kernel(const float* __restrict__ z, const float* __restrict__ p1,
+                                  const float* __restrict__ p2, float* __restrict__ x,
+                                  float* __restrict__ y, int nx, int ny, const double* L, double beta,
+                                  float mom, int use_p) {
+  const int j = blockIdx.x * FT_BX + threadIdx.x, i = blockIdx.y * FT_BY + threadIdx.y;
+  if (i >= ny || j >= nx) return;
+  const int64_t o = (int64_t)blockIdx.z * ny * nx, k = o + (int64_t)i * nx + j;
+  float xn = z[k];
+  if (use_p) xn = fmaf(-(float)(beta / *L), gtf(p1 + o, p2 + o, nx, ny, i, j), xn);
+  const float xo = x[k];
+  y[k] = fmaf(mom, xn - xo, xn);
+  x[k] = xn;
+}
+
+// power iteration helpers: *acc += sum v^2 ;  v = w / sqrt(*nw), L = 1.1 sqrt(*nw / *nv)
+__global__ void ftv_sumsq_kernel(const float* __restrict__ v, int64_t n, double* acc) {
+  double s = 0.0;
+  for (int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.y * 32 + threadIdx.x; k < n;
+       k += (int64_t)gridDim.x * 256)
+    s += (double)v[k] * (double)v[k];
+  block_sum_to(s, acc);
+}
+__global__ void ftv_normalise_kernel(const float* __restrict__ w, float* __restrict__ v, int64_t n,
+                                     const double* nv, const double* nw, double* L) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const double s = sqrt(*nw);
+  if (k < n) v[k] = (float)((double)w[k] / s);
+  if (k == 0) *L = 1.1 * s / sqrt(*nv);
+}
+__global__ void ftv_fill_kernel(float* v, int64_t n, float value) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < n) v[k] = value;
+}
+
+}  // namespace
+
+}  // namespace pyhst
+
+using namespace pyhst;
+
+extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geom_t* g, float beta,
+                              int32_t n_iter, int32_t n_inner, int32_t n_power, double* energy,
+                              double* lipschitz, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!d_data || !d_img || !g)
+    return set_error(PYHST_ERR_INVALID_ARG, "pyhst_fista_tv: null pointer");
+  if (!(beta >= 0.f) || n_iter < 0 || n_inner < 0 || n_power <= 0 || n_iter > (1 << 20))
+    return set_error(PYHST_ERR_INVALID_ARG,
+                     "pyhst_fista_tv: beta %g, n_iter %d, n_inner %d, n_power %d", (double)beta,
+                     n_iter, n_inner, n_power);
+  if (g->n_slices <= 0 || g->n_angles <= 0 || g->n_bins <= 0 || g->nx <= 0 || g->ny <= 0)
+    return set_error(PYHST_ERR_INVALID_ARG, "pyhst_fista_tv: non-positive size");
+  PYHST_TRY(require_sm100(nullptr));
+  const int S = g->n_slices, nx = g->nx, ny = g->ny;
+  const int64_t n_img = (int64_t)S * ny * nx, n1 = (int64_t)ny * nx;
+  const int64_t n_rows = (int64_t)S * g->n_angles, n_sino = n_rows * g->n_bins;
+  const int64_t data_pitch = g->sino_pitch ? g->sino_pitch : g->n_bins;
+  if ((S + 0) > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "pyhst_fista_tv: more than 65535 slices");
+
+  // workspace: y, z, grad, 4 dual stacks, residual sinogram, scalars (nv, nw, L, energy[n_iter])
+  const size_t img_bytes = ((size_t)n_img * 4 + 255) & ~(size_t)255;
+  const size_t sino_bytes = ((size_t)n_sino * 4 + 255) & ~(size_t)255;
+  const size_t sc_bytes = (size_t)(3 + n_iter) * 8;
+  void* ws = nullptr;
+  PYHST_TRY(get_workspace(WS_FISTA, 7 * img_bytes + sino_bytes + sc_bytes, &ws));
+  char* base = static_cast<char*>(ws);
+  float* y = reinterpret_cast<float*>(base);
+  float* z = reinterpret_cast<float*>(base + img_bytes);
+  float* gr = reinterpret_cast<float*>(base + 2 * img_bytes);
+  float* p[4];
+  for (int k = 0; k < 4; ++k) p[k] = reinterpret_cast<float*>(base + (3 + k) * img_bytes);
+  float* r = reinterpret_cast<float*>(base + 7 * img_bytes);
+  double* sc = reinterpret_cast<double*>(base + 7 * img_bytes + sino_bytes);
+  double *d_nv = sc, *d_nw = sc + 1, *d_L = sc + 2, *d_e = sc + 3;
+
+  pyhst_geom_t g1 = *g, gs = *g;
+  g1.n_slices = 1;
+  g1.sino_pitch = 0;
+  gs.sino_pitch = 0;
+  const dim3 blk(FT_BX, FT_BY, 1);
+  const dim3 grid_img((nx + FT_BX - 1) / FT_BX, (ny + FT_BY - 1) / FT_BY, S);
+  const unsigned red_blocks = 148 * 4;
+
+  // ---- L = 1.1 ||P^T P v|| / ||v|| after n_power iterations from v = 1, one slice (R17)
+  PYHST_CUDA_TRY(cudaMemsetAsync(sc, 0, sc_bytes, stream));
+  ftv_fill_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, stream>>>(y, n1, 1.f);
+  for (int it = 0; it < n_power; ++it) {
+    PYHST_CUDA_TRY(cudaMemsetAsync(sc, 0, 16, stream));
+    ftv_sumsq_kernel<<<red_blocks, blk, 0, stream>>>(y, n1, d_nv);
+    PYHST_TRY(pyhst_forward_project(y, r, &g1, 1.f, stream));
+    PYHST_TRY(pyhst_backproject(r, gr, &g1, 1.f, stream));
+    ftv_sumsq_kernel<<<red_blocks, blk, 0, stream>>>(gr, n1, d_nw);
+    ftv_normalise_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, stream>>>(gr, y, n1, d_nv, d_nw, d_L);
+  }
+  PYHST_CUDA_TRY(cudaGetLastError());
+
+  // ---- FISTA (R19, R20): x0 = y0 = 0, t0 = 1
+  PYHST_CUDA_TRY(cudaMemsetAsync(d_img, 0, (size_t)n_img * 4, stream));
+  PYHST_CUDA_TRY(cudaMemsetAsync(y, 0, (size_t)n_img * 4, stream));
+  const bool use_p = beta > 0.f && n_inner > 0;
+  double t = 1.0;
+  for (int k = 0; k < n_iter; ++k) {
+    PYHST_TRY(pyhst_forward_project(y, r, &gs, 1.f, stream));
+    {
+      dim3 grid((g->n_bins + FT_BX - 1) / FT_BX, (unsigned)std::min<int64_t>((n_rows + FT_BY - 1) / FT_BY, 4096), 1);
+      ftv_residual_kernel<<<grid, blk, 0, stream>>>(r, d_data, data_pitch, g->n_bins, n_rows, d_e + k);
+    }
+    PYHST_TRY(pyhst_backproject(r, gr, &gs, 1.f, stream));
+    ftv_step_kernel<<<grid_img, blk, 0, stream>>>(y, gr, z, nx, ny, d_L, (double)beta, d_e + k);
+    int cur = 0;
+    if (use_p) {
+      PYHST_CUDA_TRY(cudaMemsetAsync(p[0], 0, 2 * img_bytes, stream));  // p[0], p[1] are adjacent
+      for (int it = 0; it < n_inner; ++it) {
+        ftv_dual_kernel<<<grid_img, blk, 0, stream>>>(z, p[cur], p[cur + 1], p[2 - cur], p[3 - cur], nx,
+                                                      ny, d_L, (double)beta);
+        cur = 2 - cur;
+      }
+    }
+    const double tn = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
+    ftv_finish_kernel<<<grid_img, blk, 0, stream>>>(z, p[cur], p[cur + 1], d_img, y, nx, ny, d_L,
+                                                    (double)beta, (float)((t - 1.0) / tn), use_p ? 1 : 0);
+    t = tn;
+    PYHST_CUDA_TRY(cudaGetLastError());
+  }
+  if (energy || lipschitz) {
+    std::vector<double> h((size_t)(3 + n_iter));
+    PYHST_CUDA_TRY(cudaMemcpyAsync(h.data(), sc, sc_bytes, cudaMemcpyDeviceToHost, stream));
+    PYHST_CUDA_TRY(cudaStreamSynchronize(stream));
+    if (lipschitz) *lipschitz = h[2];
+    if (energy)
+      for (int k = 0; k < n_iter; ++k) energy[k] = h[(size_t)3 + k];
+  }
+  return PYHST_OK;
+}

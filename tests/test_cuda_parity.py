@@ -287,3 +287,43 @@ def test_invalid_arguments_are_rejected(lib):
     with pytest.raises(lib.PyhstError):
         lib.backproject(sino, w.angles, w.axis, 16, 16, pixel_size=-1.0, out=out)
     assert (out == 5.0).all()          # nothing written on error
+
+
+# ------------------------------------------------------------------------------ N1: TV-FISTA
+# FP32 iterates drift from the double oracle as rounding accumulates through the iterations
+# (SURVEY.md sec. 8(f) N1): energy within 1e-4 relative, image within 1e-3 relative L2.
+FISTA_REL_ENERGY = 1e-4
+FISTA_REL_L2 = 1e-3
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("beta,n_iter,n_inner", [(0.0, 12, 0), (0.5, 15, 20), (3.0, 10, 7)])
+def test_fista_tv_matches_oracle(lib, oracle, beta, n_iter, n_inner):
+    w = lib.workloads.config(4, shrink=8, n_slices=3)          # 128^2, 25 projections x 128 bins
+    data = w.sinogram()
+    L_want = oracle.lipschitz(w.angles, w.axis, w.n_bins, w.nx, w.ny, n_power=8)
+    want, e_want = oracle.fista_tv(data, w.angles, w.axis, w.nx, w.ny, beta, L_want, n_iter, n_inner=n_inner)
+    got, e_got, L_got = lib.fista_tv(_dev(data), w.angles, w.axis, w.nx, w.ny, beta, n_iter, n_inner=n_inner,
+                                     n_power=8)
+    assert abs(L_got - L_want) <= 1e-5 * L_want
+    np.testing.assert_allclose(e_got, e_want, rtol=FISTA_REL_ENERGY)
+    assert_parity(got.cpu().numpy(), want, "fista_tv beta=%g" % beta, rel=FISTA_REL_L2, mabs=5e-3)
+
+
+@pytest.mark.gpu
+def test_fista_tv_ragged_shapes_and_arguments(lib, oracle):
+    wl = lib.workloads
+    w = wl.custom(2, 21, 75, 50, 37, pixel_size=1.0, axis=None, drift=0.5, jitter_angles=0.01, seed=5)
+    data = wl.random_sinogram(2, 21, 75, seed=3)
+    L = oracle.lipschitz(w.angles, w.axis, 75, 50, 37, n_power=5)
+    want, e_want = oracle.fista_tv(data, w.angles, w.axis, 50, 37, 0.2, L, 6, n_inner=5)
+    got, e_got, L_got = lib.fista_tv(_dev(data), w.angles, w.axis, 50, 37, 0.2, 6, n_inner=5, n_power=5)
+    np.testing.assert_allclose(e_got, e_want, rtol=FISTA_REL_ENERGY)
+    assert_parity(got.cpu().numpy(), want, "fista_tv ragged", rel=FISTA_REL_L2, mabs=5e-3)
+    # n_iter = 0: x = 0, nothing else touched
+    got0, e0, _ = lib.fista_tv(_dev(data), w.angles, w.axis, 50, 37, 0.2, 0)
+    assert e0.size == 0 and float(got0.abs().max()) == 0.0
+    with pytest.raises(lib.binding.PyhstError):
+        lib.fista_tv(_dev(data), w.angles, w.axis, 50, 37, -1.0, 3)
+    with pytest.raises(lib.binding.PyhstError):
+        lib.fista_tv(_dev(data), w.angles, w.axis, 50, 37, 0.1, 3, n_power=0)
