@@ -152,7 +152,19 @@ def run_b200(args):
     proj = torch.empty((S, NP, B), dtype=torch.float32, device="cuda")
     updates = S * nx * ny * NP                      # per projector call, per GPU
 
+    fista = w.cfg == 4 and not args.no_fista
+    if fista:
+        # BASELINE.json configs[3]: TV-regularised FISTA, lambda = 0.01, 100 iterations, one projector
+        # pair per iteration (pyhst_fista_tv, NEXT row N1); a step = one whole reconstruction
+        n_fista = 100
+        updates *= n_fista
+        args.no_e2e = True                          # the device-resident solver has no host entry point
+
     def step():
+        if fista:
+            P.fista_tv(sino, w.angles, w.axis, nx, ny, 0.01, n_fista, n_inner=20, n_power=8,
+                       pixel_size=w.pixel_size, out=img, want_energy=False)
+            return
         P.fbp(sino, w.angles, w.axis, nx, ny, w.pixel_size, filter=w.filter, mode=w.mode, out=img)
         P.forward_project(img, w.angles, w.axis, B, w.pixel_size, out=proj)
 
@@ -261,7 +273,9 @@ def run_b200(args):
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "impl": "b200",
-        "config": _config_dict(w, world),
+        "config": _config_dict(w, world, {"step": "pyhst_fista_tv: 100 FISTA iterations (lambda 0.01, 20 dual "
+                                          "steps each), one forward/back projector pair per iteration; "
+                                          "updates counted for the 200 projector calls only"} if fista else None),
         "metrics": {"backprojection_gups": updates * world / (ms_bp * 1e-3) / 1e9 if ms_bp else None,
                     "forward_projection_gups": updates * world / (ms_fp * 1e-3) / 1e9 if ms_fp else None,
                     "fbp_slices_per_s": S * world / ((ms_filter + ms_bp) * 1e-3) if ms_bp else None,
@@ -360,6 +374,8 @@ def main():
     ap.add_argument("--cpu-slices", type=int, default=1, help="slices in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-fista", action="store_true",
+                    help="config 4: time FBP + forward projection instead of the 100-iteration TV-FISTA")
     ap.add_argument("--warmup-ref", type=int, default=0)
     ap.add_argument("--max-ref-steps", type=int, default=2)
     args = ap.parse_args()

@@ -327,3 +327,34 @@ def test_fista_tv_ragged_shapes_and_arguments(lib, oracle):
         lib.fista_tv(_dev(data), w.angles, w.axis, 50, 37, -1.0, 3)
     with pytest.raises(lib.binding.PyhstError):
         lib.fista_tv(_dev(data), w.angles, w.axis, 50, 37, 0.1, 3, n_power=0)
+
+
+@pytest.mark.gpu
+def test_fista_tv_config4_full_size(lib, oracle):
+    """BASELINE.json configs[3] at full size (8 x 1024^2, 200 x 1024) in the launch configuration
+    bench.py --config 4 times: the first iterations against the oracle on one slice (the oracle
+    needs seconds per projector pair), the 100-iteration run via properties that hold at any size."""
+    w = lib.workloads.config(4)
+    data = w.sinogram()
+    d_data = _dev(data)
+    s0 = 3
+    L_want = oracle.lipschitz(w.angles, w.axis, w.n_bins, w.nx, w.ny, n_power=8)
+    want, e_want = oracle.fista_tv(data[s0:s0 + 1], w.angles, w.axis, w.nx, w.ny, 0.01, L_want, 2, n_inner=3)
+    got, _, L_got = lib.fista_tv(d_data, w.angles, w.axis, w.nx, w.ny, 0.01, 2, n_inner=3, n_power=8)
+    assert abs(L_got - L_want) <= 1e-5 * L_want
+    assert_parity(got[s0:s0 + 1].cpu().numpy(), want, "fista_tv config 4, 2 iterations", rel=FISTA_REL_L2,
+                  mabs=5e-3)
+    _, e1, _ = lib.fista_tv(d_data[s0:s0 + 1].contiguous(), w.angles, w.axis, w.nx, w.ny, 0.01, 2, n_inner=3)
+    np.testing.assert_allclose(e1, e_want, rtol=FISTA_REL_ENERGY)
+    # 100 iterations, lambda = 0.01, 20 dual steps (the bench configuration)
+    x, e, _ = lib.fista_tv(d_data, w.angles, w.axis, w.nx, w.ny, 0.01, 100, n_inner=20, n_power=8)
+    x = x.cpu().numpy()
+    assert np.isfinite(x).all() and np.isfinite(e).all()
+    half = 0.5 * float(np.sum(data.astype(np.float64) ** 2))
+    assert e[0] == pytest.approx(half, rel=1e-6)              # y0 = 0: eq. 3 = 1/2 ||data||^2
+    assert e[-1] < 1e-3 * e[0] and e[-1] <= e[10] <= e[1]     # FISTA is not monotone, but it descends
+    # the reconstruction explains the data: P x close to data (relative residual of the noisy scan)
+    px = lib.forward_project(_dev(x), w.angles, w.axis, w.n_bins).cpu().numpy()
+    rel = np.linalg.norm((px - data).ravel()) / np.linalg.norm(data.ravel())
+    assert rel < 0.05
+    assert 2.0 * e[-1] >= (rel * np.linalg.norm(data.ravel())) ** 2 * 0.5   # energy >= its data term (y_99 ~ x)
