@@ -89,7 +89,7 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
 
 // Grow-only device workspace slots owned by the library (freed by pyhst_release_cache).
 enum WorkspaceSlot { WS_QI = 0, WS_FFT = 1, WS_WEIGHTS = 2, WS_IMG_T = 3, WS_ROWS = 4,
-                     WS_CHUNKS = 5, WS_XI = 6, WS_FISTA = 7, WS_COUNT = 8 };
+                     WS_CHUNKS = 5, WS_XI = 6, WS_FISTA = 7, WS_FPL = 8, WS_COUNT = 9 };
 int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr);
 
 // ---- interleaved sinogram layout consumed by the tiled backprojector ---------------------
@@ -173,7 +173,8 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
 void release_fp_plans();
 int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pitch,
                                   const pyhst_geom_t* g, float scale, const FpPlan& plan,
-                                  cudaStream_t stream);
+                                  bool interval, cudaStream_t stream);
+int forward_project_interval_candidates(double pixel_size);
 
 struct FpArgs {
   const float* d_img;    // [S][ny][nx]

@@ -272,6 +272,195 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Interval form of the banded gather (variant 3; measured alternative, NOT the default).
+//
+// fp_band_kernel above loads, for every (bin, line), the up to NC = 3 pixels inside the 2-bin-wide
+// hat of the bin -- three LDS.128 per 4 slices, and the kernel is bound by shared-memory
+// wavefronts.  Here a thread owns the unit INTERVAL [b-1, b) of the detector axis instead: on a
+// line at most NCI = ceil(1/|cu|) pixels have their coordinate t in it, each is loaded once and
+// used twice: with weight f = t - (b-1) for bin b (accumulator U, the thread's own bin) and with
+// 1 - f for bin b-1 (accumulator L, the neighbour's).  Two loads and four FFMA-quads per
+// (interval, line) instead of three and three.  A second kernel adds L of interval b+1 to U of
+// interval b (fp_ivl_combine_kernel).
+// Measured on config 2 (r01c): shared-memory wavefronts drop from 0.90 to 0.46 per clk per SM, but the
+// two boundary evaluations, the membership masks and the second accumulator set raise the count to
+// 60 warp instructions per (interval, line) against 43 for fp_band_kernel; the kernel becomes issue-
+// bound (80 %) and takes 67.5 ms against 49.7 ms.  Kept selectable for the next step (8 slices per
+// thread would halve the per-line overhead; it needs the two windows to fit in shared memory).
+// Which pixels belong to an interval must be decided identically by the two threads that share a
+// boundary, or a pixel at t ~ b would be counted twice or not at all: both evaluate the SAME
+// expression for the boundary -- the position u*(b, v) of t = b on the line, in double per
+// (thread, band), split into an integer (exact) and a float fraction independent of the window
+// origin, then fmaf(s, r, fraction) per line -- so the pixel sets [ceil(u*(b-1)), ceil(u*(b))) are
+// an exact partition of the line whatever the rounding.  The weights use the continuous f (a
+// pixel assigned to the "wrong" side of a boundary by rounding gets f = 1 + eps or -eps: the two
+// contributions still add up to the pixel value placed at the right coordinate).
+// For cu < 0 the line is walked in the mirrored coordinate -u, so that t always grows with it.
+// ------------------------------------------------------------------------------------------
+constexpr int IV_NB = 64;     // intervals per block: 4 warps x 16, the other 4 warps take projections 8..15
+constexpr int IV_PAIRS = IV_NB * FB_NPJ / FB_NT;   // (interval, projection) pairs per thread = 4
+
+template <int NCI>
+__global__ void __launch_bounds__(FB_NT, 3)
+fp_ivl_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_cols, XiDims dr,
+              XiDims dc, float* __restrict__ out_u, int64_t pitch_u, float* __restrict__ out_l,
+              int64_t pitch_l, int S, int P, int B, float scale, const FpProjD* __restrict__ projs,
+              const FpChunk* __restrict__ chunks, int W) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);        // [2]
+  int* sorigin = reinterpret_cast<int*>(smem + 16);          // [2]
+  FpProjD* sproj = reinterpret_cast<FpProjD*>(smem + 64);    // [FB_NPJ]
+  float4* buf = reinterpret_cast<float4*>(smem + FB_HDR);    // [2][FB_RB][W]
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const FpChunk ck = chunks[blockIdx.y];
+  const int g = blockIdx.z;
+  const int b0 = blockIdx.x * IV_NB;                         // interval b = [b-1, b), b in [b0, b0 + NB)
+  const XiDims d = ck.cls ? dc : dr;
+  const int64_t line_f4 = (int64_t)d.nu + 2 * d.zpad;
+  const float4* xi = (ck.cls ? xi_cols : xi_rows) + (int64_t)g * d.nv * line_f4;
+  const int n_bands = (d.nv + FB_RB - 1) / FB_RB;
+  const uint32_t row_bytes = (uint32_t)W * 16u;
+
+  if (tid < ck.count) sproj[tid] = projs[ck.first + tid];
+  if (tid == 0) {
+    mbar_init(&full[0], FB_RB);
+    mbar_init(&full[1], FB_RB);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  // warp 0: window origin of band k (the intervals lie inside the hats of bins b0-1 .. b0+NB-1),
+  // then one bulk copy per line of the band
+  auto produce = [&](int k) {
+    const int vb = k * FB_RB;
+    const int rows = min(FB_RB, d.nv - vb);
+    double lo = 1e300;
+    if (lane < ck.count) {
+      const FpProjD pj = sproj[lane];
+      const double ua = fma((double)(b0 - 1), pj.inv_cu, pj.k0);
+      const double ub = fma((double)(b0 + IV_NB - 1), pj.inv_cu, pj.k0);
+      const double va = pj.sD * (double)vb, vz = pj.sD * (double)(vb + rows - 1);
+      lo = fmin(fmin(ua, ub) + fmin(va, vz), lo) - (double)pj.hw;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    double of = floor(lo) - 1.0;
+    of = fmax(of, -(double)d.zpad);
+    of = fmin(of, (double)(d.nu + d.zpad - W));
+    const int origin = (int)of;
+    uint64_t* bar = &full[k & 1];
+    if (lane == 0) sorigin[k & 1] = origin;
+    if (lane < FB_RB) {
+      if (lane < rows) {
+        mbar_arrive_expect_tx(bar, row_bytes);
+        bulk_g2s(buf + ((k & 1) * FB_RB + lane) * W,
+                 xi + (int64_t)(vb + lane) * line_f4 + (origin + d.zpad), row_bytes, bar);
+      } else {
+        mbar_arrive(bar);
+      }
+    }
+  };
+
+  if (tid < 32) produce(0);
+
+  float accu[IV_PAIRS][4], accl[IV_PAIRS][4];
+#pragma unroll
+  for (int m = 0; m < IV_PAIRS; ++m)
+#pragma unroll
+    for (int sl = 0; sl < 4; ++sl) accu[m][sl] = accl[m][sl] = 0.f;
+
+  // lane pairs hold the same interval of two neighbouring projections (see fp_band_kernel)
+  const int bl = (warp & 3) * 16 + (lane >> 1);
+  const int pj0 = (lane & 1) + 8 * (warp >> 2);
+  const double bd = (double)(b0 + bl);
+
+  for (int k = 0; k < n_bands; ++k) {
+    __syncthreads();  // everyone is done with band k-1: its stage may be overwritten
+    if (k + 1 < n_bands && tid < 32) produce(k + 1);
+    mbar_wait(&full[k & 1], (uint32_t)((k >> 1) & 1));
+    const int origin = sorigin[k & 1];
+    const int vb = k * FB_RB;
+    const int rows = min(FB_RB, d.nv - vb);
+    const float4* stage = buf + (k & 1) * FB_RB * W;
+#pragma unroll
+    for (int m = 0; m < IV_PAIRS; ++m) {
+      const int pj = pj0 + 2 * m;
+      if (pj >= ck.count) break;
+      const FpProjD* sp = &sproj[pj];
+      const double inv_cu = sp->inv_cu, k0 = sp->k0, sD = sp->sD;
+      const double sigma = inv_cu >= 0.0 ? 1.0 : -1.0;
+      const int sg = inv_cu >= 0.0 ? 1 : -1;
+      // boundaries t = b-1 and t = b on the band's first line, mirrored pixel coordinate (double);
+      // the neighbour's thread evaluates the shared boundary with the identical expression
+      const double As = sigma * fma(sD, (double)vb, fma(bd - 1.0, inv_cu, k0));
+      const double Ae = sigma * fma(sD, (double)vb, fma(bd, inv_cu, k0));
+      const double aiS = rint(As), aiE = rint(Ae);
+      const float afrS = (float)(As - aiS), afrE = (float)(Ae - aiE);
+      const int dn = (int)(aiE - aiS);
+      const int base_m = sg * (int)aiS - origin;      // window index of mirrored pixel aiS
+      const float ss = (float)(sigma * sD), cuabs = sp->cuabs;
+      const int m_lo = sg > 0 ? 0 : NCI - 1, m_hi = sg > 0 ? W - NCI : W - 1;
+#pragma unroll 2
+      for (int r = 0; r < rows; ++r) {
+        const float rf = (float)r;
+        // ceil by a round-up add of 1.5 * 2^23, integer part read from the mantissa
+        const float dS = fmaf(ss, rf, afrS), dE = fmaf(ss, rf, afrE);
+        const float jmS = __fadd_ru(dS, 12582912.f), jmE = __fadd_ru(dE, 12582912.f);
+        const int kS = __float_as_int(jmS) - 0x4b400000;
+        const int n = dn + (__float_as_int(jmE) - __float_as_int(jmS));   // pixels in the interval
+        const float f0 = cuabs * ((jmS - 12582912.f) - dS);                // t - (b-1) of the first one
+        int idx = base_m + sg * kS;
+        idx = min(max(idx, m_lo), m_hi);              // only acts where the interval is off the image
+        const float4* wp = stage + r * W + idx;
+#pragma unroll
+        for (int c = 0; c < NCI; ++c) {
+          const float f = fmaf((float)c, cuabs, f0);
+          const bool in = c < n;
+          const float wu = in ? f : 0.f, wl = in ? 1.f - f : 0.f;
+          const float4 v = wp[sg * c];
+          accu[m][0] = fmaf(wu, v.x, accu[m][0]);
+          accu[m][1] = fmaf(wu, v.y, accu[m][1]);
+          accu[m][2] = fmaf(wu, v.z, accu[m][2]);
+          accu[m][3] = fmaf(wu, v.w, accu[m][3]);
+          accl[m][0] = fmaf(wl, v.x, accl[m][0]);
+          accl[m][1] = fmaf(wl, v.y, accl[m][1]);
+          accl[m][2] = fmaf(wl, v.z, accl[m][2]);
+          accl[m][3] = fmaf(wl, v.w, accl[m][3]);
+        }
+      }
+    }
+  }
+
+  // U of interval b is bin b's share, L is bin b-1's (stored at index b of out_l, b in [0, B])
+  const int b = b0 + bl;
+  if (b <= B) {
+#pragma unroll
+    for (int m = 0; m < IV_PAIRS; ++m) {
+      const int pj = pj0 + 2 * m;
+      if (pj >= ck.count) break;
+      const int p = sproj[pj].p;
+#pragma unroll
+      for (int sl = 0; sl < 4; ++sl) {
+        const int s = g * 4 + sl;
+        if (s < S) {
+          if (b < B) out_u[((int64_t)s * P + p) * pitch_u + b] = scale * accu[m][sl];
+          out_l[((int64_t)s * P + p) * pitch_l + b] = scale * accl[m][sl];
+        }
+      }
+    }
+  }
+}
+
+// y[row][b] += l[row][b + 1], b in [0, B)
+__global__ void fp_ivl_combine_kernel(float* __restrict__ y, int64_t pitch_y, const float* __restrict__ l,
+                                      int64_t pitch_l, int B, int64_t n_rows) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t row = blockIdx.y + (int64_t)blockIdx.z * gridDim.y;
+  if (b < B && row < n_rows) y[row * pitch_y + b] += l[row * pitch_l + b + 1];
+}
+
 // [S][ny][nx] -> XI rows copy [g][ny][zr + nx + zr] and XI columns copy [g][nx][zc + ny + zc]
 __global__ void repack_image_kernel(const float* __restrict__ img, int S, int ny, int nx,
                                     float4* __restrict__ xi_rows, int zr, float4* __restrict__ xi_cols,
@@ -442,9 +631,14 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
   return plan->n_chunks <= 65535;
 }
 
+// pixels that can fall into one unit interval of the detector axis on a line: floor(sqrt2/h) + 1
+int forward_project_interval_candidates(double pixel_size) {
+  return (int)std::floor(std::sqrt(2.0) / pixel_size) + 1;
+}
+
 int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pitch,
                                   const pyhst_geom_t* g, float scale, const FpPlan& plan,
-                                  cudaStream_t stream) {
+                                  bool interval, cudaStream_t stream) {
   const int n_groups = (g->n_slices + 3) / 4;
   const int W = plan.W;
   XiLayout Lr{n_groups, g->ny, g->nx, W}, Lc{n_groups, g->nx, g->ny, W};
@@ -473,6 +667,35 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
     PYHST_CUDA_TRY(cudaGetLastError());
   }
   const size_t smem = FB_HDR + (size_t)2 * FB_RB * W * 16;
+  const XiDims dr{g->ny, g->nx, W}, dc{g->nx, g->ny, W};
+  const int nci = forward_project_interval_candidates(g->pixel_size);
+  if (interval && (nci == 2 || nci == 3)) {
+    // interval kernel: U -> d_sino, L -> workspace [S P][B + 1 pitched]; then d_sino[b] += L[b + 1]
+    const int64_t n_rows = (int64_t)g->n_slices * g->n_angles;
+    const int64_t pitch_l = ((int64_t)g->n_bins + 1 + 3) & ~(int64_t)3;
+    void* wl = nullptr;
+    PYHST_TRY(get_workspace(WS_FPL, (size_t)n_rows * pitch_l * 4, &wl));
+    static size_t configured_i[2] = {0, 0};
+    auto kern_i = nci == 2 ? fp_ivl_kernel<2> : fp_ivl_kernel<3>;
+    if (smem > configured_i[nci - 2]) {
+      PYHST_CUDA_TRY(cudaFuncSetAttribute(kern_i, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      configured_i[nci - 2] = smem;
+    }
+    dim3 grid((g->n_bins + 1 + IV_NB - 1) / IV_NB, plan.n_chunks, n_groups);
+    if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
+    StageScope scope(ST_FORWARD, stream);
+    scope.kernels(2);
+    kern_i<<<grid, FB_NT, smem, stream>>>(xi_r, xi_c, dr, dc, d_sino, pitch, static_cast<float*>(wl), pitch_l,
+                                          g->n_slices, g->n_angles, g->n_bins, scale, plan.d_projs,
+                                          plan.d_chunks, W);
+    PYHST_CUDA_TRY(cudaGetLastError());
+    const unsigned gy = (unsigned)std::min<int64_t>(n_rows, 32768);
+    dim3 grid_c((g->n_bins + 255) / 256, gy, (unsigned)((n_rows + gy - 1) / gy));
+    fp_ivl_combine_kernel<<<grid_c, 256, 0, stream>>>(d_sino, pitch, static_cast<const float*>(wl), pitch_l,
+                                                      g->n_bins, n_rows);
+    PYHST_CUDA_TRY(cudaGetLastError());
+    return PYHST_OK;
+  }
   static size_t configured[3] = {0, 0, 0};
   const int vi = plan.nc == 3 ? 0 : (plan.nc == 4 ? 1 : 2);
   auto kern = plan.nc == 3 ? fp_band_kernel<3> : (plan.nc == 4 ? fp_band_kernel<4> : fp_band_kernel<6>);
@@ -484,7 +707,6 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
   if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
   StageScope scope(ST_FORWARD, stream);
   scope.kernels();
-  const XiDims dr{g->ny, g->nx, W}, dc{g->nx, g->ny, W};
   kern<<<grid, FB_NT, smem, stream>>>(xi_r, xi_c, dr, dc, d_sino, pitch, g->n_slices, g->n_angles,
                                       g->n_bins, scale, plan.d_projs, plan.d_chunks, W);
   PYHST_CUDA_TRY(cudaGetLastError());
