@@ -193,7 +193,7 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out) 
   const size_t n = (size_t)g->n_angles;
   for (auto& pl : g_fp_plans) {
     if (pl.n_angles == g->n_angles && pl.n_bins == g->n_bins && pl.nx == g->nx && pl.ny == g->ny &&
-        pl.pixel_size == g->pixel_size &&
+        pl.n_groups == (g->n_slices + 3) / 4 && pl.pixel_size == g->pixel_size &&
         std::memcmp(pl.angles.data(), g->angles_rad, n * sizeof(double)) == 0 &&
         std::memcmp(pl.axis.data(), g->axis_pos, n * sizeof(double)) == 0) {
       pl.last_use = ++g_tick;
@@ -214,6 +214,7 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out) 
   pl.n_bins = g->n_bins;
   pl.nx = g->nx;
   pl.ny = g->ny;
+  pl.n_groups = (g->n_slices + 3) / 4;
   pl.pixel_size = g->pixel_size;
   pl.angles.assign(g->angles_rad, g->angles_rad + n);
   pl.axis.assign(g->axis_pos, g->axis_pos + n);

@@ -156,7 +156,7 @@ struct FpChunk {
 };
 struct FpPlan {
   // key
-  int32_t n_angles = 0, n_bins = 0, nx = 0, ny = 0;
+  int32_t n_angles = 0, n_bins = 0, nx = 0, ny = 0, n_groups = 0;
   double pixel_size = 0;
   std::vector<double> angles, axis;
   // product

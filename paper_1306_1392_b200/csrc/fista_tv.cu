@@ -93,17 +93,25 @@ __global__ void ftv_step_kernel(const float* __restrict__ y, const float* __rest
 __global__ void ftv_dual_kernel(const float* __restrict__ z, const float* __restrict__ p1,
                                 const float* __restrict__ p2, float* __restrict__ q1,
                                 float* __restrict__ q2, int nx, int ny, const double* L, double beta) {
-  const int j = blockIdx.x * FT_BX + threadIdx.x, i = blockIdx.y * FT_BY + threadIdx.y;
-  if (i >= ny || j >= nx) return;
+  // u = z - tau G^T p of the block's tile plus one column / row of halo, through shared memory
+  __shared__ float su[FT_BY + 1][FT_BX + 1];
+  const int j0 = blockIdx.x * FT_BX, i0 = blockIdx.y * FT_BY;
   const int64_t o = (int64_t)blockIdx.z * ny * nx;
   z += o; p1 += o; p2 += o;
   const float tau = (float)(beta / *L);
   const float step = 1.f / (8.f * tau);
+  for (int e = threadIdx.y * FT_BX + threadIdx.x; e < (FT_BY + 1) * (FT_BX + 1); e += FT_BX * FT_BY) {
+    const int ii = e / (FT_BX + 1), jj = e - ii * (FT_BX + 1);
+    const int i = i0 + ii, j = j0 + jj;
+    su[ii][jj] = (i < ny && j < nx) ? fmaf(-tau, gtf(p1, p2, nx, ny, i, j), z[(int64_t)i * nx + j]) : 0.f;
+  }
+  __syncthreads();
+  const int j = j0 + threadIdx.x, i = i0 + threadIdx.y;
+  if (i >= ny || j >= nx) return;
   const int64_t k = (int64_t)i * nx + j;
-  const float u = fmaf(-tau, gtf(p1, p2, nx, ny, i, j), z[k]);
-  float a = 0.f, b = 0.f;
-  if (j + 1 < nx) a = fmaf(-tau, gtf(p1, p2, nx, ny, i, j + 1), z[k + 1]) - u;
-  if (i + 1 < ny) b = fmaf(-tau, gtf(p1, p2, nx, ny, i + 1, j), z[k + nx]) - u;
+  const float u = su[threadIdx.y][threadIdx.x];
+  const float a = j + 1 < nx ? su[threadIdx.y][threadIdx.x + 1] - u : 0.f;
+  const float b = i + 1 < ny ? su[threadIdx.y + 1][threadIdx.x] - u : 0.f;
   const float n1 = fmaf(a, step, p1[k]), n2 = fmaf(b, step, p2[k]);
   const float m = fmaxf(1.f, sqrtf(n1 * n1 + n2 * n2));
   q1[o + k] = n1 / m;

@@ -557,6 +557,8 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
   const int nc = (int)std::ceil(2.0 * std::sqrt(2.0) / h - 1e-9);
   if (nc > 6) return false;
   plan->nc = nc <= 3 ? 3 : (nc <= 4 ? 4 : 6);
+  // projections per chunk (<= FB_NPJ): picked below, once the two walk classes are known, so that
+  // the grid fills whole waves of the GPU's block slots (3 blocks per SM)
   std::vector<int> order[2];
   std::vector<FpProjD> all(P);
   for (int p = 0; p < P; ++p) {
@@ -574,6 +576,22 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
     d.cuabs = (float)std::fabs(cu);
     d.p = p;
     order[cls].push_back(p);
+  }
+  int npj = FB_NPJ;
+  {
+    int n_sm = 148;
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess)
+      cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    const int64_t slots = 3 * (int64_t)n_sm;
+    const int64_t segs = (g->n_bins + FB_NB - 1) / FB_NB, groups = (g->n_slices + 3) / 4;
+    double best = 1e300;
+    for (int c = FB_NPJ; c >= FB_NPJ / 2; c -= FB_NPJ / 2) {  // cost ~ waves x (work of a block + its fixed part)
+      // (+ 10 %: chunks that straddle a jump in angle are split)
+      const int64_t blocks = segs * groups * (int64_t)((order[0].size() + c - 1) / c + (order[1].size() + c - 1) / c) * 11 / 10;
+      const double cost = (double)((blocks + slots - 1) / slots) * (double)(c + 3);
+      if (cost < best * 0.999) { best = cost; npj = c; }
+    }
   }
   projs->clear();
   chunks->clear();
@@ -596,9 +614,9 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
       ext[p] = proj_extent(all[p], g->n_bins, nv);
       w_single = std::max(w_single, width_of(ext[p], plan->nc));
     }
-    for (size_t i = 0; i < order[cls].size(); i += FB_NPJ) {
+    for (size_t i = 0; i < order[cls].size(); i += npj) {
       Extent e = ext[order[cls][i]];
-      for (size_t j = i + 1; j < std::min(order[cls].size(), i + FB_NPJ); ++j) e = merge(e, ext[order[cls][j]]);
+      for (size_t j = i + 1; j < std::min(order[cls].size(), i + npj); ++j) e = merge(e, ext[order[cls][j]]);
       widths.push_back(width_of(e, plan->nc));
     }
   }
@@ -606,7 +624,7 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
   const int w_most = widths.empty() ? 0 : widths[(widths.size() - 1) * 9 / 10];
   const int W = std::min(std::max(std::max(w_most, w_single), plan->nc + 4), FB_WMAX);
   plan->W = W;
-  plan->npj = FB_NPJ;
+  plan->npj = npj;
   // greedy chunks: add neighbours while the window still fits
   for (int cls = 0; cls < 2; ++cls) {
     size_t i = 0;
@@ -616,7 +634,7 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
       FpChunk ck{(int32_t)projs->size(), 1, cls, 0};
       projs->push_back(all[order[cls][i]]);
       size_t j = i + 1;
-      for (; j < order[cls].size() && ck.count < FB_NPJ; ++j) {
+      for (; j < order[cls].size() && ck.count < npj; ++j) {
         const Extent m = merge(e, ext[order[cls][j]]);
         if (width_of(m, plan->nc) > W) break;
         e = m;
