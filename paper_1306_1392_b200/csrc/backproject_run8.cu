@@ -226,35 +226,41 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
         }
       }
     }
-  } else {  // pixel (x0 + rn + n, y0 + fl): 8 consecutive x per thread
-    const int y = y0 + fl;
-    if (y < ny) {
-      float v[R8_RN][8];
+  } else {
+    // pixel (x0 + rn + n, y0 + fl): lanes run along y, so the tile goes through shared memory (the
+    // window ring is free: every chunk has been consumed) and is written / added row by row
+    constexpr int TP = R8_SLOW + 1;                      // padded row of the transposed tile
+    float* ts = reinterpret_cast<float*>(buf);           // [8 slices][64 rows][TP]
+    __syncthreads();
 #pragma unroll
-      for (int n = 0; n < R8_RN; ++n)
+    for (int n = 0; n < R8_RN; ++n)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) v[n][j] = acc[n][j];
+      for (int sl = 0; sl < 8; ++sl) ts[(sl * R8_LANES + fl) * TP + rn + n] = acc[n][sl];
+    __syncthreads();
+    const bool vec_ok = (nx % 4 == 0) && ((reinterpret_cast<uintptr_t>(img) & 15) == 0);
+#pragma unroll 1
+    for (int sl = 0; sl < 8; ++sl) {
+      const int s = gA * 4 + sl;
+      if (s >= S) break;
 #pragma unroll
-      for (int sl = 0; sl < 8; ++sl) {
-        const int s = gA * 4 + sl;
-        if (s >= S) continue;
-        float* row = img + ((int64_t)s * ny + y) * nx + x0 + rn;
-        const bool vec = ((reinterpret_cast<uintptr_t>(row) & 15) == 0) && (x0 + rn + R8_RN <= nx);
+      for (int q = 0; q < 2; ++q) {
+        const int e = tid + R8_NC * q;
+        const int yl = e >> 3, xl = (e & 7) * 4;
+        const int y = y0 + yl, x = x0 + xl;
+        if (y >= ny || x >= nx) continue;
+        const float* t4 = ts + (sl * R8_LANES + yl) * TP + xl;
+        float* row = img + ((int64_t)s * ny + y) * nx + x;
+        if (vec_ok && x + 4 <= nx) {
+          float4 o = add ? *reinterpret_cast<const float4*>(row) : make_float4(0.f, 0.f, 0.f, 0.f);
+          o.x = fmaf(scale, t4[0], o.x);
+          o.y = fmaf(scale, t4[1], o.y);
+          o.z = fmaf(scale, t4[2], o.z);
+          o.w = fmaf(scale, t4[3], o.w);
+          *reinterpret_cast<float4*>(row) = o;
+        } else {
 #pragma unroll
-        for (int n4 = 0; n4 < R8_RN; n4 += 4) {
-          if (vec) {
-            float4 o = add ? *reinterpret_cast<const float4*>(row + n4) : make_float4(0.f, 0.f, 0.f, 0.f);
-            o.x = fmaf(scale, v[n4][sl], o.x);
-            o.y = fmaf(scale, v[n4 + 1][sl], o.y);
-            o.z = fmaf(scale, v[n4 + 2][sl], o.z);
-            o.w = fmaf(scale, v[n4 + 3][sl], o.w);
-            *reinterpret_cast<float4*>(row + n4) = o;
-          } else {
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-              if (x0 + rn + n4 + j < nx)
-                row[n4 + j] = fmaf(scale, v[n4 + j][sl], add ? row[n4 + j] : 0.f);
-          }
+          for (int j = 0; j < 4; ++j)
+            if (x + j < nx) row[j] = fmaf(scale, t4[j], add ? row[j] : 0.f);
         }
       }
     }
