@@ -202,9 +202,9 @@ def run_b200(args):
 
         def e2e_step():
             P.fbp_host(h_sino, w.angles, w.axis, nx, ny, w.pixel_size, filter=w.filter, mode=w.mode,
-                       out=h_img, max_slices_per_chunk=4)
+                       out=h_img, max_slices_per_chunk=8)
             P.forward_project_host(h_img, w.angles, w.axis, B, w.pixel_size, out=h_proj,
-                                   max_slices_per_chunk=4)
+                                   max_slices_per_chunk=8)
 
         for _ in range(min(args.warmup, 2) or 1):
             e2e_step()
@@ -221,7 +221,7 @@ def run_b200(args):
                "steps": n_e2e,
                "h2d_bytes_per_step": int(h_sino.numel() * 4 + h_img.numel() * 4),
                "d2h_bytes_per_step": int(h_img.numel() * 4 + h_proj.numel() * 4),
-               "api": "pyhst_fbp_host + pyhst_forward_project_host (pinned host buffers, 4-slice chunks, "
+               "api": "pyhst_fbp_host + pyhst_forward_project_host (pinned host buffers, 8-slice chunks, "
                       "copies overlapped with kernels)"}
         P.profile_read(reset=True)
         del h_sino, h_img, h_proj

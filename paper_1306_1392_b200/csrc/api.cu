@@ -312,7 +312,7 @@ static QiLayout qi_layout(int32_t n_slices, int32_t n_angles, int32_t n_bins, do
 
 // 1 = reference, 2 = tiled, 3 = run (4 slices per thread), 4 = run8 (8 slices per thread, the
 // product path); -1 = the requested variant does not cover the geometry
-static int pick_bp_kernel(double pixel_size) {
+static int pick_bp_kernel(double pixel_size, int32_t n_slices) {
   const bool tiled_ok = backproject_tiled_window(pixel_size) > 0;
   const bool run_ok = backproject_run_window(pixel_size) > 0;
   const bool run8_ok = run_ok && backproject_run8_window(pixel_size) > 0;
@@ -321,7 +321,8 @@ static int pick_bp_kernel(double pixel_size) {
     case 2: return tiled_ok ? 2 : -1;
     case 3: return run_ok ? 3 : -1;
     case 4: return run8_ok ? 4 : -1;
-    default: return run8_ok ? 4 : (run_ok ? 3 : (tiled_ok ? 2 : 1));
+    // one slice group (<= 4 slices): the 8-slice kernel would spend half of its FMAs on a duplicate
+    default: return (run8_ok && n_slices > 4) ? 4 : (run_ok ? 3 : (tiled_ok ? 2 : 1));
   }
 }
 
@@ -445,7 +446,7 @@ int pyhst_backproject(const float* d_sino, float* d_img, const pyhst_geom_t* g, 
   PYHST_TRY(get_geom_plan(g, 0.0, g->n_bins, stream, &plan));
   BpArgs a{d_img, g->n_slices, g->n_angles, g->n_bins, g->nx, g->ny, scale, plan->d_proj,
            g->pixel_size};
-  const int kern = pick_bp_kernel(g->pixel_size);
+  const int kern = pick_bp_kernel(g->pixel_size, g->n_slices);
   if (kern < 0)
     return set_error(PYHST_ERR_UNSUPPORTED, "backprojector variant %d does not cover pixel_size %g",
                      g_bp_variant, g->pixel_size);
@@ -520,7 +521,7 @@ static int fbp_device(const float* d_sino_raw, int64_t pitch, float* d_img, cons
   PYHST_TRY(get_geom_plan(g, (double)pad_left, b_out, stream, &plan));
   BpArgs a{d_img, ns, g->n_angles, b_out, g->nx, g->ny, (float)scale, plan->d_proj, g->pixel_size};
   const int64_t P = g->n_angles;
-  const int kern = pick_bp_kernel(g->pixel_size);
+  const int kern = pick_bp_kernel(g->pixel_size, ns);
   if (kern < 0)
     return set_error(PYHST_ERR_UNSUPPORTED, "backprojector variant %d does not cover pixel_size %g",
                      g_bp_variant, g->pixel_size);
