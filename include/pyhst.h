@@ -48,8 +48,11 @@ enum {
 
 /* Band-limited ramp kernels, bin width 1 (reading R8; PAPER.md:L13, L63 give no formula):
  *   Ram-Lak     h[0] = 1/4, h[n odd] = -1/(pi^2 n^2), h[n even != 0] = 0
- *   Shepp-Logan h[n] = -2 / (pi^2 (4 n^2 - 1))                                            */
-typedef enum { PYHST_FILTER_RAMLAK = 0, PYHST_FILTER_SHEPP_LOGAN = 1 } pyhst_filter_t;
+ *   Shepp-Logan h[n] = -2 / (pi^2 (4 n^2 - 1))
+ *   Hann, Hamming (NEXT row N2): Ram-Lak times the window a0 + 2 a1 cos(2 pi w), w in cycles per
+ *               bin, (a0, a1) = (0.5, 0.25) resp. (0.54, 0.23): h_w[n] = a0 h[n] + a1 (h[n-1] + h[n+1]) */
+typedef enum { PYHST_FILTER_RAMLAK = 0, PYHST_FILTER_SHEPP_LOGAN = 1, PYHST_FILTER_HANN = 2,
+               PYHST_FILTER_HAMMING = 3 } pyhst_filter_t;
 
 /* >= 180 degrees; with 360 degrees and the axis near the detector border the
  * detector "can be virtually doubled" (PYHST_SCAN_360_HALF, reading R10). */

@@ -27,6 +27,8 @@ _LIB = os.path.join(_HERE, "libpyhst_oracle.so")
 
 FILTER_RAMLAK = 0
 FILTER_SHEPP_LOGAN = 1
+FILTER_HANN = 2
+FILTER_HAMMING = 3
 SCAN_180 = 0
 SCAN_360 = 1
 SCAN_360_HALF = 2

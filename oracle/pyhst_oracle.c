@@ -60,9 +60,16 @@ int oracle_num_threads(void) {
 /* ---- R8: spatial-domain band-limited ramp kernels, bin width 1 ------------
  * Ram-Lak     : h[0] = 1/4 ; h[n] = 0 (n even, n != 0) ; h[n] = -1/(pi^2 n^2) (n odd)
  * Shepp-Logan : h[n] = -2 / (pi^2 (4 n^2 - 1))
+ * Hann (2), Hamming (3): the Ram-Lak ramp times the window a0 + 2 a1 cos(2 pi w), w in cycles per
+ *   bin (|w| <= 1/2), (a0, a1) = (0.5, 0.25) resp. (0.54, 0.23); a cosine in frequency is a pair of
+ *   unit shifts in space:  h_w[n] = a0 h[n] + a1 (h[n-1] + h[n+1])   (NEXT row N2: more windows)
  * (PAPER.md:L13, L63 only say "filtered back projection"; no formula given.) */
 double oracle_ramp_kernel(int filter, int64_t n) {
   double dn = (double)n;
+  if (filter == 2 || filter == 3) {
+    const double a0 = filter == 2 ? 0.5 : 0.54, a1 = filter == 2 ? 0.25 : 0.23;
+    return a0 * oracle_ramp_kernel(0, n) + a1 * (oracle_ramp_kernel(0, n - 1) + oracle_ramp_kernel(0, n + 1));
+  }
   if (filter == 0) {
     if (n == 0) return 0.25;
     if ((n & 1) == 0) return 0.0;
@@ -112,7 +119,7 @@ int oracle_ramp_filter(const float* in, int64_t in_pitch, double* out, int64_t n
                        int32_t n_bins_in, int32_t n_bins_out, int32_t pad_left, int filter,
                        const float* col_weights) {
   if (!in || !out || n_rows < 0 || n_bins_in <= 0 || n_bins_out <= 0 || pad_left < 0 ||
-      n_bins_out < n_bins_in + pad_left || (filter != 0 && filter != 1))
+      n_bins_out < n_bins_in + pad_left || filter < 0 || filter > 3)
     return ORACLE_ERR_INVALID_ARG;
   if (in_pitch == 0) in_pitch = n_bins_in;
   int64_t nh = (int64_t)n_bins_in + n_bins_out;         /* lags -(B_in-1) .. B_out-1 */

@@ -14,6 +14,8 @@ import numpy as np
 
 FILTER_RAMLAK = 0
 FILTER_SHEPP_LOGAN = 1
+FILTER_HANN = 2
+FILTER_HAMMING = 3
 SCAN_180 = 0
 SCAN_360 = 1
 SCAN_360_HALF = 2

@@ -51,11 +51,19 @@ __global__ void ramp_kernel_table(double* hc, int M, int filter) {
   const int l = n <= M / 2 ? n : n - M;
   const double PI = 3.14159265358979323846264338327950288;
   const double dl = (double)l;
+  auto ramlak = [PI](int m) {
+    const double dm = (double)m;
+    return m == 0 ? 0.25 : ((m & 1) ? -1.0 / (PI * PI * dm * dm) : 0.0);
+  };
   double h;
   if (filter == PYHST_FILTER_RAMLAK)
-    h = l == 0 ? 0.25 : ((l & 1) ? -1.0 / (PI * PI * dl * dl) : 0.0);
-  else
+    h = ramlak(l);
+  else if (filter == PYHST_FILTER_SHEPP_LOGAN)
     h = -2.0 / (PI * PI * (4.0 * dl * dl - 1.0));
+  else {  // Hann / Hamming window a0 + 2 a1 cos(2 pi w) on the Ram-Lak ramp = unit shifts in space
+    const double a0 = filter == PYHST_FILTER_HANN ? 0.5 : 0.54, a1 = filter == PYHST_FILTER_HANN ? 0.25 : 0.23;
+    h = a0 * ramlak(l) + a1 * (ramlak(l - 1) + ramlak(l + 1));
+  }
   hc[n] = h;
 }
 

@@ -184,7 +184,7 @@ def test_adjoint_identity_on_device(lib, B, axis):
 
 
 # ------------------------------------------------------------------------------ ramp filter
-@pytest.mark.parametrize("f", [0, 1])
+@pytest.mark.parametrize("f", [0, 1, 2, 3])
 @pytest.mark.parametrize("b_in,b_out,pad,weights", [(367, 367, 0, False), (128, 256, 0, True),
                                                     (100, 192, 92, True), (64, 64, 0, False),
                                                     (2048, 2048, 0, False)])
@@ -371,3 +371,14 @@ def test_fista_tv_config4_full_size(lib, oracle):
     rel = np.linalg.norm((px - data).ravel()) / np.linalg.norm(data.ravel())
     assert rel < 0.05
     assert 2.0 * e[-1] >= (rel * np.linalg.norm(data.ravel())) ** 2 * 0.5   # energy >= its data term (y_99 ~ x)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("f", [2, 3])
+def test_fbp_windowed_ramps(lib, oracle, f):
+    """N2: Hann / Hamming windows through the whole FBP (config 2 shrunk, drift, Poisson noise)."""
+    w = lib.workloads.config(2, shrink=8, n_slices=5)
+    sino = w.sinogram()
+    want = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, filter=f, mode=w.mode)
+    got = lib.fbp(_dev(sino), w.angles, w.axis, w.nx, w.ny, filter=f, mode=w.mode).cpu().numpy()
+    assert_parity(got, want, "fbp filter %d" % f)

@@ -177,9 +177,35 @@ def test_k6_kernel_sums_and_spectrum(oracle):
     assert np.abs(H1 - np.abs(np.sin(math.pi * k / M)) / math.pi).max() < 2.0 / M
 
 
+def test_k6_windowed_ramps(oracle):
+    """Hann / Hamming (NEXT row N2): the spectrum of the kernel is the Ram-Lak ramp |w| times the
+    window a0 + 2 a1 cos(2 pi w), w = k/M cycles per bin; the windows' own closed-form values."""
+    M = 2048
+    lag = np.fft.fftfreq(M, 1.0 / M).astype(np.int64)
+    w = np.fft.fftfreq(M)                                  # cycles per bin in [-1/2, 1/2)
+    H0 = np.fft.fft(oracle.ramp_kernel(0, lag)).real       # truncated Ram-Lak: |w| up to O(1/M)
+    for f, a0, a1 in ((2, 0.5, 0.25), (3, 0.54, 0.23)):
+        H = np.fft.fft(oracle.ramp_kernel(f, lag)).real
+        win = a0 + 2 * a1 * np.cos(2 * math.pi * w)
+        assert np.abs(H - np.abs(w) * win).max() < 3.0 / M
+        assert np.abs(H - H0 * win).max() < 1e-3           # the same truncation on both sides
+        assert win[0] == pytest.approx(1.0) and win[M // 2] == pytest.approx(a0 - 2 * a1)
+        # h_w[0] = a0/4 - 2 a1/pi^2 ; h_w[1] = -a0/pi^2 + a1/4 ; h_w[2] = -a1 (1 + 1/9)/pi^2 ; even, sums to 0
+        h = oracle.ramp_kernel(f, np.arange(-3, 4))
+        assert h[3] == pytest.approx(a0 / 4 - 2 * a1 / math.pi ** 2, rel=1e-14)
+        assert h[4] == pytest.approx(-a0 / math.pi ** 2 + a1 / 4, rel=1e-14)
+        assert h[5] == pytest.approx(-a1 * (1 + 1.0 / 9) / math.pi ** 2, rel=1e-14)
+        np.testing.assert_array_equal(h, h[::-1])
+        assert abs(oracle.ramp_kernel(f, np.arange(-20000, 20001)).sum()) < 1e-5
+    # filtering a constant row far from the ends gives ~0 (no DC), a ramp row gives ~0 too (odd part)
+    q = np.ones((1, 4001), dtype=np.float32)
+    g = oracle.ramp_filter(q, filter=2)[0]
+    assert abs(g[2000]) < 1e-4
+
+
 def test_k6_filter_of_delta_returns_kernel(oracle):
     B = 33
-    for f in (0, 1):
+    for f in (0, 1, 2, 3):
         q = np.zeros((1, B), dtype=np.float32)
         q[0, 10] = 1.0
         g = oracle.ramp_filter(q, n_bins_out=B + 7, pad_left=4, filter=f)[0]
