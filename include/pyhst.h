@@ -164,6 +164,13 @@ int pyhst_halfacq_extent(int32_t n_bins, double cbar, int32_t* n_bins_ext, int32
  * agree within FP32 rounding. */
 int pyhst_set_backproject_variant(int variant);
 
+/* PYHST_SCAN_360_HALF only (NEXT row N2): 1 (default) lets pyhst_fbp fold a scan whose projections p
+ * and p + P/2 face each other (angles differ by pi to 1e-10, equal axis, 2 x axis integer) into P/2
+ * full-width rows, lerp(g_p, t) + lerp(g_{p+P/2}, 2c - t) = lerp(g_p + flip(g_{p+P/2}), t), and
+ * backproject half as many projections; 0 always backprojects all P rows.  Scans that do not pair up
+ * take the general path either way.  Returns the previous value. */
+int pyhst_set_halfacq_stitch(int enable);
+
 /* Selects the forward-projection kernel: 0 = automatic (default), 1 = generic gather kernel (one
  * thread per bin and slice, global loads; kept for cross-checks and for pixel sizes the banded
  * kernel does not cover), 2 = banded shared-memory kernel (what 0 picks), 3 = interval form of the

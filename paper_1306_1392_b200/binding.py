@@ -25,7 +25,7 @@ _LIBNAME = "libpyhst_b200.so"
 
 # every symbol include/pyhst.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
-           "pyhst_fista_tv", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant",
+           "pyhst_fista_tv", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_set_halfacq_stitch",
            "pyhst_last_error", "pyhst_release_cache")
 
 
@@ -69,6 +69,7 @@ def _load():
     lib.pyhst_halfacq_extent.argtypes = [c_int32, c_double, POINTER(c_int32), POINTER(c_int32)]
     lib.pyhst_set_backproject_variant.argtypes = [c_int]
     lib.pyhst_set_forward_project_variant.argtypes = [c_int]
+    lib.pyhst_set_halfacq_stitch.argtypes = [c_int]
     lib.pyhst_profile_enable.argtypes = [c_int]
     lib.pyhst_profile_read.argtypes = [POINTER(c_double), POINTER(c_int64), POINTER(c_int64), c_int32]
     lib.pyhst_last_error.restype = c_char_p
@@ -250,6 +251,10 @@ def halfacq_extent(n_bins, cbar):
 
 def set_backproject_variant(variant: int) -> int:
     return int(_load().pyhst_set_backproject_variant(int(variant)))
+
+
+def set_halfacq_stitch(enable: bool) -> int:
+    return int(_load().pyhst_set_halfacq_stitch(1 if enable else 0))
 
 
 def set_forward_project_variant(variant: int) -> int:

@@ -59,6 +59,7 @@ struct Ws { void* p = nullptr; size_t bytes = 0; };
 Ws g_ws[WS_COUNT];
 int g_bp_variant = 0;
 int g_fp_variant = 0;
+int g_halfacq_stitch = 1;
 std::list<FpPlan> g_fp_plans;
 cudaStream_t g_streams[3] = {nullptr, nullptr, nullptr};
 cudaEvent_t g_events[8] = {nullptr};
@@ -367,6 +368,12 @@ int pyhst_set_backproject_variant(int variant) {
   return prev;
 }
 
+int pyhst_set_halfacq_stitch(int enable) {
+  const int prev = g_halfacq_stitch;
+  if (enable == 0 || enable == 1) g_halfacq_stitch = enable;
+  return prev;
+}
+
 int pyhst_set_forward_project_variant(int variant) {
   const int prev = g_fp_variant;
   if (variant >= 0 && variant <= 3) g_fp_variant = variant;
@@ -517,6 +524,50 @@ static int fbp_device(const float* d_sino_raw, int64_t pitch, float* d_img, cons
   }
   if ((int64_t)g->n_bins + b_out > 16384)
     return set_error(PYHST_ERR_UNSUPPORTED, "n_bins + filtered row length > 16384");
+  if (mode == PYHST_SCAN_360_HALF && g_halfacq_stitch && g_bp_variant != 1) {
+    // N2: projections p and p + P/2 face each other (angles differ by pi, same axis, 2c integer):
+    // fold the scan into P/2 full-width rows and backproject half as many projections (filter.cu)
+    const int32_t P2 = g->n_angles / 2;
+    bool ok = g->n_angles % 2 == 0 && P2 > 0;
+    std::vector<int> two_c((size_t)std::max(P2, 1));
+    int lo = 0, hi = b_out - 1;  // range of bins the folded rows must hold
+    for (int32_t p = 0; ok && p < P2; ++p) {
+      const double c2 = 2.0 * (g->axis_pos[p] + (double)pad_left);
+      ok = std::fabs(g->angles_rad[p + P2] - g->angles_rad[p] - PI) <= 1e-10 &&
+           g->axis_pos[p + P2] == g->axis_pos[p] && std::fabs(c2 - std::nearbyint(c2)) <= 1e-9 &&
+           std::fabs(c2) < 1e6;
+      if (!ok) break;
+      two_c[p] = (int)std::nearbyint(c2);
+      lo = std::min(lo, two_c[p] - (b_out - 1));
+      hi = std::max(hi, two_c[p]);
+    }
+    const int32_t off = -lo, b_st = hi - lo + 1;
+    if (ok && b_st <= 16384) {
+      const int64_t P = g->n_angles;
+      void *r1 = nullptr, *r2 = nullptr;
+      const size_t r2_bytes = (((size_t)ns * P2 * b_st * 4) + 255) & ~(size_t)255;
+      PYHST_TRY(get_workspace(WS_ROWS, (size_t)ns * P * b_out * 4, &r1));
+      PYHST_TRY(get_workspace(WS_STITCH, r2_bytes + (size_t)P2 * sizeof(int), &r2));
+      int* d_two_c = reinterpret_cast<int*>(static_cast<char*>(r2) + r2_bytes);
+      PYHST_CUDA_TRY(cudaMemcpyAsync(d_two_c, two_c.data(), (size_t)P2 * sizeof(int), cudaMemcpyHostToDevice,
+                                     stream));
+      for (int32_t s = 0; s < ns; ++s)
+        PYHST_TRY(launch_ramp_filter(d_sino_raw + (int64_t)s * P * pitch, pitch, P, g->n_bins, b_out,
+                                     pad_left, (int)f, d_w, static_cast<float*>(r1) + (int64_t)s * P * b_out,
+                                     b_out, nullptr, nullptr, 0, nullptr, stream));
+      PYHST_TRY(launch_halfacq_fold(static_cast<const float*>(r1), static_cast<float*>(r2), ns, P2, b_out,
+                                    b_st, off, d_two_c, stream));
+      std::vector<double> axis2((size_t)P2);
+      for (int32_t p = 0; p < P2; ++p) axis2[p] = g->axis_pos[p] + (double)pad_left + (double)off;
+      pyhst_geom_t g2 = *g;
+      g2.n_slices = ns;
+      g2.n_angles = P2;
+      g2.n_bins = b_st;
+      g2.sino_pitch = 0;
+      g2.axis_pos = axis2.data();
+      return pyhst_backproject(static_cast<const float*>(r2), d_img, &g2, (float)scale, stream);
+    }
+  }
   const GeomPlan* plan = nullptr;
   PYHST_TRY(get_geom_plan(g, (double)pad_left, b_out, stream, &plan));
   BpArgs a{d_img, ns, g->n_angles, b_out, g->nx, g->ny, (float)scale, plan->d_proj, g->pixel_size};

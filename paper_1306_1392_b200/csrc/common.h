@@ -89,7 +89,7 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
 
 // Grow-only device workspace slots owned by the library (freed by pyhst_release_cache).
 enum WorkspaceSlot { WS_QI = 0, WS_FFT = 1, WS_WEIGHTS = 2, WS_IMG_T = 3, WS_ROWS = 4,
-                     WS_CHUNKS = 5, WS_XI = 6, WS_FISTA = 7, WS_FPL = 8, WS_COUNT = 9 };
+                     WS_CHUNKS = 5, WS_XI = 6, WS_FISTA = 7, WS_FPL = 8, WS_STITCH = 9, WS_COUNT = 10 };
 int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr);
 
 // ---- interleaved sinogram layout consumed by the tiled backprojector ---------------------
@@ -199,6 +199,8 @@ int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int3
                        float4* d_qi, const QiLayout* L, int32_t n_slices_in, const uint8_t* d_flip,
                        cudaStream_t stream);
 int launch_halfacq_weights(float* d_w, int32_t n_bins, double cbar, cudaStream_t stream);
+int launch_halfacq_fold(const float* d_rows, float* d_out, int32_t n_slices, int32_t half_angles,
+                        int32_t b_out, int32_t b_st, int32_t off, const int* d_two_c, cudaStream_t stream);
 void release_filter_plans();
 
 // ---- device helpers: mbarrier + TMA bulk copy (inline PTX) -----------------------------------

@@ -269,4 +269,36 @@ void release_filter_plans() {
   g_spectra.clear();
 }
 
+// ---- stitched half acquisition (NEXT row N2; reading R10) -------------------------
+// A 360-degree half-acquisition scan whose projections pair up (theta_{p+P/2} = theta_p + pi, same
+// axis c, 2c integer) folds into a 180-degree scan of P/2 full-width rows: the opposite projection
+// sees the pixel at 2c - t, and lerp is symmetric, so
+//     lerp(g_p, t) + lerp(g_{p+P/2}, 2c - t) = lerp(g_p + flip(g_{p+P/2}), t),  flip(g)[b] = g[2c - b].
+// out[s][p][j], j in [0, b_st): bin b = j - off of the filtered rows' coordinate.
+__global__ void halfacq_fold_kernel(const float* __restrict__ rows, float* __restrict__ out, int P2,
+                                    int b_out, int b_st, int off, const int* __restrict__ two_c) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int p = blockIdx.y, s = blockIdx.z;
+  if (j >= b_st) return;
+  const int b = j - off, bf = two_c[p] - b;
+  const float* ra = rows + ((int64_t)s * 2 * P2 + p) * b_out;
+  const float* rb = rows + ((int64_t)s * 2 * P2 + p + P2) * b_out;
+  float v = 0.f;
+  if (b >= 0 && b < b_out) v = ra[b];
+  if (bf >= 0 && bf < b_out) v += rb[bf];
+  out[((int64_t)s * P2 + p) * b_st + j] = v;
+}
+
+int launch_halfacq_fold(const float* d_rows, float* d_out, int32_t n_slices, int32_t half_angles,
+                        int32_t b_out, int32_t b_st, int32_t off, const int* d_two_c, cudaStream_t stream) {
+  dim3 grid((b_st + 255) / 256, half_angles, n_slices);
+  if (grid.y > 65535 || grid.z > 65535)
+    return set_error(PYHST_ERR_UNSUPPORTED, "half-acquisition fold: grid too large");
+  StageScope scope(ST_FILTER, stream);
+  scope.kernels();
+  halfacq_fold_kernel<<<grid, 256, 0, stream>>>(d_rows, d_out, half_angles, b_out, b_st, off, d_two_c);
+  PYHST_CUDA_TRY(cudaGetLastError());
+  return PYHST_OK;
+}
+
 }  // namespace pyhst

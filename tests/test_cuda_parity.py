@@ -382,3 +382,39 @@ def test_fbp_windowed_ramps(lib, oracle, f):
     want = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, filter=f, mode=w.mode)
     got = lib.fbp(_dev(sino), w.angles, w.axis, w.nx, w.ny, filter=f, mode=w.mode).cpu().numpy()
     assert_parity(got, want, "fbp filter %d" % f)
+
+
+@pytest.mark.gpu
+def test_halfacq_stitched_equals_general_path(lib, oracle):
+    """N2: the folded 180-degree path of PYHST_SCAN_360_HALF against the general path (all P rows)
+    and the oracle; a scan that does not pair up (odd P, drifting axis) takes the general path."""
+    w = lib.workloads.config(3, shrink=8, n_slices=5)          # c = 237.5: 2c integer, P = 500
+    sino = w.sinogram()
+    want = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode)
+    got = lib.fbp(_dev(sino), w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode).cpu().numpy()
+    prev = lib.set_halfacq_stitch(False)
+    try:
+        gen = lib.fbp(_dev(sino), w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode).cpu().numpy()
+    finally:
+        lib.set_halfacq_stitch(prev)
+    assert_parity(got, want, "fbp half acquisition, stitched")
+    assert_parity(gen, want, "fbp half acquisition, general")
+    assert np.abs(got - gen).max() <= 2e-5 * np.abs(gen).max()
+    assert not np.array_equal(got, gen)                         # the two paths really differ
+    # unpaired scans: odd number of projections, and an axis that is not a half-integer
+    for P, axis in ((101, 50.5), (100, 50.3)):
+        ang = np.arange(P) * 2 * math.pi / P
+        ax = np.full(P, axis)
+        raw = lib.workloads.random_sinogram(2, P, 64, seed=P)
+        nxy = 100
+        want2 = oracle.fbp(raw, ang, ax, nxy, nxy, mode=lib.SCAN_360_HALF)
+        got2 = lib.fbp(_dev(raw), ang, ax, nxy, nxy, mode=lib.SCAN_360_HALF).cpu().numpy()
+        assert_parity(got2, want2, "fbp half acquisition, unpaired P=%d" % P)
+    # paired, axis left of the detector centre (pad_left > 0) and integer axis
+    P = 60
+    ang = np.arange(P) * 2 * math.pi / P
+    ax = np.full(P, 9.0)
+    raw = lib.workloads.random_sinogram(3, P, 64, seed=1)
+    want3 = oracle.fbp(raw, ang, ax, 110, 108, mode=lib.SCAN_360_HALF)
+    got3 = lib.fbp(_dev(raw), ang, ax, 110, 108, mode=lib.SCAN_360_HALF).cpu().numpy()
+    assert_parity(got3, want3, "fbp half acquisition, stitched, axis on the left")
