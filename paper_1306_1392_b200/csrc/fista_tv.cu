@@ -73,13 +73,13 @@ __global__ void ftv_residual_kernel(float* __restrict__ r, const float* __restri
 
 // z = y - g * (1/L);  *tv_acc += beta * TV(y)   (energy of eq. 3 at y, R19)
 __global__ void ftv_step_kernel(const float* __restrict__ y, const float* __restrict__ g,
-                                float* __restrict__ z, int nx, int ny, const double* L, double beta,
+                                float* __restrict__ z, int nx, int ny, const float* __restrict__ fs, double beta,
                                 double* tv_acc) {
   const int j = blockIdx.x * FT_BX + threadIdx.x, i = blockIdx.y * FT_BY + threadIdx.y;
   const int64_t o = (int64_t)blockIdx.z * ny * nx;
   double tv = 0.0;
   if (i < ny && j < nx) {
-    const float inv_l = (float)(1.0 / *L);
+    const float inv_l = fs[0];
     const int64_t k = o + (int64_t)i * nx + j;
     z[k] = fmaf(-g[k], inv_l, y[k]);
     const float a = d1f(y + o, nx, i, j), b = d2f(y + o, nx, ny, i, j);
@@ -89,45 +89,68 @@ __global__ void ftv_step_kernel(const float* __restrict__ y, const float* __rest
 }
 
 // one dual projected-gradient step (R18):  u = z - tau G^T p ;  q = p + G u / (8 tau) ;
-// p' = q / max(1, |q|)  -- p is read from (p1, p2) and written to (q1, q2) (Jacobi: ping-pong)
-__global__ void ftv_dual_kernel(const float* __restrict__ z, const float* __restrict__ p1,
-                                const float* __restrict__ p2, float* __restrict__ q1,
-                                float* __restrict__ q2, int nx, int ny, const double* L, double beta) {
-  // u = z - tau G^T p of the block's tile plus one column / row of halo, through shared memory
-  __shared__ float su[FT_BY + 1][FT_BX + 1];
-  const int j0 = blockIdx.x * FT_BX, i0 = blockIdx.y * FT_BY;
-  const int64_t o = (int64_t)blockIdx.z * ny * nx;
-  z += o; p1 += o; p2 += o;
-  const float tau = (float)(beta / *L);
-  const float step = 1.f / (8.f * tau);
-  for (int e = threadIdx.y * FT_BX + threadIdx.x; e < (FT_BY + 1) * (FT_BX + 1); e += FT_BX * FT_BY) {
-    const int ii = e / (FT_BX + 1), jj = e - ii * (FT_BX + 1);
-    const int i = i0 + ii, j = j0 + jj;
-    su[ii][jj] = (i < ny && j < nx) ? fmaf(-tau, gtf(p1, p2, nx, ny, i, j), z[(int64_t)i * nx + j]) : 0.f;
-  }
+// p' = q / max(1, |q|)  -- p is read from (p1, p2) and written to (q1, q2) (Jacobi: ping-pong).
+// u of the block's tile plus one row / column of halo goes through shared memory (32-bit offsets
+// inside a slice; the halo row is filled by the first warp, the halo column by the first lane of
+// every row).  INTERIOR: the tile and its halo touch no image border -- no boundary tests.
+template <bool INTERIOR>
+__device__ __forceinline__ void ftv_dual_tile(const float* __restrict__ z, const float* __restrict__ p1,
+                                              const float* __restrict__ p2, float* __restrict__ q1,
+                                              float* __restrict__ q2, int nx, int ny, float tau,
+                                              float step, float (&su)[FT_BY + 1][FT_BX + 1]) {
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int j = blockIdx.x * FT_BX + tx, i = blockIdx.y * FT_BY + ty;
+  auto uval = [&](int ii, int jj) -> float {
+    const int kk = ii * nx + jj;
+    if (INTERIOR) return fmaf(-tau, (p1[kk - 1] - p1[kk]) + (p2[kk - nx] - p2[kk]), z[kk]);
+    if (ii >= ny || jj >= nx) return 0.f;
+    float v = 0.f;                                       // (G^T p)[ii, jj], see gtf()
+    if (jj > 0) v += p1[kk - 1];
+    if (jj + 1 < nx) v -= p1[kk];
+    if (ii > 0) v += p2[kk - nx];
+    if (ii + 1 < ny) v -= p2[kk];
+    return fmaf(-tau, v, z[kk]);
+  };
+  su[ty][tx] = uval(i, j);
+  if (ty == 0) su[FT_BY][tx] = uval(blockIdx.y * FT_BY + FT_BY, j);
+  if (tx == 0) su[ty][FT_BX] = uval(i, blockIdx.x * FT_BX + FT_BX);
   __syncthreads();
-  const int j = j0 + threadIdx.x, i = i0 + threadIdx.y;
-  if (i >= ny || j >= nx) return;
-  const int64_t k = (int64_t)i * nx + j;
-  const float u = su[threadIdx.y][threadIdx.x];
-  const float a = j + 1 < nx ? su[threadIdx.y][threadIdx.x + 1] - u : 0.f;
-  const float b = i + 1 < ny ? su[threadIdx.y + 1][threadIdx.x] - u : 0.f;
+  if (!INTERIOR && (i >= ny || j >= nx)) return;
+  const int k = i * nx + j;
+  const float u = su[ty][tx];
+  const float a = (INTERIOR || j + 1 < nx) ? su[ty][tx + 1] - u : 0.f;
+  const float b = (INTERIOR || i + 1 < ny) ? su[ty + 1][tx] - u : 0.f;
   const float n1 = fmaf(a, step, p1[k]), n2 = fmaf(b, step, p2[k]);
   const float m = fmaxf(1.f, sqrtf(n1 * n1 + n2 * n2));
-  q1[o + k] = n1 / m;
-  q2[o + k] = n2 / m;
+  q1[k] = n1 / m;
+  q2[k] = n2 / m;
+}
+
+__global__ void ftv_dual_kernel(const float* __restrict__ z, const float* __restrict__ p1,
+                                const float* __restrict__ p2, float* __restrict__ q1,
+                                float* __restrict__ q2, int nx, int ny, const float* __restrict__ fs) {
+  __shared__ float su[FT_BY + 1][FT_BX + 1];
+  const int64_t o = (int64_t)blockIdx.z * ny * nx;
+  const float tau = fs[1], step = fs[2];
+  const int j0 = blockIdx.x * FT_BX, i0 = blockIdx.y * FT_BY;
+  // note: the non-symmetric sum order of the border path, (+p1[k-1] - p1[k]) + (p2[k-nx] - p2[k]),
+  // is kept by the interior path only up to FP32 rounding of the four-term sum
+  if (j0 > 0 && i0 > 0 && j0 + FT_BX + 1 < nx && i0 + FT_BY + 1 < ny)
+    ftv_dual_tile<true>(z + o, p1 + o, p2 + o, q1 + o, q2 + o, nx, ny, tau, step, su);
+  else
+    ftv_dual_tile<false>(z + o, p1 + o, p2 + o, q1 + o, q2 + o, nx, ny, tau, step, su);
 }
 
 // x+ = z - tau G^T p (tau = 0: x+ = z);  y = x+ + mom (x+ - x);  x = x+
 __global__ void ftv_finish_kernel(const float* __restrict__ z, const float* __restrict__ p1,
                                   const float* __restrict__ p2, float* __restrict__ x,
-                                  float* __restrict__ y, int nx, int ny, const double* L, double beta,
-                                  float mom, int use_p) {
+                                  float* __restrict__ y, int nx, int ny, const float* __restrict__ fs, float mom,
+                                  int use_p) {
   const int j = blockIdx.x * FT_BX + threadIdx.x, i = blockIdx.y * FT_BY + threadIdx.y;
   if (i >= ny || j >= nx) return;
   const int64_t o = (int64_t)blockIdx.z * ny * nx, k = o + (int64_t)i * nx + j;
   float xn = z[k];
-  if (use_p) xn = fmaf(-(float)(beta / *L), gtf(p1 + o, p2 + o, nx, ny, i, j), xn);
+  if (use_p) xn = fmaf(-fs[1], gtf(p1 + o, p2 + o, nx, ny, i, j), xn);
   const float xo = x[k];
   y[k] = fmaf(mom, xn - xo, xn);
   x[k] = xn;
@@ -147,6 +170,13 @@ __global__ void ftv_normalise_kernel(const float* __restrict__ w, float* __restr
   const double s = sqrt(*nw);
   if (k < n) v[k] = (float)((double)w[k] / s);
   if (k == 0) *L = 1.1 * s / sqrt(*nv);
+}
+// fs[0] = 1/L, fs[1] = tau = beta/L, fs[2] = 1/(8 tau): the per-thread constants of the loop, once
+__global__ void ftv_scalars_kernel(const double* L, double beta, float* fs) {
+  fs[0] = (float)(1.0 / *L);
+  const float tau = (float)(beta / *L);
+  fs[1] = tau;
+  fs[2] = 1.f / (8.f * tau);
 }
 __global__ void ftv_fill_kernel(float* v, int64_t n, float value) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -181,9 +211,9 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
   // workspace: y, z, grad, 4 dual stacks, residual sinogram, scalars (nv, nw, L, energy[n_iter])
   const size_t img_bytes = ((size_t)n_img * 4 + 255) & ~(size_t)255;
   const size_t sino_bytes = ((size_t)n_sino * 4 + 255) & ~(size_t)255;
-  const size_t sc_bytes = (size_t)(3 + n_iter) * 8;
+  const size_t sc_bytes = (size_t)(3 + n_iter) * 8;   // doubles: nv, nw, L, energy[n_iter]; then 4 floats
   void* ws = nullptr;
-  PYHST_TRY(get_workspace(WS_FISTA, 7 * img_bytes + sino_bytes + sc_bytes, &ws));
+  PYHST_TRY(get_workspace(WS_FISTA, 7 * img_bytes + sino_bytes + sc_bytes + 16, &ws));
   char* base = static_cast<char*>(ws);
   float* y = reinterpret_cast<float*>(base);
   float* z = reinterpret_cast<float*>(base + img_bytes);
@@ -193,6 +223,7 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
   float* r = reinterpret_cast<float*>(base + 7 * img_bytes);
   double* sc = reinterpret_cast<double*>(base + 7 * img_bytes + sino_bytes);
   double *d_nv = sc, *d_nw = sc + 1, *d_L = sc + 2, *d_e = sc + 3;
+  float* d_fs = reinterpret_cast<float*>(sc + 3 + n_iter);
 
   pyhst_geom_t g1 = *g, gs = *g;
   g1.n_slices = 1;
@@ -213,6 +244,7 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
     ftv_sumsq_kernel<<<red_blocks, blk, 0, stream>>>(gr, n1, d_nw);
     ftv_normalise_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, stream>>>(gr, y, n1, d_nv, d_nw, d_L);
   }
+  ftv_scalars_kernel<<<1, 1, 0, stream>>>(d_L, (double)beta, d_fs);
   PYHST_CUDA_TRY(cudaGetLastError());
 
   // ---- FISTA (R19, R20): x0 = y0 = 0, t0 = 1
@@ -227,19 +259,19 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
       ftv_residual_kernel<<<grid, blk, 0, stream>>>(r, d_data, data_pitch, g->n_bins, n_rows, d_e + k);
     }
     PYHST_TRY(pyhst_backproject(r, gr, &gs, 1.f, stream));
-    ftv_step_kernel<<<grid_img, blk, 0, stream>>>(y, gr, z, nx, ny, d_L, (double)beta, d_e + k);
+    ftv_step_kernel<<<grid_img, blk, 0, stream>>>(y, gr, z, nx, ny, d_fs, (double)beta, d_e + k);
     int cur = 0;
     if (use_p) {
       PYHST_CUDA_TRY(cudaMemsetAsync(p[0], 0, 2 * img_bytes, stream));  // p[0], p[1] are adjacent
       for (int it = 0; it < n_inner; ++it) {
         ftv_dual_kernel<<<grid_img, blk, 0, stream>>>(z, p[cur], p[cur + 1], p[2 - cur], p[3 - cur], nx,
-                                                      ny, d_L, (double)beta);
+                                                      ny, d_fs);
         cur = 2 - cur;
       }
     }
     const double tn = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
-    ftv_finish_kernel<<<grid_img, blk, 0, stream>>>(z, p[cur], p[cur + 1], d_img, y, nx, ny, d_L,
-                                                    (double)beta, (float)((t - 1.0) / tn), use_p ? 1 : 0);
+    ftv_finish_kernel<<<grid_img, blk, 0, stream>>>(z, p[cur], p[cur + 1], d_img, y, nx, ny, d_fs,
+                                                    (float)((t - 1.0) / tn), use_p ? 1 : 0);
     t = tn;
     PYHST_CUDA_TRY(cudaGetLastError());
   }
