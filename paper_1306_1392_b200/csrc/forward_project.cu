@@ -213,6 +213,7 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
   const int par = lane & 1;
   const double bd = (double)(b0 + bl);
   const int idx_hi = W - NC;
+  float4 vlast = make_float4(0.f, 0.f, 0.f, 0.f);
 
   for (int k = 0; k < n_bands; ++k) {
     __syncthreads();  // everyone is done with band k-1: its stage may be overwritten
@@ -232,7 +233,7 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
       const int ai = __double2int_rn(A);
       const float afr = (float)(A - (double)ai);
       const float s = sp->s, hw = sp->hw, cuabs = sp->cuabs;
-#pragma unroll 2
+#pragma unroll 4
       for (int r = 0; r < rows; ++r) {
         const float dfr = fmaf(s, (float)r, afr);
         // first pixel that can lie inside the strip: ceil(dfr - hw) by a round-up add of
@@ -246,7 +247,11 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
           const float w = fmaxf(0.f, fmaf(-cuabs, fabsf(d0 + (float)c), 1.f));
-          const float4 v = wp[c];
+          // the last candidate lies outside the strip for most bins of a steep projection: its load
+          // is predicated on the weight (a quarter-warp with no taker costs no shared-memory
+          // wavefront); the register then keeps an older, finite pixel that is multiplied by 0
+          if (c < NC - 1 || w > 0.f) vlast = wp[c];
+          const float4 v = vlast;
           acc[m][0] = fmaf(w, v.x, acc[m][0]);
           acc[m][1] = fmaf(w, v.y, acc[m][1]);
           acc[m][2] = fmaf(w, v.z, acc[m][2]);
