@@ -137,11 +137,16 @@ constexpr int FB_WMAX = 416;  // window capacity (float4 per line): 2 x 8 x 416 
 
 struct XiDims { int32_t nv, nu, zpad; };
 
-template <int NC>
-__global__ void __launch_bounds__(FB_NT, 3)
+// MINB = blocks per SM the register budget is cut for (3: 80 registers; 4: 64, for windows small
+// enough that four blocks fit in shared memory).  n_split > 1: blockIdx.z = group * n_split + h and
+// the block walks only the h-th part of the bands; part h > 0 writes its sums to part[h - 1] (same
+// layout as sino, pitch part_pitch), fp_split_combine_kernel adds them -- small scans then fill the GPU.
+template <int NC, int MINB, bool SPLIT>
+__global__ void __launch_bounds__(FB_NT, MINB)
 fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_cols, XiDims dr,
                XiDims dc, float* __restrict__ sino, int64_t pitch, int S, int P, int B, float scale,
-               const FpProjD* __restrict__ projs, const FpChunk* __restrict__ chunks, int W) {
+               const FpProjD* __restrict__ projs, const FpChunk* __restrict__ chunks, int W,
+               int n_split, float* __restrict__ part, int64_t part_pitch, int64_t part_stride) {
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);        // [2]
   int* sorigin = reinterpret_cast<int*>(smem + 16);          // [2]
@@ -150,12 +155,14 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
 
   const int tid = threadIdx.x, lane = tid & 31;
   const FpChunk ck = chunks[blockIdx.y];
-  const int g = blockIdx.z;
+  const int g = SPLIT ? blockIdx.z / n_split : blockIdx.z, hs = SPLIT ? blockIdx.z - g * n_split : 0;
   const int b0 = blockIdx.x * FB_NB;
   const XiDims d = ck.cls ? dc : dr;
   const int64_t line_f4 = (int64_t)d.nu + 2 * d.zpad;
   const float4* xi = (ck.cls ? xi_cols : xi_rows) + (int64_t)g * d.nv * line_f4;
-  const int n_bands = (d.nv + FB_RB - 1) / FB_RB;
+  const int n_bands_all = (d.nv + FB_RB - 1) / FB_RB;
+  const int k0 = SPLIT ? (int)((int64_t)hs * n_bands_all / n_split) : 0;
+  const int n_bands = SPLIT ? (int)((int64_t)(hs + 1) * n_bands_all / n_split) : n_bands_all;
   const uint32_t row_bytes = (uint32_t)W * 16u;
 
   if (tid < ck.count) sproj[tid] = projs[ck.first + tid];
@@ -185,12 +192,12 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
     of = fmax(of, -(double)d.zpad);
     of = fmin(of, (double)(d.nu + d.zpad - W));
     const int origin = (int)of;
-    uint64_t* bar = &full[k & 1];
-    if (lane == 0) sorigin[k & 1] = origin;
+    uint64_t* bar = &full[(k - k0) & 1];
+    if (lane == 0) sorigin[(k - k0) & 1] = origin;
     if (lane < FB_RB) {
       if (lane < rows) {
         mbar_arrive_expect_tx(bar, row_bytes);
-        bulk_g2s(buf + ((k & 1) * FB_RB + lane) * W,
+        bulk_g2s(buf + (((k - k0) & 1) * FB_RB + lane) * W,
                  xi + (int64_t)(vb + lane) * line_f4 + (origin + d.zpad), row_bytes, bar);
       } else {
         mbar_arrive(bar);
@@ -198,7 +205,7 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
     }
   };
 
-  if (tid < 32) produce(0);
+  if (tid < 32 && k0 < n_bands) produce(k0);
 
   float acc[FB_PAIRS][4];
 #pragma unroll
@@ -215,14 +222,14 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
   const int idx_hi = W - NC;
   float4 vlast = make_float4(0.f, 0.f, 0.f, 0.f);
 
-  for (int k = 0; k < n_bands; ++k) {
+  for (int k = k0; k < n_bands; ++k) {
     __syncthreads();  // everyone is done with band k-1: its stage may be overwritten
     if (k + 1 < n_bands && tid < 32) produce(k + 1);
-    mbar_wait(&full[k & 1], (uint32_t)((k >> 1) & 1));
-    const int origin = sorigin[k & 1];
+    mbar_wait(&full[(k - k0) & 1], (uint32_t)(((k - k0) >> 1) & 1));
+    const int origin = sorigin[(k - k0) & 1];
     const int vb = k * FB_RB;
     const int rows = min(FB_RB, d.nv - vb);
-    const float4* stage = buf + (k & 1) * FB_RB * W;
+    const float4* stage = buf + ((k - k0) & 1) * FB_RB * W;
 #pragma unroll
     for (int m = 0; m < FB_PAIRS; ++m) {
       const int pj = par + 2 * m;
@@ -271,10 +278,25 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
 #pragma unroll
       for (int sl = 0; sl < 4; ++sl) {
         const int s = g * 4 + sl;
-        if (s < S) sino[((int64_t)s * P + p) * pitch + b] = scale * acc[m][sl];
+        if (s < S) {
+          if (!SPLIT || hs == 0) sino[((int64_t)s * P + p) * pitch + b] = scale * acc[m][sl];
+          else part[(int64_t)(hs - 1) * part_stride + ((int64_t)s * P + p) * part_pitch + b] = scale * acc[m][sl];
+        }
       }
     }
   }
+}
+
+// y[row][b] += sum_h part[h][row][b]
+__global__ void fp_split_combine_kernel(float* __restrict__ y, int64_t pitch_y, const float* __restrict__ part,
+                                        int64_t part_pitch, int64_t part_stride, int n_parts, int B,
+                                        int64_t n_rows) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t row = blockIdx.y + (int64_t)blockIdx.z * gridDim.y;
+  if (b >= B || row >= n_rows) return;
+  float v = y[row * pitch_y + b];
+  for (int h = 0; h < n_parts; ++h) v += part[(int64_t)h * part_stride + row * part_pitch + b];
+  y[row * pitch_y + b] = v;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -582,22 +604,6 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
     d.p = p;
     order[cls].push_back(p);
   }
-  int npj = FB_NPJ;
-  {
-    int n_sm = 148;
-    int dev = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess)
-      cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-    const int64_t slots = 3 * (int64_t)n_sm;
-    const int64_t segs = (g->n_bins + FB_NB - 1) / FB_NB, groups = (g->n_slices + 3) / 4;
-    double best = 1e300;
-    for (int c = FB_NPJ; c >= FB_NPJ / 2; c -= FB_NPJ / 2) {  // cost ~ waves x (work of a block + its fixed part)
-      // (+ 10 %: chunks that straddle a jump in angle are split)
-      const int64_t blocks = segs * groups * (int64_t)((order[0].size() + c - 1) / c + (order[1].size() + c - 1) / c) * 11 / 10;
-      const double cost = (double)((blocks + slots - 1) / slots) * (double)(c + 3);
-      if (cost < best * 0.999) { best = cost; npj = c; }
-    }
-  }
   projs->clear();
   chunks->clear();
   plan->any_rows = !order[0].empty();
@@ -607,11 +613,7 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
   for (int cls = 0; cls < 2; ++cls)
     std::stable_sort(order[cls].begin(), order[cls].end(),
                      [&](int a, int b) { return g->angles_rad[a] < g->angles_rad[b]; });
-  // window width: wide enough for ~all chunks of FB_NPJ neighbours (the 90th percentile of their
-  // widths: a chunk that straddles a jump in angle, e.g. 45 -> 135 degrees inside a walk class, is
-  // simply split below) and for every single projection; at most the capacity
   std::vector<Extent> ext(P);
-  std::vector<int> widths;
   int w_single = 0;
   for (int cls = 0; cls < 2; ++cls) {
     const int nv = cls ? g->nx : g->ny;
@@ -619,15 +621,47 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
       ext[p] = proj_extent(all[p], g->n_bins, nv);
       w_single = std::max(w_single, width_of(ext[p], plan->nc));
     }
-    for (size_t i = 0; i < order[cls].size(); i += npj) {
-      Extent e = ext[order[cls][i]];
-      for (size_t j = i + 1; j < std::min(order[cls].size(), i + npj); ++j) e = merge(e, ext[order[cls][j]]);
-      widths.push_back(width_of(e, plan->nc));
+  }
+  // window width for chunks of c neighbours: wide enough for ~all of them (the 90th percentile of
+  // their widths: a chunk that straddles a jump in angle, e.g. 45 -> 135 degrees inside a walk
+  // class, is simply split below) and for every single projection; at most the capacity
+  auto window_for = [&](int c) {
+    std::vector<int> widths;
+    for (int cls = 0; cls < 2; ++cls)
+      for (size_t i = 0; i < order[cls].size(); i += c) {
+        Extent e = ext[order[cls][i]];
+        for (size_t j = i + 1; j < std::min(order[cls].size(), i + c); ++j) e = merge(e, ext[order[cls][j]]);
+        widths.push_back(width_of(e, plan->nc));
+      }
+    std::sort(widths.begin(), widths.end());
+    const int w_most = widths.empty() ? 0 : widths[(widths.size() - 1) * 9 / 10];
+    return std::min(std::max(std::max(w_most, w_single), plan->nc + 4), FB_WMAX);
+  };
+  // projections per chunk: 16, 8 or 4.  Many neighbours share one staged window (good for dense
+  // angle lists), but their strips fan out (sparse lists: config 4's 16 neighbours span 14 degrees
+  // and need the full 416-pixel window, two blocks per SM).  Cost model, calibrated on configs 2 and 4:
+  // waves of the GPU's block slots (fractional above one) x (projections + fixed part + window
+  // staging) of one block.
+  int npj = FB_NPJ, W = window_for(FB_NPJ);
+  {
+    int n_sm = 148, dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    const int64_t segs = (g->n_bins + FB_NB - 1) / FB_NB, groups = (g->n_slices + 3) / 4;
+    double best = 1e300;
+    for (int c = FB_NPJ; c >= 4; c /= 2) {
+      const int w = window_for(c);
+      const size_t smem = FB_HDR + (size_t)2 * FB_RB * w * 16;
+      const int64_t per_sm = std::max<int64_t>(1, std::min<int64_t>(3, (int64_t)(227 * 1024) / (int64_t)(smem + 1024)));
+      // (+ 10 %: chunks that straddle a jump in angle are split)
+      const int64_t blocks = segs * groups * (int64_t)((order[0].size() + c - 1) / c + (order[1].size() + c - 1) / c) * 11 / 10;
+      const int64_t slots = per_sm * n_sm;
+      const double cost = std::max(1.0, (double)blocks / (double)slots) * ((double)c + 1.0 + (double)w / 64.0);
+      if (std::getenv("PYHST_DEBUG"))
+        std::fprintf(stderr, "[pyhst] fp chunk size %d: W %d, %lld blocks, %lld slots, cost %.1f\n", c, w,
+                     (long long)blocks, (long long)slots, cost);
+      if (cost < best * 0.999) { best = cost; npj = c; W = w; }
     }
   }
-  std::sort(widths.begin(), widths.end());
-  const int w_most = widths.empty() ? 0 : widths[(widths.size() - 1) * 9 / 10];
-  const int W = std::min(std::max(std::max(w_most, w_single), plan->nc + 4), FB_WMAX);
   plan->W = W;
   plan->npj = npj;
   // greedy chunks: add neighbours while the window still fits
@@ -719,19 +753,48 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
     PYHST_CUDA_TRY(cudaGetLastError());
     return PYHST_OK;
   }
-  static size_t configured[3] = {0, 0, 0};
-  const int vi = plan.nc == 3 ? 0 : (plan.nc == 4 ? 1 : 2);
-  auto kern = plan.nc == 3 ? fp_band_kernel<3> : (plan.nc == 4 ? fp_band_kernel<4> : fp_band_kernel<6>);
+  // blocks per SM: 3 (80 registers), or 4 (64 registers) when four windows fit in shared memory;
+  // small grids are split along the lines so that they fill the block slots (deterministic:
+  // partial sums go to a workspace and are added by a second kernel)
+  int n_sm = 148, dev = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  const bool four = plan.nc == 3 && smem <= 56 * 1024;
+  const int64_t blocks = (int64_t)((g->n_bins + FB_NB - 1) / FB_NB) * plan.n_chunks * n_groups;
+  const int64_t slots = (int64_t)n_sm * (four ? 4 : 3);
+  const int n_bands_min = (std::min(g->nx, g->ny) + FB_RB - 1) / FB_RB;
+  int n_split = (int)std::max<int64_t>(1, std::min<int64_t>(4, slots / std::max<int64_t>(blocks, 1)));
+  n_split = std::max(1, std::min(n_split, n_bands_min / 8));
+  static size_t configured[5] = {0, 0, 0, 0, 0};
+  const int vi = four ? 3 : (plan.nc == 3 ? (n_split > 1 ? 4 : 0) : (plan.nc == 4 ? 1 : 2));
+  auto kern = four ? fp_band_kernel<3, 4, true>
+                   : (plan.nc == 3 ? (n_split > 1 ? fp_band_kernel<3, 3, true> : fp_band_kernel<3, 3, false>)
+                                   : (plan.nc == 4 ? fp_band_kernel<4, 3, true> : fp_band_kernel<6, 3, true>));
   if (smem > configured[vi]) {
     PYHST_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured[vi] = smem;
   }
-  dim3 grid((g->n_bins + FB_NB - 1) / FB_NB, plan.n_chunks, n_groups);
+  const int64_t n_rows = (int64_t)g->n_slices * g->n_angles;
+  float* part = nullptr;
+  const int64_t part_pitch = g->n_bins, part_stride = n_rows * part_pitch;
+  if (n_split > 1) {
+    void* wp = nullptr;
+    PYHST_TRY(get_workspace(WS_FPL, (size_t)(n_split - 1) * part_stride * 4, &wp));
+    part = static_cast<float*>(wp);
+  }
+  dim3 grid((g->n_bins + FB_NB - 1) / FB_NB, plan.n_chunks, n_groups * n_split);
   if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
   StageScope scope(ST_FORWARD, stream);
-  scope.kernels();
+  scope.kernels(n_split > 1 ? 2 : 1);
   kern<<<grid, FB_NT, smem, stream>>>(xi_r, xi_c, dr, dc, d_sino, pitch, g->n_slices, g->n_angles,
-                                      g->n_bins, scale, plan.d_projs, plan.d_chunks, W);
+                                      g->n_bins, scale, plan.d_projs, plan.d_chunks, W, n_split, part,
+                                      part_pitch, part_stride);
+  PYHST_CUDA_TRY(cudaGetLastError());
+  if (n_split > 1) {
+    const unsigned gy = (unsigned)std::min<int64_t>(n_rows, 32768);
+    dim3 grid_c((g->n_bins + 255) / 256, gy, (unsigned)((n_rows + gy - 1) / gy));
+    fp_split_combine_kernel<<<grid_c, 256, 0, stream>>>(d_sino, pitch, part, part_pitch, part_stride,
+                                                        n_split - 1, g->n_bins, n_rows);
+  }
   PYHST_CUDA_TRY(cudaGetLastError());
   return PYHST_OK;
 }
