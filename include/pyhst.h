@@ -174,8 +174,9 @@ int pyhst_set_halfacq_stitch(int enable);
 /* Selects the forward-projection kernel: 0 = automatic (default), 1 = generic gather kernel (one
  * thread per bin and slice, global loads; kept for cross-checks and for pixel sizes the banded
  * kernel does not cover), 2 = banded shared-memory kernel (what 0 picks), 3 = interval form of the
- * banded kernel (fewer shared-memory loads, more instructions; slower on B200, kept for
- * comparison).  Returns the previous value. */
+ * banded kernel (fewer shared-memory loads, more instructions), 4 = interval form with 8 slices per
+ * thread (stacks with an even number of slice groups and 16-projection chunks, else as 3); both
+ * are slower than 2 on B200 and kept for comparison.  Returns the previous value. */
 int pyhst_set_forward_project_variant(int variant);
 
 /* Stage accounting for bench.py / tests.  Stages of the hot path, in call order: */

@@ -376,7 +376,7 @@ int pyhst_set_halfacq_stitch(int enable) {
 
 int pyhst_set_forward_project_variant(int variant) {
   const int prev = g_fp_variant;
-  if (variant >= 0 && variant <= 3) g_fp_variant = variant;
+  if (variant >= 0 && variant <= 4) g_fp_variant = variant;
   return prev;
 }
 
@@ -486,7 +486,7 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
     const FpPlan* fplan = nullptr;
     PYHST_TRY(get_fp_plan(g, stream, &fplan));
     if (fplan->n_chunks > 0)
-      return launch_forward_project_banded(d_img, d_sino, pitch, g, scale, *fplan, g_fp_variant == 3, stream);
+      return launch_forward_project_banded(d_img, d_sino, pitch, g, scale, *fplan, g_fp_variant == 3 ? 1 : (g_fp_variant == 4 ? 2 : 0), stream);
     if (g_fp_variant == 2)
       return set_error(PYHST_ERR_UNSUPPORTED, "banded forward projector does not cover pixel_size %g",
                        g->pixel_size);

@@ -173,7 +173,7 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
 void release_fp_plans();
 int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pitch,
                                   const pyhst_geom_t* g, float scale, const FpPlan& plan,
-                                  bool interval, cudaStream_t stream);
+                                  int interval_groups, cudaStream_t stream);
 int forward_project_interval_candidates(double pixel_size);
 
 struct FpArgs {

@@ -313,8 +313,11 @@ __global__ void fp_split_combine_kernel(float* __restrict__ y, int64_t pitch_y, 
 // Measured on config 2 (r01c): shared-memory wavefronts drop from 0.90 to 0.46 per clk per SM, but the
 // two boundary evaluations, the membership masks and the second accumulator set raise the count to
 // 60 warp instructions per (interval, line) against 43 for fp_band_kernel; the kernel becomes issue-
-// bound (80 %) and takes 67.5 ms against 49.7 ms.  Kept selectable for the next step (8 slices per
-// thread would halve the per-line overhead; it needs the two windows to fit in shared memory).
+// bound (80 %) and takes 67.5 ms against 49.7 ms.  With 8 slices per thread (NG = 2, variant 4: the
+// per-line logic is shared by twice the FMAs; bands of 4 lines so that both windows fit) and a
+// three-stage mbarrier ring instead of the per-band block barrier it reaches 49.2 ms against the
+// banded kernel's 47.8 ms: fewer instructions (42.6e9 vs 46.4e9) but two blocks per SM and ~11
+// instructions per line of double-precision boundary set-up per 4-line band.  Kept selectable.
 // Which pixels belong to an interval must be decided identically by the two threads that share a
 // boundary, or a pixel at t ~ b would be counted twice or not at all: both evaluate the SAME
 // expression for the boundary -- the position u*(b, v) of t = b on the line, in double per
@@ -328,41 +331,53 @@ __global__ void fp_split_combine_kernel(float* __restrict__ y, int64_t pitch_y, 
 constexpr int IV_NB = 64;     // intervals per block: 4 warps x 16, the other 4 warps take projections 8..15
 constexpr int IV_PAIRS = IV_NB * FB_NPJ / FB_NT;   // (interval, projection) pairs per thread = 4
 
-template <int NCI>
-__global__ void __launch_bounds__(FB_NT, 3)
+// NG = slice groups per block (1: 4 slices per thread, bands of RB = 8 lines; 2: 8 slices per thread --
+// the boundary / membership / weight logic of a line is shared by twice the FMA work -- bands of RB = 4
+// lines so that both groups' windows fit in shared memory).
+template <int NCI, int NG, int RB>
+__global__ void __launch_bounds__(FB_NT, NG == 2 ? 2 : 3)
 fp_ivl_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_cols, XiDims dr,
               XiDims dc, float* __restrict__ out_u, int64_t pitch_u, float* __restrict__ out_l,
               int64_t pitch_l, int S, int P, int B, float scale, const FpProjD* __restrict__ projs,
               const FpChunk* __restrict__ chunks, int W) {
   extern __shared__ __align__(128) unsigned char smem[];
-  uint64_t* full = reinterpret_cast<uint64_t*>(smem);        // [2]
-  int* sorigin = reinterpret_cast<int*>(smem + 16);          // [2]
+  constexpr int NSTG = 3;                                    // stages of the band ring
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);        // [NSTG]
+  uint64_t* empty = reinterpret_cast<uint64_t*>(smem + 24);  // [NSTG]
+  int* sorigin = reinterpret_cast<int*>(smem + 48);          // [NSTG]
   FpProjD* sproj = reinterpret_cast<FpProjD*>(smem + 64);    // [FB_NPJ]
-  float4* buf = reinterpret_cast<float4*>(smem + FB_HDR);    // [2][FB_RB][W]
+  float4* buf = reinterpret_cast<float4*>(smem + FB_HDR);    // [NSTG][RB][NG][W]
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const FpChunk ck = chunks[blockIdx.y];
-  const int g = blockIdx.z;
+  const int gA = blockIdx.z * NG;
   const int b0 = blockIdx.x * IV_NB;                         // interval b = [b-1, b), b in [b0, b0 + NB)
   const XiDims d = ck.cls ? dc : dr;
   const int64_t line_f4 = (int64_t)d.nu + 2 * d.zpad;
-  const float4* xi = (ck.cls ? xi_cols : xi_rows) + (int64_t)g * d.nv * line_f4;
-  const int n_bands = (d.nv + FB_RB - 1) / FB_RB;
+  const float4* xi = (ck.cls ? xi_cols : xi_rows) + (int64_t)gA * d.nv * line_f4;
+  const int64_t group_f4 = (int64_t)d.nv * line_f4;
+  const int n_bands = (d.nv + RB - 1) / RB;
   const uint32_t row_bytes = (uint32_t)W * 16u;
 
   if (tid < ck.count) sproj[tid] = projs[ck.first + tid];
   if (tid == 0) {
-    mbar_init(&full[0], FB_RB);
-    mbar_init(&full[1], FB_RB);
+#pragma unroll
+    for (int q = 0; q < NSTG; ++q) {
+      mbar_init(&full[q], RB);
+      mbar_init(&empty[q], FB_NT / 32);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
-  // warp 0: window origin of band k (the intervals lie inside the hats of bins b0-1 .. b0+NB-1),
+  // one warp (the role rotates): waits until the stage of band k - NSTG has been read by every warp,
+  // then window origin of band k (the intervals lie inside the hats of bins b0-1 .. b0+NB-1),
   // then one bulk copy per line of the band
   auto produce = [&](int k) {
-    const int vb = k * FB_RB;
-    const int rows = min(FB_RB, d.nv - vb);
+    const int st = k % NSTG;
+    if (k >= NSTG) mbar_wait(&empty[st], (uint32_t)(((k / NSTG) - 1) & 1));
+    const int vb = k * RB;
+    const int rows = min(RB, d.nv - vb);
     double lo = 1e300;
     if (lane < ck.count) {
       const FpProjD pj = sproj[lane];
@@ -377,26 +392,28 @@ fp_ivl_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_
     of = fmax(of, -(double)d.zpad);
     of = fmin(of, (double)(d.nu + d.zpad - W));
     const int origin = (int)of;
-    uint64_t* bar = &full[k & 1];
-    if (lane == 0) sorigin[k & 1] = origin;
-    if (lane < FB_RB) {
+    uint64_t* bar = &full[st];
+    if (lane == 0) sorigin[st] = origin;
+    if (lane < RB) {
       if (lane < rows) {
-        mbar_arrive_expect_tx(bar, row_bytes);
-        bulk_g2s(buf + ((k & 1) * FB_RB + lane) * W,
-                 xi + (int64_t)(vb + lane) * line_f4 + (origin + d.zpad), row_bytes, bar);
+        mbar_arrive_expect_tx(bar, NG * row_bytes);
+#pragma unroll
+        for (int q = 0; q < NG; ++q)
+          bulk_g2s(buf + ((st * RB + lane) * NG + q) * W,
+                   xi + q * group_f4 + (int64_t)(vb + lane) * line_f4 + (origin + d.zpad), row_bytes, bar);
       } else {
         mbar_arrive(bar);
       }
     }
   };
 
-  if (tid < 32) produce(0);
+  if (tid < 32) produce(0);   // bands are issued one ahead of the one being read
 
-  float accu[IV_PAIRS][4], accl[IV_PAIRS][4];
+  float accu[IV_PAIRS][4 * NG], accl[IV_PAIRS][4 * NG];
 #pragma unroll
   for (int m = 0; m < IV_PAIRS; ++m)
 #pragma unroll
-    for (int sl = 0; sl < 4; ++sl) accu[m][sl] = accl[m][sl] = 0.f;
+    for (int sl = 0; sl < 4 * NG; ++sl) accu[m][sl] = accl[m][sl] = 0.f;
 
   // lane pairs hold the same interval of two neighbouring projections (see fp_band_kernel)
   const int bl = (warp & 3) * 16 + (lane >> 1);
@@ -404,13 +421,13 @@ fp_ivl_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_
   const double bd = (double)(b0 + bl);
 
   for (int k = 0; k < n_bands; ++k) {
-    __syncthreads();  // everyone is done with band k-1: its stage may be overwritten
-    if (k + 1 < n_bands && tid < 32) produce(k + 1);
-    mbar_wait(&full[k & 1], (uint32_t)((k >> 1) & 1));
-    const int origin = sorigin[k & 1];
-    const int vb = k * FB_RB;
-    const int rows = min(FB_RB, d.nv - vb);
-    const float4* stage = buf + (k & 1) * FB_RB * W;
+    if (k + 1 < n_bands && warp == ((k + 1) & 7)) produce(k + 1);
+    const int st = k % NSTG;
+    mbar_wait(&full[st], (uint32_t)((k / NSTG) & 1));
+    const int origin = sorigin[st];
+    const int vb = k * RB;
+    const int rows = min(RB, d.nv - vb);
+    const float4* stage = buf + st * RB * NG * W;
 #pragma unroll
     for (int m = 0; m < IV_PAIRS; ++m) {
       const int pj = pj0 + 2 * m;
@@ -429,8 +446,9 @@ fp_ivl_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_
       const int base_m = sg * (int)aiS - origin;      // window index of mirrored pixel aiS
       const float ss = (float)(sigma * sD), cuabs = sp->cuabs;
       const int m_lo = sg > 0 ? 0 : NCI - 1, m_hi = sg > 0 ? W - NCI : W - 1;
-#pragma unroll 2
-      for (int r = 0; r < rows; ++r) {
+#pragma unroll
+      for (int r = 0; r < RB; ++r) {
+        if (r >= rows) break;
         const float rf = (float)r;
         // ceil by a round-up add of 1.5 * 2^23, integer part read from the mantissa
         const float dS = fmaf(ss, rf, afrS), dE = fmaf(ss, rf, afrE);
@@ -440,24 +458,29 @@ fp_ivl_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_
         const float f0 = cuabs * ((jmS - 12582912.f) - dS);                // t - (b-1) of the first one
         int idx = base_m + sg * kS;
         idx = min(max(idx, m_lo), m_hi);              // only acts where the interval is off the image
-        const float4* wp = stage + r * W + idx;
+        const float4* wp = stage + r * NG * W + idx;
 #pragma unroll
         for (int c = 0; c < NCI; ++c) {
           const float f = fmaf((float)c, cuabs, f0);
           const bool in = c < n;
           const float wu = in ? f : 0.f, wl = in ? 1.f - f : 0.f;
-          const float4 v = wp[sg * c];
-          accu[m][0] = fmaf(wu, v.x, accu[m][0]);
-          accu[m][1] = fmaf(wu, v.y, accu[m][1]);
-          accu[m][2] = fmaf(wu, v.z, accu[m][2]);
-          accu[m][3] = fmaf(wu, v.w, accu[m][3]);
-          accl[m][0] = fmaf(wl, v.x, accl[m][0]);
-          accl[m][1] = fmaf(wl, v.y, accl[m][1]);
-          accl[m][2] = fmaf(wl, v.z, accl[m][2]);
-          accl[m][3] = fmaf(wl, v.w, accl[m][3]);
+#pragma unroll
+          for (int q = 0; q < NG; ++q) {
+            const float4 v = wp[q * W + sg * c];
+            accu[m][4 * q + 0] = fmaf(wu, v.x, accu[m][4 * q + 0]);
+            accu[m][4 * q + 1] = fmaf(wu, v.y, accu[m][4 * q + 1]);
+            accu[m][4 * q + 2] = fmaf(wu, v.z, accu[m][4 * q + 2]);
+            accu[m][4 * q + 3] = fmaf(wu, v.w, accu[m][4 * q + 3]);
+            accl[m][4 * q + 0] = fmaf(wl, v.x, accl[m][4 * q + 0]);
+            accl[m][4 * q + 1] = fmaf(wl, v.y, accl[m][4 * q + 1]);
+            accl[m][4 * q + 2] = fmaf(wl, v.z, accl[m][4 * q + 2]);
+            accl[m][4 * q + 3] = fmaf(wl, v.w, accl[m][4 * q + 3]);
+          }
         }
       }
     }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[st]);
   }
 
   // U of interval b is bin b's share, L is bin b-1's (stored at index b of out_l, b in [0, B])
@@ -469,8 +492,8 @@ fp_ivl_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_
       if (pj >= ck.count) break;
       const int p = sproj[pj].p;
 #pragma unroll
-      for (int sl = 0; sl < 4; ++sl) {
-        const int s = g * 4 + sl;
+      for (int sl = 0; sl < 4 * NG; ++sl) {
+        const int s = gA * 4 + sl;
         if (s < S) {
           if (b < B) out_u[((int64_t)s * P + p) * pitch_u + b] = scale * accu[m][sl];
           out_l[((int64_t)s * P + p) * pitch_l + b] = scale * accl[m][sl];
@@ -695,7 +718,8 @@ int forward_project_interval_candidates(double pixel_size) {
 
 int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pitch,
                                   const pyhst_geom_t* g, float scale, const FpPlan& plan,
-                                  bool interval, cudaStream_t stream) {
+                                  int interval_groups, cudaStream_t stream) {
+  const bool interval = interval_groups > 0;
   const int n_groups = (g->n_slices + 3) / 4;
   const int W = plan.W;
   XiLayout Lr{n_groups, g->ny, g->nx, W}, Lc{n_groups, g->nx, g->ny, W};
@@ -732,17 +756,23 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
     const int64_t pitch_l = ((int64_t)g->n_bins + 1 + 3) & ~(int64_t)3;
     void* wl = nullptr;
     PYHST_TRY(get_workspace(WS_FPL, (size_t)n_rows * pitch_l * 4, &wl));
-    static size_t configured_i[2] = {0, 0};
-    auto kern_i = nci == 2 ? fp_ivl_kernel<2> : fp_ivl_kernel<3>;
-    if (smem > configured_i[nci - 2]) {
-      PYHST_CUDA_TRY(cudaFuncSetAttribute(kern_i, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      configured_i[nci - 2] = smem;
+    // 8 slices per thread (two groups per block, bands of 4 lines) when the stack has an even number
+    // of slice groups and full 16-projection chunks (the thread map gives projections 8..15 to warps 4..7)
+    const bool two = nci == 2 && n_groups % 2 == 0 && plan.npj == FB_NPJ && interval_groups == 2;
+    static size_t configured_i[3] = {0, 0, 0};
+    auto kern_i = two ? fp_ivl_kernel<2, 2, 4> : (nci == 2 ? fp_ivl_kernel<2, 1, 8> : fp_ivl_kernel<3, 1, 8>);
+    const int ci = two ? 2 : nci - 2;
+    if (smem > configured_i[ci]) {
+      PYHST_CUDA_TRY(cudaFuncSetAttribute(kern_i, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)(FB_HDR + (size_t)3 * FB_RB * W * 16)));
+      configured_i[ci] = smem;
     }
-    dim3 grid((g->n_bins + 1 + IV_NB - 1) / IV_NB, plan.n_chunks, n_groups);
+    const size_t smem_i = FB_HDR + (size_t)3 * FB_RB * W * 16;   // three stages of RB x NG = 8 lines
+    dim3 grid((g->n_bins + 1 + IV_NB - 1) / IV_NB, plan.n_chunks, two ? n_groups / 2 : n_groups);
     if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
     StageScope scope(ST_FORWARD, stream);
     scope.kernels(2);
-    kern_i<<<grid, FB_NT, smem, stream>>>(xi_r, xi_c, dr, dc, d_sino, pitch, static_cast<float*>(wl), pitch_l,
+    kern_i<<<grid, FB_NT, smem_i, stream>>>(xi_r, xi_c, dr, dc, d_sino, pitch, static_cast<float*>(wl), pitch_l,
                                           g->n_slices, g->n_angles, g->n_bins, scale, plan.d_projs,
                                           plan.d_chunks, W);
     PYHST_CUDA_TRY(cudaGetLastError());

@@ -137,7 +137,7 @@ FP_CASES = [
 ]
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 @pytest.mark.parametrize("case", FP_CASES)
 def test_forward_project_matches_oracle(lib, oracle, case, variant):
     S, P, B, nx, ny, h, axis, drift = case
