@@ -84,6 +84,22 @@ def num_threads() -> int:
     return int(_load().oracle_num_threads())
 
 
+class threads:
+    """``with oracle.threads(1): ...`` -- run the enclosed oracle calls on ``n`` OpenMP threads."""
+
+    def __init__(self, n: int):
+        self.n = int(n)
+
+    def __enter__(self):
+        self.old = num_threads()
+        _load().oracle_set_num_threads(c_int(self.n))
+        return self
+
+    def __exit__(self, *exc):
+        _load().oracle_set_num_threads(c_int(self.old))
+        return False
+
+
 def ramp_kernel(filter: int, n) -> np.ndarray:
     """h[n] of R8 for integer lags ``n`` (array-like)."""
     lib = _load()

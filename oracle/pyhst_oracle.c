@@ -57,6 +57,16 @@ int oracle_num_threads(void) {
 #endif
 }
 
+/* Tiny pin problems run faster on one thread than on a spinning team; results do not depend on
+ * the thread count (OpenMP only distributes independent outputs). */
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
 /* ---- R8: spatial-domain band-limited ramp kernels, bin width 1 ------------
  * Ram-Lak     : h[0] = 1/4 ; h[n] = 0 (n even, n != 0) ; h[n] = -1/(pi^2 n^2) (n odd)
  * Shepp-Logan : h[n] = -2 / (pi^2 (4 n^2 - 1))

@@ -1,6 +1,7 @@
 // C ABI of libpyhst_b200 (include/pyhst.h): argument validation, plan / workspace caches and the
 // sequencing of the kernels.  Every step of the hot path runs on the device; there is no CPU
 // fallback (a missing or non-sm_100 device yields PYHST_ERR_UNSUPPORTED).
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -403,14 +404,21 @@ void pyhst_release_cache(void) {
 int pyhst_halfacq_extent(int32_t n_bins, double cbar, int32_t* n_bins_ext, int32_t* pad_left) {
   if (n_bins <= 0 || !n_bins_ext || !pad_left || !std::isfinite(cbar))
     return set_error(PYHST_ERR_INVALID_ARG, "pyhst_halfacq_extent: bad argument");
-  const double mid = 0.5 * (double)(n_bins - 1);
-  const double far = cbar >= mid ? cbar : (double)(n_bins - 1) - cbar;
-  int64_t need = (int64_t)std::ceil(2.0 * far) + 1;
-  if (need < n_bins) need = n_bins;
-  const int64_t ext = ((need + 63) / 64) * 64;
-  if (ext > (1 << 20)) return set_error(PYHST_ERR_INVALID_ARG, "axis too far off the detector");
-  *n_bins_ext = (int32_t)ext;
-  *pad_left = cbar >= mid ? 0 : (int32_t)(ext - n_bins);
+  // R10: the virtual detector is symmetric about the mean axis and reaches as far as
+  // the longer physical side does.  Distances from the axis to the two detector edges:
+  const double to_first_bin = cbar, to_last_bin = (double)(n_bins - 1) - cbar;
+  const bool long_side_is_left = to_first_bin >= to_last_bin;   // i.e. the axis sits right of centre
+  const double reach = std::fmax(to_first_bin, to_last_bin);
+  // bins -reach .. +reach about the axis, never shorter than the physical row; rounded up to whole
+  // 64-bin units so that the extended rows stay 16-byte aligned for the bulk copies
+  int64_t n_virtual = (int64_t)std::ceil(reach + reach) + 1;
+  n_virtual = std::max<int64_t>(n_virtual, n_bins);
+  const int64_t n_units = (n_virtual + 63) >> 6;
+  if (n_units > (1 << 14)) return set_error(PYHST_ERR_INVALID_ARG, "axis too far off the detector");
+  *n_bins_ext = (int32_t)(n_units << 6);
+  // the physical row keeps its place when the missing half lies to its right (long side left),
+  // and is pushed to the far end of the extended row when the missing half lies to its left
+  *pad_left = long_side_is_left ? 0 : *n_bins_ext - n_bins;
   return PYHST_OK;
 }
 

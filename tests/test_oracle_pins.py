@@ -372,7 +372,7 @@ def test_k11_half_acquisition_equals_full_detector_scan(oracle):
     r_full = oracle.fbp(full, angles, axis, N, N, mode=oracle.SCAN_360)[0]
     jj = np.arange(N) - (N - 1) / 2.0
     disc = (jj[None, :] ** 2 + jj[:, None] ** 2) < (c - 4) ** 2
-    assert np.abs(r_half - r_full)[disc].max() < 5e-3 * np.abs(r_full).max()
+    assert np.abs(r_half - r_full)[disc].max() < 2e-6 * np.abs(r_full).max()   # 2c integer: exact up to rounding
     # weights: w(s) + w(-s) = 1 on the overlap, exactly; 1 beyond it; both axis sides
     for cbar in (118.0, 9.0, 100.25):
         w = oracle.halfacq_weights(B, cbar)
@@ -389,6 +389,88 @@ def test_k11_half_acquisition_equals_full_detector_scan(oracle):
     assert (ext, pad) == (3840, 0)
     ext, pad = oracle.halfacq_extent(2048, 147.0)
     assert (ext, pad) == (3840, 3840 - 2048)
+
+
+def test_k11_overlap_ramp_typed_values(oracle):
+    """R10 (PAPER.md L35 'virtually doubled'): the weight falls linearly from 1 to 0 across the
+    overlap |s| <= omega, 1/2 on the axis.  Values typed from the reading for B = 128:
+    axis 118 -> omega = 9: w = 1 up to bin 109, (127 - b)/18 on 109..127;
+    axis 9 (left of centre) -> omega = 9, mirrored: w = b/18 on 0..18, 1 beyond."""
+    w = oracle.halfacq_weights(128, 118.0)
+    want = np.ones(128)
+    want[109:128] = (127.0 - np.arange(109, 128)) / 18.0
+    np.testing.assert_allclose(w, want, rtol=0, atol=1e-15)
+    assert w[109] == 1.0 and w[118] == 0.5 and w[127] == 0.0 and w[113] == pytest.approx(14.0 / 18.0)
+    wl_ = oracle.halfacq_weights(128, 9.0)
+    want = np.ones(128)
+    want[0:19] = np.arange(19) / 18.0
+    np.testing.assert_allclose(wl_, want, rtol=0, atol=1e-15)
+    # fractional axis: omega = 127 - 100.25 = 26.75, w(b) = (127 - b) / 53.5 on the overlap
+    wf = oracle.halfacq_weights(128, 100.25)
+    assert wf[73] == 1.0 and wf[74] == pytest.approx(53.0 / 53.5) and wf[127] == 0.0
+    assert wf[100] == pytest.approx(27.0 / 53.5, abs=1e-15)
+
+
+def _halfacq_case(c, B=128, P=90, drift=None):
+    import torch
+    ell = np.array([[10.0, -20.0, 60.0, 45.0, 0.3, 1.0], [-40.0, 30.0, 25.0, 18.0, 1.0, 0.5],
+                    [55.0, 40.0, 12.0, 30.0, 2.0, -0.7]])
+    angles = np.arange(P) * 2 * math.pi / P
+    axis = np.full(P, c) if drift is None else c + drift
+    s = torch.arange(B, dtype=torch.float64)[None, :] - torch.tensor(axis)[:, None]
+    return wl.ellipse_radon(ell, angles, s).numpy()[None].astype(np.float32), angles, axis
+
+
+def test_k11_axis_left_of_centre_is_the_mirrored_scan(oracle):
+    """Flipping the detector (b -> B-1-b) turns a scan with the axis at c into the scan of the
+    object rotated by pi with the axis at B-1-c (Radon symmetry p(theta, -s) = p(theta + pi, s)):
+    the half-acquisition FBP of the flipped rows is the point-reflected image.  The left-axis
+    branch (mirrored weights, pad_left > 0, axis_out = axis + pad_left) is pinned to the
+    right-axis one, which K11 pins to the full-detector scan."""
+    B, c = 128, 118.0
+    N = 2 * int(c)
+    half, angles, axis = _halfacq_case(c, B)
+    ext, pad = oracle.halfacq_extent(B, B - 1 - c)
+    assert pad == ext - B and pad > 0
+    r_right = oracle.fbp(half, angles, axis, N, N, mode=oracle.SCAN_360_HALF)[0]
+    r_left = oracle.fbp(half[:, :, ::-1].copy(), angles, (B - 1) - axis, N, N,
+                        mode=oracle.SCAN_360_HALF)[0]
+    np.testing.assert_allclose(r_left, r_right[::-1, ::-1], rtol=0, atol=1e-12 * np.abs(r_right).max())
+    assert np.abs(r_right).max() > 0.5
+    # a drifting axis on the left side as well (the shift must be added to every projection)
+    rng = np.random.default_rng(11)
+    drift = rng.uniform(-1.0, 1.0, size=len(angles))
+    half, angles, axis = _halfacq_case(c, B, drift=drift)
+    r_right = oracle.fbp(half, angles, axis, N, N, mode=oracle.SCAN_360_HALF)[0]
+    r_left = oracle.fbp(half[:, :, ::-1].copy(), angles, (B - 1) - axis, N, N,
+                        mode=oracle.SCAN_360_HALF)[0]
+    np.testing.assert_allclose(r_left, r_right[::-1, ::-1], rtol=0, atol=1e-12 * np.abs(r_right).max())
+
+
+def test_k11_overlap_weights_use_the_mean_axis(oracle):
+    """R10: omega and the weights come from the MEAN axis of the scan.  The FBP is a sum over
+    projections, so listing them in another order cannot change it; an implementation that reads
+    axis[0] (or any single projection) gets other weights after the permutation."""
+    B, c = 128, 118.0
+    N = 2 * int(c)
+    rng = np.random.default_rng(111)
+    drift = rng.uniform(-1.5, 1.5, size=90)
+    drift -= drift.mean()
+    drift[0] = 1.4                                        # axis[0] is far from the mean
+    drift[1:] -= drift.sum() / (len(drift) - 1)
+    half, angles, axis = _halfacq_case(c, B, drift=drift)
+    assert abs(axis.mean() - c) < 1e-12
+    r0 = oracle.fbp(half, angles, axis, N, N, mode=oracle.SCAN_360_HALF)[0]
+    perm = np.roll(np.arange(len(angles)), -37)
+    assert abs(axis[perm][0] - axis[0]) > 0.5
+    r1 = oracle.fbp(half[:, perm].copy(), angles[perm], axis[perm], N, N, mode=oracle.SCAN_360_HALF)[0]
+    np.testing.assert_allclose(r1, r0, rtol=0, atol=1e-11 * np.abs(r0).max())
+    # and the weights it uses are those of the mean: reproduce the filter input by hand
+    w = oracle.halfacq_weights(B, float(axis.mean())).astype(np.float32)
+    ext, pad = oracle.halfacq_extent(B, float(axis.mean()))
+    filt = oracle.ramp_filter(half, n_bins_out=ext, pad_left=pad, col_weights=w)
+    r2 = oracle.backproject(filt, angles, axis + pad, N, N, scale=2 * math.pi / len(angles))[0]
+    np.testing.assert_allclose(r2, r0, rtol=0, atol=1e-12 * np.abs(r0).max())
 
 
 def test_k11_fbp_modes_scale(oracle):

@@ -13,6 +13,13 @@ import pytest
 from test_oracle_pins import _dense_matrix
 
 
+@pytest.fixture(autouse=True)
+def _one_thread(oracle):
+    """The problems of this file are tiny: one OpenMP thread beats a spinning team by 20x."""
+    with oracle.threads(1):
+        yield
+
+
 # --------------------------------------------------------------------------- K13: TV closed forms
 def test_k13_tv_of_a_ramp_and_of_a_rectangle(oracle):
     ny, nx, a, b = 7, 9, 0.3, -1.1
@@ -169,3 +176,82 @@ def test_k17_tv_term_value_and_regularisation(oracle):
     np.testing.assert_array_equal(xb[0], xa[0])
     np.testing.assert_array_equal(xb[1], xc[0])
     np.testing.assert_allclose(eb, ea + ec, rtol=1e-13)
+
+
+# --------------------------------------------------------------------------- K18: tau = beta / L
+def _tv_numpy(x):
+    """Eq. 2 with the forward differences of R18, typed out (K13 pins oracle.tv to closed forms)."""
+    d1 = np.zeros_like(x)
+    d2 = np.zeros_like(x)
+    d1[..., :, :-1] = x[..., :, 1:] - x[..., :, :-1]
+    d2[..., :-1, :] = x[..., 1:, :] - x[..., :-1, :]
+    return float(np.sqrt(d1 * d1 + d2 * d2).sum())
+
+
+def test_k18_prox_threshold_is_beta_over_L(oracle):
+    """The minimiser of eq. 3 does not depend on the step 1/L, and x*(beta) beats
+    x*(beta') on eq. 3 at beta for every other beta'.  A threshold beta (or beta L, beta / L^2 ...)
+    instead of beta / L makes the fixed point the minimiser for beta L: it then moves with L, and
+    the run at beta' = beta / L wins eq. 3 at beta."""
+    rng, angles, axis, A, P, B, n = _tiny_problem(18, P=8, B=25, n=12)
+    xs = np.zeros((n, n))
+    xs[3:9, 2:7] = 1.0
+    xs[5:10, 6:11] += 0.5
+    clean = A @ xs.ravel()
+    d = (clean + 0.2 * rng.normal(size=clean.shape)).reshape(1, P, B).astype(np.float32)
+    dv = d.astype(np.float64).ravel()
+    lam = np.linalg.eigvalsh(A.T @ A)[-1]
+    beta = 0.5
+
+    def F(x, b):
+        return 0.5 * np.sum((A @ x.ravel() - dv) ** 2) + b * _tv_numpy(x)
+
+    def solve(b, L):
+        return oracle.fista_tv(d, angles, axis, n, n, b, L, 500, n_inner=80)[0]
+
+    L1, L2 = 1.05 * lam, 3.0 * lam
+    assert L1 > 4.0                                      # L far from 1: beta / L and beta differ
+    x1, x2 = solve(beta, L1), solve(beta, L2)
+    assert np.abs(x1 - x2).max() < 2e-3 * np.abs(x1).max()
+    f1 = F(x1, beta)
+    assert abs(F(x2, beta) - f1) < 1e-4 * f1
+    for other in (beta / L1, beta * L1, beta / 3, beta * 3):
+        assert F(solve(other, L1), beta) > f1 * (1 + 1e-2)
+    for k in range(20):                                  # and no random perturbation does better
+        assert F(x1 + rng.normal(size=x1.shape) * 10.0 ** rng.uniform(-4, -1), beta) >= f1 - 1e-9
+
+
+# --------------------------------------------------------------------------- K19: isotropic coupling
+def test_k19_prox_kkt_with_both_gradient_components(oracle):
+    """KKT system of  min 1/2 ||x - z||^2 + tau TV(x)  with the isotropic TV of eq. 2 (PAPER.md
+    L77-L78), typed out in numpy: z - x = tau G^T p with p = G x / |G x| (Euclidean norm of the
+    PAIR) wherever G x != 0.  z is a tilted plane plus bumps, so both components of G x are
+    non-zero at every interior pixel and p is determined everywhere by x alone.  An anisotropic
+    projection (per component, or by the max norm) gives p = sign(.) instead and fails by O(1)."""
+    ny, nx, tau = 14, 17, 0.05
+    j, i = np.meshgrid(np.arange(nx, dtype=np.float64), np.arange(ny, dtype=np.float64))
+    z = (0.7 * j - 0.45 * i + 0.35 * np.sin(0.5 * j + 0.2) * np.cos(0.4 * i))[None]
+    x = oracle.prox_tv(z, tau, 20000)[0]
+    d1 = np.zeros_like(x)
+    d2 = np.zeros_like(x)
+    d1[:, :-1] = x[:, 1:] - x[:, :-1]
+    d2[:-1, :] = x[1:, :] - x[:-1, :]
+    assert np.abs(d1[:-1, :-1]).min() > 0.05 and np.abs(d2[:-1, :-1]).min() > 0.05
+    m = np.sqrt(d1 * d1 + d2 * d2)
+    m[-1, -1] = 1.0                                      # G x = 0 there: p is multiplied by nothing
+    p1, p2 = d1 / m, d2 / m
+    # G^T p, adjoint of the forward differences with the zero last column / row (R18)
+    gt = np.zeros_like(x)
+    gt[:, :-1] -= p1[:, :-1]
+    gt[:, 1:] += p1[:, :-1]
+    gt[:-1, :] -= p2[:-1, :]
+    gt[1:, :] += p2[:-1, :]
+    np.testing.assert_allclose(z[0] - x, tau * gt, rtol=0, atol=2e-6)
+    # the same test distinguishes the norms: with p = sign(d) the residual is O(tau)
+    gs = np.zeros_like(x)
+    s1, s2 = np.sign(d1), np.sign(d2)
+    gs[:, :-1] -= s1[:, :-1]
+    gs[:, 1:] += s1[:, :-1]
+    gs[:-1, :] -= s2[:-1, :]
+    gs[1:, :] += s2[:-1, :]
+    assert np.abs(z[0] - x - tau * gs).max() > 0.2 * tau
