@@ -10,12 +10,22 @@
  * - `d_*` pointers are DEVICE pointers owned by the caller (4-byte aligned); `h_*` pointers
  *   and the arrays inside pyhst_geom_t are HOST pointers that need only live for the duration
  *   of the call (the library copies them).
- * - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = default stream).
- *   There is no implicit device synchronisation in the d_* entry points: errors detectable at
- *   enqueue time are returned, asynchronous faults surface at the caller's next sync.
- *   The *_host entry points synchronise `stream` before returning.
- * - Internal workspace (filtered sinogram, filter spectra, per-projection geometry tables,
- *   TMA tensor maps) lives in a cache keyed by shapes; pyhst_release_cache() frees it.
+ * - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = default stream) of the
+ *   CURRENT device.  Errors detectable at enqueue time are returned, asynchronous faults surface
+ *   at the caller's next sync.  The *_host entry points synchronise `stream` before returning.
+ * - Concurrency rule: ONE CALL IN FLIGHT PER DEVICE.  All library state (workspace, plans, geometry
+ *   tables) is kept per device and shared by that device's calls, so the library serialises them:
+ *   entry points may be called from any thread and on any stream, but a call takes the device's
+ *   lock while it enqueues, and a call on another stream than the previous one first makes its
+ *   stream wait (cudaStreamWaitEvent, on the device, no host block) for the previous call's work.
+ *   Calls on one stream cost nothing extra.  Different devices are independent.
+ * - Synchronisation: in steady state (same shapes as an earlier call) the d_* entry points only
+ *   enqueue.  The FIRST call with a new shape, filter or geometry builds plans and may grow the
+ *   workspace: cudaMalloc / cudaFree of a grown block, one-time cuFFT plan creation and the
+ *   one-time ramp-spectrum set-up synchronise the device or `stream`.  Warm the shapes up once
+ *   (one call per shape) before a latency-critical loop or a CUDA-graph capture.
+ * - Internal workspace (filtered sinogram, filter spectra, per-projection geometry tables)
+ *   lives in a per-device cache keyed by shapes; pyhst_release_cache() frees it on every device.
  * - There is no CPU fallback: a missing/non-sm_100 device yields PYHST_ERR_UNSUPPORTED.
  * - On any error nothing is written to the output buffers and pyhst_last_error() describes it.
  *
@@ -155,29 +165,6 @@ int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geom_t* g, flo
  * far = max(cbar, n_bins-1-cbar); *n_bins_ext = ceil(2 far) + 1 rounded up to a multiple of
  * 64; *pad_left = 0 if the axis is right of the detector centre else n_bins_ext - n_bins. */
 int pyhst_halfacq_extent(int32_t n_bins, double cbar, int32_t* n_bins_ext, int32_t* pad_left);
-
-/* Selects the backprojection kernel: 0 = automatic (default), 1 = reference one-thread-per-
- * pixel kernel (global loads; kept for cross-checks), 2 = tiled shared-memory kernel, 3 = run
- * kernel with 4 slices per thread, 4 = run kernel with 8 slices per thread (what 0 picks for
- * pixel sizes below sqrt(2) bins).  A variant that does not cover the geometry makes the next
- * call return PYHST_ERR_UNSUPPORTED.  Returns the previous value.  Test/bench hook; results
- * agree within FP32 rounding. */
-int pyhst_set_backproject_variant(int variant);
-
-/* PYHST_SCAN_360_HALF only (NEXT row N2): 1 (default) lets pyhst_fbp fold a scan whose projections p
- * and p + P/2 face each other (angles differ by pi to 1e-10, equal axis, 2 x axis integer) into P/2
- * full-width rows, lerp(g_p, t) + lerp(g_{p+P/2}, 2c - t) = lerp(g_p + flip(g_{p+P/2}), t), and
- * backproject half as many projections; 0 always backprojects all P rows.  Scans that do not pair up
- * take the general path either way.  Returns the previous value. */
-int pyhst_set_halfacq_stitch(int enable);
-
-/* Selects the forward-projection kernel: 0 = automatic (default), 1 = generic gather kernel (one
- * thread per bin and slice, global loads; kept for cross-checks and for pixel sizes the banded
- * kernel does not cover), 2 = banded shared-memory kernel (what 0 picks), 3 = interval form of the
- * banded kernel (fewer shared-memory loads, more instructions), 4 = interval form with 8 slices per
- * thread (stacks with an even number of slice groups and 16-projection chunks, else as 3); both
- * are slower than 2 on B200 and kept for comparison.  Returns the previous value. */
-int pyhst_set_forward_project_variant(int variant);
 
 /* Stage accounting for bench.py / tests.  Stages of the hot path, in call order: */
 enum {

@@ -1,0 +1,41 @@
+/*
+ * pyhst_test.h -- test / bench hooks of libpyhst_b200 (NOT part of the product API of pyhst.h).
+ *
+ * Process-wide switches that select older or alternative kernels for cross-checks.  They are
+ * plain globals read at the start of a call: set them only while no call is in flight.  Every
+ * variant computes the operation pyhst.h defines; results agree within FP32 rounding.
+ */
+#ifndef PYHST_TEST_H_
+#define PYHST_TEST_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Selects the backprojection kernel: 0 = automatic (default), 1 = reference one-thread-per-
+ * pixel kernel (global loads; kept for cross-checks), 2 = tiled shared-memory kernel, 3 = run
+ * kernel with 4 slices per thread, 4 = run kernel with 8 slices per thread (what 0 picks for
+ * pixel sizes below sqrt(2) bins).  A variant that does not cover the geometry makes the next
+ * call return PYHST_ERR_UNSUPPORTED.  Returns the previous value.  Test/bench hook; results
+ * agree within FP32 rounding. */
+int pyhst_set_backproject_variant(int variant);
+
+/* PYHST_SCAN_360_HALF only (NEXT row N2): 1 (default) lets pyhst_fbp fold a scan whose projections p
+ * and p + P/2 face each other (angles differ by pi to 1e-10, equal axis, 2 x axis integer) into P/2
+ * full-width rows, lerp(g_p, t) + lerp(g_{p+P/2}, 2c - t) = lerp(g_p + flip(g_{p+P/2}), t), and
+ * backproject half as many projections; 0 always backprojects all P rows.  Scans that do not pair up
+ * take the general path either way.  Returns the previous value. */
+int pyhst_set_halfacq_stitch(int enable);
+
+/* Selects the forward-projection kernel: 0 = automatic (default), 1 = generic gather kernel (one
+ * thread per bin and slice, global loads; kept for cross-checks and for pixel sizes the banded
+ * kernel does not cover), 2 = banded shared-memory kernel (what 0 picks), 3 = interval form of the
+ * banded kernel (fewer shared-memory loads, more instructions), 4 = interval form with 8 slices per
+ * thread (stacks with an even number of slice groups and 16-projection chunks, else as 3); both
+ * are slower than 2 on B200 and kept for comparison.  Returns the previous value. */
+int pyhst_set_forward_project_variant(int variant);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PYHST_TEST_H_ */

@@ -6,6 +6,8 @@
 #include <cstdlib>
 #include <cstring>
 #include <list>
+#include <map>
+#include <memory>
 #include <mutex>
 
 #include "common.h"
@@ -51,20 +53,88 @@ int require_sm100(int* n_sm) {
   return PYHST_OK;
 }
 
-// ---- caches ------------------------------------------------------------------------------
+// ---- per-device state ----------------------------------------------------------------------
+struct Ws { void* p = nullptr; size_t bytes = 0; uint64_t gen = 0; };
+struct DeviceCtx {
+  int device = 0;
+  std::recursive_mutex mu;      // held by the open CallScope(s) of one thread
+  int depth = 0;                // nesting of entry points inside the outermost call
+  cudaEvent_t last_done = nullptr;
+  cudaStream_t last_stream = nullptr;
+  bool have_last = false;
+  std::list<GeomPlan> geom;
+  std::list<FpPlan> fp_plans;
+  Ws ws[WS_COUNT];
+  cudaStream_t streams[3] = {nullptr, nullptr, nullptr};
+  cudaEvent_t events[8] = {nullptr};
+  uint64_t tick = 0;
+};
+
 namespace {
-std::mutex g_mu;
-std::list<GeomPlan> g_geom;
-uint64_t g_tick = 0;
-struct Ws { void* p = nullptr; size_t bytes = 0; };
-Ws g_ws[WS_COUNT];
+std::mutex g_map_mu;
+std::map<int, std::unique_ptr<DeviceCtx>> g_ctx;
 int g_bp_variant = 0;
 int g_fp_variant = 0;
 int g_halfacq_stitch = 1;
-std::list<FpPlan> g_fp_plans;
-cudaStream_t g_streams[3] = {nullptr, nullptr, nullptr};
-cudaEvent_t g_events[8] = {nullptr};
+
+DeviceCtx* ctx_of(int dev) {
+  std::lock_guard<std::mutex> lock(g_map_mu);
+  auto& slot = g_ctx[dev];
+  if (!slot) {
+    slot.reset(new DeviceCtx());
+    slot->device = dev;
+  }
+  return slot.get();
+}
+// state of the current device; only called inside an open CallScope (or under its own lock)
+DeviceCtx& ctx() { return *ctx_of(std::max(0, current_device())); }
 }  // namespace
+
+int current_device() {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) {
+    cudaGetLastError();
+    return -1;
+  }
+  return dev;
+}
+
+bool first_use_on_device(uint64_t* mask) {
+  const int dev = std::max(0, current_device()) & 63;
+  if ((*mask >> dev) & 1) return false;
+  *mask |= (uint64_t)1 << dev;
+  return true;
+}
+
+size_t& PerDeviceSize::here() { return v[std::max(0, current_device()) & 63]; }
+
+CallScope::CallScope(cudaStream_t stream_) : stream(stream_) {
+  const int dev = current_device();
+  if (dev < 0) return;   // no device: the entry point's require_sm100() reports it
+  ctx = ctx_of(dev);
+  ctx->mu.lock();
+  if (ctx->depth++ == 0 && ctx->have_last && ctx->last_stream != stream) {
+    cudaError_t e = cudaStreamWaitEvent(stream, ctx->last_done, 0);
+    if (e != cudaSuccess)
+      status = set_error(PYHST_ERR_CUDA, "cudaStreamWaitEvent on the previous call failed: %s",
+                         cudaGetErrorString(e));
+  }
+}
+
+CallScope::~CallScope() {
+  if (!ctx) return;
+  if (--ctx->depth == 0) {
+    if (!ctx->last_done) cudaEventCreateWithFlags(&ctx->last_done, cudaEventDisableTiming);
+    if (ctx->last_done && cudaEventRecord(ctx->last_done, stream) == cudaSuccess) {
+      ctx->last_stream = stream;
+      ctx->have_last = true;
+    } else {
+      cudaGetLastError();
+      ctx->have_last = false;
+    }
+  }
+  ctx->mu.unlock();
+}
 
 // ---- stage accounting --------------------------------------------------------------------
 namespace {
@@ -113,7 +183,10 @@ void StageScope::library(int n) {
 
 int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cudaStream_t stream,
                   const GeomPlan** out) {
-  std::lock_guard<std::mutex> lock(g_mu);
+  DeviceCtx& c = ctx();
+  std::lock_guard<std::recursive_mutex> lock(c.mu);
+  auto& g_geom = c.geom;
+  uint64_t& g_tick = c.tick;
   const size_t n = (size_t)g->n_angles;
   for (auto& pl : g_geom) {
     if (pl.n_angles == g->n_angles && pl.n_bins == n_bins && pl.pixel_size == g->pixel_size &&
@@ -191,7 +264,10 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
 }
 
 int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out) {
-  std::lock_guard<std::mutex> lock(g_mu);
+  DeviceCtx& c = ctx();
+  std::lock_guard<std::recursive_mutex> lock(c.mu);
+  auto& g_fp_plans = c.fp_plans;
+  uint64_t& g_tick = c.tick;
   const size_t n = (size_t)g->n_angles;
   for (auto& pl : g_fp_plans) {
     if (pl.n_angles == g->n_angles && pl.n_bins == g->n_bins && pl.nx == g->nx && pl.ny == g->ny &&
@@ -243,23 +319,17 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out) 
   return PYHST_OK;
 }
 
-void release_fp_plans() {
-  for (auto& pl : g_fp_plans) {
-    cudaFree(pl.d_projs);
-    cudaFree(pl.d_chunks);
-  }
-  g_fp_plans.clear();
-}
-
 int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr) {
-  std::lock_guard<std::mutex> lock(g_mu);
-  Ws& w = g_ws[slot];
+  DeviceCtx& c = ctx();
+  std::lock_guard<std::recursive_mutex> lock(c.mu);
+  Ws& w = c.ws[slot];
   if (w.bytes < bytes) {
     if (w.p) {
       cudaFree(w.p);  // synchronises the device: nothing can still be using the old block
       w.p = nullptr;
       w.bytes = 0;
     }
+    ++w.gen;
     cudaError_t e = cudaMalloc(&w.p, bytes);
     if (e != cudaSuccess) {
       cudaGetLastError();
@@ -271,6 +341,12 @@ int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr) {
   }
   *ptr = w.p;
   return PYHST_OK;
+}
+
+uint64_t workspace_generation(WorkspaceSlot slot) {
+  DeviceCtx& c = ctx();
+  std::lock_guard<std::recursive_mutex> lock(c.mu);
+  return c.ws[slot].gen;
 }
 
 // ---- validation --------------------------------------------------------------------------
@@ -382,23 +458,42 @@ int pyhst_set_forward_project_variant(int variant) {
 }
 
 void pyhst_release_cache(void) {
-  cudaDeviceSynchronize();
+  int prev = current_device();
+  std::vector<DeviceCtx*> all;
+  {
+    std::lock_guard<std::mutex> lock(g_map_mu);
+    for (auto& kv : g_ctx) all.push_back(kv.second.get());
+  }
+  for (DeviceCtx* c : all) {
+    std::lock_guard<std::recursive_mutex> lock(c->mu);
+    if (cudaSetDevice(c->device) != cudaSuccess) { cudaGetLastError(); continue; }
+    cudaDeviceSynchronize();
+    for (auto& pl : c->fp_plans) {
+      cudaFree(pl.d_projs);
+      cudaFree(pl.d_chunks);
+    }
+    c->fp_plans.clear();
+    for (auto& pl : c->geom) {
+      cudaFree(pl.d_proj);
+      cudaFree(pl.d_run);
+      cudaFree(pl.d_flip);
+      cudaFreeHost(pl.h_pinned);
+    }
+    c->geom.clear();
+    for (int i = 0; i < WS_COUNT; ++i) {
+      if (c->ws[i].p) cudaFree(c->ws[i].p);
+      c->ws[i].p = nullptr;
+      c->ws[i].bytes = 0;
+      ++c->ws[i].gen;
+    }
+    for (auto& st : c->streams) if (st) { cudaStreamDestroy(st); st = nullptr; }
+    for (auto& e : c->events) if (e) { cudaEventDestroy(e); e = nullptr; }
+    if (c->last_done) { cudaEventDestroy(c->last_done); c->last_done = nullptr; }
+    c->have_last = false;
+  }
   release_filter_plans();
-  std::lock_guard<std::mutex> lock(g_mu);
-  release_fp_plans();
-  for (auto& pl : g_geom) {
-    cudaFree(pl.d_proj);
-    cudaFree(pl.d_run);
-    cudaFree(pl.d_flip);
-    cudaFreeHost(pl.h_pinned);
-  }
-  g_geom.clear();
-  for (int i = 0; i < WS_COUNT; ++i) {
-    if (g_ws[i].p) cudaFree(g_ws[i].p);
-    g_ws[i] = Ws();
-  }
-  for (auto& s : g_streams) if (s) { cudaStreamDestroy(s); s = nullptr; }
-  for (auto& e : g_events) if (e) { cudaEventDestroy(e); e = nullptr; }
+  if (prev >= 0) cudaSetDevice(prev);
+  cudaGetLastError();
 }
 
 int pyhst_halfacq_extent(int32_t n_bins, double cbar, int32_t* n_bins_ext, int32_t* pad_left) {
@@ -444,6 +539,7 @@ int pyhst_ramp_filter(const float* d_in, float* d_out, int64_t n_rows, int32_t n
   if ((int64_t)n_bins_in + n_bins_out > 16384)
     return set_error(PYHST_ERR_UNSUPPORTED, "n_bins_in + n_bins_out > 16384");
   PYHST_TRY(require_sm100(nullptr));
+  PYHST_CALL_SCOPE(static_cast<cudaStream_t>(stream));
   return launch_ramp_filter(d_in, n_bins_in, n_rows, n_bins_in, n_bins_out, pad_left, (int)f,
                             d_col_weights, d_out, out_pitch, nullptr, nullptr, 0, nullptr,
                             static_cast<cudaStream_t>(stream));
@@ -457,6 +553,7 @@ int pyhst_backproject(const float* d_sino, float* d_img, const pyhst_geom_t* g, 
   PYHST_TRY(check_ptr(d_img, "d_img"));
   PYHST_TRY(check_geom(g, &pitch));
   PYHST_TRY(require_sm100(nullptr));
+  PYHST_CALL_SCOPE(stream);
   const GeomPlan* plan = nullptr;
   PYHST_TRY(get_geom_plan(g, 0.0, g->n_bins, stream, &plan));
   BpArgs a{d_img, g->n_slices, g->n_angles, g->n_bins, g->nx, g->ny, scale, plan->d_proj,
@@ -488,6 +585,7 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
   PYHST_TRY(check_ptr(d_sino, "d_sino"));
   PYHST_TRY(check_geom(g, &pitch));
   PYHST_TRY(require_sm100(nullptr));
+  PYHST_CALL_SCOPE(stream);
   const GeomPlan* plan = nullptr;
   PYHST_TRY(get_geom_plan(g, 0.0, g->n_bins, stream, &plan));
   if (g_fp_variant != 1) {
@@ -627,6 +725,7 @@ int pyhst_fbp(const float* d_sino_raw, float* d_img, const pyhst_geom_t* g, pyhs
   PYHST_TRY(check_ptr(d_sino_raw, "d_sino_raw"));
   PYHST_TRY(check_ptr(d_img, "d_img"));
   PYHST_TRY(check_fbp(g, f, mode, &pitch));
+  PYHST_CALL_SCOPE(static_cast<cudaStream_t>(stream));
   return fbp_device(d_sino_raw, pitch, d_img, g, g->n_slices, f, mode, static_cast<cudaStream_t>(stream));
 }
 
@@ -639,13 +738,15 @@ template <class Body>
 static int host_pipeline(const float* h_in, size_t in_floats_per_slice, float* h_out,
                          size_t out_floats_per_slice, int32_t n_slices, int32_t chunk,
                          cudaStream_t user, Body body) {
+  PYHST_CALL_SCOPE(user);   // the device's lock is held until the pipeline has drained
+  DeviceCtx& c = *_call_scope.ctx;
   const size_t in_bytes = (size_t)chunk * in_floats_per_slice * 4;
   const size_t out_bytes = (size_t)chunk * out_floats_per_slice * 4;
   for (int i = 0; i < 3; ++i)
-    if (!g_streams[i]) PYHST_CUDA_TRY(cudaStreamCreateWithFlags(&g_streams[i], cudaStreamNonBlocking));
+    if (!c.streams[i]) PYHST_CUDA_TRY(cudaStreamCreateWithFlags(&c.streams[i], cudaStreamNonBlocking));
   for (int i = 0; i < 8; ++i)
-    if (!g_events[i]) PYHST_CUDA_TRY(cudaEventCreateWithFlags(&g_events[i], cudaEventDisableTiming));
-  cudaStream_t s_in = g_streams[0], s_k = g_streams[1], s_out = g_streams[2];
+    if (!c.events[i]) PYHST_CUDA_TRY(cudaEventCreateWithFlags(&c.events[i], cudaEventDisableTiming));
+  cudaStream_t s_in = c.streams[0], s_k = c.streams[1], s_out = c.streams[2];
   void *d_in[2], *d_out[2];
   void* blk = nullptr;
   PYHST_TRY(get_workspace(WS_CHUNKS, 2 * in_bytes + 2 * out_bytes, &blk));
@@ -653,30 +754,46 @@ static int host_pipeline(const float* h_in, size_t in_floats_per_slice, float* h
   d_in[1] = static_cast<char*>(blk) + in_bytes;
   d_out[0] = static_cast<char*>(blk) + 2 * in_bytes;
   d_out[1] = static_cast<char*>(blk) + 2 * in_bytes + out_bytes;
-  cudaEvent_t ev_start = g_events[0];
-  cudaEvent_t ev_in[2] = {g_events[1], g_events[2]}, ev_k[2] = {g_events[3], g_events[4]},
-              ev_out[2] = {g_events[5], g_events[6]};
-  PYHST_CUDA_TRY(cudaEventRecord(ev_start, user));
-  for (int i = 0; i < 3; ++i) PYHST_CUDA_TRY(cudaStreamWaitEvent(g_streams[i], ev_start, 0));
-  int n = 0;
-  for (int32_t s0 = 0; s0 < n_slices; s0 += chunk, ++n) {
-    const int32_t ns = std::min(chunk, n_slices - s0);
-    const int b = n & 1;
-    if (n >= 2) PYHST_CUDA_TRY(cudaStreamWaitEvent(s_in, ev_k[b], 0));   // kernels of chunk n-2 read d_in[b]
-    PYHST_CUDA_TRY(cudaMemcpyAsync(d_in[b], h_in + (size_t)s0 * in_floats_per_slice,
-                                   (size_t)ns * in_floats_per_slice * 4, cudaMemcpyHostToDevice, s_in));
-    PYHST_CUDA_TRY(cudaEventRecord(ev_in[b], s_in));
-    PYHST_CUDA_TRY(cudaStreamWaitEvent(s_k, ev_in[b], 0));
-    if (n >= 2) PYHST_CUDA_TRY(cudaStreamWaitEvent(s_k, ev_out[b], 0));  // D2H of chunk n-2 reads d_out[b]
-    PYHST_TRY(body(static_cast<const float*>(d_in[b]), static_cast<float*>(d_out[b]), ns, s_k));
-    PYHST_CUDA_TRY(cudaEventRecord(ev_k[b], s_k));
-    PYHST_CUDA_TRY(cudaStreamWaitEvent(s_out, ev_k[b], 0));
-    PYHST_CUDA_TRY(cudaMemcpyAsync(h_out + (size_t)s0 * out_floats_per_slice, d_out[b],
-                                   (size_t)ns * out_floats_per_slice * 4, cudaMemcpyDeviceToHost, s_out));
-    PYHST_CUDA_TRY(cudaEventRecord(ev_out[b], s_out));
+  cudaEvent_t ev_start = c.events[0];
+  cudaEvent_t ev_in[2] = {c.events[1], c.events[2]}, ev_k[2] = {c.events[3], c.events[4]},
+              ev_out[2] = {c.events[5], c.events[6]};
+  // the enqueue loop; whatever it returns, the copies it has started are drained below, so that no
+  // DMA touches the caller's host buffers after the call has returned (also on error)
+  auto enqueue = [&]() -> int {
+    PYHST_CUDA_TRY(cudaEventRecord(ev_start, user));
+    for (int i = 0; i < 3; ++i) PYHST_CUDA_TRY(cudaStreamWaitEvent(c.streams[i], ev_start, 0));
+    int n = 0;
+    for (int32_t s0 = 0; s0 < n_slices; s0 += chunk, ++n) {
+      const int32_t ns = std::min(chunk, n_slices - s0);
+      const int b = n & 1;
+      if (n >= 2) PYHST_CUDA_TRY(cudaStreamWaitEvent(s_in, ev_k[b], 0));   // kernels of chunk n-2 read d_in[b]
+      PYHST_CUDA_TRY(cudaMemcpyAsync(d_in[b], h_in + (size_t)s0 * in_floats_per_slice,
+                                     (size_t)ns * in_floats_per_slice * 4, cudaMemcpyHostToDevice, s_in));
+      PYHST_CUDA_TRY(cudaEventRecord(ev_in[b], s_in));
+      PYHST_CUDA_TRY(cudaStreamWaitEvent(s_k, ev_in[b], 0));
+      if (n >= 2) PYHST_CUDA_TRY(cudaStreamWaitEvent(s_k, ev_out[b], 0));  // D2H of chunk n-2 reads d_out[b]
+      PYHST_TRY(body(static_cast<const float*>(d_in[b]), static_cast<float*>(d_out[b]), ns, s_k));
+      PYHST_CUDA_TRY(cudaEventRecord(ev_k[b], s_k));
+      PYHST_CUDA_TRY(cudaStreamWaitEvent(s_out, ev_k[b], 0));
+      PYHST_CUDA_TRY(cudaMemcpyAsync(h_out + (size_t)s0 * out_floats_per_slice, d_out[b],
+                                     (size_t)ns * out_floats_per_slice * 4, cudaMemcpyDeviceToHost, s_out));
+      PYHST_CUDA_TRY(cudaEventRecord(ev_out[b], s_out));
+    }
+    return PYHST_OK;
+  };
+  const int rc = enqueue();
+  cudaError_t drain = cudaSuccess;
+  for (int i = 0; i < 3; ++i) {
+    cudaError_t e = cudaStreamSynchronize(c.streams[i]);
+    if (e != cudaSuccess && drain == cudaSuccess) drain = e;
   }
-  for (int i = 0; i < 3; ++i) PYHST_CUDA_TRY(cudaStreamSynchronize(g_streams[i]));
-  PYHST_CUDA_TRY(cudaStreamSynchronize(user));
+  {
+    cudaError_t e = cudaStreamSynchronize(user);
+    if (e != cudaSuccess && drain == cudaSuccess) drain = e;
+  }
+  if (rc != PYHST_OK) return rc;
+  if (drain != cudaSuccess)
+    return set_error(PYHST_ERR_CUDA, "host pipeline: %s while draining the copies", cudaGetErrorString(drain));
   return PYHST_OK;
 }
 

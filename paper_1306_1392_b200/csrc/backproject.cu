@@ -486,11 +486,11 @@ int launch_backproject_run(const float4* d_qi, const QiLayout& L, const BpArgs& 
   const size_t smem = SMEM_HDR + (size_t)2 * NA * W * 16;
   if (smem > 200 * 1024)
     return set_error(PYHST_ERR_UNSUPPORTED, "run backprojector: pixel size too large");
-  static size_t configured = 0;
-  if (smem > configured) {
+  static PerDeviceSize configured;
+  if (smem > configured.here()) {
     PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)smem));
-    configured = smem;
+    configured.here() = smem;
   }
   dim3 grid((a.nx + TX - 1) / TX, (a.ny + TY - 1) / TY, L.n_groups);
   if (grid.y > 65535 || grid.z > 65535)
@@ -508,7 +508,10 @@ int backproject_tiled_window(double pixel_size) {
   const double span = pixel_size * sqrt((double)((TX - 1) * (TX - 1) + (TY - 1) * (TY - 1)));
   const double w = ceil(span) + 5.0;
   if (w > 1024.0) return 0;
-  return ((int)w + 3) & ~3;
+  const int W = ((int)w + 3) & ~3;
+  // same limit as launch_backproject_tiled: beyond it pick_bp_kernel falls back to the reference kernel
+  if (SMEM_HDR + (size_t)2 * NA * W * 16 > 200 * 1024) return 0;
+  return W;
 }
 
 int launch_backproject_tiled(const float4* d_qi, const QiLayout& L, const BpArgs& a,
@@ -519,11 +522,11 @@ int launch_backproject_tiled(const float4* d_qi, const QiLayout& L, const BpArgs
   const size_t smem = SMEM_HDR + (size_t)2 * NA * W * 16;
   if (smem > 200 * 1024)
     return set_error(PYHST_ERR_UNSUPPORTED, "tiled backprojector: pixel size too large");
-  static size_t configured = 0;
-  if (smem > configured) {
+  static PerDeviceSize configured;
+  if (smem > configured.here()) {
     PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)smem));
-    configured = smem;
+    configured.here() = smem;
   }
   dim3 grid((a.nx + TX - 1) / TX, (a.ny + TY - 1) / TY, L.n_groups);
   if (grid.y > 65535 || grid.z > 65535)

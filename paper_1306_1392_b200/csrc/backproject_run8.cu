@@ -283,13 +283,12 @@ template <int WS, int NS>
 int launch_run8(const float4* d_qi, const QiLayout& L, const BpArgs& a, const RunProj* d_run,
                 int32_t n_a, int32_t n_b, int W, cudaStream_t stream) {
   const size_t smem = R8_HDR + (size_t)NS * R8_NA * 2 * WS * 16;
-  static bool configured = false;
-  if (!configured) {
+  static uint64_t configured = 0;   // one bit per device (cudaFuncSetAttribute is per device)
+  if (first_use_on_device(&configured)) {
     PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<0, WS, NS>,
                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<1, WS, NS>,
                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = true;
   }
   const unsigned gz = (unsigned)((L.n_groups + 1) / 2);
   dim3 grid_a((a.nx + R8_LANES - 1) / R8_LANES, (a.ny + R8_SLOW - 1) / R8_SLOW, gz);

@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "../../include/pyhst.h"
+#include "../../include/pyhst_test.h"
 
 namespace pyhst {
 
@@ -52,6 +53,37 @@ struct StageScope {
 // sm_100 device present and current?  (no CPU fallback: anything else is UNSUPPORTED)
 int require_sm100(int* n_sm);
 
+// ---- per-device state and call serialisation (include/pyhst.h "ONE CALL IN FLIGHT PER DEVICE") ----
+// Every public compute entry point opens a CallScope first: it takes the current device's lock for
+// the duration of the enqueue (re-entrant: entry points call one another) and, when the outermost
+// call runs on another stream than the previous call on this device, makes `stream` wait on the
+// device for that call's last kernel.  All caches below (workspace, plans, tables) belong to the
+// device of the open scope.
+struct DeviceCtx;
+struct CallScope {
+  explicit CallScope(cudaStream_t stream);
+  ~CallScope();
+  CallScope(const CallScope&) = delete;
+  CallScope& operator=(const CallScope&) = delete;
+  int status = PYHST_OK;   // PYHST_ERR_* if the device could not be queried / the wait not enqueued
+  DeviceCtx* ctx = nullptr;
+  cudaStream_t stream;
+};
+#define PYHST_CALL_SCOPE(stream)             \
+  ::pyhst::CallScope _call_scope(stream);    \
+  if (_call_scope.status != PYHST_OK) return _call_scope.status
+
+int current_device();  // cudaGetDevice, -1 on failure
+// true exactly once per (mask, device): cudaFuncSetAttribute and friends are per device.
+// Call inside a CallScope (the device lock makes it race-free).
+bool first_use_on_device(uint64_t* mask);
+// per-device table of sizes already configured (index = device), for kernels whose dynamic
+// shared-memory limit grows with the geometry
+struct PerDeviceSize {
+  size_t v[64] = {0};
+  size_t& here();
+};
+
 // ---- per-projection geometry, built in double on the host (reading R11) -----------------
 // t_p(i,j) = c + ch * (j - j0) + sh * (i - i0),  ch = h cos(theta_p), sh = h sin(theta_p)
 struct ProjGeom {
@@ -91,6 +123,9 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
 enum WorkspaceSlot { WS_QI = 0, WS_FFT = 1, WS_WEIGHTS = 2, WS_IMG_T = 3, WS_ROWS = 4,
                      WS_CHUNKS = 5, WS_XI = 6, WS_FISTA = 7, WS_FPL = 8, WS_STITCH = 9, WS_COUNT = 10 };
 int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr);
+// bumped whenever the slot's block is (re)allocated or released: lets a user of the slot remember
+// "I initialised this very block" without being fooled by a recycled address
+uint64_t workspace_generation(WorkspaceSlot slot);
 
 // ---- interleaved sinogram layout consumed by the tiled backprojector ---------------------
 // QI[g][p][zpad + b][sl]: slice group g = s / 4, sl = s % 4, one float4 per (g, p, bin);
@@ -170,7 +205,6 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out);
 // fills the host tables of a plan; returns false if the banded kernel cannot cover the geometry
 bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* projs,
                      std::vector<FpChunk>* chunks);  // forward_project.cu
-void release_fp_plans();
 int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pitch,
                                   const pyhst_geom_t* g, float scale, const FpPlan& plan,
                                   int interval_groups, cudaStream_t stream);

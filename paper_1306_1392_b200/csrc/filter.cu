@@ -31,9 +31,9 @@ namespace {
 
 std::mutex g_mu;
 struct Spectrum { float* d_H = nullptr; };                    // [M/2 + 1], H[k] / M
-std::map<std::pair<int, int>, Spectrum> g_spectra;            // (filter, M)
+std::map<std::tuple<int, int, int>, Spectrum> g_spectra;      // (device, filter, M)
 struct FftPlans { cufftHandle r2c = 0, c2r = 0; };
-std::map<std::pair<int, int>, FftPlans> g_plans;              // (M, batch)
+std::map<std::tuple<int, int, int>, FftPlans> g_plans;        // (device, M, batch)
 
 // smallest M = 2^a * {1, 3, 5} with M >= n (cuFFT is efficient for these radices)
 int fft_length(int64_t n) {
@@ -73,7 +73,7 @@ __global__ void spectrum_to_float(const cufftDoubleComplex* Hd, float* H, int nk
 }
 
 int get_spectrum(int filter, int M, cudaStream_t stream, const float** out) {
-  auto key = std::make_pair(filter, M);
+  auto key = std::make_tuple(current_device(), filter, M);
   auto it = g_spectra.find(key);
   if (it != g_spectra.end()) { *out = it->second.d_H; return PYHST_OK; }
   const int nk = M / 2 + 1;
@@ -100,7 +100,7 @@ int get_spectrum(int filter, int M, cudaStream_t stream, const float** out) {
 }
 
 int get_plans(int M, int batch, FftPlans* out) {
-  auto key = std::make_pair(M, batch);
+  auto key = std::make_tuple(current_device(), M, batch);
   auto it = g_plans.find(key);
   if (it != g_plans.end()) { *out = it->second; return PYHST_OK; }
   FftPlans pl;

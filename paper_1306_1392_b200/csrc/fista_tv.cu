@@ -22,19 +22,37 @@ namespace {
 
 constexpr int FT_BX = 32, FT_BY = 8;
 
-// block-wide sum of a float into a double accumulator in global memory
-__device__ __forceinline__ void block_sum_to(double v, double* dst) {
-  __shared__ double part[FT_BX * FT_BY / 32];
+// Deterministic two-stage sum: every block stores the sum of its threads' values (fixed shuffle /
+// warp order) into part[linear block index]; ftv_reduce_kernel then adds the partials to the
+// accumulator in a fixed order.  (Round 1 used atomicAdd(double): the order of the additions, hence
+// the last bits of L, of the energies and of every iterate, changed from run to run.)
+__device__ __forceinline__ void block_sum_to(double v, double* part) {
+  __shared__ double wsum[FT_BX * FT_BY / 32];
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   const int t = threadIdx.y * blockDim.x + threadIdx.x;
-  if ((t & 31) == 0) part[t >> 5] = v;
+  if ((t & 31) == 0) wsum[t >> 5] = v;
   __syncthreads();
   if (t == 0) {
     double s = 0.0;
-    for (int w = 0; w < (int)(blockDim.x * blockDim.y) / 32; ++w) s += part[w];
-    atomicAdd(dst, s);
+    for (int w = 0; w < (int)(blockDim.x * blockDim.y) / 32; ++w) s += wsum[w];
+    part[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = s;
   }
+}
+
+// *dst += sum_k part[k], k < n: thread t adds part[t], part[t + 1024], ... in that order, then a
+// fixed binary tree over the 1024 threads
+__global__ void __launch_bounds__(1024) ftv_reduce_kernel(const double* __restrict__ part, int n, double* dst) {
+  __shared__ double sh[1024];
+  double s = 0.0;
+  for (int k = threadIdx.x; k < n; k += 1024) s += part[k];
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *dst += sh[0];
 }
 
 // forward differences, zero at the last column / row (R18)
@@ -68,7 +86,7 @@ __global__ void ftv_residual_kernel(float* __restrict__ r, const float* __restri
       acc += 0.5 * (double)v * (double)v;
     }
   }
-  block_sum_to(acc, half_acc);
+  block_sum_to(acc, half_acc);   // half_acc = partials [gridDim.x * gridDim.y]
 }
 
 // z = y - g * (1/L);  *tv_acc += beta * TV(y)   (energy of eq. 3 at y, R19)
@@ -202,6 +220,7 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
   if (g->n_slices <= 0 || g->n_angles <= 0 || g->n_bins <= 0 || g->nx <= 0 || g->ny <= 0)
     return set_error(PYHST_ERR_INVALID_ARG, "pyhst_fista_tv: non-positive size");
   PYHST_TRY(require_sm100(nullptr));
+  PYHST_CALL_SCOPE(stream);
   const int S = g->n_slices, nx = g->nx, ny = g->ny;
   const int64_t n_img = (int64_t)S * ny * nx, n1 = (int64_t)ny * nx;
   const int64_t n_rows = (int64_t)S * g->n_angles, n_sino = n_rows * g->n_bins;
@@ -212,8 +231,15 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
   const size_t img_bytes = ((size_t)n_img * 4 + 255) & ~(size_t)255;
   const size_t sino_bytes = ((size_t)n_sino * 4 + 255) & ~(size_t)255;
   const size_t sc_bytes = (size_t)(3 + n_iter) * 8;   // doubles: nv, nw, L, energy[n_iter]; then 4 floats
+  // per-block partial sums of the reductions (deterministic two-stage sums)
+  const int64_t n_part_img = (int64_t)((nx + FT_BX - 1) / FT_BX) * ((ny + FT_BY - 1) / FT_BY) * S;
+  const int64_t res_gy = std::min<int64_t>((n_rows + FT_BY - 1) / FT_BY, 4096);
+  const int64_t n_part_res = (int64_t)((g->n_bins + FT_BX - 1) / FT_BX) * res_gy;
+  const int64_t n_part = std::max<int64_t>(std::max(n_part_img, n_part_res), 148 * 4);
+  if (n_part > (1 << 30)) return set_error(PYHST_ERR_UNSUPPORTED, "pyhst_fista_tv: stack too large");
+  const size_t part_off = (7 * img_bytes + sino_bytes + sc_bytes + 16 + 255) & ~(size_t)255;
   void* ws = nullptr;
-  PYHST_TRY(get_workspace(WS_FISTA, 7 * img_bytes + sino_bytes + sc_bytes + 16, &ws));
+  PYHST_TRY(get_workspace(WS_FISTA, part_off + (size_t)n_part * 8, &ws));
   char* base = static_cast<char*>(ws);
   float* y = reinterpret_cast<float*>(base);
   float* z = reinterpret_cast<float*>(base + img_bytes);
@@ -224,6 +250,7 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
   double* sc = reinterpret_cast<double*>(base + 7 * img_bytes + sino_bytes);
   double *d_nv = sc, *d_nw = sc + 1, *d_L = sc + 2, *d_e = sc + 3;
   float* d_fs = reinterpret_cast<float*>(sc + 3 + n_iter);
+  double* d_part = reinterpret_cast<double*>(base + part_off);
 
   pyhst_geom_t g1 = *g, gs = *g;
   g1.n_slices = 1;
@@ -238,10 +265,12 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
   ftv_fill_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, stream>>>(y, n1, 1.f);
   for (int it = 0; it < n_power; ++it) {
     PYHST_CUDA_TRY(cudaMemsetAsync(sc, 0, 16, stream));
-    ftv_sumsq_kernel<<<red_blocks, blk, 0, stream>>>(y, n1, d_nv);
+    ftv_sumsq_kernel<<<red_blocks, blk, 0, stream>>>(y, n1, d_part);
+    ftv_reduce_kernel<<<1, 1024, 0, stream>>>(d_part, (int)red_blocks, d_nv);
     PYHST_TRY(pyhst_forward_project(y, r, &g1, 1.f, stream));
     PYHST_TRY(pyhst_backproject(r, gr, &g1, 1.f, stream));
-    ftv_sumsq_kernel<<<red_blocks, blk, 0, stream>>>(gr, n1, d_nw);
+    ftv_sumsq_kernel<<<red_blocks, blk, 0, stream>>>(gr, n1, d_part);
+    ftv_reduce_kernel<<<1, 1024, 0, stream>>>(d_part, (int)red_blocks, d_nw);
     ftv_normalise_kernel<<<(unsigned)((n1 + 255) / 256), 256, 0, stream>>>(gr, y, n1, d_nv, d_nw, d_L);
   }
   ftv_scalars_kernel<<<1, 1, 0, stream>>>(d_L, (double)beta, d_fs);
@@ -255,11 +284,13 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
   for (int k = 0; k < n_iter; ++k) {
     PYHST_TRY(pyhst_forward_project(y, r, &gs, 1.f, stream));
     {
-      dim3 grid((g->n_bins + FT_BX - 1) / FT_BX, (unsigned)std::min<int64_t>((n_rows + FT_BY - 1) / FT_BY, 4096), 1);
-      ftv_residual_kernel<<<grid, blk, 0, stream>>>(r, d_data, data_pitch, g->n_bins, n_rows, d_e + k);
+      dim3 grid((g->n_bins + FT_BX - 1) / FT_BX, (unsigned)res_gy, 1);
+      ftv_residual_kernel<<<grid, blk, 0, stream>>>(r, d_data, data_pitch, g->n_bins, n_rows, d_part);
+      ftv_reduce_kernel<<<1, 1024, 0, stream>>>(d_part, (int)n_part_res, d_e + k);
     }
     PYHST_TRY(pyhst_backproject(r, gr, &gs, 1.f, stream));
-    ftv_step_kernel<<<grid_img, blk, 0, stream>>>(y, gr, z, nx, ny, d_fs, (double)beta, d_e + k);
+    ftv_step_kernel<<<grid_img, blk, 0, stream>>>(y, gr, z, nx, ny, d_fs, (double)beta, d_part);
+    ftv_reduce_kernel<<<1, 1024, 0, stream>>>(d_part, (int)n_part_img, d_e + k);
     int cur = 0;
     if (use_p) {
       PYHST_CUDA_TRY(cudaMemsetAsync(p[0], 0, 2 * img_bytes, stream));  // p[0], p[1] are adjacent

@@ -729,15 +729,18 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
   float4* xi_r = plan.any_rows ? static_cast<float4*>(ws) : nullptr;
   float4* xi_c = plan.any_cols ? reinterpret_cast<float4*>(static_cast<char*>(ws) + bytes_r) : nullptr;
   // the zero pads are written once per (block, layout); the repack only touches the interior
-  static const void* pads_ptr = nullptr;
-  static size_t pads_key[6] = {0};
-  const size_t key[6] = {bytes_r, bytes_c, (size_t)g->nx, (size_t)g->ny, (size_t)W, (size_t)n_groups};
+  // ("this very block": device + the slot's allocation generation, so that a block freed by
+  // pyhst_release_cache or regrown and handed back at the same address is zeroed again)
+  struct PadsKey { size_t k[8]; };
+  static PadsKey pads[64];
+  const PadsKey key = {{bytes_r, bytes_c, (size_t)g->nx, (size_t)g->ny, (size_t)W, (size_t)n_groups,
+                        (size_t)workspace_generation(WS_XI), (size_t)reinterpret_cast<uintptr_t>(ws)}};
+  PadsKey& seen = pads[std::max(0, current_device()) & 63];
   {
     StageScope scope(ST_TRANSPOSE, stream);
-    if (pads_ptr != ws || std::memcmp(pads_key, key, sizeof(key)) != 0) {
+    if (std::memcmp(&seen, &key, sizeof(key)) != 0) {
       PYHST_CUDA_TRY(cudaMemsetAsync(ws, 0, bytes_r + bytes_c, stream));
-      pads_ptr = ws;
-      std::memcpy(pads_key, key, sizeof(key));
+      seen = key;
     }
     dim3 block(32, 8, 1);
     dim3 grid((g->nx + 31) / 32, (g->ny + 31) / 32, n_groups);
@@ -759,13 +762,13 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
     // 8 slices per thread (two groups per block, bands of 4 lines) when the stack has an even number
     // of slice groups and full 16-projection chunks (the thread map gives projections 8..15 to warps 4..7)
     const bool two = nci == 2 && n_groups % 2 == 0 && plan.npj == FB_NPJ && interval_groups == 2;
-    static size_t configured_i[3] = {0, 0, 0};
+    static PerDeviceSize configured_i[3];
     auto kern_i = two ? fp_ivl_kernel<2, 2, 4> : (nci == 2 ? fp_ivl_kernel<2, 1, 8> : fp_ivl_kernel<3, 1, 8>);
     const int ci = two ? 2 : nci - 2;
-    if (smem > configured_i[ci]) {
+    if (smem > configured_i[ci].here()) {
       PYHST_CUDA_TRY(cudaFuncSetAttribute(kern_i, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)(FB_HDR + (size_t)3 * FB_RB * W * 16)));
-      configured_i[ci] = smem;
+      configured_i[ci].here() = smem;
     }
     const size_t smem_i = FB_HDR + (size_t)3 * FB_RB * W * 16;   // three stages of RB x NG = 8 lines
     dim3 grid((g->n_bins + 1 + IV_NB - 1) / IV_NB, plan.n_chunks, two ? n_groups / 2 : n_groups);
@@ -794,14 +797,14 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
   const int n_bands_min = (std::min(g->nx, g->ny) + FB_RB - 1) / FB_RB;
   int n_split = (int)std::max<int64_t>(1, std::min<int64_t>(4, slots / std::max<int64_t>(blocks, 1)));
   n_split = std::max(1, std::min(n_split, n_bands_min / 8));
-  static size_t configured[5] = {0, 0, 0, 0, 0};
+  static PerDeviceSize configured[5];
   const int vi = four ? 3 : (plan.nc == 3 ? (n_split > 1 ? 4 : 0) : (plan.nc == 4 ? 1 : 2));
   auto kern = four ? fp_band_kernel<3, 4, true>
                    : (plan.nc == 3 ? (n_split > 1 ? fp_band_kernel<3, 3, true> : fp_band_kernel<3, 3, false>)
                                    : (plan.nc == 4 ? fp_band_kernel<4, 3, true> : fp_band_kernel<6, 3, true>));
-  if (smem > configured[vi]) {
+  if (smem > configured[vi].here()) {
     PYHST_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured[vi] = smem;
+    configured[vi].here() = smem;
   }
   const int64_t n_rows = (int64_t)g->n_slices * g->n_angles;
   float* part = nullptr;

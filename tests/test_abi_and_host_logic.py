@@ -21,10 +21,14 @@ def cuda_lib():
     return ctypes.CDLL(build.build())
 
 
-def _declared_symbols():
-    src = open(os.path.join(ROOT, "include", "pyhst.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(pyhst_[a-z0-9_]+)\s*\(", src)))
+def _declared_symbols(headers=None):
+    inc = os.path.join(ROOT, "include")
+    names = set()
+    for h in headers or sorted(f for f in os.listdir(inc) if f.endswith(".h")):
+        src = open(os.path.join(inc, h)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names |= set(re.findall(r"\b(pyhst_[a-z0-9_]+)\s*\(", src))
+    return sorted(names)
 
 
 def test_header_symbols_are_exported(cuda_lib):
@@ -32,6 +36,17 @@ def test_header_symbols_are_exported(cuda_lib):
     assert {"pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp"} <= set(names)
     for n in names:
         assert hasattr(cuda_lib, n), "libpyhst_b200.so does not export %s" % n
+
+
+def test_header_states_the_concurrency_rule_and_keeps_test_hooks_out():
+    """pyhst.h promises stream-ordered calls: it must say how calls on several streams / threads /
+    devices are ordered and where a call may synchronise; kernel-variant switches are test hooks."""
+    text = open(os.path.join(ROOT, "include", "pyhst.h")).read()
+    assert "ONE CALL IN FLIGHT PER DEVICE" in text and "cudaStreamWaitEvent" in text
+    assert "FIRST call with a new shape" in text
+    public = _declared_symbols(["pyhst.h"])
+    assert not [n for n in public if n.startswith("pyhst_set_")]
+    assert "pyhst_set_backproject_variant" in _declared_symbols(["pyhst_test.h"])
 
 
 def test_binding_lists_every_header_symbol():

@@ -240,21 +240,6 @@ def _sample_points(rng, n, slices, ny, nx):
     return np.concatenate([pts, np.array(corners)], axis=0).astype(np.int32)
 
 
-@pytest.mark.parametrize("cfg,n_slices", [(2, 16), (3, 4), (5, 8)])
-def test_fbp_full_size_sampled(lib, oracle, cfg, n_slices):
-    """BASELINE.json's full sizes in the launch configuration bench.py times (config 5 with 8 of its
-    64 slices): the oracle evaluates sampled pixels one by one."""
-    w = lib.workloads.config(cfg, n_slices=n_slices)
-    rng = np.random.default_rng(cfg)
-    check = [0, n_slices - 1] if cfg != 5 else [n_slices - 3]
-    sino = w.sinogram()
-    got = lib.fbp(_dev(sino), w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode).cpu().numpy()
-    pts = _sample_points(rng, 400, check, w.ny, w.nx)
-    want = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode, pts=pts)
-    g = got[pts[:, 0], pts[:, 1], pts[:, 2]]
-    assert_parity(g, want, "fbp cfg%d full size (sampled)" % cfg)
-
-
 def test_projector_pair_config4_full(lib, oracle):
     """Config 4 (iterative): the pair P, P^T at full size on sampled rows / pixels + the K3 identity."""
     import torch
@@ -418,3 +403,71 @@ def test_halfacq_stitched_equals_general_path(lib, oracle):
     want3 = oracle.fbp(raw, ang, ax, 110, 108, mode=lib.SCAN_360_HALF)
     got3 = lib.fbp(_dev(raw), ang, ax, 110, 108, mode=lib.SCAN_360_HALF).cpu().numpy()
     assert_parity(got3, want3, "fbp half acquisition, stitched, axis on the left")
+
+
+# ------------------------------------------------------------------------------ library state
+@pytest.mark.gpu
+def test_calls_on_two_streams_are_serialised(lib, oracle):
+    """include/pyhst.h, concurrency rule: all calls of a device share one workspace; calls on
+    different streams are ordered on the device by the library (cudaStreamWaitEvent), so two
+    streams that alternate between two shapes -- which regrow / reuse the same QI and FFT
+    blocks -- still give the serial results."""
+    import torch
+    wl = lib.workloads
+    wa = wl.config(2, shrink=8, n_slices=6)            # 256^2, 250 projections
+    wb = wl.custom(9, 90, 300, 200, 170, drift=1.0, seed=4)
+    sa, sb = _dev(wa.sinogram()), _dev(wl.random_sinogram(9, 90, 300, seed=9))
+    ref_a = lib.fbp(sa, wa.angles, wa.axis, wa.nx, wa.ny, filter=wa.filter)
+    ref_b = lib.fbp(sb, wb.angles, wb.axis, 200, 170)
+    ref_p = lib.forward_project(ref_b, wb.angles, wb.axis, 300)
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    out_a = [torch.empty_like(ref_a) for _ in range(4)]
+    out_b = [torch.empty_like(ref_b) for _ in range(4)]
+    out_p = [torch.empty_like(ref_p) for _ in range(4)]
+    for k in range(4):                                  # no host synchronisation in between
+        lib.fbp(sa, wa.angles, wa.axis, wa.nx, wa.ny, filter=wa.filter, out=out_a[k], stream=s1)
+        lib.fbp(sb, wb.angles, wb.axis, 200, 170, out=out_b[k], stream=s2)
+        lib.forward_project(ref_b, wb.angles, wb.axis, 300, out=out_p[k], stream=s1)
+    torch.cuda.synchronize()
+    for k in range(4):
+        assert torch.equal(out_a[k], ref_a) and torch.equal(out_b[k], ref_b) and torch.equal(out_p[k], ref_p)
+    assert_parity(ref_a.cpu().numpy(), oracle.fbp(wa.sinogram(), wa.angles, wa.axis, wa.nx, wa.ny, filter=wa.filter),
+                  "fbp (serial reference of the two-stream test)")
+
+
+@pytest.mark.gpu
+def test_forward_projector_pads_survive_a_released_cache(lib, oracle):
+    """The banded forward projector relies on zero pads around its interleaved image copy and writes
+    them only once per block: after pyhst_release_cache() (or a regrown workspace) the block may come
+    back at the same address holding anything, and must be zeroed again."""
+    import torch
+    wl = lib.workloads
+    w = wl.custom(4, 40, 200, 150, 140, drift=1.0, seed=8)
+    x = _dev(wl.random_image(4, 140, 150, seed=2))
+    want = oracle.forward_project(x.cpu().numpy(), w.angles, w.axis, 200)
+    got = lib.forward_project(x, w.angles, w.axis, 200)
+    assert_parity(got.cpu().numpy(), want, "forward_project before release")
+    for _ in range(3):
+        lib.release_cache()
+        junk = [torch.full((1 << 22,), float("nan"), device="cuda") for _ in range(8)]   # dirty the freed blocks
+        del junk
+        torch.cuda.empty_cache()
+        got = lib.forward_project(x, w.angles, w.axis, 200)
+        assert_parity(got.cpu().numpy(), want, "forward_project after release_cache")
+
+
+@pytest.mark.gpu
+def test_large_pixel_size_falls_back_to_the_reference_kernel(lib, oracle):
+    """pixel_size ~ 6: the staged window of the tiled kernels would exceed shared memory; the
+    automatic pick must take the one-thread-per-pixel kernel instead of failing."""
+    wl = lib.workloads
+    w = wl.custom(2, 24, 700, 90, 80, pixel_size=6.0, drift=0.5, seed=6)
+    sino = wl.random_sinogram(2, 24, 700, seed=6)
+    want = oracle.backproject(sino, w.angles, w.axis, 90, 80, pixel_size=6.0)
+    got = lib.backproject(_dev(sino), w.angles, w.axis, 90, 80, pixel_size=6.0).cpu().numpy()
+    assert_parity(got, want, "backproject pixel_size 6")
+    x = wl.random_image(2, 80, 90, seed=6)
+    wantp = oracle.forward_project(x, w.angles, w.axis, 700, pixel_size=6.0)
+    gotp = lib.forward_project(_dev(x), w.angles, w.axis, 700, pixel_size=6.0).cpu().numpy()
+    assert_parity(gotp, wantp, "forward_project pixel_size 6")
