@@ -289,3 +289,136 @@ def fista_tv(data, angles, axis, nx, ny, beta, L, n_iter, n_inner=20, pixel_size
                                c_int32(ny), c_double(pixel_size), c_double(beta), c_double(L),
                                c_int32(n_iter), c_int32(n_inner), _p(energy, c_double)), "fista_tv")
     return x, energy[:n_iter]
+
+
+def ista_tv(data, angles, axis, nx, ny, beta, L, n_iter, n_inner=20, pixel_size=1.0):
+    """ISTA: fista_tv without the momentum.  -> (x float64, energy float64 [n_iter])."""
+    lib = _load()
+    data = _f32(data)
+    s, p, b, angles, axis = _geom(data.shape, angles, axis)
+    x = np.empty((s, ny, nx), dtype=np.float64)
+    energy = np.zeros(max(n_iter, 1), dtype=np.float64)
+    _check(lib.oracle_ista_tv(_p(data, c_float), c_int64(b), _p(x, c_double), c_int32(s), c_int32(p),
+                              c_int32(b), _p(angles, c_double), _p(axis, c_double), c_int32(nx),
+                              c_int32(ny), c_double(pixel_size), c_double(beta), c_double(L),
+                              c_int32(n_iter), c_int32(n_inner), _p(energy, c_double)), "ista_tv")
+    return x, energy[:n_iter]
+
+
+FILTER_COSINE = 4
+
+
+# ---- NEXT row N4: ring filter (PAPER.md L61) and the estimators of sec. 4 (L149-L162) ----------
+def ring_filter(sino, half_width, model=None):
+    """sino float32 [S,P,B] (model: same shape or None) -> float64 [S,P,B] (reading R21)."""
+    lib = _load()
+    sino = _f32(sino)
+    s, p, b = sino.shape
+    mod = None if model is None else _f32(model)
+    if mod is not None and mod.shape != sino.shape:
+        raise ValueError("model must have the sinogram's shape")
+    out = np.empty((s, p, b), dtype=np.float64)
+    _check(lib.oracle_ring_filter(_p(sino, c_float), _p(mod, c_float) if mod is not None else None,
+                                  c_int64(b), _p(out, c_double), c_int32(s), c_int32(p), c_int32(b),
+                                  c_int32(half_width)), "ring_filter")
+    return out
+
+
+def ecohe(a, b):
+    """eq. 11 per slice: Cos(a - b, a) for stacks a = I(beta), b = I(0+) [S, ...] -> float64 [S]."""
+    lib = _load()
+    a, b = _f32(a), _f32(b)
+    if a.shape != b.shape:
+        raise ValueError("shapes differ")
+    s = a.shape[0]
+    out = np.empty(s, dtype=np.float64)
+    _check(lib.oracle_ecohe(_p(a, c_float), _p(b, c_float), c_int32(s), c_int64(a[0].size), _p(out, c_double)),
+           "ecohe")
+    return out
+
+
+def cv_distance(img, data_excl, angles_excl, axis_excl, pixel_size=1.0):
+    """Cross-validation distance (L149): sum over the excluded projections of ||P x - data||^2, per slice."""
+    lib = _load()
+    img, data = _f32(img), _f32(data_excl)
+    s, ny, nx = img.shape
+    s2, e, b = data.shape
+    angles, axis = _f64(angles_excl), _f64(axis_excl)
+    if s2 != s or angles.shape != (e,) or axis.shape != (e,):
+        raise ValueError("shape mismatch")
+    out = np.empty(s, dtype=np.float64)
+    _check(lib.oracle_cv_distance(_p(img, c_float), _p(data, c_float), c_int64(b), c_int32(s), c_int32(e),
+                                  c_int32(b), _p(angles, c_double), _p(axis, c_double), c_int32(nx),
+                                  c_int32(ny), c_double(pixel_size), _p(out, c_double)), "cv_distance")
+    return out
+
+
+# ---- NEXT row N3: overlapping-patch dictionary reconstruction (PAPER.md L102-L145, Alg. 1) ------
+def patch_grid(ny, nx, m, st):
+    na, nb = c_int32(0), c_int32(0)
+    _check(_load().oracle_patch_grid(c_int32(ny), c_int32(nx), c_int32(m), c_int32(st), ctypes.byref(na),
+                                     ctypes.byref(nb)), "patch_grid")
+    return int(na.value), int(nb.value)
+
+
+def patch_maps(ny, nx, m, st):
+    """(core [ny,nx] int32 = C_j, cover [ny,nx] int32 = N_v(j))."""
+    core = np.empty((ny, nx), dtype=np.int32)
+    cover = np.empty((ny, nx), dtype=np.int32)
+    _check(_load().oracle_patch_maps(c_int32(ny), c_int32(nx), c_int32(m), c_int32(st), _p(core, c_int32),
+                                     _p(cover, c_int32)), "patch_maps")
+    return core, cover
+
+
+def patch_gradient(W, D, data, angles, axis, nx, ny, m, st, rho, pixel_size=1.0):
+    """Algorithm 1 for one slice.  W [N,Nc] f64, D [Nc,m*m] f64, data f32 [P,B] -> (G [N,Nc], X [ny,nx], f)."""
+    lib = _load()
+    W, D, data = _f64(W), _f64(D), _f32(data)
+    p, b = data.shape
+    angles, axis = _f64(angles), _f64(axis)
+    n_atoms = D.shape[0]
+    G = np.empty_like(W)
+    X = np.empty((ny, nx), dtype=np.float64)
+    f = c_double(0.0)
+    _check(lib.oracle_patch_gradient(_p(W, c_double), _p(D, c_double), _p(data, c_float), c_int64(b), c_int32(p),
+                                     c_int32(b), _p(angles, c_double), _p(axis, c_double), c_int32(nx), c_int32(ny),
+                                     c_double(pixel_size), c_int32(m), c_int32(st), c_int32(n_atoms), c_double(rho),
+                                     _p(G, c_double), _p(X, c_double), ctypes.byref(f)), "patch_gradient")
+    return G, X, float(f.value)
+
+
+def soft_threshold(v, t):
+    v = _f64(v)
+    out = np.empty_like(v)
+    _load().oracle_soft_threshold(_p(v, c_double), c_int64(v.size), c_double(t), _p(out, c_double))
+    return out
+
+
+def patch_lipschitz(D, angles, axis, n_bins, nx, ny, m, st, rho, pixel_size=1.0, n_power=8) -> float:
+    lib = _load()
+    D = _f64(D)
+    angles, axis = _f64(angles), _f64(axis)
+    out = c_double(0.0)
+    _check(lib.oracle_patch_lipschitz(_p(D, c_double), c_int32(angles.shape[0]), c_int32(n_bins),
+                                      _p(angles, c_double), _p(axis, c_double), c_int32(nx), c_int32(ny),
+                                      c_double(pixel_size), c_int32(m), c_int32(st), c_int32(D.shape[0]),
+                                      c_double(rho), c_int32(n_power), ctypes.byref(out)), "patch_lipschitz")
+    return float(out.value)
+
+
+def patch_fista(D, data, angles, axis, nx, ny, m, st, rho, beta, Lw, n_iter, pixel_size=1.0):
+    """-> (W [N,Nc] f64, X [ny,nx] f64, energy [n_iter])."""
+    lib = _load()
+    D, data = _f64(D), _f32(data)
+    p, b = data.shape
+    angles, axis = _f64(angles), _f64(axis)
+    na, nb = patch_grid(ny, nx, m, st)
+    W = np.empty((na * nb, D.shape[0]), dtype=np.float64)
+    X = np.empty((ny, nx), dtype=np.float64)
+    energy = np.zeros(max(n_iter, 1), dtype=np.float64)
+    _check(lib.oracle_patch_fista(_p(D, c_double), _p(data, c_float), c_int64(b), c_int32(p), c_int32(b),
+                                  _p(angles, c_double), _p(axis, c_double), c_int32(nx), c_int32(ny),
+                                  c_double(pixel_size), c_int32(m), c_int32(st), c_int32(D.shape[0]), c_double(rho),
+                                  c_double(beta), c_double(Lw), c_int32(n_iter), _p(W, c_double), _p(X, c_double),
+                                  _p(energy, c_double)), "patch_fista")
+    return W, X, energy[:n_iter]

@@ -73,9 +73,20 @@ void oracle_set_num_threads(int n) {
  * Hann (2), Hamming (3): the Ram-Lak ramp times the window a0 + 2 a1 cos(2 pi w), w in cycles per
  *   bin (|w| <= 1/2), (a0, a1) = (0.5, 0.25) resp. (0.54, 0.23); a cosine in frequency is a pair of
  *   unit shifts in space:  h_w[n] = a0 h[n] + a1 (h[n-1] + h[n+1])   (NEXT row N2: more windows)
+ * Cosine (4): the ramp times cos(pi w) = (e^{i pi w} + e^{-i pi w}) / 2, a pair of HALF-bin shifts of
+ *   the continuous band-limited ramp  h(x) = int_{-1/2}^{1/2} |w| e^{2 pi i w x} dw
+ *                                          = sin(pi x) / (2 pi x) + (cos(pi x) - 1) / (2 pi^2 x^2):
+ *   h_c[n] = (h(n - 1/2) + h(n + 1/2)) / 2,  with  h(m + 1/2) = (-1)^m / (2 pi (m + 1/2)) - 1 / (2 pi^2 (m + 1/2)^2)
  * (PAPER.md:L13, L63 only say "filtered back projection"; no formula given.) */
+static double ramp_at_half_integer(int64_t m) { /* h(m + 1/2) */
+  double x = (double)m + 0.5;
+  double sgn = (m & 1) ? -1.0 : 1.0;
+  return sgn / (2.0 * ORACLE_PI * x) - 1.0 / (2.0 * ORACLE_PI * ORACLE_PI * x * x);
+}
+
 double oracle_ramp_kernel(int filter, int64_t n) {
   double dn = (double)n;
+  if (filter == 4) return 0.5 * (ramp_at_half_integer(n - 1) + ramp_at_half_integer(n));
   if (filter == 2 || filter == 3) {
     const double a0 = filter == 2 ? 0.5 : 0.54, a1 = filter == 2 ? 0.25 : 0.23;
     return a0 * oracle_ramp_kernel(0, n) + a1 * (oracle_ramp_kernel(0, n - 1) + oracle_ramp_kernel(0, n + 1));
@@ -129,7 +140,7 @@ int oracle_ramp_filter(const float* in, int64_t in_pitch, double* out, int64_t n
                        int32_t n_bins_in, int32_t n_bins_out, int32_t pad_left, int filter,
                        const float* col_weights) {
   if (!in || !out || n_rows < 0 || n_bins_in <= 0 || n_bins_out <= 0 || pad_left < 0 ||
-      n_bins_out < n_bins_in + pad_left || filter < 0 || filter > 3)
+      n_bins_out < n_bins_in + pad_left || filter < 0 || filter > 4)
     return ORACLE_ERR_INVALID_ARG;
   if (in_pitch == 0) in_pitch = n_bins_in;
   int64_t nh = (int64_t)n_bins_in + n_bins_out;         /* lags -(B_in-1) .. B_out-1 */
@@ -537,10 +548,10 @@ int oracle_lipschitz(int32_t n_angles, int32_t n_bins, const double* angles, con
  *     t_{k+1} = (1 + sqrt(1 + 4 t_k^2)) / 2 ;  y_{k+1} = x_{k+1} + (t_k - 1)/t_{k+1} (x_{k+1} - x_k)
  * data: float32 [S][P][pitch] widened exactly; x_out = x_{n_iter} [S][ny][nx] in double; energy
  * (nullable) [n_iter], summed over the slices of the stack. */
-int oracle_fista_tv(const float* data, int64_t pitch, double* x_out, int32_t n_slices,
-                    int32_t n_angles, int32_t n_bins, const double* angles, const double* axis,
-                    int32_t nx, int32_t ny, double h, double beta, double L, int32_t n_iter,
-                    int32_t n_inner, double* energy) {
+static int tv_solver(const float* data, int64_t pitch, double* x_out, int32_t n_slices,
+                     int32_t n_angles, int32_t n_bins, const double* angles, const double* axis,
+                     int32_t nx, int32_t ny, double h, double beta, double L, int32_t n_iter,
+                     int32_t n_inner, double* energy, int accelerated) {
   int rc = check_geom(n_slices, n_angles, n_bins, angles, axis, nx, ny, h);
   if (rc || !data || !x_out || !(L > 0.0) || !(beta >= 0.0) || n_iter < 0 || n_inner < 0)
     return rc ? rc : ORACLE_ERR_INVALID_ARG;
@@ -571,7 +582,7 @@ int oracle_fista_tv(const float* data, int64_t pitch, double* x_out, int32_t n_s
     rc = oracle_prox_tv(z, g, n_slices, ny, nx, beta / L, n_inner); /* g := x_{k+1} */
     if (rc) break;
     const double tn = 0.5 * (1.0 + sqrt(1.0 + 4.0 * t * t));
-    const double mom = (t - 1.0) / tn;
+    const double mom = accelerated ? (t - 1.0) / tn : 0.0;   /* ISTA: y_{k+1} = x_{k+1} */
     for (int64_t i = 0; i < n; ++i) {
       yk[i] = g[i] + mom * (g[i] - xk[i]);
       xk[i] = g[i];
@@ -580,5 +591,357 @@ int oracle_fista_tv(const float* data, int64_t pitch, double* x_out, int32_t n_s
   }
   memcpy(x_out, xk, sizeof(double) * (size_t)n);
   free(xk);
+  return rc;
+}
+
+int oracle_fista_tv(const float* data, int64_t pitch, double* x_out, int32_t n_slices,
+                    int32_t n_angles, int32_t n_bins, const double* angles, const double* axis,
+                    int32_t nx, int32_t ny, double h, double beta, double L, int32_t n_iter,
+                    int32_t n_inner, double* energy) {
+  return tv_solver(data, pitch, x_out, n_slices, n_angles, n_bins, angles, axis, nx, ny, h, beta, L,
+                   n_iter, n_inner, energy, 1);
+}
+
+/* ISTA ("ISTA ... or the accelerated FISTA ... can be used"): the same iteration
+ * without the momentum, y_{k+1} = x_{k+1}; energy[k] is then eq. 3 at the iterate x_k itself and
+ * does not increase from one iteration to the next (exact proximal step, L >= lambda_max). */
+int oracle_ista_tv(const float* data, int64_t pitch, double* x_out, int32_t n_slices,
+                   int32_t n_angles, int32_t n_bins, const double* angles, const double* axis,
+                   int32_t nx, int32_t ny, double h, double beta, double L, int32_t n_iter,
+                   int32_t n_inner, double* energy) {
+  return tv_solver(data, pitch, x_out, n_slices, n_angles, n_bins, angles, axis, nx, ny, h, beta, L,
+                   n_iter, n_inner, energy, 0);
+}
+
+/* ============================================================================
+ * NEXT row N4: ring-artefact filter (sec. 2.3) and the
+ * parameter-selection estimators of sec. 4 (L149-L162, eq. 10-11).
+ * ========================================================================== */
+
+/* Ring filter: "The filter reduces first the sinogram to a 1D signal by summing
+ * over the projection-angles.  An high-frequencies filter is then applied in an attempt to
+ * extract these features and the result is subtracted from the sinogram."  The optional model
+ * (L61: "thresholding the bone in a first reconstructed slice.  The thresholded signal is then
+ * subtracted to the data before application of the high-pass filter") is a sinogram of the same
+ * shape -- the projection of the thresholded slice -- or NULL.  Readings R21, the
+ * paper names neither the normalisation nor the high-pass filter:
+ *   m[b]  = (1/P) sum_p (q[p,b] - model[p,b])          angular MEAN (a per-bin error e[b] that sits
+ *                                                      in every row sums to P e[b])
+ *   lp[b] = mean of m over the bins b-r .. b+r that exist (centred moving average, window
+ *           clipped at the detector edges), r = half_width >= 1
+ *   hp[b] = m[b] - lp[b] ;   out[p,b] = q[p,b] - hp[b]  for every projection p.
+ * in: float32 [S][P][pitch]; out: double [S][P][B]. */
+int oracle_ring_filter(const float* sino, const float* model, int64_t pitch, double* out,
+                       int32_t n_slices, int32_t n_angles, int32_t n_bins, int32_t half_width) {
+  if (!sino || !out || n_slices <= 0 || n_angles <= 0 || n_bins <= 0 || half_width < 1)
+    return ORACLE_ERR_INVALID_ARG;
+  if (pitch == 0) pitch = n_bins;
+  int rc = ORACLE_OK;
+#pragma omp parallel for schedule(static)
+  for (int32_t s = 0; s < n_slices; ++s) {
+    double* m = (double*)malloc(sizeof(double) * 2 * (size_t)n_bins);
+    if (!m) { rc = ORACLE_ERR_NOMEM; continue; }
+    double* hp = m + n_bins;
+    for (int32_t b = 0; b < n_bins; ++b) {
+      double acc = 0.0;
+      for (int32_t p = 0; p < n_angles; ++p) {
+        int64_t o = ((int64_t)s * n_angles + p) * pitch + b;
+        acc += (double)sino[o] - (model ? (double)model[o] : 0.0);
+      }
+      m[b] = acc / (double)n_angles;
+    }
+    for (int32_t b = 0; b < n_bins; ++b) {
+      int32_t lo = b - half_width < 0 ? 0 : b - half_width;
+      int32_t hi = b + half_width > n_bins - 1 ? n_bins - 1 : b + half_width;
+      double acc = 0.0;
+      for (int32_t k = lo; k <= hi; ++k) acc += m[k];
+      hp[b] = m[b] - acc / (double)(hi - lo + 1);
+    }
+    for (int32_t p = 0; p < n_angles; ++p)
+      for (int32_t b = 0; b < n_bins; ++b)
+        out[((int64_t)s * n_angles + p) * n_bins + b] =
+            (double)sino[((int64_t)s * n_angles + p) * pitch + b] - hp[b];
+    free(m);
+  }
+  return rc;
+}
+
+/* Decoherence estimator, eq. 11:
+ *   E_cohe = Cos(I(beta) - I(0+), I(beta)) = <a - b, a> / (||a - b|| ||a||),  a = I(beta), b = I(0+),
+ * one value per slice of the stacks a, b [S][n] (float32, widened exactly).  A zero norm gives 0. */
+int oracle_ecohe(const float* a, const float* b, int32_t n_slices, int64_t n, double* out) {
+  if (!a || !b || !out || n_slices <= 0 || n <= 0) return ORACLE_ERR_INVALID_ARG;
+  for (int32_t s = 0; s < n_slices; ++s) {
+    double dot = 0.0, nd = 0.0, na = 0.0;
+    for (int64_t k = 0; k < n; ++k) {
+      double av = (double)a[s * n + k], d = av - (double)b[s * n + k];
+      dot += d * av;
+      nd += d * d;
+      na += av * av;
+    }
+    out[s] = (nd > 0.0 && na > 0.0) ? dot / (sqrt(nd) * sqrt(na)) : 0.0;
+  }
+  return ORACLE_OK;
+}
+
+/* Cross-validation estimator: "we reconstruct the slice using all the projections
+ * except a selected one at a given angle.  Then we calculate the quadratic distance between the
+ * reconstructed sample projection and the data for the excluded angle."  Given the reconstruction
+ * x [S][ny][nx] (made without the excluded projections) and the excluded projections' geometry
+ * (n_excl angles / axis positions) and data [S][n_excl][pitch]:
+ *   out[s] = sum_{e < n_excl} sum_b ( (P x)[s,e,b] - data[s,e,b] )^2 . */
+int oracle_cv_distance(const float* img, const float* data, int64_t pitch, int32_t n_slices,
+                       int32_t n_excl, int32_t n_bins, const double* angles, const double* axis,
+                       int32_t nx, int32_t ny, double h, double* out) {
+  int rc = check_geom(n_slices, n_excl, n_bins, angles, axis, nx, ny, h);
+  if (rc || !img || !data || !out) return rc ? rc : ORACLE_ERR_INVALID_ARG;
+  if (pitch == 0) pitch = n_bins;
+  double* y = (double*)malloc(sizeof(double) * (size_t)n_bins);
+  if (!y) return ORACLE_ERR_NOMEM;
+  for (int32_t s = 0; s < n_slices; ++s) {
+    double acc = 0.0;
+    for (int32_t e = 0; e < n_excl; ++e) {
+      fp_row(img + (int64_t)s * ny * nx, y, n_bins, axis[e], h, cos(angles[e]), sin(angles[e]), nx, ny, 1.0);
+      for (int32_t b = 0; b < n_bins; ++b) {
+        double d = y[b] - (double)data[((int64_t)s * n_excl + e) * pitch + b];
+        acc += d * d;
+      }
+    }
+    out[s] = acc;
+  }
+  free(y);
+  return ORACLE_OK;
+}
+
+/* ============================================================================
+ * NEXT row N3: overlapping-patch dictionary reconstruction,
+ * PAPER.md L102-L145 (sec. 3.2.1-3.2.2, eq. 4-9) and Algorithm 1 (L201-L228).
+ *
+ *   x_i = sum_p 1^c_p(i) sum_k w_kp phi_k(i - r_p)                                   (eq. 7)
+ *   f(w) = || y - Pi x ||^2 + rho sum_{p,i} 1_p(i) (x_i - sum_k w_kp phi_k(i - r_p))^2   (eq. 8)
+ *   F(w) = f(w) + beta ||w||_1, minimised by FISTA; "the L1 norm shrinking step is trivial" (L141)
+ *
+ * Matrices as in L145: D [Nc][m*m] (row k = basis function phi_k, row-major m x m), W [N][Nc],
+ * P = W D [N][m*m] (row p = the patch p rebuilt from its coefficients), G [N][Nc].
+ * Readings R16, R22-R24 of DESIGN.md (the paper gives no patch placement, tie-break, rho, m, Nc,
+ * step size):
+ *   R22 patches m x m on a regular grid of stride st (1 <= st <= m) that covers the image (eq. 4):
+ *       origins oy[a] = min(a st, ny - m), a < na = ceil((ny - m)/st) + 1 (ox[b] likewise),
+ *       patch index p = a nb + b, r_p = (oy[a], ox[b]), centre C_p = r_p + (m-1)/2;
+ *       core map (eq. 5-6): C_j = the patch whose centre is closest to j in the L1 norm, the
+ *       smallest p among equals; N_v(j) = number of patches that contain j.
+ *   R16 the residual image is R = Pi^T (Pi x - y) (eq. 9), not Alg. 1's Bp(data - Fp(X));
+ *       L226's garbled "P_{r_p+i}" is P_{p i}.
+ *   R23 step 1/Lw, Lw = 1.1 x the power-iteration estimate of the largest eigenvalue of the
+ *       Hessian of f (f is quadratic: grad f(w) = H w + g0; H v = grad f(v) evaluated with y = 0).
+ *   R24 w_0 = 0, Beck-Teboulle momentum as R20; energy[k] = F(v_k) at the point v_k where the
+ *       gradient of iteration k is taken.
+ * One slice per call (slices are independent; the dictionary is shared).
+ * ========================================================================== */
+
+static int32_t patch_count_1d(int32_t n, int32_t m, int32_t st) {
+  return n <= m ? 1 : (n - m + st - 1) / st + 1;
+}
+static int32_t patch_origin_1d(int32_t a, int32_t n, int32_t m, int32_t st) {
+  int32_t o = a * st;
+  return o > n - m ? n - m : o;
+}
+
+int oracle_patch_grid(int32_t ny, int32_t nx, int32_t m, int32_t st, int32_t* na, int32_t* nb) {
+  if (ny < m || nx < m || m <= 0 || st <= 0 || st > m || !na || !nb) return ORACLE_ERR_INVALID_ARG;
+  *na = patch_count_1d(ny, m, st);
+  *nb = patch_count_1d(nx, m, st);
+  return ORACLE_OK;
+}
+
+/* core[j] = C_j (eq. 5-6, brute force over all patches), cover[j] = N_v(j) (eq. 4). */
+int oracle_patch_maps(int32_t ny, int32_t nx, int32_t m, int32_t st, int32_t* core, int32_t* cover) {
+  int32_t na, nb;
+  int rc = oracle_patch_grid(ny, nx, m, st, &na, &nb);
+  if (rc || !core || !cover) return rc ? rc : ORACLE_ERR_INVALID_ARG;
+  const double half = 0.5 * (double)(m - 1);
+  for (int32_t iy = 0; iy < ny; ++iy)
+    for (int32_t ix = 0; ix < nx; ++ix) {
+      double best = 1e300;
+      int32_t bestp = -1, nv = 0;
+      for (int32_t a = 0; a < na; ++a)
+        for (int32_t b = 0; b < nb; ++b) {
+          int32_t oy = patch_origin_1d(a, ny, m, st), ox = patch_origin_1d(b, nx, m, st);
+          if (iy >= oy && iy < oy + m && ix >= ox && ix < ox + m) ++nv;
+          double d = fabs((double)iy - ((double)oy + half)) + fabs((double)ix - ((double)ox + half));
+          if (d < best) { best = d; bestp = a * nb + b; }
+        }
+      core[(int64_t)iy * nx + ix] = bestp;
+      cover[(int64_t)iy * nx + ix] = nv;
+    }
+  return ORACLE_OK;
+}
+
+/* Algorithm 1 in the paper's order.  W [N][Nc], D [Nc][m*m], data float32 [P][pitch] (one slice).
+ * Outputs (each nullable): G [N][Nc] = grad f(W) (eq. 9), X [ny][nx] (eq. 7), *fval = f(W) (eq. 8). */
+int oracle_patch_gradient(const double* W, const double* D, const float* data, int64_t pitch,
+                          int32_t n_angles, int32_t n_bins, const double* angles, const double* axis,
+                          int32_t nx, int32_t ny, double h, int32_t m, int32_t st, int32_t n_atoms,
+                          double rho, double* G, double* X_out, double* fval) {
+  int rc = check_geom(1, n_angles, n_bins, angles, axis, nx, ny, h);
+  int32_t na, nb;
+  if (!rc) rc = oracle_patch_grid(ny, nx, m, st, &na, &nb);
+  if (rc || !W || !D || !data || n_atoms <= 0 || !(rho >= 0.0)) return rc ? rc : ORACLE_ERR_INVALID_ARG;
+  if (pitch == 0) pitch = n_bins;
+  const int64_t N = (int64_t)na * nb, mm = (int64_t)m * m, npix = (int64_t)ny * nx;
+  const int64_t nsino = (int64_t)n_angles * n_bins;
+  double* P = (double*)calloc((size_t)(2 * N * mm + 3 * npix + nsino), sizeof(double));
+  int32_t* core = (int32_t*)malloc(sizeof(int32_t) * 2 * (size_t)npix);
+  if (!P || !core) { free(P); free(core); return ORACLE_ERR_NOMEM; }
+  double* Pp = P + N * mm;          /* P' */
+  double* X = Pp + N * mm;
+  double* R = X + npix;
+  double* S = R + npix;
+  double* r = S + npix;             /* residual sinogram */
+  int32_t* cover = core + npix;
+  oracle_patch_maps(ny, nx, m, st, core, cover);
+  /* P <- W . D */
+  for (int64_t p = 0; p < N; ++p)
+    for (int64_t e = 0; e < mm; ++e) {
+      double acc = 0.0;
+      for (int32_t k = 0; k < n_atoms; ++k) acc += W[p * n_atoms + k] * D[(int64_t)k * mm + e];
+      P[p * mm + e] = acc;
+    }
+  /* for all image positions j: p <- C_j; i <- j - r_p; X_j <- P_{p i} */
+  for (int32_t jy = 0; jy < ny; ++jy)
+    for (int32_t jx = 0; jx < nx; ++jx) {
+      int32_t p = core[(int64_t)jy * nx + jx];
+      int32_t oy = patch_origin_1d(p / nb, ny, m, st), ox = patch_origin_1d(p % nb, nx, m, st);
+      X[(int64_t)jy * nx + jx] = P[(int64_t)p * mm + (int64_t)(jy - oy) * m + (jx - ox)];
+    }
+  /* R = Pi^T (Pi X - data)   (R16: the sign of eq. 9) */
+  rc = oracle_forward_project_f64(X, r, 1, n_angles, n_bins, angles, axis, nx, ny, h, 1.0);
+  double fid = 0.0;
+  for (int32_t p = 0; p < n_angles && !rc; ++p)
+    for (int32_t b = 0; b < n_bins; ++b) {
+      r[(int64_t)p * n_bins + b] -= (double)data[(int64_t)p * pitch + b];
+      fid += r[(int64_t)p * n_bins + b] * r[(int64_t)p * n_bins + b];
+    }
+  if (!rc) rc = oracle_backproject_f64(r, n_bins, R, 1, n_angles, n_bins, angles, axis, nx, ny, h, 1.0);
+  /* S <- sum of all the patches covering each pixel; similarity term of eq. 8 */
+  double sim = 0.0;
+  for (int64_t p = 0; p < N; ++p) {
+    int32_t oy = patch_origin_1d((int32_t)(p / nb), ny, m, st), ox = patch_origin_1d((int32_t)(p % nb), nx, m, st);
+    for (int32_t iy = 0; iy < m; ++iy)
+      for (int32_t ix = 0; ix < m; ++ix) {
+        int64_t j = (int64_t)(oy + iy) * nx + (ox + ix);
+        double v = P[p * mm + (int64_t)iy * m + ix];
+        S[j] += v;
+        sim += (X[j] - v) * (X[j] - v);
+      }
+  }
+  /* P' per Algorithm 1 */
+  for (int64_t p = 0; p < N; ++p) {
+    int32_t oy = patch_origin_1d((int32_t)(p / nb), ny, m, st), ox = patch_origin_1d((int32_t)(p % nb), nx, m, st);
+    for (int32_t iy = 0; iy < m; ++iy)
+      for (int32_t ix = 0; ix < m; ++ix) {
+        int64_t j = (int64_t)(oy + iy) * nx + (ox + ix), e = (int64_t)iy * m + ix;
+        double v = 0.0;
+        if (core[j] == (int32_t)p) v += R[j] + rho * ((double)cover[j] * X[j] - S[j]);
+        v += rho * (P[p * mm + e] - X[j]);
+        Pp[p * mm + e] = v;
+      }
+  }
+  /* G <- 2 P' . D^T */
+  if (G)
+    for (int64_t p = 0; p < N; ++p)
+      for (int32_t k = 0; k < n_atoms; ++k) {
+        double acc = 0.0;
+        for (int64_t e = 0; e < mm; ++e) acc += Pp[p * mm + e] * D[(int64_t)k * mm + e];
+        G[p * n_atoms + k] = 2.0 * acc;
+      }
+  if (X_out) memcpy(X_out, X, sizeof(double) * (size_t)npix);
+  if (fval) *fval = fid + rho * sim;
+  free(P); free(core);
+  return rc;
+}
+
+/* "the L1 norm shrinking step is trivial" (L141): soft threshold sign(v) max(|v| - t, 0). */
+void oracle_soft_threshold(const double* v, int64_t n, double t, double* out) {
+  for (int64_t k = 0; k < n; ++k) {
+    double a = fabs(v[k]) - t;
+    out[k] = a > 0.0 ? (v[k] > 0.0 ? a : -a) : 0.0;
+  }
+}
+
+/* R23: Lw = 1.1 ||H v_n|| / ||v_n|| after n_power iterations v <- H v / ||H v|| from v = 1, where
+ * H v = grad f(v) with zero data (f is quadratic in w). */
+int oracle_patch_lipschitz(const double* D, int32_t n_angles, int32_t n_bins, const double* angles,
+                           const double* axis, int32_t nx, int32_t ny, double h, int32_t m, int32_t st,
+                           int32_t n_atoms, double rho, int32_t n_power, double* Lw) {
+  int32_t na, nb;
+  int rc = oracle_patch_grid(ny, nx, m, st, &na, &nb);
+  if (rc || !Lw || n_power <= 0) return rc ? rc : ORACLE_ERR_INVALID_ARG;
+  const int64_t n = (int64_t)na * nb * n_atoms;
+  double* v = (double*)malloc(sizeof(double) * 2 * (size_t)n);
+  float* zero = (float*)calloc((size_t)n_angles * (size_t)n_bins, sizeof(float));
+  if (!v || !zero) { free(v); free(zero); return ORACLE_ERR_NOMEM; }
+  double* g = v + n;
+  for (int64_t k = 0; k < n; ++k) v[k] = 1.0;
+  double ratio = 0.0;
+  for (int32_t it = 0; it < n_power && !rc; ++it) {
+    rc = oracle_patch_gradient(v, D, zero, n_bins, n_angles, n_bins, angles, axis, nx, ny, h, m, st,
+                               n_atoms, rho, g, NULL, NULL);
+    double nv = 0.0, ng = 0.0;
+    for (int64_t k = 0; k < n; ++k) { nv += v[k] * v[k]; ng += g[k] * g[k]; }
+    ratio = sqrt(ng) / sqrt(nv);
+    for (int64_t k = 0; k < n; ++k) v[k] = g[k] / sqrt(ng);
+  }
+  *Lw = 1.1 * ratio;
+  free(v); free(zero);
+  return rc;
+}
+
+/* FISTA on the coefficients (L139-L141; R23, R24):
+ *   w_0 = v_0 = 0, t_0 = 1;  for k < n_iter:
+ *     G = grad f(v_k) (Algorithm 1);  energy[k] = f(v_k) + beta ||v_k||_1
+ *     w_{k+1} = shrink(v_k - G / Lw, beta / Lw);  momentum as R20.
+ * W_out [N][Nc] = w_{n_iter}; X_out [ny][nx] = the image of eq. 7 at w_{n_iter} (nullable). */
+int oracle_patch_fista(const double* D, const float* data, int64_t pitch, int32_t n_angles,
+                       int32_t n_bins, const double* angles, const double* axis, int32_t nx, int32_t ny,
+                       double h, int32_t m, int32_t st, int32_t n_atoms, double rho, double beta,
+                       double Lw, int32_t n_iter, double* W_out, double* X_out, double* energy) {
+  int32_t na, nb;
+  int rc = oracle_patch_grid(ny, nx, m, st, &na, &nb);
+  if (rc || !D || !data || !W_out || !(Lw > 0.0) || !(beta >= 0.0) || n_iter < 0)
+    return rc ? rc : ORACLE_ERR_INVALID_ARG;
+  const int64_t n = (int64_t)na * nb * n_atoms;
+  double* w = (double*)calloc((size_t)(4 * n), sizeof(double));
+  if (!w) return ORACLE_ERR_NOMEM;
+  double* v = w + n;
+  double* g = v + n;
+  double* wn = g + n;
+  double t = 1.0;
+  for (int32_t k = 0; k < n_iter && !rc; ++k) {
+    double f = 0.0, l1 = 0.0;
+    rc = oracle_patch_gradient(v, D, data, pitch, n_angles, n_bins, angles, axis, nx, ny, h, m, st,
+                               n_atoms, rho, g, NULL, &f);
+    if (rc) break;
+    for (int64_t i = 0; i < n; ++i) l1 += fabs(v[i]);
+    if (energy) energy[k] = f + beta * l1;
+    for (int64_t i = 0; i < n; ++i) g[i] = v[i] - g[i] / Lw;
+    oracle_soft_threshold(g, n, beta / Lw, wn);
+    const double tn = 0.5 * (1.0 + sqrt(1.0 + 4.0 * t * t));
+    const double mom = (t - 1.0) / tn;
+    for (int64_t i = 0; i < n; ++i) {
+      v[i] = wn[i] + mom * (wn[i] - w[i]);
+      w[i] = wn[i];
+    }
+    t = tn;
+  }
+  memcpy(W_out, w, sizeof(double) * (size_t)n);
+  if (!rc && X_out) {
+    float* zero = (float*)calloc((size_t)n_angles * (size_t)n_bins, sizeof(float));
+    if (!zero) rc = ORACLE_ERR_NOMEM;
+    else rc = oracle_patch_gradient(w, D, zero, n_bins, n_angles, n_bins, angles, axis, nx, ny, h, m,
+                                    st, n_atoms, rho, NULL, X_out, NULL);
+    free(zero);
+  }
+  free(w);
   return rc;
 }
