@@ -60,9 +60,12 @@ enum {
  *   Ram-Lak     h[0] = 1/4, h[n odd] = -1/(pi^2 n^2), h[n even != 0] = 0
  *   Shepp-Logan h[n] = -2 / (pi^2 (4 n^2 - 1))
  *   Hann, Hamming (NEXT row N2): Ram-Lak times the window a0 + 2 a1 cos(2 pi w), w in cycles per
- *               bin, (a0, a1) = (0.5, 0.25) resp. (0.54, 0.23): h_w[n] = a0 h[n] + a1 (h[n-1] + h[n+1]) */
+ *               bin, (a0, a1) = (0.5, 0.25) resp. (0.54, 0.23): h_w[n] = a0 h[n] + a1 (h[n-1] + h[n+1])
+ *   Cosine      Ram-Lak times cos(pi w): a pair of half-bin shifts of the continuous band-limited ramp,
+ *               h_c[n] = (h(n-1/2) + h(n+1/2)) / 2,  h(m+1/2) = (-1)^m / (2 pi (m+1/2)) - 1 / (2 pi^2 (m+1/2)^2)
+ *               (reading R8c; h_c[0] = 1/pi - 2/pi^2) */
 typedef enum { PYHST_FILTER_RAMLAK = 0, PYHST_FILTER_SHEPP_LOGAN = 1, PYHST_FILTER_HANN = 2,
-               PYHST_FILTER_HAMMING = 3 } pyhst_filter_t;
+               PYHST_FILTER_HAMMING = 3, PYHST_FILTER_COSINE = 4 } pyhst_filter_t;
 
 /* >= 180 degrees; with 360 degrees and the axis near the detector border the
  * detector "can be virtually doubled" (PYHST_SCAN_360_HALF, reading R10). */
@@ -160,6 +163,47 @@ int pyhst_forward_project_host(const float* h_img, float* h_sino, const pyhst_ge
 int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geom_t* g, float beta,
                    int32_t n_iter, int32_t n_inner, int32_t n_power, double* energy,
                    double* lipschitz, void* stream);
+
+/* ISTA ("ISTA ... or the accelerated FISTA ... can be used"): pyhst_fista_tv without
+ * the momentum (y_{k+1} = x_{k+1}); same arguments, workspace and errors.  energy[k] is then eq. 3
+ * at the iterate x_k itself and does not increase from one iteration to the next. */
+int pyhst_ista_tv(const float* d_data, float* d_img, const pyhst_geom_t* g, float beta,
+                  int32_t n_iter, int32_t n_inner, int32_t n_power, double* energy,
+                  double* lipschitz, void* stream);
+
+/* NEXT row N4 -- ring-artefact filter (sec. 2.3: "The filter reduces first the sinogram
+ * to a 1D signal by summing over the projection-angles.  An high-frequencies filter is then applied in
+ * an attempt to extract these features and the result is subtracted from the sinogram"; reading R21):
+ *   m[s][b]  = (1/P) sum_p (sino[s][p][b] - model[s][p][b])       angular mean, per slice
+ *   hp[s][b] = m[s][b] - mean of m[s] over the bins b-r .. b+r that exist    (r = half_width >= 1)
+ *   out[s][p][b] = sino[s][p][b] - hp[s][b]                        for every projection p
+ *   d_sino   DEVICE [n_slices][n_angles][pitch] f32, read
+ *   d_model  DEVICE, same layout, or NULL (= 0): the projection of the thresholded first reconstruction
+ *            (L61: "thresholding the bone ... The thresholded signal is then subtracted to the data
+ *            before application of the high-pass filter")
+ *   d_out    DEVICE, same layout, written; may be d_sino itself (in place)
+ * pitch 0 => n_bins.  Errors: null pointers, sizes <= 0, half_width < 1, pitch < n_bins -> INVALID_ARG. */
+int pyhst_ring_filter(const float* d_sino, const float* d_model, float* d_out, int32_t n_slices,
+                      int32_t n_angles, int32_t n_bins, int64_t pitch, int32_t half_width, void* stream);
+
+/* NEXT row N4 -- decoherence-maximising estimator, eq. 11:
+ *   E_cohe[s] = Cos(I(beta) - I(0+), I(beta)) = <a - b, a> / (||a - b|| ||a||),  a = d_img_beta[s], b = d_img_0[s]
+ * one fused pass over the two stacks, sums in double, fixed summation order (deterministic).
+ *   d_img_beta, d_img_0  DEVICE [n_slices][n_per_slice] f32, read
+ *   h_out                HOST [n_slices]; the call synchronises `stream`.  A zero norm gives 0. */
+int pyhst_ecohe(const float* d_img_beta, const float* d_img_0, int32_t n_slices, int64_t n_per_slice,
+                double* h_out, void* stream);
+
+/* NEXT row N4 -- cross-validation estimator ("we reconstruct the slice using all the
+ * projections except a selected one at a given angle.  Then we calculate the quadratic distance between
+ * the reconstructed sample projection and the data for the excluded angle"):
+ *   h_out[s] = sum_{e < g_excl->n_angles} sum_b ( (P x)[s][e][b] - d_data_excl[s][e][b] )^2
+ * g_excl describes ONLY the excluded projections (their angles / axis positions; n_slices, n_bins, nx,
+ * ny, pixel_size as in the reconstruction; sino_pitch = row pitch of d_data_excl).  The reconstruction
+ * d_img is made by the caller from the remaining projections (e.g. pyhst_fista_tv with the reduced
+ * angle list).  P = pyhst_forward_project (scale 1); the call synchronises `stream`. */
+int pyhst_cv_distance(const float* d_img, const float* d_data_excl, const pyhst_geom_t* g_excl,
+                      double* h_out, void* stream);
 
 /* Extended row length / left padding of the virtually doubled detector (R10):
  * far = max(cbar, n_bins-1-cbar); *n_bins_ext = ceil(2 far) + 1 rounded up to a multiple of

@@ -16,6 +16,7 @@ FILTER_RAMLAK = 0
 FILTER_SHEPP_LOGAN = 1
 FILTER_HANN = 2
 FILTER_HAMMING = 3
+FILTER_COSINE = 4
 SCAN_180 = 0
 SCAN_360 = 1
 SCAN_360_HALF = 2
@@ -23,9 +24,9 @@ SCAN_360_HALF = 2
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBNAME = "libpyhst_b200.so"
 
-# every symbol include/pyhst.h declares
+# every symbol include/*.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
-           "pyhst_fista_tv", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_set_halfacq_stitch",
+           "pyhst_fista_tv", "pyhst_ista_tv", "pyhst_ring_filter", "pyhst_ecohe", "pyhst_cv_distance", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_set_halfacq_stitch",
            "pyhst_last_error", "pyhst_release_cache")
 
 
@@ -66,6 +67,11 @@ def _load():
     lib.pyhst_forward_project_host.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_int32, c_void_p]
     lib.pyhst_fista_tv.argtypes = [c_void_p, c_void_p, POINTER(Geom), c_float, c_int32, c_int32, c_int32,
                                    POINTER(c_double), POINTER(c_double), c_void_p]
+    lib.pyhst_ista_tv.argtypes = lib.pyhst_fista_tv.argtypes
+    lib.pyhst_ring_filter.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int64, c_int32,
+                                      c_void_p]
+    lib.pyhst_ecohe.argtypes = [c_void_p, c_void_p, c_int32, c_int64, POINTER(c_double), c_void_p]
+    lib.pyhst_cv_distance.argtypes = [c_void_p, c_void_p, POINTER(Geom), POINTER(c_double), c_void_p]
     lib.pyhst_halfacq_extent.argtypes = [c_int32, c_double, POINTER(c_int32), POINTER(c_int32)]
     lib.pyhst_set_backproject_variant.argtypes = [c_int]
     lib.pyhst_set_forward_project_variant.argtypes = [c_int]
@@ -171,23 +177,70 @@ def fbp(d_sino_raw, angles, axis, nx, ny, pixel_size=1.0, filter=FILTER_RAMLAK, 
 
 
 def fista_tv(d_data, angles, axis, nx, ny, beta, n_iter, n_inner=20, n_power=8, pixel_size=1.0, out=None,
-             want_energy=True, stream=None):
-    """pyhst_fista_tv: float32 CUDA data [S,P,B] -> (x [S,ny,nx] CUDA, energy float64 [n_iter], L).
+             want_energy=True, stream=None, accelerated=True):
+    """pyhst_fista_tv (accelerated=False: pyhst_ista_tv): float32 CUDA data [S,P,B] ->
+    (x [S,ny,nx] CUDA, energy float64 [n_iter], L).
     With want_energy=False nothing is copied back and the call does not synchronise."""
     import torch
     lib = _load()
+    fn = lib.pyhst_fista_tv if accelerated else lib.pyhst_ista_tv
     s, p, b = d_data.shape
     if out is None:
         out = torch.empty((s, ny, nx), dtype=torch.float32, device=d_data.device)
     g = _geom(s, p, b, angles, axis, nx, ny, pixel_size)
     energy = np.zeros(max(int(n_iter), 1), dtype=np.float64)
     lip = c_double(0.0)
-    _check(lib.pyhst_fista_tv(_dev(d_data, "d_data"), _dev(out, "out"), ctypes.byref(g), float(beta),
-                              int(n_iter), int(n_inner), int(n_power),
-                              energy.ctypes.data_as(POINTER(c_double)) if want_energy else None,
-                              ctypes.byref(lip) if want_energy else None, _stream(stream)),
-           "pyhst_fista_tv")
+    _check(fn(_dev(d_data, "d_data"), _dev(out, "out"), ctypes.byref(g), float(beta),
+              int(n_iter), int(n_inner), int(n_power),
+              energy.ctypes.data_as(POINTER(c_double)) if want_energy else None,
+              ctypes.byref(lip) if want_energy else None, _stream(stream)),
+           "pyhst_fista_tv" if accelerated else "pyhst_ista_tv")
     return out, energy[:int(n_iter)], float(lip.value)
+
+
+def ista_tv(*args, **kwargs):
+    """pyhst_ista_tv: fista_tv without the momentum."""
+    return fista_tv(*args, accelerated=False, **kwargs)
+
+
+def ring_filter(d_sino, half_width, model=None, out=None, stream=None):
+    """pyhst_ring_filter: float32 CUDA [S,P,B] (+ optional model of the same shape) -> [S,P,B]."""
+    import torch
+    lib = _load()
+    s, p, b = d_sino.shape
+    if out is None:
+        out = torch.empty_like(d_sino)
+    _check(lib.pyhst_ring_filter(_dev(d_sino, "d_sino"), None if model is None else _dev(model, "model"),
+                                 _dev(out, "out"), s, p, b, c_int64(b), int(half_width), _stream(stream)),
+           "pyhst_ring_filter")
+    return out
+
+
+def ecohe(d_img_beta, d_img_0, stream=None):
+    """pyhst_ecohe: eq. 11 per slice of two float32 CUDA stacks [S, ...] -> float64 [S] (host)."""
+    lib = _load()
+    s = d_img_beta.shape[0]
+    if tuple(d_img_beta.shape) != tuple(d_img_0.shape):
+        raise PyhstError("stacks must have the same shape")
+    out = np.zeros(s, dtype=np.float64)
+    _check(lib.pyhst_ecohe(_dev(d_img_beta, "d_img_beta"), _dev(d_img_0, "d_img_0"), s,
+                           c_int64(d_img_beta[0].numel()), out.ctypes.data_as(POINTER(c_double)), _stream(stream)),
+           "pyhst_ecohe")
+    return out
+
+
+def cv_distance(d_img, d_data_excl, angles_excl, axis_excl, pixel_size=1.0, stream=None):
+    """pyhst_cv_distance: sum over the excluded projections of ||P x - data||^2 per slice -> float64 [S]."""
+    lib = _load()
+    s, ny, nx = d_img.shape
+    s2, e, b = d_data_excl.shape
+    if s2 != s:
+        raise PyhstError("d_img and d_data_excl must have the same number of slices")
+    g = _geom(s, e, b, angles_excl, axis_excl, nx, ny, pixel_size)
+    out = np.zeros(s, dtype=np.float64)
+    _check(lib.pyhst_cv_distance(_dev(d_img, "d_img"), _dev(d_data_excl, "d_data_excl"), ctypes.byref(g),
+                                 out.ctypes.data_as(POINTER(c_double)), _stream(stream)), "pyhst_cv_distance")
+    return out
 
 
 def _host_ptr(a, name):

@@ -534,7 +534,7 @@ int pyhst_ramp_filter(const float* d_in, float* d_out, int64_t n_rows, int32_t n
   if (out_pitch < n_bins_out)
     return set_error(PYHST_ERR_INVALID_ARG, "out_pitch %lld < n_bins_out %d", (long long)out_pitch,
                      n_bins_out);
-  if ((int)f < PYHST_FILTER_RAMLAK || (int)f > PYHST_FILTER_HAMMING)
+  if ((int)f < PYHST_FILTER_RAMLAK || (int)f > PYHST_FILTER_COSINE)
     return set_error(PYHST_ERR_INVALID_ARG, "unknown filter %d", (int)f);
   if ((int64_t)n_bins_in + n_bins_out > 16384)
     return set_error(PYHST_ERR_UNSUPPORTED, "n_bins_in + n_bins_out > 16384");
@@ -712,7 +712,7 @@ static int fbp_device(const float* d_sino_raw, int64_t pitch, float* d_img, cons
 
 static int check_fbp(const pyhst_geom_t* g, pyhst_filter_t f, pyhst_scan_t mode, int64_t* pitch) {
   PYHST_TRY(check_geom(g, pitch));
-  if ((int)f < PYHST_FILTER_RAMLAK || (int)f > PYHST_FILTER_HAMMING)
+  if ((int)f < PYHST_FILTER_RAMLAK || (int)f > PYHST_FILTER_COSINE)
     return set_error(PYHST_ERR_INVALID_ARG, "unknown filter %d", (int)f);
   if (mode != PYHST_SCAN_180 && mode != PYHST_SCAN_360 && mode != PYHST_SCAN_360_HALF)
     return set_error(PYHST_ERR_INVALID_ARG, "unknown scan mode %d", (int)mode);

@@ -60,7 +60,15 @@ __global__ void ramp_kernel_table(double* hc, int M, int filter) {
     h = ramlak(l);
   else if (filter == PYHST_FILTER_SHEPP_LOGAN)
     h = -2.0 / (PI * PI * (4.0 * dl * dl - 1.0));
-  else {  // Hann / Hamming window a0 + 2 a1 cos(2 pi w) on the Ram-Lak ramp = unit shifts in space
+  else if (filter == PYHST_FILTER_COSINE) {
+    // window cos(pi w) = half-bin shifts of the continuous band-limited ramp (R8c):
+    // ramp(m + 1/2) = (-1)^m / (2 pi (m + 1/2)) - 1 / (2 pi^2 (m + 1/2)^2)
+    auto half_shifted = [PI](int m) {
+      const double x = (double)m + 0.5;
+      return ((m & 1) ? -1.0 : 1.0) / (2.0 * PI * x) - 1.0 / (2.0 * PI * PI * x * x);
+    };
+    h = 0.5 * (half_shifted(l - 1) + half_shifted(l));
+  } else {  // Hann / Hamming window a0 + 2 a1 cos(2 pi w) on the Ram-Lak ramp = unit shifts in space
     const double a0 = filter == PYHST_FILTER_HANN ? 0.5 : 0.54, a1 = filter == PYHST_FILTER_HANN ? 0.25 : 0.23;
     h = a0 * ramlak(l) + a1 * (ramlak(l - 1) + ramlak(l + 1));
   }

@@ -207,9 +207,9 @@ __global__ void ftv_fill_kernel(float* v, int64_t n, float value) {
 
 using namespace pyhst;
 
-extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geom_t* g, float beta,
-                              int32_t n_iter, int32_t n_inner, int32_t n_power, double* energy,
-                              double* lipschitz, void* stream_) {
+static int tv_solver(const float* d_data, float* d_img, const pyhst_geom_t* g, float beta,
+                     int32_t n_iter, int32_t n_inner, int32_t n_power, double* energy,
+                     double* lipschitz, void* stream_, bool accelerated) {
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   if (!d_data || !d_img || !g)
     return set_error(PYHST_ERR_INVALID_ARG, "pyhst_fista_tv: null pointer");
@@ -302,7 +302,7 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
     }
     const double tn = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
     ftv_finish_kernel<<<grid_img, blk, 0, stream>>>(z, p[cur], p[cur + 1], d_img, y, nx, ny, d_fs,
-                                                    (float)((t - 1.0) / tn), use_p ? 1 : 0);
+                                                    accelerated ? (float)((t - 1.0) / tn) : 0.f, use_p ? 1 : 0);
     t = tn;
     PYHST_CUDA_TRY(cudaGetLastError());
   }
@@ -315,4 +315,17 @@ extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geo
       for (int k = 0; k < n_iter; ++k) energy[k] = h[(size_t)3 + k];
   }
   return PYHST_OK;
+}
+
+extern "C" int pyhst_fista_tv(const float* d_data, float* d_img, const pyhst_geom_t* g, float beta,
+                              int32_t n_iter, int32_t n_inner, int32_t n_power, double* energy,
+                              double* lipschitz, void* stream) {
+  return tv_solver(d_data, d_img, g, beta, n_iter, n_inner, n_power, energy, lipschitz, stream, true);
+}
+
+// ISTA: no momentum, y_{k+1} = x_{k+1}
+extern "C" int pyhst_ista_tv(const float* d_data, float* d_img, const pyhst_geom_t* g, float beta,
+                             int32_t n_iter, int32_t n_inner, int32_t n_power, double* energy,
+                             double* lipschitz, void* stream) {
+  return tv_solver(d_data, d_img, g, beta, n_iter, n_inner, n_power, energy, lipschitz, stream, false);
 }

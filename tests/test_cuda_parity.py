@@ -471,3 +471,102 @@ def test_large_pixel_size_falls_back_to_the_reference_kernel(lib, oracle):
     wantp = oracle.forward_project(x, w.angles, w.axis, 700, pixel_size=6.0)
     gotp = lib.forward_project(_dev(x), w.angles, w.axis, 700, pixel_size=6.0).cpu().numpy()
     assert_parity(gotp, wantp, "forward_project pixel_size 6")
+
+
+# ------------------------------------------------------------------------------ N2: cosine window
+@pytest.mark.gpu
+def test_cosine_window_filter_and_fbp(lib, oracle):
+    rng = np.random.default_rng(44)
+    rows = rng.normal(size=(5, 300)).astype(np.float32)
+    want = oracle.ramp_filter(rows, n_bins_out=340, pad_left=17, filter=oracle.FILTER_COSINE)
+    got = lib.ramp_filter(_dev(rows), n_bins_out=340, pad_left=17, filter=lib.FILTER_COSINE).cpu().numpy()
+    assert_parity(got, want, "ramp_filter cosine")
+    w = lib.workloads.config(2, shrink=8, n_slices=5)
+    sino = w.sinogram()
+    want = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, filter=oracle.FILTER_COSINE, mode=w.mode)
+    got = lib.fbp(_dev(sino), w.angles, w.axis, w.nx, w.ny, filter=lib.FILTER_COSINE, mode=w.mode).cpu().numpy()
+    assert_parity(got, want, "fbp cosine window")
+
+
+# ------------------------------------------------------------------------------ N1: ISTA switch
+@pytest.mark.gpu
+def test_ista_tv_matches_oracle_and_descends(lib, oracle):
+    w = lib.workloads.config(4, shrink=8, n_slices=3)
+    data = w.sinogram()
+    L = oracle.lipschitz(w.angles, w.axis, w.n_bins, w.nx, w.ny, n_power=8)
+    want, e_want = oracle.ista_tv(data, w.angles, w.axis, w.nx, w.ny, 0.5, L, 15, n_inner=20)
+    got, e_got, L_got = lib.ista_tv(_dev(data), w.angles, w.axis, w.nx, w.ny, 0.5, 15, n_inner=20, n_power=8)
+    assert abs(L_got - L) <= 1e-5 * L
+    np.testing.assert_allclose(e_got, e_want, rtol=FISTA_REL_ENERGY)
+    assert_parity(got.cpu().numpy(), want, "ista_tv", rel=FISTA_REL_L2, mabs=5e-3)
+    # the energy of eq. 3 does not increase under ISTA (inexact prox: to rounding)
+    _, e_long, _ = lib.ista_tv(_dev(data), w.angles, w.axis, w.nx, w.ny, 0.5, 60, n_inner=40, n_power=8)
+    assert np.all(np.diff(e_long) <= 1e-5 * e_long[0])
+    # two runs are bit-identical (deterministic reductions)
+    got2, e2, L2 = lib.ista_tv(_dev(data), w.angles, w.axis, w.nx, w.ny, 0.5, 15, n_inner=20, n_power=8)
+    assert L2 == L_got and np.array_equal(e2, e_got) and bool((got2 == got).all())
+
+
+# ------------------------------------------------------------------------------ N4
+@pytest.mark.gpu
+@pytest.mark.parametrize("S,P,B,r,with_model", [(1, 1, 40, 1, False), (3, 50, 211, 4, True), (2, 333, 1000, 15, False),
+                                                (5, 64, 2048, 9, True)])
+def test_ring_filter_matches_oracle(lib, oracle, S, P, B, r, with_model):
+    rng = np.random.default_rng(S * 1000 + B)
+    sino = (rng.normal(size=(S, P, B)) + 0.5 * rng.normal(size=(S, 1, B))).astype(np.float32)   # per-bin errors
+    model = rng.normal(size=(S, P, B)).astype(np.float32) if with_model else None
+    want = oracle.ring_filter(sino, r, model=model)
+    got = lib.ring_filter(_dev(sino), r, model=None if model is None else _dev(model)).cpu().numpy()
+    assert_parity(got, want, "ring_filter")
+    d = _dev(sino)
+    lib.ring_filter(d, r, model=None if model is None else _dev(model), out=d)                   # in place
+    assert np.array_equal(d.cpu().numpy(), got)
+    with pytest.raises(lib.PyhstError):
+        lib.ring_filter(_dev(sino), 0)
+
+
+@pytest.mark.gpu
+def test_ring_filter_removes_rings_from_a_reconstruction(lib, oracle):
+    """End to end: per-bin detector errors give rings in the FBP; the filter removes most of them."""
+    w = lib.workloads.config(2, shrink=8, n_slices=2)
+    clean = w.sinogram()
+    rng = np.random.default_rng(61)
+    err = np.zeros(w.n_bins, dtype=np.float32)
+    err[rng.choice(w.n_bins, 12, replace=False)] = rng.choice([-0.05, 0.05], 12).astype(np.float32)
+    dirty = clean + err[None, None, :]
+    rec = lambda s: lib.fbp(s, w.angles, w.axis, w.nx, w.ny, filter=w.filter).cpu().numpy()
+    r_clean, r_dirty = rec(_dev(clean)), rec(_dev(dirty))
+    r_fixed = rec(lib.ring_filter(_dev(dirty), 3))
+    e_dirty = np.linalg.norm(r_dirty - r_clean)
+    e_fixed = np.linalg.norm(r_fixed - r_clean)
+    assert e_fixed < 0.45 * e_dirty
+
+
+@pytest.mark.gpu
+def test_ecohe_and_cv_distance_match_oracle(lib, oracle):
+    wl = lib.workloads
+    rng = np.random.default_rng(62)
+    a = rng.normal(size=(3, 201, 187)).astype(np.float32)
+    b = (a + 0.3 * rng.normal(size=a.shape)).astype(np.float32)
+    want = oracle.ecohe(a, b)
+    got = lib.ecohe(_dev(a), _dev(b))
+    np.testing.assert_allclose(got, want, rtol=1e-12, atol=1e-14)
+    assert lib.ecohe(_dev(a), _dev(a)).tolist() == [0.0, 0.0, 0.0]
+    assert np.array_equal(lib.ecohe(_dev(a), _dev(b)), got)                # deterministic
+    # cross-validation: leave two projections out of a config-4-like scan
+    w = wl.config(4, shrink=8, n_slices=2)
+    data = w.sinogram()
+    excl = [7, 19]
+    keep = [p for p in range(w.n_angles) if p not in excl]
+    x, _, _ = lib.fista_tv(_dev(np.ascontiguousarray(data[:, keep])), w.angles[keep], w.axis[keep], w.nx, w.ny,
+                           0.05, 30, n_inner=10)
+    d_excl = np.ascontiguousarray(data[:, excl])
+    want = oracle.cv_distance(x.cpu().numpy(), d_excl, w.angles[excl], w.axis[excl])
+    got = lib.cv_distance(x, _dev(d_excl), w.angles[excl], w.axis[excl])
+    np.testing.assert_allclose(got, want, rtol=2e-5)
+    # estimator curve: E_cohe between a weakly and a strongly regularised reconstruction is finite and in [-1, 1]
+    x0, _, _ = lib.fista_tv(_dev(np.ascontiguousarray(data[:, keep])), w.angles[keep], w.axis[keep], w.nx, w.ny,
+                            1e-4, 30, n_inner=10)
+    e = lib.ecohe(x, x0)
+    assert np.all(np.abs(e) <= 1.0) and np.all(np.isfinite(e))
+    np.testing.assert_allclose(e, oracle.ecohe(x.cpu().numpy(), x0.cpu().numpy()), rtol=1e-10, atol=1e-13)
