@@ -205,6 +205,44 @@ int pyhst_ecohe(const float* d_img_beta, const float* d_img_0, int32_t n_slices,
 int pyhst_cv_distance(const float* d_img, const float* d_data_excl, const pyhst_geom_t* g_excl,
                       double* h_out, void* stream);
 
+/* NEXT row N3 -- overlapping-patch dictionary reconstruction, PAPER.md L102-L145 (sec. 3.2, eq. 4-9)
+ * and Algorithm 1 (L201-L228); readings R16, R22-R24 of DESIGN.md.
+ *   x_i = sum_p 1^c_p(i) sum_k w_kp phi_k(i - r_p)                                       (eq. 7)
+ *   f(w) = ||y - P x||^2 + rho sum_{p,i} 1_p(i) (x_i - sum_k w_kp phi_k(i - r_p))^2       (eq. 8)
+ *   F(w) = f(w) + beta ||w||_1, minimised by FISTA with the soft-threshold step (L139-L141).
+ * Patches are m x m on a regular grid of stride `stride` (1 <= stride <= m): origins
+ * min(a * stride, n - m), a < na (pyhst_patch_grid), patch index p = a * nb + b; the core of a patch
+ * (eq. 5-6) is the set of pixels whose L1-closest patch centre is its own (smallest p among equals).
+ * Matrices as in L145: D [n_atoms][m*m] (row k = basis function phi_k, row-major m x m, shared by
+ * all slices), W [n_slices][N][n_atoms] with N = na * nb, G like W.  All DEVICE, float32. */
+typedef struct {
+  int32_t m, stride, n_atoms;
+  float rho;                        /* weight of the similarity term of eq. 8, >= 0 */
+} pyhst_patch_t;
+
+/* Pure host function: number of patch rows / columns that cover an ny x nx image (eq. 4). */
+int pyhst_patch_grid(int32_t ny, int32_t nx, int32_t m, int32_t stride, int32_t* na, int32_t* nb);
+
+/* Algorithm 1: P <- W D; X from the patch cores (eq. 7); R <- P^T (P X - data) (eq. 9's sign, R16);
+ * S <- sum of the covering patches; P' per Algorithm 1; G <- 2 P' D^T  (= grad f(W), eq. 9).
+ *   d_data [n_slices][n_angles][sino_pitch]  read;   g as for pyhst_forward_project
+ *   d_G    [n_slices][N][n_atoms]  written, or NULL (then only X / f are computed)
+ *   d_X    [n_slices][ny][nx]      written, or NULL
+ *   h_fval HOST scalar = f(W) of eq. 8 summed over the slices, or NULL; if given the call synchronises.
+ * Errors: null pointers, stride > m or < 1, m < 1, image smaller than a patch, rho < 0 -> INVALID_ARG. */
+int pyhst_patch_gradient(const float* d_W, const float* d_D, const float* d_data, const pyhst_geom_t* g,
+                         const pyhst_patch_t* pp, float* d_G, float* d_X, double* h_fval, void* stream);
+
+/* FISTA on the coefficients (R23, R24): w_0 = 0; step 1/Lw with Lw = 1.1 x the power-iteration estimate
+ * (n_power iterations from w = 1) of the largest eigenvalue of the Hessian of f; w_{k+1} =
+ * shrink(v_k - grad f(v_k)/Lw, beta/Lw); Beck-Teboulle momentum.  energy[k] = f(v_k) + beta ||v_k||_1.
+ *   d_W [n_slices][N][n_atoms] written (w after n_iter iterations); d_X [n_slices][ny][nx] = eq. 7 at the
+ *   result, or NULL; energy HOST [n_iter] or NULL; lipschitz HOST scalar or NULL (either one: the call
+ *   synchronises). */
+int pyhst_patch_fista(const float* d_D, const float* d_data, const pyhst_geom_t* g, const pyhst_patch_t* pp,
+                      float beta, int32_t n_iter, int32_t n_power, float* d_W, float* d_X, double* energy,
+                      double* lipschitz, void* stream);
+
 /* Extended row length / left padding of the virtually doubled detector (R10):
  * far = max(cbar, n_bins-1-cbar); *n_bins_ext = ceil(2 far) + 1 rounded up to a multiple of
  * 64; *pad_left = 0 if the axis is right of the detector centre else n_bins_ext - n_bins. */

@@ -26,7 +26,8 @@ _LIBNAME = "libpyhst_b200.so"
 
 # every symbol include/*.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
-           "pyhst_fista_tv", "pyhst_ista_tv", "pyhst_ring_filter", "pyhst_ecohe", "pyhst_cv_distance", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_set_halfacq_stitch",
+           "pyhst_fista_tv", "pyhst_ista_tv", "pyhst_ring_filter", "pyhst_ecohe", "pyhst_cv_distance", "pyhst_patch_grid",
+           "pyhst_patch_gradient", "pyhst_patch_fista", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_set_halfacq_stitch",
            "pyhst_last_error", "pyhst_release_cache")
 
 
@@ -72,6 +73,11 @@ def _load():
                                       c_void_p]
     lib.pyhst_ecohe.argtypes = [c_void_p, c_void_p, c_int32, c_int64, POINTER(c_double), c_void_p]
     lib.pyhst_cv_distance.argtypes = [c_void_p, c_void_p, POINTER(Geom), POINTER(c_double), c_void_p]
+    lib.pyhst_patch_grid.argtypes = [c_int32, c_int32, c_int32, c_int32, POINTER(c_int32), POINTER(c_int32)]
+    lib.pyhst_patch_gradient.argtypes = [c_void_p, c_void_p, c_void_p, POINTER(Geom), POINTER(Patch), c_void_p,
+                                         c_void_p, POINTER(c_double), c_void_p]
+    lib.pyhst_patch_fista.argtypes = [c_void_p, c_void_p, POINTER(Geom), POINTER(Patch), c_float, c_int32, c_int32,
+                                      c_void_p, c_void_p, POINTER(c_double), POINTER(c_double), c_void_p]
     lib.pyhst_halfacq_extent.argtypes = [c_int32, c_double, POINTER(c_int32), POINTER(c_int32)]
     lib.pyhst_set_backproject_variant.argtypes = [c_int]
     lib.pyhst_set_forward_project_variant.argtypes = [c_int]
@@ -241,6 +247,54 @@ def cv_distance(d_img, d_data_excl, angles_excl, axis_excl, pixel_size=1.0, stre
     _check(lib.pyhst_cv_distance(_dev(d_img, "d_img"), _dev(d_data_excl, "d_data_excl"), ctypes.byref(g),
                                  out.ctypes.data_as(POINTER(c_double)), _stream(stream)), "pyhst_cv_distance")
     return out
+
+
+class Patch(ctypes.Structure):
+    _fields_ = [("m", c_int32), ("stride", c_int32), ("n_atoms", c_int32), ("rho", c_float)]
+
+
+def patch_grid(ny, nx, m, stride):
+    na, nb = c_int32(0), c_int32(0)
+    _check(_load().pyhst_patch_grid(ny, nx, m, stride, ctypes.byref(na), ctypes.byref(nb)), "pyhst_patch_grid")
+    return int(na.value), int(nb.value)
+
+
+def patch_gradient(d_W, d_D, d_data, angles, axis, nx, ny, m, stride, rho, pixel_size=1.0, want_f=True,
+                   stream=None):
+    """pyhst_patch_gradient (Algorithm 1): W [S,N,Nc], D [Nc,m*m], data [S,P,B] (float32 CUDA) ->
+    (G [S,N,Nc], X [S,ny,nx], f)."""
+    import torch
+    lib = _load()
+    s, p, b = d_data.shape
+    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size)
+    pp = Patch(int(m), int(stride), int(d_D.shape[0]), float(rho))
+    G = torch.empty_like(d_W)
+    X = torch.empty((s, ny, nx), dtype=torch.float32, device=d_W.device)
+    f = c_double(0.0)
+    _check(lib.pyhst_patch_gradient(_dev(d_W, "d_W"), _dev(d_D, "d_D"), _dev(d_data, "d_data"), ctypes.byref(g),
+                                    ctypes.byref(pp), _dev(G, "G"), _dev(X, "X"),
+                                    ctypes.byref(f) if want_f else None, _stream(stream)), "pyhst_patch_gradient")
+    return G, X, float(f.value)
+
+
+def patch_fista(d_D, d_data, angles, axis, nx, ny, m, stride, rho, beta, n_iter, n_power=8, pixel_size=1.0,
+                want_energy=True, stream=None):
+    """pyhst_patch_fista -> (W [S,N,Nc] CUDA, X [S,ny,nx] CUDA, energy float64 [n_iter], Lw)."""
+    import torch
+    lib = _load()
+    s, p, b = d_data.shape
+    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size)
+    pp = Patch(int(m), int(stride), int(d_D.shape[0]), float(rho))
+    na, nb = patch_grid(ny, nx, m, stride)
+    W = torch.empty((s, na * nb, d_D.shape[0]), dtype=torch.float32, device=d_data.device)
+    X = torch.empty((s, ny, nx), dtype=torch.float32, device=d_data.device)
+    energy = np.zeros(max(int(n_iter), 1), dtype=np.float64)
+    lip = c_double(0.0)
+    _check(lib.pyhst_patch_fista(_dev(d_D, "d_D"), _dev(d_data, "d_data"), ctypes.byref(g), ctypes.byref(pp),
+                                 float(beta), int(n_iter), int(n_power), _dev(W, "W"), _dev(X, "X"),
+                                 energy.ctypes.data_as(POINTER(c_double)) if want_energy else None,
+                                 ctypes.byref(lip) if want_energy else None, _stream(stream)), "pyhst_patch_fista")
+    return W, X, energy[:int(n_iter)], float(lip.value)
 
 
 def _host_ptr(a, name):

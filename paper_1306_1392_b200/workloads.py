@@ -336,3 +336,21 @@ def random_image(n_slices, ny, nx, seed=0) -> np.ndarray:
 
 def random_sinogram(n_slices, n_angles, n_bins, seed=0) -> np.ndarray:
     return _rng(7, seed).standard_normal((n_slices, n_angles, n_bins)).astype(np.float32)
+
+
+def dct_dictionary(m: int, n_atoms: int, seed: int = 0) -> np.ndarray:
+    """Seeded over-complete dictionary [n_atoms, m*m] (float32, unit-norm rows) standing in for the
+    learned basis of ref. [4] (fig. 5: not available).  Rows = separable 2-D cosines
+    cos(pi (i + 1/2) u / q) cos(pi (j + 1/2) v / q) on an over-complete frequency grid q = ceil(sqrt(
+    n_atoms)) >= m (the first row is the constant patch); a seeded permutation picks which of the q^2
+    products are kept when n_atoms < q^2.  Holds none of the method's arithmetic."""
+    q = int(math.ceil(math.sqrt(n_atoms)))
+    q = max(q, m)
+    i = np.arange(m) + 0.5
+    basis = np.cos(math.pi * np.outer(np.arange(q), i) / q)          # [q, m]
+    atoms = np.einsum("ui,vj->uvij", basis, basis).reshape(q * q, m * m)
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 77 + seed))
+    order = np.concatenate([[0], 1 + rng.permutation(q * q - 1)])[:n_atoms]
+    D = atoms[np.sort(order)]
+    D = D / np.linalg.norm(D, axis=1, keepdims=True)
+    return np.ascontiguousarray(D, dtype=np.float32)

@@ -570,3 +570,62 @@ def test_ecohe_and_cv_distance_match_oracle(lib, oracle):
     e = lib.ecohe(x, x0)
     assert np.all(np.abs(e) <= 1.0) and np.all(np.isfinite(e))
     np.testing.assert_allclose(e, oracle.ecohe(x.cpu().numpy(), x0.cpu().numpy()), rtol=1e-10, atol=1e-13)
+
+
+# ------------------------------------------------------------------------------ N3: overlapping patches
+PATCH_REL_L2 = 2e-5      # two projector calls + two FP32 GEMMs (K <= 256) on top of each other
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("ny,nx,m,st,n_atoms,rho", [(64, 64, 8, 4, 128, 0.5), (70, 93, 8, 3, 100, 1.5),
+                                                    (40, 52, 4, 4, 16, 0.0), (33, 47, 6, 5, 40, 0.2)])
+def test_patch_gradient_matches_oracle(lib, oracle, ny, nx, m, st, n_atoms, rho):
+    """Algorithm 1 (PAPER.md L201-L228) on the device against the oracle: X (eq. 7), f (eq. 8), G (eq. 9);
+    ragged grids (last patch pulled back), non-overlapping patches, two slices."""
+    wl = lib.workloads
+    P, B = 25, int(1.5 * max(nx, ny)) | 1
+    w = wl.custom(2, P, B, nx, ny, drift=0.7, jitter_angles=0.01, seed=m + st)
+    data = wl.random_sinogram(2, P, B, seed=ny)
+    D = wl.dct_dictionary(m, n_atoms, seed=1)
+    na, nb = oracle.patch_grid(ny, nx, m, st)
+    assert lib.patch_grid(ny, nx, m, st) == (na, nb)
+    rng = np.random.default_rng(nx)
+    W = (rng.normal(size=(2, na * nb, n_atoms)) * (rng.uniform(size=(2, na * nb, n_atoms)) < 0.2)).astype(np.float32)
+    G, X, f = lib.patch_gradient(_dev(W), _dev(D), _dev(data), w.angles, w.axis, nx, ny, m, st, rho)
+    f_want = 0.0
+    for s in range(2):
+        Gw, Xw, fw = oracle.patch_gradient(W[s].astype(np.float64), D.astype(np.float64), data[s], w.angles, w.axis,
+                                           nx, ny, m, st, rho)
+        assert_parity(X[s].cpu().numpy(), Xw, "patch X slice %d" % s)
+        assert_parity(G[s].cpu().numpy(), Gw, "patch G slice %d" % s, rel=PATCH_REL_L2, mabs=2e-4)
+        f_want += fw
+    assert f == pytest.approx(f_want, rel=1e-5)
+
+
+@pytest.mark.gpu
+def test_patch_fista_matches_oracle(lib, oracle):
+    """FISTA on the coefficients (R23, R24): Lipschitz estimate, energies and iterates against the oracle
+    on a reduced-projection scan (few projections + noise), 8 x 8 patches, stride 4,
+    2x over-complete dictionary; then the long run descends and sparsifies."""
+    wl = lib.workloads
+    w = wl.config(4, shrink=16, n_slices=2)                  # 64^2, 12 projections x 64 bins
+    data = w.sinogram()
+    m, st, n_atoms, rho, beta = 8, 4, 128, 0.3, 0.05
+    D = wl.dct_dictionary(m, n_atoms)
+    Lw = oracle.patch_lipschitz(D.astype(np.float64), w.angles, w.axis, w.n_bins, w.nx, w.ny, m, st, rho, n_power=6)
+    Wg, Xg, eg, Lg = lib.patch_fista(_dev(D), _dev(data), w.angles, w.axis, w.nx, w.ny, m, st, rho, beta, 12, n_power=6)
+    assert abs(Lg - Lw) <= 2e-5 * Lw
+    e_want = np.zeros(12)
+    for s in range(2):
+        Ww, Xw, ew = oracle.patch_fista(D.astype(np.float64), data[s], w.angles, w.axis, w.nx, w.ny, m, st, rho, beta,
+                                        Lw, 12)
+        e_want += ew
+        assert_parity(Xg[s].cpu().numpy(), Xw, "patch FISTA image, slice %d" % s, rel=1e-3, mabs=5e-3)
+        assert_parity(Wg[s].cpu().numpy(), Ww, "patch FISTA coefficients, slice %d" % s, rel=2e-3, mabs=1e-2)
+    np.testing.assert_allclose(eg, e_want, rtol=1e-4)
+    Wl, Xl, el, _ = lib.patch_fista(_dev(D), _dev(data), w.angles, w.axis, w.nx, w.ny, m, st, rho, beta, 150, n_power=6)
+    assert el[-1] < 0.2 * el[0] and np.isfinite(el).all()
+    frac_zero = float((Wl == 0).float().mean())
+    assert frac_zero > 0.5                                   # the L1 term switches most coefficients off
+    with pytest.raises(lib.PyhstError):
+        lib.patch_gradient(Wl, _dev(D), _dev(data), w.angles, w.axis, w.nx, w.ny, m, 9, rho)   # stride > m
