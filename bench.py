@@ -5,9 +5,12 @@
 
 A *step* is one pass of the whole hot path over one synthetic batch:
 pyhst_fbp (a1 ramp filter -> a2 backprojection = a4) followed by pyhst_forward_project (a3) of the
-reconstructed stack.  `value` counts the pixel*projection*slice updates of BOTH projector calls per
-second of step time (GUPS); `metrics` breaks the step down per stage (CUDA events recorded by the
-library on the launching stream): backprojection GUPS, forward-projection GUPS, FBP slices/s.
+reconstructed stack.  `value` is BASELINE.json's metric, backprojection GUPS: the pixel*projection*
+slice updates of the backprojection divided by the device time of the backprojection stage inside
+the step (CUDA events recorded by the library on the launching stream); `metrics` carries the other
+half of the metric (FBP slices/s = slices / (filter + backprojection time)), the forward projector
+and the composite step; `roofline` is the backprojector's, `roofline_other` the forward projector's
+and the ramp filter's.
 
 N > 1 (torchrun, one rank per GPU): slices are independent, every rank runs the
 same per-GPU stack (weak scaling, no data-path collective); time = max over ranks.
@@ -30,7 +33,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "projector updates/s over one hot-path step (ramp filter + backprojection + forward projection)"
+METRIC = "backprojection GUPS (pixel*projection*slice updates/s of the backprojection stage; FBP slices/s in metrics)"
+METRIC_STEP = "projector updates/s over one hot-path step (ramp filter + backprojection + forward projection)"
 UNIT = "GUPS"
 FP32_LANES_PER_SM = 128          # FP32 FMA lanes per SM per clock (4 SMSP x 32)
 LANE_OPS_PER_UPDATE = 2          # lerp FMA + accumulate FMA
@@ -109,6 +113,22 @@ def _workload(P, args):
     return w
 
 
+def _executed_bp_fraction(w):
+    """Share of the nominal S*nx*ny*P backprojection updates the library executes: the stitched
+    360-degree half-acquisition path (pyhst_test.h pyhst_set_halfacq_stitch) folds
+    facing projections and backprojects P/2 rows when the scan pairs up (same test as csrc/api.cu)."""
+    import math
+    import numpy as np
+    if w.mode != 2 or w.n_angles % 2:
+        return 1.0
+    h = w.n_angles // 2
+    a, c = np.asarray(w.angles), np.asarray(w.axis)
+    c2 = 2.0 * c[:h]
+    ok = (np.abs(a[h:] - a[:h] - math.pi) <= 1e-10).all() and (c[h:] == c[:h]).all() and \
+         (np.abs(c2 - np.rint(c2)) <= 1e-9).all()
+    return 0.5 if ok else 1.0
+
+
 def _config_dict(w, world, extra=None):
     d = {"workload": "BASELINE.json configs[%d] (%s): %d slices x %dx%d, %d projections x %d bins per GPU"
                      % (w.cfg - 1, w.name, w.n_slices, w.ny, w.nx, w.n_angles, w.n_bins),
@@ -151,6 +171,7 @@ def run_b200(args):
     img = torch.empty((S, ny, nx), dtype=torch.float32, device="cuda")
     proj = torch.empty((S, NP, B), dtype=torch.float32, device="cuda")
     updates = S * nx * ny * NP                      # per projector call, per GPU
+    updates_call = updates
 
     fista = w.cfg == 4 and not args.no_fista
     if fista:
@@ -200,24 +221,40 @@ def run_b200(args):
         h_img = torch.empty((S, ny, nx), dtype=torch.float32, pin_memory=True)
         h_proj = torch.empty((S, NP, B), dtype=torch.float32, pin_memory=True)
 
-        def e2e_step():
+        def e2e_fbp():
             P.fbp_host(h_sino, w.angles, w.axis, nx, ny, w.pixel_size, filter=w.filter, mode=w.mode,
                        out=h_img, max_slices_per_chunk=8)
+
+        def e2e_fp():
             P.forward_project_host(h_img, w.angles, w.axis, B, w.pixel_size, out=h_proj,
                                    max_slices_per_chunk=8)
 
         for _ in range(min(args.warmup, 2) or 1):
-            e2e_step()
+            e2e_fbp()
+            e2e_fp()
         n_e2e = max(1, min(args.steps, 5))
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(n_e2e):
-            e2e_step()
+        t_fbp = t_fp = 0.0
+        for _ in range(n_e2e):                      # the *_host calls synchronise before returning
+            t0 = time.perf_counter()
+            e2e_fbp()
+            t1 = time.perf_counter()
+            e2e_fp()
+            t_fbp += t1 - t0
+            t_fp += time.perf_counter() - t1
         torch.cuda.synchronize()
-        ms_e2e = sharding.max_over_ranks((time.perf_counter() - t0) * 1e3, dist if world > 1 else None) / n_e2e
-        e2e = {"value": 2 * updates * world / (ms_e2e * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms_e2e,
+        mx = lambda v: sharding.max_over_ranks(v, dist if world > 1 else None)
+        ms_fbp_h, ms_fp_h = mx(t_fbp * 1e3) / n_e2e, mx(t_fp * 1e3) / n_e2e
+        ms_e2e = ms_fbp_h + ms_fp_h
+        e2e = {"value": updates * world / (ms_fbp_h * 1e-3) / 1e9, "unit": UNIT,
+               "what": "backprojection updates / wall time of pyhst_fbp_host (ramp filter + backprojection with the "
+                       "H2D copy of the raw sinograms and the D2H copy of the slices inside the timed region)",
+               "fbp_slices_per_s": S * world / (ms_fbp_h * 1e-3),
+               "forward_projection_gups": updates * world / (ms_fp_h * 1e-3) / 1e9,
+               "step_gups": 2 * updates * world / (ms_e2e * 1e-3) / 1e9,
+               "ms_fbp_host": ms_fbp_h, "ms_forward_project_host": ms_fp_h, "ms_per_step": ms_e2e,
                "steps": n_e2e,
                "h2d_bytes_per_step": int(h_sino.numel() * 4 + h_img.numel() * 4),
                "d2h_bytes_per_step": int(h_img.numel() * 4 + h_proj.numel() * 4),
@@ -236,21 +273,25 @@ def run_b200(args):
     f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     peak_tflops = n_sm * FP32_LANES_PER_SM * 2 * f_max / 1e12   # FP32 FMA issue peak at max clock
 
-    def kernel_roofline(stage, name):
+    bp_exec = _executed_bp_fraction(w)
+
+    def kernel_roofline(stage, name, executed=1.0, calls_per_step=1):
         # one "launch" of the roofline = one call of the stage (all S*nx*ny*P updates); the run8
         # backprojector covers it with two kernel launches (class A, then class B projections)
         ms, launches, _ = stages[stage]
         if launches == 0:
             return None
-        kernels_per_call = max(1, round(launches / args.steps))
-        launches = args.steps
+        kernels_per_call = max(1, round(launches / (args.steps * calls_per_step)))
+        launches = args.steps * calls_per_step
         avg_ms = ms / launches
-        ach = updates * LANE_OPS_PER_UPDATE * 2 / (avg_ms * 1e-3) / 1e12
+        upd = updates_call * executed
+        ach = upd * LANE_OPS_PER_UPDATE * 2 / (avg_ms * 1e-3) / 1e12
         r = {"kernel": name, "bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s",
              "frac": ach / peak_tflops, "traffic": None, "avg_ms": avg_ms, "launches": launches,
              "kernels_per_launch": kernels_per_call,
-             "updates_per_launch": updates, "flop_per_update": 2 * LANE_OPS_PER_UPDATE,
-             "gups": updates / (avg_ms * 1e-3) / 1e9,
+             "updates_per_launch": upd, "nominal_updates_per_launch": updates_call,
+             "flop_per_update": 2 * LANE_OPS_PER_UPDATE,
+             "gups": upd / (avg_ms * 1e-3) / 1e9,
              "peak_note": "%d SMs x 128 FP32 lanes x 2 flop x %.0f MHz (sm_max_mhz, %s peaks file); "
                           "algorithmic work = 2 FMA per (pixel, projection, slice)"
                           % (n_sm, f_max / 1e6, peaks_kind)}
@@ -259,33 +300,69 @@ def run_b200(args):
         tr = _traffic().get(stage)
         if tr is not None:
             r["traffic"] = tr
+            r["traffic_source"] = "stored: " + str(_traffic().get("_source", "profiles/traffic.json (ncu --set full capture)"))
         return r
 
-    roofs = [x for x in (kernel_roofline("backproject", "bp_run8_kernel<0> + bp_run8_kernel<1>"),
-                         kernel_roofline("forward_project", "fp_band_kernel")) if x]
-    roofs.sort(key=lambda r: -r["avg_ms"] * r["launches"])
+    calls = n_fista if fista else 1
+    r_bp = kernel_roofline("backproject", "bp_run8_kernel<0> + bp_run8_kernel<1>", executed=bp_exec, calls_per_step=calls)
+    r_fp = kernel_roofline("forward_project", "fp_band_kernel", calls_per_step=calls)
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
     ms_bp = stages["backproject"][0] / args.steps
     ms_fp = (stages["forward_project"][0] + stages["transpose"][0]) / args.steps
     ms_filter = stages["ramp_filter"][0] / args.steps
+    ms_tv = stages["tv_solver"][0] / args.steps
+    others = []
+    if ms_filter > 0 and not fista:
+        # a1 is HBM-bound: algorithmic bytes = one read of the raw row + one write of the filtered row
+        fbytes = 4.0 * S * NP * (B + (B if w.mode != 2 else P.halfacq_extent(B, float(w.axis.mean()))[0]))
+        others.append({"kernel": "ramp filter (a1)", "bound": "hbm", "achieved": fbytes / (ms_filter * 1e-3) / 1e9,
+                       "peak": hbm, "unit": "GB/s", "frac": fbytes / (ms_filter * 1e-3) / 1e9 / hbm,
+                       "traffic": None, "avg_ms": ms_filter, "bytes_per_launch": fbytes,
+                       "peak_note": "hbm_gbs of MEASURED_PEAKS.json (%s); algorithmic bytes = 4 (B_in + B_out) per row" % peaks_kind})
+    if fista and ms_tv > 0:
+        # N1: the dual steps dominate the solver's own kernels; algorithmic bytes of ONE dual step =
+        # read z, p1, p2 + write p1', p2' = 5 image stacks
+        dbytes = 5.0 * 4.0 * S * nx * ny
+        n_dual = n_fista * 20
+        others.append({"kernel": "ftv_dual_fused_kernel (+ residual / step / finish kernels of pyhst_fista_tv)",
+                       "bound": "hbm", "achieved": dbytes * n_dual / (ms_tv * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                       "frac": dbytes * n_dual / (ms_tv * 1e-3) / 1e9 / hbm, "traffic": None,
+                       "avg_ms": ms_tv / n_dual, "launches": n_dual, "bytes_per_launch": dbytes,
+                       "note": "one 'launch' = one dual step of 168 MB algorithmic traffic at config 4; the fused kernel "
+                               "runs 5 steps per kernel launch out of shared memory, so the fraction can exceed 1",
+                       "peak_note": "hbm_gbs of MEASURED_PEAKS.json (%s)" % peaks_kind})
     own = sum(v[1] for v in stages.values())
+    bp_gups = updates_call * calls * world / (ms_bp * 1e-3) / 1e9 if ms_bp else None
+    if fista:
+        roofs = sorted([x for x in (r_bp, r_fp) if x], key=lambda r: -r["avg_ms"] * r["launches"])
+        metric, value = METRIC_STEP + " -- pyhst_fista_tv solve", 2 * updates * world / (ms_step * 1e-3) / 1e9
+    else:
+        roofs = [x for x in (r_bp, r_fp) if x]       # the stated metric is the backprojector's: it leads
+        metric, value = METRIC, bp_gups
     line = {
-        "metric": METRIC, "value": 2 * updates * world / (ms_step * 1e-3) / 1e9, "unit": UNIT,
+        "metric": metric, "value": value, "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "impl": "b200",
         "config": _config_dict(w, world, {"step": "pyhst_fista_tv: 100 FISTA iterations (lambda 0.01, 20 dual "
                                           "steps each), one forward/back projector pair per iteration; "
                                           "updates counted for the 200 projector calls only"} if fista else None),
-        "metrics": {"backprojection_gups": updates * world / (ms_bp * 1e-3) / 1e9 if ms_bp else None,
+        "metrics": {"backprojection_gups": bp_gups,
+                    "backprojection_gups_executed": bp_gups * bp_exec if bp_gups else None,
+                    "backprojection_executed_fraction": bp_exec,
                     "forward_projection_gups": updates * world / (ms_fp * 1e-3) / 1e9 if ms_fp else None,
-                    "fbp_slices_per_s": S * world / ((ms_filter + ms_bp) * 1e-3) if ms_bp else None,
+                    "fbp_slices_per_s": S * world / ((ms_filter + ms_bp) * 1e-3) if (ms_bp and not fista) else None,
+                    "step_gups": 2 * updates * world / (ms_step * 1e-3) / 1e9,
                     "ms_ramp_filter": ms_filter, "ms_backproject": ms_bp, "ms_forward_project": ms_fp,
-                    "note": "per-stage device ms of rank 0 (CUDA events recorded by the library on the "
-                            "launching stream, inside the timed region)"},
+                    "ms_tv_solver_kernels": ms_tv,
+                    "note": "per-stage device ms of rank 0 (CUDA events recorded by the library on the launching "
+                            "stream, inside the timed region); backprojection_gups counts the nominal S*nx*ny*P "
+                            "updates, _executed what the kernel really does (the stitched half-acquisition path "
+                            "backprojects P/2 folded rows)"},
         "clocks": clocks, "e2e": e2e,
         "gpu_launches": own, "gpu_launches_per_step": own / args.steps,
         "library_launches": {"cufft_execs": sum(v[2] for v in stages.values())},
-        "roofline": roofs[0] if roofs else None, "roofline_other": roofs[1:],
+        "roofline": roofs[0] if roofs else None, "roofline_other": roofs[1:] + others,
     }
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(P.workloads, args)

@@ -255,7 +255,8 @@ enum {
   PYHST_STAGE_BACKPROJECT = 2, /* a2: the backprojection kernel                                  */
   PYHST_STAGE_TRANSPOSE = 3,   /* a3: image transpose for the column walk                        */
   PYHST_STAGE_FORWARD = 4,     /* a3: the forward-projection kernel                              */
-  PYHST_N_STAGES = 5
+  PYHST_STAGE_TV = 5,          /* N1: the solver's own kernels (residual, gradient step, dual steps, momentum) */
+  PYHST_N_STAGES = 6
 };
 /* pyhst_profile_enable(1): from now on every stage is bracketed by a pair of CUDA events recorded
  * on the stream the stage is launched on (no synchronisation is added).  Returns the previous

@@ -35,6 +35,11 @@ int pyhst_set_halfacq_stitch(int enable);
  * are slower than 2 on B200 and kept for comparison.  Returns the previous value. */
 int pyhst_set_forward_project_variant(int variant);
 
+/* Selects the ramp-filter implementation: 0 = automatic (default: the fused shared-memory FFT kernel for
+ * rows of up to 4096 filtered bins, cuFFT beyond), 1 = the cuFFT path (pad/weight, R2C, x H, C2R, crop:
+ * five passes), 2 = the fused kernel (UNSUPPORTED for longer rows).  Returns the previous value. */
+int pyhst_set_filter_variant(int variant);
+
 #ifdef __cplusplus
 }
 #endif

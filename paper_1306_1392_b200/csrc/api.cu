@@ -76,6 +76,7 @@ std::map<int, std::unique_ptr<DeviceCtx>> g_ctx;
 int g_bp_variant = 0;
 int g_fp_variant = 0;
 int g_halfacq_stitch = 1;
+int g_filter_variant = 0;
 
 DeviceCtx* ctx_of(int dev) {
   std::lock_guard<std::mutex> lock(g_map_mu);
@@ -89,6 +90,8 @@ DeviceCtx* ctx_of(int dev) {
 // state of the current device; only called inside an open CallScope (or under its own lock)
 DeviceCtx& ctx() { return *ctx_of(std::max(0, current_device())); }
 }  // namespace
+
+int filter_variant() { return g_filter_variant; }
 
 int current_device() {
   int dev = -1;
@@ -451,6 +454,12 @@ int pyhst_set_halfacq_stitch(int enable) {
   return prev;
 }
 
+int pyhst_set_filter_variant(int variant) {
+  const int prev = g_filter_variant;
+  if (variant >= 0 && variant <= 2) g_filter_variant = variant;
+  return prev;
+}
+
 int pyhst_set_forward_project_variant(int variant) {
   const int prev = g_fp_variant;
   if (variant >= 0 && variant <= 4) g_fp_variant = variant;
@@ -657,10 +666,9 @@ static int fbp_device(const float* d_sino_raw, int64_t pitch, float* d_img, cons
       int* d_two_c = reinterpret_cast<int*>(static_cast<char*>(r2) + r2_bytes);
       PYHST_CUDA_TRY(cudaMemcpyAsync(d_two_c, two_c.data(), (size_t)P2 * sizeof(int), cudaMemcpyHostToDevice,
                                      stream));
-      for (int32_t s = 0; s < ns; ++s)
-        PYHST_TRY(launch_ramp_filter(d_sino_raw + (int64_t)s * P * pitch, pitch, P, g->n_bins, b_out,
-                                     pad_left, (int)f, d_w, static_cast<float*>(r1) + (int64_t)s * P * b_out,
-                                     b_out, nullptr, nullptr, 0, nullptr, stream));
+      // rows of the whole stack are equally pitched: one call filters all ns * P of them
+      PYHST_TRY(launch_ramp_filter(d_sino_raw, pitch, (int64_t)ns * P, g->n_bins, b_out, pad_left, (int)f, d_w,
+                                   static_cast<float*>(r1), b_out, nullptr, nullptr, 0, nullptr, stream));
       PYHST_TRY(launch_halfacq_fold(static_cast<const float*>(r1), static_cast<float*>(r2), ns, P2, b_out,
                                     b_st, off, d_two_c, stream));
       std::vector<double> axis2((size_t)P2);
@@ -685,21 +693,26 @@ static int fbp_device(const float* d_sino_raw, int64_t pitch, float* d_img, cons
   if (kern == 1) {
     void* rows = nullptr;
     PYHST_TRY(get_workspace(WS_ROWS, (size_t)ns * P * b_out * 4, &rows));
-    for (int32_t s = 0; s < ns; ++s)
-      PYHST_TRY(launch_ramp_filter(d_sino_raw + (int64_t)s * P * pitch, pitch, P, g->n_bins, b_out,
-                                   pad_left, (int)f, d_w, static_cast<float*>(rows) + (int64_t)s * P * b_out,
-                                   b_out, nullptr, nullptr, 0, nullptr, stream));
+    PYHST_TRY(launch_ramp_filter(d_sino_raw, pitch, (int64_t)ns * P, g->n_bins, b_out, pad_left, (int)f, d_w,
+                                 static_cast<float*>(rows), b_out, nullptr, nullptr, 0, nullptr, stream));
     return launch_backproject_reference(static_cast<const float*>(rows), b_out, a, stream);
   }
   const QiLayout L = qi_layout(ns, g->n_angles, b_out, g->pixel_size);
   void* qi = nullptr;
   PYHST_TRY(get_workspace(WS_QI, L.bytes(), &qi));
-  for (int32_t grp = 0; grp < L.n_groups; ++grp) {
-    const int32_t n_in = std::min(4, ns - grp * 4);
-    PYHST_TRY(launch_ramp_filter(d_sino_raw + (int64_t)grp * 4 * P * pitch, pitch, (int64_t)n_in * P,
-                                 g->n_bins, b_out, pad_left, (int)f, d_w, nullptr, 0,
-                                 static_cast<float4*>(qi) + (int64_t)grp * L.group_f4(), &L, n_in,
-                                 kern >= 3 ? plan->d_flip : nullptr, stream));
+  if (filter_variant() != 1 && ramp_fused_log2m(b_out)) {
+    // fused filter: every slice group in one launch, written straight into the interleaved layout
+    PYHST_TRY(launch_ramp_filter_fused(d_sino_raw, pitch, (int64_t)ns * P, g->n_bins, b_out, pad_left, (int)f, d_w,
+                                       nullptr, 0, static_cast<float4*>(qi), &L, ns,
+                                       kern >= 3 ? plan->d_flip : nullptr, stream));
+  } else {
+    for (int32_t grp = 0; grp < L.n_groups; ++grp) {
+      const int32_t n_in = std::min(4, ns - grp * 4);
+      PYHST_TRY(launch_ramp_filter(d_sino_raw + (int64_t)grp * 4 * P * pitch, pitch, (int64_t)n_in * P,
+                                   g->n_bins, b_out, pad_left, (int)f, d_w, nullptr, 0,
+                                   static_cast<float4*>(qi) + (int64_t)grp * L.group_f4(), &L, n_in,
+                                   kern >= 3 ? plan->d_flip : nullptr, stream));
+    }
   }
   if (kern == 4)
     return launch_backproject_run8(static_cast<const float4*>(qi), L, a, plan->d_run, plan->n_a, plan->n_b,

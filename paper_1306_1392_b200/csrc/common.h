@@ -39,7 +39,7 @@ int set_error(int status, const char* fmt, ...);
 // with CUDA events on the launching stream.
 enum Stage { ST_FILTER = PYHST_STAGE_FILTER, ST_REPACK = PYHST_STAGE_REPACK,
              ST_BACKPROJECT = PYHST_STAGE_BACKPROJECT, ST_TRANSPOSE = PYHST_STAGE_TRANSPOSE,
-             ST_FORWARD = PYHST_STAGE_FORWARD, ST_COUNT = PYHST_N_STAGES };
+             ST_FORWARD = PYHST_STAGE_FORWARD, ST_TV = PYHST_STAGE_TV, ST_COUNT = PYHST_N_STAGES };
 struct StageScope {
   StageScope(Stage st, cudaStream_t stream);
   ~StageScope();
@@ -232,6 +232,14 @@ int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int3
                        const float* d_col_weights, float* d_out, int64_t out_pitch,
                        float4* d_qi, const QiLayout* L, int32_t n_slices_in, const uint8_t* d_flip,
                        cudaStream_t stream);
+// fused shared-memory FFT filter (filter_fused.cu): same contract as launch_ramp_filter
+int ramp_fused_log2m(int32_t n_bins_out);   // 0 if the rows are too long for it
+int launch_ramp_filter_fused(const float* d_in, int64_t in_pitch, int64_t n_rows, int32_t n_bins_in,
+                             int32_t n_bins_out, int32_t pad_left, int filter, const float* d_col_weights,
+                             float* d_out, int64_t out_pitch, float4* d_qi, const QiLayout* L, int32_t n_slices_in,
+                             const uint8_t* d_flip, cudaStream_t stream);
+void release_fused_filter_tables();
+int filter_variant();   // 0 automatic, 1 cuFFT path, 2 fused kernel (pyhst_test.h)
 int launch_halfacq_weights(float* d_w, int32_t n_bins, double cbar, cudaStream_t stream);
 int launch_halfacq_fold(const float* d_rows, float* d_out, int32_t n_slices, int32_t half_angles,
                         int32_t b_out, int32_t b_st, int32_t off, const int* d_two_c, cudaStream_t stream);

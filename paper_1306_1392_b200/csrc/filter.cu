@@ -206,6 +206,16 @@ int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int3
                        float4* d_qi, const QiLayout* L, int32_t n_slices_in, const uint8_t* d_flip,
                        cudaStream_t stream) {
   if (n_rows == 0) return PYHST_OK;
+  {
+    // product path: the fused shared-memory FFT kernel (one read, one write); cuFFT for longer rows
+    const int variant = filter_variant();
+    const bool fused_ok = ramp_fused_log2m(n_bins_out) != 0;
+    if (variant == 2 && !fused_ok)
+      return set_error(PYHST_ERR_UNSUPPORTED, "fused ramp filter does not cover rows of %d bins", n_bins_out);
+    if (variant != 1 && fused_ok)
+      return launch_ramp_filter_fused(d_in, in_pitch, n_rows, n_bins_in, n_bins_out, pad_left, filter, d_col_weights,
+                                      d_out, out_pitch, d_qi, L, n_slices_in, d_flip, stream);
+  }
   std::lock_guard<std::mutex> lock(g_mu);
   const int M = fft_length(2 * (int64_t)n_bins_out);
   const int Mp = M + 2, nk = M / 2 + 1;
@@ -267,6 +277,7 @@ int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int3
 }
 
 void release_filter_plans() {
+  release_fused_filter_tables();
   std::lock_guard<std::mutex> lock(g_mu);
   for (auto& kv : g_plans) {
     cufftDestroy(kv.second.r2c);

@@ -7,7 +7,7 @@
 // library) and a handful of element-wise / 5-point-stencil kernels over the image stack:
 //   r = P y - data, 1/2 ||r||^2            ftv_residual_kernel
 //   z = y - P^T r / L, TV(y)               ftv_step_kernel
-//   n_inner dual projected-gradient steps  ftv_dual_kernel   (p ping-pongs between two buffers)
+//   n_inner dual projected-gradient steps  ftv_dual_fused_kernel (5 steps per launch on a shared-memory tile)
 //   x+ = z - tau G^T p, momentum           ftv_finish_kernel
 // All scalars (L, the energies) stay on the device: the loop enqueues without a host sync.
 #include <algorithm>
@@ -63,7 +63,7 @@ __device__ __forceinline__ float d2f(const float* x, int nx, int ny, int i, int 
   return i + 1 < ny ? x[(int64_t)(i + 1) * nx + j] - x[(int64_t)i * nx + j] : 0.f;
 }
 // (G^T p)[i,j] = p1[i,j-1] - p1[i,j] + p2[i-1,j] - p2[i,j]; p1 of the last column and p2 of the
-// last row are identically zero (they are never made non-zero by ftv_dual_kernel)
+// last row are identically zero (they are never made non-zero by the dual steps)
 __device__ __forceinline__ float gtf(const float* p1, const float* p2, int nx, int ny, int i, int j) {
   float v = 0.f;
   if (j > 0) v += p1[(int64_t)i * nx + j - 1];
@@ -106,57 +106,87 @@ __global__ void ftv_step_kernel(const float* __restrict__ y, const float* __rest
   if (tv_acc) block_sum_to(tv, tv_acc);
 }
 
-// one dual projected-gradient step (R18):  u = z - tau G^T p ;  q = p + G u / (8 tau) ;
-// p' = q / max(1, |q|)  -- p is read from (p1, p2) and written to (q1, q2) (Jacobi: ping-pong).
-// u of the block's tile plus one row / column of halo goes through shared memory (32-bit offsets
-// inside a slice; the halo row is filled by the first warp, the halo column by the first lane of
-// every row).  INTERIOR: the tile and its halo touch no image border -- no boundary tests.
-template <bool INTERIOR>
-__device__ __forceinline__ void ftv_dual_tile(const float* __restrict__ z, const float* __restrict__ p1,
-                                              const float* __restrict__ p2, float* __restrict__ q1,
-                                              float* __restrict__ q2, int nx, int ny, float tau,
-                                              float step, float (&su)[FT_BY + 1][FT_BX + 1]) {
-  const int tx = threadIdx.x, ty = threadIdx.y;
-  const int j = blockIdx.x * FT_BX + tx, i = blockIdx.y * FT_BY + ty;
-  auto uval = [&](int ii, int jj) -> float {
-    const int kk = ii * nx + jj;
-    if (INTERIOR) return fmaf(-tau, (p1[kk - 1] - p1[kk]) + (p2[kk - nx] - p2[kk]), z[kk]);
-    if (ii >= ny || jj >= nx) return 0.f;
-    float v = 0.f;                                       // (G^T p)[ii, jj], see gtf()
-    if (jj > 0) v += p1[kk - 1];
-    if (jj + 1 < nx) v -= p1[kk];
-    if (ii > 0) v += p2[kk - nx];
-    if (ii + 1 < ny) v -= p2[kk];
-    return fmaf(-tau, v, z[kk]);
-  };
-  su[ty][tx] = uval(i, j);
-  if (ty == 0) su[FT_BY][tx] = uval(blockIdx.y * FT_BY + FT_BY, j);
-  if (tx == 0) su[ty][FT_BX] = uval(i, blockIdx.x * FT_BX + FT_BX);
-  __syncthreads();
-  if (!INTERIOR && (i >= ny || j >= nx)) return;
-  const int k = i * nx + j;
-  const float u = su[ty][tx];
-  const float a = (INTERIOR || j + 1 < nx) ? su[ty][tx + 1] - u : 0.f;
-  const float b = (INTERIOR || i + 1 < ny) ? su[ty + 1][tx] - u : 0.f;
-  const float n1 = fmaf(a, step, p1[k]), n2 = fmaf(b, step, p2[k]);
-  const float m = fmaxf(1.f, sqrtf(n1 * n1 + n2 * n2));
-  q1[k] = n1 / m;
-  q2[k] = n2 / m;
-}
+// Dual projected-gradient steps (R18):  u = z - tau G^T p ;  q = p + G u / (8 tau) ;  p' = q / max(1, |q|)
+// -- p is read from (p1, p2) and written to (q1, q2) (Jacobi: ping-pong between two buffer pairs).
+// K dual steps per launch (temporal blocking): the block stages z, p1, p2 of its 64 x 32 tile plus a
+// halo of K cells into shared memory, iterates the Jacobi step K times there (u, then p in place) and
+// writes the tile's p after K steps.  A cell's value after one step depends on its neighbours at
+// distance 1, so what enters from the edge of the staged region spoils one more ring per step and
+// never reaches the tile; every cell of the tile goes through exactly the arithmetic of K single steps.  HBM traffic per step falls from 5 arrays to
+// (3 x 1.3 + 2) / K arrays.  Cells outside the image hold p = z = u = 0 and are never updated
+// (p1 of the last column and p2 of the last row stay zero by construction: their differences are 0).
+constexpr int FD_TX = 64, FD_TY = 32, FD_KMAX = 5, FD_NT = 256;
+constexpr int FD_RW = FD_TX + 2 * FD_KMAX, FD_RH = FD_TY + 2 * FD_KMAX;
 
-__global__ void ftv_dual_kernel(const float* __restrict__ z, const float* __restrict__ p1,
-                                const float* __restrict__ p2, float* __restrict__ q1,
-                                float* __restrict__ q2, int nx, int ny, const float* __restrict__ fs) {
-  __shared__ float su[FT_BY + 1][FT_BX + 1];
+__global__ void __launch_bounds__(FD_NT)
+ftv_dual_fused_kernel(const float* __restrict__ z, const float* __restrict__ p1, const float* __restrict__ p2,
+                      float* __restrict__ q1, float* __restrict__ q2, int nx, int ny,
+                      const float* __restrict__ fs, int K, int p_is_zero) {
+  extern __shared__ float sm[];
+  const int rw = FD_TX + 2 * K, rh = FD_TY + 2 * K, n = rw * rh;
+  float* sz = sm;
+  float* s1 = sm + FD_RW * FD_RH;
+  float* s2 = s1 + FD_RW * FD_RH;
+  float* su = s2 + FD_RW * FD_RH;
   const int64_t o = (int64_t)blockIdx.z * ny * nx;
+  const int gx0 = blockIdx.x * FD_TX - K, gy0 = blockIdx.y * FD_TY - K;
   const float tau = fs[1], step = fs[2];
-  const int j0 = blockIdx.x * FT_BX, i0 = blockIdx.y * FT_BY;
-  // note: the non-symmetric sum order of the border path, (+p1[k-1] - p1[k]) + (p2[k-nx] - p2[k]),
-  // is kept by the interior path only up to FP32 rounding of the four-term sum
-  if (j0 > 0 && i0 > 0 && j0 + FT_BX + 1 < nx && i0 + FT_BY + 1 < ny)
-    ftv_dual_tile<true>(z + o, p1 + o, p2 + o, q1 + o, q2 + o, nx, ny, tau, step, su);
-  else
-    ftv_dual_tile<false>(z + o, p1 + o, p2 + o, q1 + o, q2 + o, nx, ny, tau, step, su);
+  for (int e = threadIdx.x; e < n; e += FD_NT) {
+    const int ly = e / rw, lx = e - ly * rw;
+    const int gy = gy0 + ly, gx = gx0 + lx;
+    const bool in = gy >= 0 && gy < ny && gx >= 0 && gx < nx;
+    const int64_t k = o + (int64_t)gy * nx + gx;
+    sz[e] = in ? z[k] : 0.f;
+    s1[e] = (in && !p_is_zero) ? p1[k] : 0.f;
+    s2[e] = (in && !p_is_zero) ? p2[k] : 0.f;
+  }
+  __syncthreads();
+  // the cells of a thread are e = tid, tid + 256, ...: (ly, lx) advance by (256 / rw, 256 % rw) with a
+  // carry -- no division in the loops
+  const int dy = FD_NT / rw, dx = FD_NT - dy * rw;
+  const int ly0 = (int)threadIdx.x / rw, lx0 = (int)threadIdx.x - ly0 * rw;
+  for (int it = 0; it < K; ++it) {
+    {
+      int ly = ly0, lx = lx0;
+      for (int e = threadIdx.x; e < n; e += FD_NT) {
+        const float l1 = lx > 0 ? s1[e - 1] : 0.f, t2 = ly > 0 ? s2[e - rw] : 0.f;
+        su[e] = fmaf(-tau, (l1 - s1[e]) + (t2 - s2[e]), sz[e]);
+        lx += dx;
+        ly += dy;
+        if (lx >= rw) { lx -= rw; ++ly; }
+      }
+    }
+    __syncthreads();
+    {
+      int ly = ly0, lx = lx0;
+      for (int e = threadIdx.x; e < n; e += FD_NT) {
+        const int gy = gy0 + ly, gx = gx0 + lx;
+        if (gy >= 0 && gy < ny && gx >= 0 && gx < nx) {
+          const float u = su[e];
+          const float a = (gx + 1 < nx && lx + 1 < rw) ? su[e + 1] - u : 0.f;
+          const float b = (gy + 1 < ny && ly + 1 < rh) ? su[e + rw] - u : 0.f;
+          const float n1 = fmaf(a, step, s1[e]), n2 = fmaf(b, step, s2[e]);
+          // p = q / max(1, |q|) = q * min(1, 1/|q|)
+          const float inv = fminf(1.f, rsqrtf(fmaf(n1, n1, n2 * n2)));
+          s1[e] = n1 * inv;
+          s2[e] = n2 * inv;
+        }
+        lx += dx;
+        ly += dy;
+        if (lx >= rw) { lx -= rw; ++ly; }
+      }
+    }
+    __syncthreads();
+  }
+  for (int e = threadIdx.x; e < FD_TX * FD_TY; e += FD_NT) {
+    const int ty = e / FD_TX, tx = e - ty * FD_TX;
+    const int gy = blockIdx.y * FD_TY + ty, gx = blockIdx.x * FD_TX + tx;
+    if (gy >= ny || gx >= nx) continue;
+    const int l = (ty + K) * rw + tx + K;
+    const int64_t k = o + (int64_t)gy * nx + gx;
+    q1[k] = s1[l];
+    q2[k] = s2[l];
+  }
 }
 
 // x+ = z - tau G^T p (tau = 0: x+ = z);  y = x+ + mom (x+ - x);  x = x+
@@ -276,6 +306,13 @@ static int tv_solver(const float* d_data, float* d_img, const pyhst_geom_t* g, f
   ftv_scalars_kernel<<<1, 1, 0, stream>>>(d_L, (double)beta, d_fs);
   PYHST_CUDA_TRY(cudaGetLastError());
 
+  const size_t fd_smem = (size_t)4 * FD_RW * FD_RH * sizeof(float);
+  {
+    static uint64_t configured = 0;
+    if (first_use_on_device(&configured))
+      PYHST_CUDA_TRY(cudaFuncSetAttribute(ftv_dual_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)fd_smem));
+  }
   // ---- FISTA (R19, R20): x0 = y0 = 0, t0 = 1
   PYHST_CUDA_TRY(cudaMemsetAsync(d_img, 0, (size_t)n_img * 4, stream));
   PYHST_CUDA_TRY(cudaMemsetAsync(y, 0, (size_t)n_img * 4, stream));
@@ -284,20 +321,27 @@ static int tv_solver(const float* d_data, float* d_img, const pyhst_geom_t* g, f
   for (int k = 0; k < n_iter; ++k) {
     PYHST_TRY(pyhst_forward_project(y, r, &gs, 1.f, stream));
     {
+      StageScope scope(ST_TV, stream);
+      scope.kernels(2);
       dim3 grid((g->n_bins + FT_BX - 1) / FT_BX, (unsigned)res_gy, 1);
       ftv_residual_kernel<<<grid, blk, 0, stream>>>(r, d_data, data_pitch, g->n_bins, n_rows, d_part);
       ftv_reduce_kernel<<<1, 1024, 0, stream>>>(d_part, (int)n_part_res, d_e + k);
     }
     PYHST_TRY(pyhst_backproject(r, gr, &gs, 1.f, stream));
+    StageScope scope(ST_TV, stream);
+    scope.kernels(3 + (use_p ? (n_inner + FD_KMAX - 1) / FD_KMAX : 0));
     ftv_step_kernel<<<grid_img, blk, 0, stream>>>(y, gr, z, nx, ny, d_fs, (double)beta, d_part);
     ftv_reduce_kernel<<<1, 1024, 0, stream>>>(d_part, (int)n_part_img, d_e + k);
     int cur = 0;
     if (use_p) {
-      PYHST_CUDA_TRY(cudaMemsetAsync(p[0], 0, 2 * img_bytes, stream));  // p[0], p[1] are adjacent
-      for (int it = 0; it < n_inner; ++it) {
-        ftv_dual_kernel<<<grid_img, blk, 0, stream>>>(z, p[cur], p[cur + 1], p[2 - cur], p[3 - cur], nx,
-                                                      ny, d_fs);
+      // n_inner dual steps, FD_KMAX per launch; the first launch starts from p = 0 without reading it
+      const dim3 grid_d((nx + FD_TX - 1) / FD_TX, (ny + FD_TY - 1) / FD_TY, S);
+      for (int done = 0; done < n_inner;) {
+        const int kk = std::min(FD_KMAX, n_inner - done);
+        ftv_dual_fused_kernel<<<grid_d, FD_NT, fd_smem, stream>>>(z, p[cur], p[cur + 1], p[2 - cur], p[3 - cur], nx,
+                                                                 ny, d_fs, kk, done == 0 ? 1 : 0);
         cur = 2 - cur;
+        done += kk;
       }
     }
     const double tn = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));

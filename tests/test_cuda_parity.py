@@ -629,3 +629,52 @@ def test_patch_fista_matches_oracle(lib, oracle):
     assert frac_zero > 0.5                                   # the L1 term switches most coefficients off
     with pytest.raises(lib.PyhstError):
         lib.patch_gradient(Wl, _dev(D), _dev(data), w.angles, w.axis, w.nx, w.ny, m, 9, rho)   # stride > m
+
+
+# ------------------------------------------------------------------------------ N2: fused FFT filter
+@pytest.mark.gpu
+@pytest.mark.parametrize("f", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("b_in,b_out,pad,weights,rows", [(367, 367, 0, False, 7), (128, 256, 0, True, 4),
+                                                         (100, 192, 92, True, 9), (20, 20, 0, False, 1),
+                                                         (2048, 2048, 0, False, 6), (2048, 3840, 0, True, 5),
+                                                         (2560, 2560, 0, False, 3), (4096, 4096, 0, False, 2)])
+def test_fused_ramp_filter_matches_oracle_and_cufft_path(lib, oracle, f, b_in, b_out, pad, weights, rows):
+    """N2: the fused shared-memory FFT kernel (FFT lengths 64 .. 8192, every radix schedule 8..8 [4|2]) against
+    the oracle's direct convolution and against the cuFFT path."""
+    rng = np.random.default_rng(b_in + 7 * f)
+    x = rng.normal(size=(rows, b_in)).astype(np.float32)
+    w = rng.uniform(0, 1, b_in).astype(np.float32) if weights else None
+    want = oracle.ramp_filter(x, n_bins_out=b_out, pad_left=pad, filter=f, col_weights=w)
+    dw = None if w is None else _dev(w)
+    prev = lib.set_filter_variant(2)
+    try:
+        got = lib.ramp_filter(_dev(x), n_bins_out=b_out, pad_left=pad, filter=f, col_weights=dw).cpu().numpy()
+        lib.set_filter_variant(1)
+        ref = lib.ramp_filter(_dev(x), n_bins_out=b_out, pad_left=pad, filter=f, col_weights=dw).cpu().numpy()
+    finally:
+        lib.set_filter_variant(prev)
+    assert_parity(got, want, "fused ramp filter")
+    assert_parity(ref, want, "cuFFT ramp filter")
+
+
+@pytest.mark.gpu
+def test_fbp_through_both_filter_paths(lib, oracle):
+    """pyhst_fbp writes the interleaved layout straight from the filter: both filter paths, ragged slice
+    group, reversed rows (360-degree angles), half acquisition (weights + extension)."""
+    for cfg, shrink, n_slices in ((2, 8, 6), (3, 8, 3), (5, 8, 5)):
+        w = lib.workloads.config(cfg, shrink=shrink, n_slices=n_slices)
+        sino = w.sinogram()
+        want = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode)
+        for variant in (1, 2):
+            prev = lib.set_filter_variant(variant)
+            try:
+                got = lib.fbp(_dev(sino), w.angles, w.axis, w.nx, w.ny, filter=w.filter, mode=w.mode).cpu().numpy()
+            finally:
+                lib.set_filter_variant(prev)
+            assert_parity(got, want, "fbp cfg%d, filter variant %d" % (cfg, variant))
+    with pytest.raises(lib.PyhstError):
+        prev = lib.set_filter_variant(2)
+        try:
+            lib.ramp_filter(_dev(np.zeros((2, 5000), dtype=np.float32)))        # M would be 16384
+        finally:
+            lib.set_filter_variant(prev)
