@@ -15,7 +15,8 @@ extern "C" {
 /* Selects the backprojection kernel: 0 = automatic (default), 1 = reference one-thread-per-
  * pixel kernel (global loads; kept for cross-checks), 2 = tiled shared-memory kernel, 3 = run
  * kernel with 4 slices per thread, 4 = run kernel with 8 slices per thread (what 0 picks for
- * pixel sizes below sqrt(2) bins).  A variant that does not cover the geometry makes the next
+ * pixel sizes below sqrt(2) bins), 6 = the same with the interpolation written as packed FFMA2 (8 fewer
+ * warp instructions per step, same time: an FFMA2 costs two issue slots on sm_100a, profiles/r02_micro.md).  A variant that does not cover the geometry makes the next
  * call return PYHST_ERR_UNSUPPORTED.  Returns the previous value.  Test/bench hook; results
  * agree within FP32 rounding. */
 int pyhst_set_backproject_variant(int variant);
@@ -39,6 +40,12 @@ int pyhst_set_forward_project_variant(int variant);
  * rows of up to 4096 filtered bins, cuFFT beyond), 1 = the cuFFT path (pad/weight, R2C, x H, C2R, crop:
  * five passes), 2 = the fused kernel (UNSUPPORTED for longer rows).  Returns the previous value. */
 int pyhst_set_filter_variant(int variant);
+
+/* Selects the kernel of the two GEMMs of pyhst_patch_gradient / pyhst_patch_fista: 0 = automatic (default: the
+ * tcgen05 3xTF32 tensor-core kernel when the shapes allow it -- n_atoms and m*m multiples of 32 resp. 16, at
+ * most 256, operands 16-byte aligned -- else the FP32 SIMT kernel), 1 = FP32 SIMT kernel, 2 = tensor-core
+ * kernel (UNSUPPORTED for other shapes).  Returns the previous value. */
+int pyhst_set_patch_gemm_variant(int variant);
 
 #ifdef __cplusplus
 }

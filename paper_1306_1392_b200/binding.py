@@ -27,7 +27,7 @@ _LIBNAME = "libpyhst_b200.so"
 # every symbol include/*.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
            "pyhst_fista_tv", "pyhst_ista_tv", "pyhst_ring_filter", "pyhst_ecohe", "pyhst_cv_distance", "pyhst_patch_grid",
-           "pyhst_patch_gradient", "pyhst_patch_fista", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_set_halfacq_stitch", "pyhst_set_filter_variant",
+           "pyhst_patch_gradient", "pyhst_patch_fista", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_set_halfacq_stitch", "pyhst_set_filter_variant", "pyhst_set_patch_gemm_variant",
            "pyhst_last_error", "pyhst_release_cache")
 
 
@@ -83,6 +83,7 @@ def _load():
     lib.pyhst_set_forward_project_variant.argtypes = [c_int]
     lib.pyhst_set_halfacq_stitch.argtypes = [c_int]
     lib.pyhst_set_filter_variant.argtypes = [c_int]
+    lib.pyhst_set_patch_gemm_variant.argtypes = [c_int]
     lib.pyhst_profile_enable.argtypes = [c_int]
     lib.pyhst_profile_read.argtypes = [POINTER(c_double), POINTER(c_int64), POINTER(c_int64), c_int32]
     lib.pyhst_last_error.restype = c_char_p
@@ -368,6 +369,11 @@ def set_halfacq_stitch(enable: bool) -> int:
 def set_filter_variant(variant: int) -> int:
     """0 automatic, 1 cuFFT path, 2 fused shared-memory FFT kernel; returns the previous value."""
     return int(_load().pyhst_set_filter_variant(int(variant)))
+
+
+def set_patch_gemm_variant(variant: int) -> int:
+    """0 automatic, 1 FP32 SIMT GEMM, 2 tcgen05 3xTF32 GEMM; returns the previous value."""
+    return int(_load().pyhst_set_patch_gemm_variant(int(variant)))
 
 
 def set_forward_project_variant(variant: int) -> int:

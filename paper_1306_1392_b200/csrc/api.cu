@@ -77,6 +77,7 @@ int g_bp_variant = 0;
 int g_fp_variant = 0;
 int g_halfacq_stitch = 1;
 int g_filter_variant = 0;
+int g_patch_gemm_variant = 0;
 
 DeviceCtx* ctx_of(int dev) {
   std::lock_guard<std::mutex> lock(g_map_mu);
@@ -92,6 +93,8 @@ DeviceCtx& ctx() { return *ctx_of(std::max(0, current_device())); }
 }  // namespace
 
 int filter_variant() { return g_filter_variant; }
+int patch_gemm_variant() { return g_patch_gemm_variant; }
+bool run8_packed() { return g_bp_variant == 6; }
 
 int current_device() {
   int dev = -1;
@@ -402,6 +405,7 @@ static int pick_bp_kernel(double pixel_size, int32_t n_slices) {
     case 2: return tiled_ok ? 2 : -1;
     case 3: return run_ok ? 3 : -1;
     case 4: return run8_ok ? 4 : -1;
+    case 6: return run8_ok ? 4 : -1;   // run8 with packed FFMA2 interpolation (measured alternative)
     // one slice group (<= 4 slices): the 8-slice kernel would spend half of its FMAs on a duplicate
     default: return (run8_ok && n_slices > 4) ? 4 : (run_ok ? 3 : (tiled_ok ? 2 : 1));
   }
@@ -444,13 +448,19 @@ int pyhst_profile_read(double* ms, int64_t* kernels, int64_t* fft_execs, int32_t
 
 int pyhst_set_backproject_variant(int variant) {
   const int prev = g_bp_variant;
-  if (variant >= 0 && variant <= 4) g_bp_variant = variant;
+  if (variant >= 0 && variant <= 6 && variant != 5) g_bp_variant = variant;
   return prev;
 }
 
 int pyhst_set_halfacq_stitch(int enable) {
   const int prev = g_halfacq_stitch;
   if (enable == 0 || enable == 1) g_halfacq_stitch = enable;
+  return prev;
+}
+
+int pyhst_set_patch_gemm_variant(int variant) {
+  const int prev = g_patch_gemm_variant;
+  if (variant >= 0 && variant <= 2) g_patch_gemm_variant = variant;
   return prev;
 }
 

@@ -92,6 +92,72 @@ __device__ __forceinline__ void r8_run(float (&acc)[R8_RN][8], uint32_t addr, fl
   }
 }
 
+
+// (c0, c1) += (a0, a1) * (s, s): one packed FFMA2.  An FFMA2 takes ONE issue slot and holds the FMA pipe for
+// two cycles (r02 microbenchmarks, profiles/r02_micro.md: 4 FFMA2 + 4 IADD3 issue in 8 cycles), so the
+// ALU-pipe overhead of the run loop (FSEL moves, IADD3, FSETP) and its LDS issue in the FFMA2's shadow.
+__device__ __forceinline__ uint64_t r8_pair(float s) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %1};" : "=l"(r) : "f"(s));
+  return r;
+}
+__device__ __forceinline__ void r8_ffma2(float& c0, float& c1, float a0, float a1, uint64_t s2) {
+  asm("{\n\t.reg .b64 ra, rc;\n\t"
+      "mov.b64 ra, {%2, %3};\n\t"
+      "mov.b64 rc, {%0, %1};\n\t"
+      "fma.rn.f32x2 rc, ra, %4, rc;\n\t"
+      "mov.b64 {%0, %1}, rc;\n\t}"
+      : "+f"(c0), "+f"(c1)
+      : "f"(a0), "f"(a1), "l"(s2));
+}
+
+// r8_run with the interpolation written as packed FFMA2 (two slices per instruction); the tap moves are
+// all FSEL-class (ALU pipe), so that the FMA pipe only carries the FFMA2s and the three weight FADDs.
+template <int GOFF>
+__device__ __forceinline__ void r8_run_packed(float (&acc)[R8_RN][8], uint32_t addr, float f, const float dl) {
+  float4 qa, qb, ra, rb;
+  R8_LD4(qa, addr);
+  R8_LD4(qb, addr + 16);
+  R8_LD4(ra, addr + GOFF);
+  R8_LD4(rb, addr + GOFF + 16);
+#pragma unroll
+  for (int n = 0; n < R8_RN; ++n) {
+    const uint64_t w2 = r8_pair(1.f - f), f2 = r8_pair(f);
+    r8_ffma2(acc[n][0], acc[n][1], qa.x, qa.y, w2);
+    r8_ffma2(acc[n][2], acc[n][3], qa.z, qa.w, w2);
+    r8_ffma2(acc[n][4], acc[n][5], ra.x, ra.y, w2);
+    r8_ffma2(acc[n][6], acc[n][7], ra.z, ra.w, w2);
+    r8_ffma2(acc[n][0], acc[n][1], qb.x, qb.y, f2);
+    r8_ffma2(acc[n][2], acc[n][3], qb.z, qb.w, f2);
+    r8_ffma2(acc[n][4], acc[n][5], rb.x, rb.y, f2);
+    r8_ffma2(acc[n][6], acc[n][7], rb.z, rb.w, f2);
+    if (n + 1 < R8_RN) {
+      asm volatile(
+          "{\n\t"
+          ".reg .pred p;\n\t"
+          "add.rn.f32 %17, %17, %18;\n\t"
+          "setp.ge.f32 p, %17, 0f3F800000;\n\t"
+          "@p add.rn.f32 %17, %17, 0fBF800000;\n\t"
+          "@p mov.f32 %0, %4;\n\t"
+          "@p mov.f32 %1, %5;\n\t"
+          "@p mov.f32 %2, %6;\n\t"
+          "@p mov.f32 %3, %7;\n\t"
+          "@p mov.f32 %8, %12;\n\t"
+          "@p mov.f32 %9, %13;\n\t"
+          "@p mov.f32 %10, %14;\n\t"
+          "@p mov.f32 %11, %15;\n\t"
+          "@p add.u32 %16, %16, 16;\n\t"
+          "@p ld.shared.v4.f32 {%4, %5, %6, %7}, [%16+16];\n\t"
+          "@p ld.shared.v4.f32 {%12, %13, %14, %15}, [%16+%19];\n\t"
+          "}"
+          : "+f"(qa.x), "+f"(qa.y), "+f"(qa.z), "+f"(qa.w), "+f"(qb.x), "+f"(qb.y), "+f"(qb.z),
+            "+f"(qb.w), "+f"(ra.x), "+f"(ra.y), "+f"(ra.z), "+f"(ra.w), "+f"(rb.x), "+f"(rb.y),
+            "+f"(rb.z), "+f"(rb.w), "+r"(addr), "+f"(f)
+          : "f"(dl), "n"(GOFF + 16));
+    }
+  }
+}
+
 }  // namespace
 
 // PASS 0: entries [e0, e0 + ne) are class A (lanes along x, runs along y), tile 64 (x) x 32 (y).
@@ -101,7 +167,7 @@ __device__ __forceinline__ void r8_run(float (&acc)[R8_RN][8], uint32_t addr, fl
 // constant offset from the first one's); W <= WS bins are staged.  NS = stages; chunks are issued
 // NS - 2 ahead of the one being consumed (the producing warp may then run ahead of the slowest
 // warp by up to two chunks without waiting).
-template <int PASS, int WS, int NS>
+template <int PASS, int WS, int NS, bool PACKED>
 __global__ void __launch_bounds__(R8_NT, 2)
 bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* img, int S,
                int n_groups, int P, int B, int nx, int ny, float scale,
@@ -199,7 +265,8 @@ bp_run8_kernel(const float4* __restrict__ qi, int64_t row_f4, int zpad, float* i
       const int k = __float_as_int(tm) - 0x4b000000;
       const float f0 = t - (tm - 8388608.f);
       const uint32_t addr = sb + (uint32_t)a * (2u * WS * 16u) + (uint32_t)k * 16u;
-      r8_run<WS * 16>(acc, addr, f0, gg.y);
+      if (PACKED) r8_run_packed<WS * 16>(acc, addr, f0, gg.y);
+      else r8_run<WS * 16>(acc, addr, f0, gg.y);
     }
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(&empty[st]);
@@ -279,15 +346,15 @@ int backproject_run8_window(double pixel_size) {
 
 namespace {
 
-template <int WS, int NS>
+template <int WS, int NS, bool PACKED>
 int launch_run8(const float4* d_qi, const QiLayout& L, const BpArgs& a, const RunProj* d_run,
                 int32_t n_a, int32_t n_b, int W, cudaStream_t stream) {
   const size_t smem = R8_HDR + (size_t)NS * R8_NA * 2 * WS * 16;
   static uint64_t configured = 0;   // one bit per device (cudaFuncSetAttribute is per device)
   if (first_use_on_device(&configured)) {
-    PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<0, WS, NS>,
+    PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<0, WS, NS, PACKED>,
                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<1, WS, NS>,
+    PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<1, WS, NS, PACKED>,
                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   }
   const unsigned gz = (unsigned)((L.n_groups + 1) / 2);
@@ -298,14 +365,14 @@ int launch_run8(const float4* d_qi, const QiLayout& L, const BpArgs& a, const Ru
   StageScope scope(ST_BACKPROJECT, stream);
   if (n_a > 0 || n_b == 0) {  // n_a == n_b == 0 cannot happen (n_angles > 0)
     scope.kernels();
-    bp_run8_kernel<0, WS, NS><<<grid_a, R8_NT, smem, stream>>>(
+    bp_run8_kernel<0, WS, NS, PACKED><<<grid_a, R8_NT, smem, stream>>>(
         d_qi, L.row_f4(), L.zpad, a.d_img, a.n_slices, L.n_groups, L.n_angles, a.n_bins, a.nx, a.ny,
         a.scale, d_run, 0, n_a, 0, W);
     PYHST_CUDA_TRY(cudaGetLastError());
   }
   if (n_b > 0) {
     scope.kernels();
-    bp_run8_kernel<1, WS, NS><<<grid_b, R8_NT, smem, stream>>>(
+    bp_run8_kernel<1, WS, NS, PACKED><<<grid_b, R8_NT, smem, stream>>>(
         d_qi, L.row_f4(), L.zpad, a.d_img, a.n_slices, L.n_groups, L.n_angles, a.n_bins, a.nx, a.ny,
         a.scale, d_run, n_a, n_b, n_a > 0 ? 1 : 0, W);
     PYHST_CUDA_TRY(cudaGetLastError());
@@ -321,8 +388,12 @@ int launch_backproject_run8(const float4* d_qi, const QiLayout& L, const BpArgs&
   if (W == 0 || W > L.n_bins + 2 * L.zpad || L.zpad < W + 2)
     return set_error(PYHST_ERR_UNSUPPORTED, "run8 backprojector: window %d does not fit", W);
   // two instantiations: slots of 80 bins, 4 stages (pixel size <= 1.03), or 112 bins, 3 stages
-  if (W <= 80) return launch_run8<80, 4>(d_qi, L, a, d_run, n_a, n_b, W, stream);
-  return launch_run8<112, 3>(d_qi, L, a, d_run, n_a, n_b, W, stream);
+  const bool packed = run8_packed();
+  if (W <= 80)
+    return packed ? launch_run8<80, 4, true>(d_qi, L, a, d_run, n_a, n_b, W, stream)
+                  : launch_run8<80, 4, false>(d_qi, L, a, d_run, n_a, n_b, W, stream);
+  return packed ? launch_run8<112, 3, true>(d_qi, L, a, d_run, n_a, n_b, W, stream)
+                : launch_run8<112, 3, false>(d_qi, L, a, d_run, n_a, n_b, W, stream);
 }
 
 }  // namespace pyhst

@@ -240,6 +240,12 @@ int launch_ramp_filter_fused(const float* d_in, int64_t in_pitch, int64_t n_rows
                              const uint8_t* d_flip, cudaStream_t stream);
 void release_fused_filter_tables();
 int filter_variant();   // 0 automatic, 1 cuFFT path, 2 fused kernel (pyhst_test.h)
+// tensor-core GEMM of Algorithm 1 (patch_gemm_tc.cu): C[M x N] = alpha A[M x K] B, per slice of a stack
+bool patch_gemm_tc_covers(int N, int K);
+int launch_patch_gemm_tc(const float* A, const float* Bm, float* C, int64_t M, int N, int K, float alpha,
+                         bool trans_b, int n_slices, cudaStream_t stream);
+bool run8_packed();       // run8 backprojector: packed FFMA2 interpolation (test variant 6) instead of scalar FFMA
+int patch_gemm_variant();   // 0 automatic, 1 FP32 SIMT kernel, 2 tcgen05 3xTF32 kernel (pyhst_test.h)
 int launch_halfacq_weights(float* d_w, int32_t n_bins, double cbar, cudaStream_t stream);
 int launch_halfacq_fold(const float* d_rows, float* d_out, int32_t n_slices, int32_t half_angles,
                         int32_t b_out, int32_t b_st, int32_t off, const int* d_two_c, cudaStream_t stream);
@@ -279,6 +285,20 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
           smem_u32(dst)),
       "l"(src), "r"(bytes), "r"(smem_u32(bar))
       : "memory");
+}
+
+// (c0, c1) += (a0, a1) * s: one packed FFMA2 (ptxas encodes the broadcast scalar operand directly).  On
+// sm_100a an FFMA2 takes one issue slot and holds the FMA pipe for two cycles, so ALU-pipe / LSU
+// instructions issue in its shadow (profiles/r02_micro.md).
+__device__ __forceinline__ void ffma2_bcast(float& c0, float& c1, float a0, float a1, float s) {
+  asm("{\n\t.reg .b64 ra, rs, rc;\n\t"
+      "mov.b64 ra, {%2, %3};\n\t"
+      "mov.b64 rs, {%4, %4};\n\t"
+      "mov.b64 rc, {%0, %1};\n\t"
+      "fma.rn.f32x2 rc, ra, rs, rc;\n\t"
+      "mov.b64 {%0, %1}, rc;\n\t}"
+      : "+f"(c0), "+f"(c1)
+      : "f"(a0), "f"(a1), "f"(s));
 }
 
 #endif  // __CUDACC__

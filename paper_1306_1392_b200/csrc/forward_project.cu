@@ -259,10 +259,8 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
           // wavefront); the register then keeps an older, finite pixel that is multiplied by 0
           if (c < NC - 1 || w > 0.f) vlast = wp[c];
           const float4 v = vlast;
-          acc[m][0] = fmaf(w, v.x, acc[m][0]);
-          acc[m][1] = fmaf(w, v.y, acc[m][1]);
-          acc[m][2] = fmaf(w, v.z, acc[m][2]);
-          acc[m][3] = fmaf(w, v.w, acc[m][3]);
+          ffma2_bcast(acc[m][0], acc[m][1], v.x, v.y, w);
+          ffma2_bcast(acc[m][2], acc[m][3], v.z, v.w, w);
         }
       }
     }

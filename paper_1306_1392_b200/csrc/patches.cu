@@ -13,8 +13,9 @@
 //   G  <- 2 P' D^T                patch_gemm_kernel<true>    (the second GEMM)
 // The core map C_j and the cover count N_v(j) are evaluated per pixel in integer arithmetic (the
 // doubled L1 distance |2i - 2o - (m-1)| is exact), never stored.
-// The two GEMMs are tall and skinny (N ~ 1e5 patches, K and the other side 64..256): FP32 SIMT
-// tiles here; FP32 accumulation keeps the projector pair's parity bar (rel-L2 1e-5).
+// The two GEMMs are tall and skinny (N ~ 1e5 patches, K and the other side 64..256): the tcgen05
+// 3xTF32 tensor-core kernel of patch_gemm_tc.cu when the shapes allow it, else the FP32 SIMT tiles
+// here; both keep the gradient's parity bar (rel-L2 2e-5).
 #include <algorithm>
 #include <cmath>
 #include <vector>
@@ -279,6 +280,23 @@ __global__ void scalars_kernel(const double* L, double beta, float* fs) {
   fs[1] = (float)(beta / *L);
 }
 
+// C[z][M x N] = alpha A[z][M x K] B for every slice z; B = Bm[K x N] or, trans_b, Bm[N x K]^T
+int patch_gemm(const float* A, const float* Bm, float* C, int64_t M, int N, int K, float alpha, bool trans_b, int S,
+               cudaStream_t stream) {
+  const int variant = patch_gemm_variant();
+  const bool aligned = ((reinterpret_cast<uintptr_t>(A) | reinterpret_cast<uintptr_t>(Bm) |
+                         reinterpret_cast<uintptr_t>(C)) & 15) == 0 && (M * K) % 4 == 0 && (M * N) % 4 == 0;
+  const bool tc_ok = aligned && patch_gemm_tc_covers(N, K);
+  if (variant == 2 && !tc_ok)
+    return set_error(PYHST_ERR_UNSUPPORTED, "tensor-core patch GEMM does not cover N = %d, K = %d", N, K);
+  if (variant != 1 && tc_ok) return launch_patch_gemm_tc(A, Bm, C, M, N, K, alpha, trans_b, S, stream);
+  const dim3 grid((unsigned)((M + GM_BM - 1) / GM_BM), (N + GM_BN - 1) / GM_BN, S);
+  if (trans_b) patch_gemm_kernel<true><<<grid, GM_NT, 0, stream>>>(A, Bm, C, M, N, K, alpha);
+  else patch_gemm_kernel<false><<<grid, GM_NT, 0, stream>>>(A, Bm, C, M, N, K, alpha);
+  PYHST_CUDA_TRY(cudaGetLastError());
+  return PYHST_OK;
+}
+
 struct PatchWs {
   float *P, *Pp, *X, *S, *R, *r;
   double* part;
@@ -319,8 +337,7 @@ int patch_gradient_device(const float* d_W, const float* d_D, const float* d_dat
   const int64_t data_pitch = g->sino_pitch ? g->sino_pitch : g->n_bins;
   const int64_t n_rows = (int64_t)S * g->n_angles;
   // P <- W D
-  patch_gemm_kernel<false><<<dim3((unsigned)((N + GM_BM - 1) / GM_BM), (mm + GM_BN - 1) / GM_BN, S), GM_NT, 0, stream>>>(
-      d_W, d_D, w.P, N, mm, n_atoms, 1.f);
+  PYHST_TRY(patch_gemm(d_W, d_D, w.P, N, mm, n_atoms, 1.f, false, S, stream));
   // X, S, similarity
   const dim3 blk(32, 8, 1), grid_img((pg.nx + 31) / 32, (pg.ny + 7) / 8, S);
   patch_compose_kernel<<<grid_img, blk, 0, stream>>>(w.P, pg, w.X, w.S, d_f ? w.part : nullptr);
@@ -339,8 +356,7 @@ int patch_gradient_device(const float* d_W, const float* d_D, const float* d_dat
   // P' and G <- 2 P' D^T
   const int64_t n_total = (int64_t)S * N * mm;
   patch_pprime_kernel<<<(unsigned)((n_total + 255) / 256), 256, 0, stream>>>(w.P, w.X, w.S, w.R, pg, rho, w.Pp, n_total);
-  patch_gemm_kernel<true><<<dim3((unsigned)((N + GM_BM - 1) / GM_BM), (n_atoms + GM_BN - 1) / GM_BN, S), GM_NT, 0, stream>>>(
-      w.Pp, d_D, d_G, N, n_atoms, mm, 2.f);
+  PYHST_TRY(patch_gemm(w.Pp, d_D, d_G, N, n_atoms, mm, 2.f, true, S, stream));
   PYHST_CUDA_TRY(cudaGetLastError());
   return PYHST_OK;
 }
@@ -461,9 +477,7 @@ extern "C" int pyhst_patch_fista(const float* d_D, const float* d_data, const py
     PYHST_CUDA_TRY(cudaGetLastError());
   }
   if (d_X) {  // the image of eq. 7 at the final coefficients
-    patch_gemm_kernel<false><<<dim3((unsigned)(((int64_t)pg.na * pg.nb + GM_BM - 1) / GM_BM),
-                                    (pg.m * pg.m + GM_BN - 1) / GM_BN, S), GM_NT, 0, stream>>>(
-        d_W, d_D, w.P, (int64_t)pg.na * pg.nb, pg.m * pg.m, pp->n_atoms, 1.f);
+    PYHST_TRY(patch_gemm(d_W, d_D, w.P, (int64_t)pg.na * pg.nb, pg.m * pg.m, pp->n_atoms, 1.f, false, S, stream));
     patch_compose_kernel<<<dim3((pg.nx + 31) / 32, (pg.ny + 7) / 8, S), dim3(32, 8, 1), 0, stream>>>(w.P, pg, d_X, w.S,
                                                                                                     nullptr);
     PYHST_CUDA_TRY(cudaGetLastError());

@@ -60,7 +60,7 @@ BP_CASES = [
 ]
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3, 4])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 6])
 @pytest.mark.parametrize("case", BP_CASES)
 def test_backproject_matches_oracle(lib, oracle, case, variant):
     S, P, B, nx, ny, h, axis, drift = case
@@ -678,3 +678,34 @@ def test_fbp_through_both_filter_paths(lib, oracle):
             lib.ramp_filter(_dev(np.zeros((2, 5000), dtype=np.float32)))        # M would be 16384
         finally:
             lib.set_filter_variant(prev)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("m,st,n_atoms", [(8, 4, 128), (8, 8, 64), (16, 9, 64), (8, 5, 256)])
+def test_patch_gradient_tensor_core_gemm(lib, oracle, m, st, n_atoms):
+    """The tcgen05 3xTF32 GEMM (pyhst_test.h variant 2) against the oracle and against the FP32 SIMT GEMM:
+    ragged last tile of patches (N not a multiple of 128), K = 32 .. 256, N = 16 .. 256, two slices."""
+    wl = lib.workloads
+    ny, nx = 77, 102
+    P, B = 21, 155
+    w = wl.custom(2, P, B, nx, ny, drift=0.5, jitter_angles=0.01, seed=m + n_atoms)
+    data = wl.random_sinogram(2, P, B, seed=n_atoms)
+    D = wl.dct_dictionary(m, n_atoms, seed=2)
+    na, nb = oracle.patch_grid(ny, nx, m, st)
+    rng = np.random.default_rng(n_atoms)
+    W = rng.normal(size=(2, na * nb, n_atoms)).astype(np.float32)
+    out = {}
+    for variant in (1, 2):
+        prev = lib.set_patch_gemm_variant(variant)
+        try:
+            out[variant] = lib.patch_gradient(_dev(W), _dev(D), _dev(data), w.angles, w.axis, nx, ny, m, st, 0.8)
+        finally:
+            lib.set_patch_gemm_variant(prev)
+    for s in range(2):
+        Gw, Xw, fw = oracle.patch_gradient(W[s].astype(np.float64), D.astype(np.float64), data[s], w.angles, w.axis,
+                                           nx, ny, m, st, 0.8)
+        for variant in (1, 2):
+            G, X, f = out[variant]
+            assert_parity(X[s].cpu().numpy(), Xw, "patch X, GEMM variant %d" % variant)
+            assert_parity(G[s].cpu().numpy(), Gw, "patch G, GEMM variant %d" % variant, rel=PATCH_REL_L2, mabs=2e-4)
+    assert not np.array_equal(out[1][0].cpu().numpy(), out[2][0].cpu().numpy())    # the two kernels really differ
