@@ -108,84 +108,97 @@ __global__ void ftv_step_kernel(const float* __restrict__ y, const float* __rest
 
 // Dual projected-gradient steps (R18):  u = z - tau G^T p ;  q = p + G u / (8 tau) ;  p' = q / max(1, |q|)
 // -- p is read from (p1, p2) and written to (q1, q2) (Jacobi: ping-pong between two buffer pairs).
-// K dual steps per launch (temporal blocking): the block stages z, p1, p2 of its 64 x 32 tile plus a
-// halo of K cells into shared memory, iterates the Jacobi step K times there (u, then p in place) and
-// writes the tile's p after K steps.  A cell's value after one step depends on its neighbours at
-// distance 1, so what enters from the edge of the staged region spoils one more ring per step and
-// never reaches the tile; every cell of the tile goes through exactly the arithmetic of K single steps.  HBM traffic per step falls from 5 arrays to
-// (3 x 1.3 + 2) / K arrays.  Cells outside the image hold p = z = u = 0 and are never updated
-// (p1 of the last column and p2 of the last row stay zero by construction: their differences are 0).
-constexpr int FD_TX = 64, FD_TY = 32, FD_KMAX = 5, FD_NT = 256;
+// K dual steps per launch (temporal blocking): the block owns a 64 x 32 tile of the image plus a halo of K
+// cells and iterates the Jacobi step K times on it.  A cell's value after one step depends on its neighbours
+// at distance 1, so what enters from the edge of the staged region spoils one more ring per step and never
+// reaches the tile; every cell of the tile goes through exactly the arithmetic of K single steps.  HBM traffic
+// per step falls from 5 arrays to (3 x 1.5 + 2) / K arrays.
+// Register blocking: a thread owns a column segment of FD_SEG = 14 cells (3 segments x (64 + 2K) columns <= 222
+// threads) and keeps their z, p1, p2 and u in registers for all K steps; only what a NEIGHBOUR needs goes
+// through shared memory: p1 (read by the cell to the right), u (read by the cell to the left) and, at the
+// segment ends, p2 of the last row / u of the first row.  Two block barriers per step.
+// Cells outside the image hold p = z = 0 and are never updated (p1 of the last column and p2 of the last row
+// stay zero by construction: their differences are 0).
+constexpr int FD_TX = 64, FD_TY = 32, FD_KMAX = 5, FD_NT = 256, FD_SEG = 14, FD_NSEG = 3;
 constexpr int FD_RW = FD_TX + 2 * FD_KMAX, FD_RH = FD_TY + 2 * FD_KMAX;
+static_assert(FD_SEG * FD_NSEG >= FD_RH && FD_RW * FD_NSEG <= FD_NT, "thread map of the fused dual kernel");
 
 __global__ void __launch_bounds__(FD_NT)
 ftv_dual_fused_kernel(const float* __restrict__ z, const float* __restrict__ p1, const float* __restrict__ p2,
                       float* __restrict__ q1, float* __restrict__ q2, int nx, int ny,
                       const float* __restrict__ fs, int K, int p_is_zero) {
-  extern __shared__ float sm[];
-  const int rw = FD_TX + 2 * K, rh = FD_TY + 2 * K, n = rw * rh;
-  float* sz = sm;
-  float* s1 = sm + FD_RW * FD_RH;
-  float* s2 = s1 + FD_RW * FD_RH;
-  float* su = s2 + FD_RW * FD_RH;
+  __shared__ float S1[FD_RH][FD_RW];          // p1 as of the last completed step
+  __shared__ float SU[FD_RH][FD_RW];          // u of the current step
+  __shared__ float E2[FD_NSEG][FD_RW];        // p2 of the last row of every segment
+  const int rw = FD_TX + 2 * K, rh = FD_TY + 2 * K;
+  const int col = (int)threadIdx.x % rw, seg = (int)threadIdx.x / rw;
+  const bool active = seg < FD_NSEG;
+  const int row0 = seg * FD_SEG;
   const int64_t o = (int64_t)blockIdx.z * ny * nx;
-  const int gx0 = blockIdx.x * FD_TX - K, gy0 = blockIdx.y * FD_TY - K;
+  const int gx = blockIdx.x * FD_TX - K + col, gy0 = blockIdx.y * FD_TY - K + row0;
   const float tau = fs[1], step = fs[2];
-  for (int e = threadIdx.x; e < n; e += FD_NT) {
-    const int ly = e / rw, lx = e - ly * rw;
-    const int gy = gy0 + ly, gx = gx0 + lx;
-    const bool in = gy >= 0 && gy < ny && gx >= 0 && gx < nx;
-    const int64_t k = o + (int64_t)gy * nx + gx;
-    sz[e] = in ? z[k] : 0.f;
-    s1[e] = (in && !p_is_zero) ? p1[k] : 0.f;
-    s2[e] = (in && !p_is_zero) ? p2[k] : 0.f;
+  const bool x_in = gx >= 0 && gx < nx, right_ok = gx + 1 < nx && col + 1 < rw;
+
+  float vz[FD_SEG], v1[FD_SEG], v2[FD_SEG], vu[FD_SEG];
+  if (active) {
+#pragma unroll
+    for (int r = 0; r < FD_SEG; ++r) {
+      const int gy = gy0 + r;
+      const bool in = x_in && gy >= 0 && gy < ny && row0 + r < rh;
+      const int64_t k = o + (int64_t)gy * nx + gx;
+      vz[r] = in ? z[k] : 0.f;
+      v1[r] = (in && !p_is_zero) ? p1[k] : 0.f;
+      v2[r] = (in && !p_is_zero) ? p2[k] : 0.f;
+      if (row0 + r < rh) S1[row0 + r][col] = v1[r];
+    }
+    E2[seg][col] = v2[FD_SEG - 1];
   }
   __syncthreads();
-  // the cells of a thread are e = tid, tid + 256, ...: (ly, lx) advance by (256 / rw, 256 % rw) with a
-  // carry -- no division in the loops
-  const int dy = FD_NT / rw, dx = FD_NT - dy * rw;
-  const int ly0 = (int)threadIdx.x / rw, lx0 = (int)threadIdx.x - ly0 * rw;
   for (int it = 0; it < K; ++it) {
-    {
-      int ly = ly0, lx = lx0;
-      for (int e = threadIdx.x; e < n; e += FD_NT) {
-        const float l1 = lx > 0 ? s1[e - 1] : 0.f, t2 = ly > 0 ? s2[e - rw] : 0.f;
-        su[e] = fmaf(-tau, (l1 - s1[e]) + (t2 - s2[e]), sz[e]);
-        lx += dx;
-        ly += dy;
-        if (lx >= rw) { lx -= rw; ++ly; }
+    if (active) {
+      float above = seg > 0 ? E2[seg - 1][col] : 0.f;    // p2 of the cell above the segment
+#pragma unroll
+      for (int r = 0; r < FD_SEG; ++r) {
+        if (row0 + r < rh) {
+          const float l1 = col > 0 ? S1[row0 + r][col - 1] : 0.f;
+          vu[r] = fmaf(-tau, (l1 - v1[r]) + (above - v2[r]), vz[r]);
+          SU[row0 + r][col] = vu[r];
+        }
+        above = v2[r];
       }
     }
     __syncthreads();
-    {
-      int ly = ly0, lx = lx0;
-      for (int e = threadIdx.x; e < n; e += FD_NT) {
-        const int gy = gy0 + ly, gx = gx0 + lx;
-        if (gy >= 0 && gy < ny && gx >= 0 && gx < nx) {
-          const float u = su[e];
-          const float a = (gx + 1 < nx && lx + 1 < rw) ? su[e + 1] - u : 0.f;
-          const float b = (gy + 1 < ny && ly + 1 < rh) ? su[e + rw] - u : 0.f;
-          const float n1 = fmaf(a, step, s1[e]), n2 = fmaf(b, step, s2[e]);
+    if (active) {
+#pragma unroll
+      for (int r = 0; r < FD_SEG; ++r) {
+        const int gy = gy0 + r, row = row0 + r;
+        if (row < rh && x_in && gy >= 0 && gy < ny) {
+          const float u = vu[r];
+          const float ur = right_ok ? SU[row][col + 1] - u : 0.f;
+          float ub = 0.f;
+          if (gy + 1 < ny && row + 1 < rh) ub = (r + 1 < FD_SEG ? vu[r + 1] : SU[row + 1][col]) - u;
+          const float n1 = fmaf(ur, step, v1[r]), n2 = fmaf(ub, step, v2[r]);
           // p = q / max(1, |q|) = q * min(1, 1/|q|)
           const float inv = fminf(1.f, rsqrtf(fmaf(n1, n1, n2 * n2)));
-          s1[e] = n1 * inv;
-          s2[e] = n2 * inv;
+          v1[r] = n1 * inv;
+          v2[r] = n2 * inv;
+          S1[row][col] = v1[r];
         }
-        lx += dx;
-        ly += dy;
-        if (lx >= rw) { lx -= rw; ++ly; }
       }
+      E2[seg][col] = v2[FD_SEG - 1];
     }
     __syncthreads();
   }
-  for (int e = threadIdx.x; e < FD_TX * FD_TY; e += FD_NT) {
-    const int ty = e / FD_TX, tx = e - ty * FD_TX;
-    const int gy = blockIdx.y * FD_TY + ty, gx = blockIdx.x * FD_TX + tx;
-    if (gy >= ny || gx >= nx) continue;
-    const int l = (ty + K) * rw + tx + K;
-    const int64_t k = o + (int64_t)gy * nx + gx;
-    q1[k] = s1[l];
-    q2[k] = s2[l];
+  if (active && col >= K && col < K + FD_TX && x_in) {
+#pragma unroll
+    for (int r = 0; r < FD_SEG; ++r) {
+      const int row = row0 + r, gy = gy0 + r;
+      if (row >= K && row < K + FD_TY && gy < ny) {
+        const int64_t k = o + (int64_t)gy * nx + gx;
+        q1[k] = v1[r];
+        q2[k] = v2[r];
+      }
+    }
   }
 }
 
@@ -306,13 +319,6 @@ static int tv_solver(const float* d_data, float* d_img, const pyhst_geom_t* g, f
   ftv_scalars_kernel<<<1, 1, 0, stream>>>(d_L, (double)beta, d_fs);
   PYHST_CUDA_TRY(cudaGetLastError());
 
-  const size_t fd_smem = (size_t)4 * FD_RW * FD_RH * sizeof(float);
-  {
-    static uint64_t configured = 0;
-    if (first_use_on_device(&configured))
-      PYHST_CUDA_TRY(cudaFuncSetAttribute(ftv_dual_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)fd_smem));
-  }
   // ---- FISTA (R19, R20): x0 = y0 = 0, t0 = 1
   PYHST_CUDA_TRY(cudaMemsetAsync(d_img, 0, (size_t)n_img * 4, stream));
   PYHST_CUDA_TRY(cudaMemsetAsync(y, 0, (size_t)n_img * 4, stream));
@@ -338,7 +344,7 @@ static int tv_solver(const float* d_data, float* d_img, const pyhst_geom_t* g, f
       const dim3 grid_d((nx + FD_TX - 1) / FD_TX, (ny + FD_TY - 1) / FD_TY, S);
       for (int done = 0; done < n_inner;) {
         const int kk = std::min(FD_KMAX, n_inner - done);
-        ftv_dual_fused_kernel<<<grid_d, FD_NT, fd_smem, stream>>>(z, p[cur], p[cur + 1], p[2 - cur], p[3 - cur], nx,
+        ftv_dual_fused_kernel<<<grid_d, FD_NT, 0, stream>>>(z, p[cur], p[cur + 1], p[2 - cur], p[3 - cur], nx,
                                                                  ny, d_fs, kk, done == 0 ? 1 : 0);
         cur = 2 - cur;
         done += kk;
