@@ -269,7 +269,7 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
   return PYHST_OK;
 }
 
-int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out) {
+int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, bool want_diag, const FpPlan** out) {
   DeviceCtx& c = ctx();
   std::lock_guard<std::recursive_mutex> lock(c.mu);
   auto& g_fp_plans = c.fp_plans;
@@ -277,7 +277,7 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out) 
   const size_t n = (size_t)g->n_angles;
   for (auto& pl : g_fp_plans) {
     if (pl.n_angles == g->n_angles && pl.n_bins == g->n_bins && pl.nx == g->nx && pl.ny == g->ny &&
-        pl.n_groups == (g->n_slices + 3) / 4 && pl.pixel_size == g->pixel_size &&
+        pl.n_groups == (g->n_slices + 3) / 4 && pl.pixel_size == g->pixel_size && pl.want_diag == want_diag &&
         std::memcmp(pl.angles.data(), g->angles_rad, n * sizeof(double)) == 0 &&
         std::memcmp(pl.axis.data(), g->axis_pos, n * sizeof(double)) == 0) {
       pl.last_use = ++g_tick;
@@ -291,6 +291,9 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out) 
       if (it->last_use < lru->last_use) lru = it;
     cudaFree(lru->d_projs);  // synchronises: no kernel can still be reading them
     cudaFree(lru->d_chunks);
+    cudaFree(lru->fd.d_projs);
+    cudaFree(lru->fd.d_chunks);
+    cudaFree(lru->fd.d_ranges);
     g_fp_plans.erase(lru);
   }
   FpPlan pl;
@@ -302,9 +305,41 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out) 
   pl.pixel_size = g->pixel_size;
   pl.angles.assign(g->angles_rad, g->angles_rad + n);
   pl.axis.assign(g->axis_pos, g->axis_pos + n);
+  pl.want_diag = want_diag;
   std::vector<FpProjD> projs;
   std::vector<FpChunk> chunks;
-  if (build_fp_tables(g, &pl, &projs, &chunks)) {
+  std::vector<int32_t> legacy;
+  if (want_diag) {
+    // diagonal-line interval kernel for every projection it covers; the banded tables then hold
+    // only the rest (projections within 2^-12 rad of an image axis, windows that do not fit)
+    std::vector<FdProj> dprojs;
+    std::vector<FdChunk> dchunks;
+    std::vector<int32_t> ranges;
+    FpPlan probe = pl;
+    if (build_fd_tables(g, &pl.fd, &dprojs, &dchunks, &ranges, &legacy) &&
+        (legacy.empty() || build_fp_tables(g, &probe, &projs, &chunks, &legacy))) {
+      pl.diag = true;
+      pl.n_legacy = (int32_t)legacy.size();
+      PYHST_CUDA_TRY(cudaMalloc(&pl.fd.d_projs, dprojs.size() * sizeof(FdProj)));
+      PYHST_CUDA_TRY(cudaMalloc(&pl.fd.d_chunks, dchunks.size() * sizeof(FdChunk)));
+      PYHST_CUDA_TRY(cudaMalloc(&pl.fd.d_ranges, ranges.size() * sizeof(int32_t)));
+      PYHST_CUDA_TRY(cudaMemcpyAsync(pl.fd.d_projs, dprojs.data(), dprojs.size() * sizeof(FdProj),
+                                     cudaMemcpyHostToDevice, stream));
+      PYHST_CUDA_TRY(cudaMemcpyAsync(pl.fd.d_chunks, dchunks.data(), dchunks.size() * sizeof(FdChunk),
+                                     cudaMemcpyHostToDevice, stream));
+      PYHST_CUDA_TRY(cudaMemcpyAsync(pl.fd.d_ranges, ranges.data(), ranges.size() * sizeof(int32_t),
+                                     cudaMemcpyHostToDevice, stream));
+      if (std::getenv("PYHST_DEBUG"))
+        fprintf(stderr, "[pyhst] fp diag plan: P=%d B=%d %dx%d h=%g -> W=%d chunks=%d n_bx=%d legacy=%d\n",
+                g->n_angles, g->n_bins, g->nx, g->ny, g->pixel_size, pl.fd.W, pl.fd.n_chunks, pl.fd.n_bx,
+                pl.n_legacy);
+    }
+    projs.clear();
+    chunks.clear();
+  }
+  if (pl.diag && legacy.empty()) {
+    pl.n_chunks = 0;
+  } else if (build_fp_tables(g, &pl, &projs, &chunks, pl.diag ? &legacy : nullptr)) {
     PYHST_CUDA_TRY(cudaMalloc(&pl.d_projs, projs.size() * sizeof(FpProjD)));
     PYHST_CUDA_TRY(cudaMalloc(&pl.d_chunks, chunks.size() * sizeof(FpChunk)));
     // pageable sources: the copies are complete (staged) when the calls return
@@ -472,7 +507,7 @@ int pyhst_set_filter_variant(int variant) {
 
 int pyhst_set_forward_project_variant(int variant) {
   const int prev = g_fp_variant;
-  if (variant >= 0 && variant <= 4) g_fp_variant = variant;
+  if (variant >= 0 && variant <= 5) g_fp_variant = variant;
   return prev;
 }
 
@@ -490,6 +525,9 @@ void pyhst_release_cache(void) {
     for (auto& pl : c->fp_plans) {
       cudaFree(pl.d_projs);
       cudaFree(pl.d_chunks);
+      cudaFree(pl.fd.d_projs);
+      cudaFree(pl.fd.d_chunks);
+      cudaFree(pl.fd.d_ranges);
     }
     c->fp_plans.clear();
     for (auto& pl : c->geom) {
@@ -609,7 +647,15 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
   PYHST_TRY(get_geom_plan(g, 0.0, g->n_bins, stream, &plan));
   if (g_fp_variant != 1) {
     const FpPlan* fplan = nullptr;
-    PYHST_TRY(get_fp_plan(g, stream, &fplan));
+    PYHST_TRY(get_fp_plan(g, stream, g_fp_variant == 0 || g_fp_variant == 5, &fplan));
+    if (fplan->diag) {
+      PYHST_TRY(launch_forward_project_diag(d_img, d_sino, pitch, g, scale, fplan->fd, stream));
+      if (fplan->n_chunks > 0)
+        return launch_forward_project_banded(d_img, d_sino, pitch, g, scale, *fplan, 0, stream);
+      return PYHST_OK;
+    }
+    if (g_fp_variant == 5)
+      return set_error(PYHST_ERR_UNSUPPORTED, "diagonal-line forward projector does not cover this geometry");
     if (fplan->n_chunks > 0)
       return launch_forward_project_banded(d_img, d_sino, pitch, g, scale, *fplan, g_fp_variant == 3 ? 1 : (g_fp_variant == 4 ? 2 : 0), stream);
     if (g_fp_variant == 2)

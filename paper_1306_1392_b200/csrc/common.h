@@ -121,7 +121,7 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
 
 // Grow-only device workspace slots owned by the library (freed by pyhst_release_cache).
 enum WorkspaceSlot { WS_QI = 0, WS_FFT = 1, WS_WEIGHTS = 2, WS_IMG_T = 3, WS_ROWS = 4,
-                     WS_CHUNKS = 5, WS_XI = 6, WS_FISTA = 7, WS_FPL = 8, WS_STITCH = 9, WS_COUNT = 10 };
+                     WS_CHUNKS = 5, WS_XI = 6, WS_FISTA = 7, WS_FPL = 8, WS_STITCH = 9, WS_XD = 10, WS_COUNT = 11 };
 int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr);
 // bumped whenever the slot's block is (re)allocated or released: lets a user of the slot remember
 // "I initialised this very block" without being fooled by a recycled address
@@ -189,10 +189,38 @@ struct FpChunk {
   int32_t cls;           // 0: lines are image rows, 1: lines are image columns
   int32_t pad_;
 };
+// ---- diagonal-line interval projector (forward_project_diag.cu) ----------------------------------
+// Position (in kappa = sgn * stored position k, so that t grows with it) of t = m on stored line w:
+//   ks(m, w) = K0 + m inv + sD w      (double, R11)
+struct FdProj {
+  double K0, inv, sD;
+  float s, sig;        // (float)sD, |sigma| = h (|cos| + |sin|) = bins per pixel along the line
+  int32_t p, pad_;     // projection index in the caller's order
+};
+struct FdChunk {
+  int32_t first, count;   // range in the permuted FdProj table
+  int32_t layout;         // 0: lines are diagonals i - j, 1: anti-diagonals i + j
+  int32_t sgn, skew;      // stored position = sgn * kappa; stored positions the strips move per line, rounded
+  int32_t mul16;          // 16 * sgn: byte step of the stage per kappa
+  int32_t pad_[2];
+};
+struct FdPlan {
+  int32_t n_chunks = 0, n_bx = 0, W = 0, zpad = 0, n_lines_alloc = 0;
+  FdProj* d_projs = nullptr;
+  FdChunk* d_chunks = nullptr;
+  int32_t* d_ranges = nullptr;   // [n_chunks][n_bx][2]
+};
+
 struct FpPlan {
   // key
   int32_t n_angles = 0, n_bins = 0, nx = 0, ny = 0, n_groups = 0;
   double pixel_size = 0;
+  bool want_diag = false;
+  // diagonal-line kernel: covers every projection except `n_legacy` ones (too close to an image axis,
+  // or a window that does not fit), which the banded tables below then hold alone
+  bool diag = false;
+  int32_t n_legacy = 0;
+  FdPlan fd;
   std::vector<double> angles, axis;
   // product
   int32_t npj = 0, W = 0, nc = 0, n_chunks = 0;
@@ -201,10 +229,17 @@ struct FpPlan {
   FpChunk* d_chunks = nullptr;
   uint64_t last_use = 0;
 };
-int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, const FpPlan** out);  // api.cu
-// fills the host tables of a plan; returns false if the banded kernel cannot cover the geometry
+int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, bool want_diag, const FpPlan** out);  // api.cu
+// fills the host tables of a plan (for the projections listed in `subset`, all if null); returns false if
+// the banded kernel cannot cover the geometry
 bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* projs,
-                     std::vector<FpChunk>* chunks);  // forward_project.cu
+                     std::vector<FpChunk>* chunks, const std::vector<int32_t>* subset = nullptr);  // forward_project.cu
+// diagonal-line kernel: host tables (projections it does not cover are listed in `legacy`); false if it
+// covers none
+bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* projs, std::vector<FdChunk>* chunks,
+                     std::vector<int32_t>* ranges, std::vector<int32_t>* legacy);  // forward_project_diag.cu
+int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch, const pyhst_geom_t* g,
+                                float scale, const FdPlan& plan, cudaStream_t stream);
 int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pitch,
                                   const pyhst_geom_t* g, float scale, const FpPlan& plan,
                                   int interval_groups, cudaStream_t stream);

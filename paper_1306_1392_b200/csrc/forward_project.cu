@@ -598,7 +598,7 @@ Extent merge(const Extent& a, const Extent& b) {
 }  // namespace
 
 bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* projs,
-                     std::vector<FpChunk>* chunks) {
+                     std::vector<FpChunk>* chunks, const std::vector<int32_t>* subset) {
   const int P = g->n_angles;
   const double h = g->pixel_size;
   // candidates per line: the open strip of width 2 / |cu| <= 2 sqrt(2) / h holds at most nc pixels
@@ -609,7 +609,11 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
   // the grid fills whole waves of the GPU's block slots (3 blocks per SM)
   std::vector<int> order[2];
   std::vector<FpProjD> all(P);
+  std::vector<char> wanted(P, subset ? 0 : 1);
+  if (subset)
+    for (int32_t p : *subset) wanted[p] = 1;
   for (int p = 0; p < P; ++p) {
+    if (!wanted[p]) continue;
     const double ch = h * std::cos(g->angles_rad[p]), sh = h * std::sin(g->angles_rad[p]);
     const int cls = std::fabs(ch) >= std::fabs(sh) ? 0 : 1;
     const double cu = cls ? sh : ch, cv = cls ? ch : sh;
@@ -795,6 +799,7 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
   const int n_bands_min = (std::min(g->nx, g->ny) + FB_RB - 1) / FB_RB;
   int n_split = (int)std::max<int64_t>(1, std::min<int64_t>(4, slots / std::max<int64_t>(blocks, 1)));
   n_split = std::max(1, std::min(n_split, n_bands_min / 8));
+  if (plan.diag) n_split = 1;   // the tables hold a subset of the projections: the combine pass would touch every row
   static PerDeviceSize configured[5];
   const int vi = four ? 3 : (plan.nc == 3 ? (n_split > 1 ? 4 : 0) : (plan.nc == 4 ? 1 : 2));
   auto kern = four ? fp_band_kernel<3, 4, true>

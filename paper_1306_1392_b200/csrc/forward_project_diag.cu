@@ -1,0 +1,589 @@
+// Forward projection P = (P^T)^T, the product kernel (include/pyhst.h a3; PAPER.md:L65, L71-L73
+// eq. 1, L211 Alg. 1 "Fp"; readings R6, R11, R13 of DESIGN.md):
+//
+//   y[s,p,b] = scale * sum_{i,j} Lambda(t_p(i,j) - b) x[s,i,j],   Lambda(u) = max(0, 1 - |u|)
+//
+// fp_diag_kernel: interval form of the gather on DIAGONAL image lines.
+//
+//   * Interval form: a thread owns unit intervals [m, m+1) of the detector axis.  A pixel whose
+//     coordinate t falls into the interval is loaded once from shared memory and used twice, with
+//     weight f = t - m for bin m+1 and 1 - f for bin m.  No atomics; each bin is the sum of the
+//     upper share of the interval below it and the lower share of the interval above it.
+//   * Diagonal lines: along a line of pixels (j + k, i +- k) the coordinate t moves by
+//     |sigma| = h (|cos| + |sin|) >= 1 bin per pixel, so an interval holds AT MOST ONE pixel of a
+//     line -- one candidate, one predicate, no second-candidate logic (on image rows or columns
+//     the step is h max(|cos|, |sin|) <= 1: up to two pixels per interval and line, and half of
+//     the executed FMAs carry weight zero).  The image is stored sheared (XD, below), so that a
+//     diagonal is a contiguous run of float4 (4 slices) and a band of diagonals is staged by TMA
+//     bulk copies like the rows of the banded kernel.
+//   * A thread owns FD_M = 2 neighbouring intervals of one projection and 4 NG slices: three
+//     boundaries serve two intervals, the middle bin has one accumulator.
+//   * Which pixel belongs to which interval is decided identically by the two threads that share
+//     a boundary: both evaluate the SAME expression for it -- ks(m, w) = K0 + m inv + sD w in
+//     double per (boundary, band), split into an integer and a float fraction, then
+//     fmaf(s, r, fraction) per line and a round-up add of 1.5 * 2^23 + integer -- so the sets
+//     [ceil(ks(m)), ceil(ks(m+1))) partition the line whatever the rounding.  With
+//     |sigma| >= 1 + 2^-12 such a set has at most one element; projections closer to an image
+//     axis than that (and pixel sizes below 1 bin) go to the banded kernel (forward_project.cu).
+//   * The weight f = |sigma| (ceil(ks) - ks) uses the continuous position (R11: double per band,
+//     FP32 only for the in-band offset).
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "common.h"
+
+namespace pyhst {
+
+namespace {
+
+constexpr int FD_NB = 64;      // intervals per block (FD_NB - 1 complete bins)
+constexpr int FD_NPJ = 16;     // projections per block (at most)
+constexpr int FD_M = 2;        // neighbouring intervals per thread
+constexpr int FD_NT = FD_NB / FD_M * FD_NPJ;   // 512 threads, one (interval pair, projection) each
+constexpr int FD_RB = 8;       // lines per band
+constexpr int FD_UNR = 4;      // lines unrolled together (register budget)
+constexpr int FD_NSTG = 3;     // stages of the band ring
+constexpr int FD_WMAX = 128;   // window capacity (float4 per line)
+constexpr int FD_PW = FD_WMAX + FD_RB;   // row pitch of a stage (float4): room for the per-line skew
+constexpr int FD_HDR = 1024;   // mbarriers, origins, FdProj table
+constexpr float FD_MAGIC = 12582912.f;   // 1.5 * 2^23
+
+// smem bytes of one launch
+constexpr size_t fd_smem(int ng) { return FD_HDR + (size_t)FD_NSTG * FD_RB * ng * FD_PW * 16; }
+
+struct FdParams {
+  const float4* xd[2];     // sheared image, layout 0 (diagonals i - j) and 1 (anti-diagonals i + j)
+  int64_t line_f4;         // float4 per stored line (nx + 2 zpad)
+  int64_t group_f4;        // float4 per slice group (line_f4 * stored lines)
+  int32_t zpad;
+  float* sino;
+  int64_t pitch;
+  int32_t S, P, B;
+  float scale;
+  const FdProj* projs;
+  const FdChunk* chunks;
+  const int2* ranges;      // [n_chunks][n_bx]: lines [x, y) the block walks
+  int32_t n_bx, W;
+};
+
+// One line of one interval, NG slice groups: predicated on `jlo < jhi` (the interval holds the
+// pixel ceil(ks_lo)), two LDS.128 and 8 NG FFMA.  al / au: accumulators of bins m and m + 1.
+template <int NG>
+__device__ __forceinline__ void fd_line(float (&al)[4 * NG], float (&au)[4 * NG], float jlo, float jhi,
+                                        float f, float g, uint32_t addr) {
+  if constexpr (NG == 2) {
+    asm volatile("{\n\t"
+        ".reg .pred p;\n\t"
+        ".reg .f32 v<8>;\n\t"
+        "setp.lt.f32 p, %16, %17;\n\t"
+        "ld.shared.v4.f32 {v0, v1, v2, v3}, [%20];\n\t"
+        "ld.shared.v4.f32 {v4, v5, v6, v7}, [%20+%21];\n\t"
+        "@p fma.rn.f32 %0, %19, v0, %0;\n\t"
+        "@p fma.rn.f32 %1, %19, v1, %1;\n\t"
+        "@p fma.rn.f32 %2, %19, v2, %2;\n\t"
+        "@p fma.rn.f32 %3, %19, v3, %3;\n\t"
+        "@p fma.rn.f32 %8, %18, v0, %8;\n\t"
+        "@p fma.rn.f32 %9, %18, v1, %9;\n\t"
+        "@p fma.rn.f32 %10, %18, v2, %10;\n\t"
+        "@p fma.rn.f32 %11, %18, v3, %11;\n\t"
+        "@p fma.rn.f32 %4, %19, v4, %4;\n\t"
+        "@p fma.rn.f32 %5, %19, v5, %5;\n\t"
+        "@p fma.rn.f32 %6, %19, v6, %6;\n\t"
+        "@p fma.rn.f32 %7, %19, v7, %7;\n\t"
+        "@p fma.rn.f32 %12, %18, v4, %12;\n\t"
+        "@p fma.rn.f32 %13, %18, v5, %13;\n\t"
+        "@p fma.rn.f32 %14, %18, v6, %14;\n\t"
+        "@p fma.rn.f32 %15, %18, v7, %15;\n\t"
+        "}"
+        : "+f"(al[0]), "+f"(al[1]), "+f"(al[2]), "+f"(al[3]), "+f"(al[4]), "+f"(al[5]), "+f"(al[6]), "+f"(al[7]),
+          "+f"(au[0]), "+f"(au[1]), "+f"(au[2]), "+f"(au[3]), "+f"(au[4]), "+f"(au[5]), "+f"(au[6]), "+f"(au[7])
+        : "f"(jlo), "f"(jhi), "f"(f), "f"(g), "r"(addr), "n"(FD_RB * FD_PW * 16));
+  } else {
+    asm volatile("{\n\t"
+        ".reg .pred p;\n\t"
+        ".reg .f32 v<4>;\n\t"
+        "setp.lt.f32 p, %8, %9;\n\t"
+        "ld.shared.v4.f32 {v0, v1, v2, v3}, [%12];\n\t"
+        "@p fma.rn.f32 %0, %11, v0, %0;\n\t"
+        "@p fma.rn.f32 %1, %11, v1, %1;\n\t"
+        "@p fma.rn.f32 %2, %11, v2, %2;\n\t"
+        "@p fma.rn.f32 %3, %11, v3, %3;\n\t"
+        "@p fma.rn.f32 %4, %10, v0, %4;\n\t"
+        "@p fma.rn.f32 %5, %10, v1, %5;\n\t"
+        "@p fma.rn.f32 %6, %10, v2, %6;\n\t"
+        "@p fma.rn.f32 %7, %10, v3, %7;\n\t"
+        "}"
+        : "+f"(al[0]), "+f"(al[1]), "+f"(al[2]), "+f"(al[3]), "+f"(au[0]), "+f"(au[1]), "+f"(au[2]), "+f"(au[3])
+        : "f"(jlo), "f"(jhi), "f"(f), "f"(g), "r"(addr));
+  }
+}
+
+template <int NG>
+__global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);              // [NSTG]
+  uint64_t* empty = reinterpret_cast<uint64_t*>(smem + 32);        // [NSTG]
+  int* sorigin = reinterpret_cast<int*>(smem + 64);                // [NSTG]
+  FdProj* sproj = reinterpret_cast<FdProj*>(smem + 128);           // [FD_NPJ] x 48 B
+  float4* buf = reinterpret_cast<float4*>(smem + FD_HDR);          // [NSTG][NG][RB][PW]
+  constexpr int STAGE_F4 = NG * FD_RB * FD_PW;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const FdChunk ck = prm.chunks[blockIdx.y];
+  const int gA = blockIdx.z * NG;
+  const int mB = blockIdx.x * (FD_NB - 1) - 1;      // intervals [m, m+1), m in [mB, mB + NB)
+  const int2 rg = prm.ranges[(int64_t)blockIdx.y * prm.n_bx + blockIdx.x];
+  const int n_bands = (rg.y - rg.x + FD_RB - 1) / FD_RB;
+  const int W = prm.W;
+  const uint32_t row_bytes = (uint32_t)W * 16u;
+  const float4* xd = (ck.layout ? prm.xd[1] : prm.xd[0]) + (int64_t)gA * prm.group_f4;
+  const int sgn = ck.sgn, skew = ck.skew;
+  const int bias = skew < 0 ? FD_RB - 1 : 0;
+
+  if (tid < ck.count) sproj[tid] = prm.projs[ck.first + tid];
+  if (tid == 0) {
+#pragma unroll
+    for (int q = 0; q < FD_NSTG; ++q) {
+      mbar_init(&full[q], FD_RB);
+      mbar_init(&empty[q], FD_NT / 32);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  // one warp (the role rotates): waits until the stage of band k - NSTG has been read by every
+  // warp, computes the window origin of band k in double (the lowest stored position, over the
+  // chunk's projections, of the block's outer boundaries on the band's first and last line, the
+  // per-line skew taken off), then issues one bulk copy per line and slice group.  Line r of the
+  // band is staged from stored position origin + skew * r.
+  auto produce = [&](int k) {
+    const int st = k % FD_NSTG;
+    if (k >= FD_NSTG) mbar_wait(&empty[st], (uint32_t)(((k / FD_NSTG) - 1) & 1));
+    const int w0 = rg.x + k * FD_RB;
+    double lo = 1e300;
+    if (lane < ck.count) {
+      const FdProj pj = sproj[lane];
+      // stored position of t = m on line w: sgn * ks(m, w); the block's pixels lie between the two
+      // outer boundaries
+      const double e0 = fma((double)mB, pj.inv, pj.K0), e1 = fma((double)(mB + FD_NB), pj.inv, pj.K0);
+      const double ea = sgn > 0 ? e0 : -e1;                      // lowest stored position on line 0
+      const double da = (double)sgn * pj.sD;                     // its change per line
+      const double a0 = fma(da, (double)w0, ea);
+      const double a1 = fma(da, (double)(w0 + FD_RB - 1), ea) - (double)(skew * (FD_RB - 1));
+      lo = fmin(a0, a1);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    const int origin = (int)floor(lo) - 2;
+    uint64_t* bar = &full[st];
+    if (lane == 0) sorigin[st] = origin;
+    if (lane < FD_RB) {
+      mbar_arrive_expect_tx(bar, NG * row_bytes);
+      const float4* src = xd + (int64_t)(w0 + lane) * prm.line_f4 + (prm.zpad + origin + skew * lane);
+      float4* dst = buf + st * STAGE_F4 + lane * FD_PW + bias + skew * lane;
+#pragma unroll
+      for (int q = 0; q < NG; ++q) bulk_g2s(dst + q * FD_RB * FD_PW, src + q * prm.group_f4, row_bytes, bar);
+    }
+  };
+
+  if (warp == 0 && n_bands > 0) produce(0);
+  if (warp == 1 && n_bands > 1) produce(1);
+
+  // bins mB + 2 jp + {0, 1, 2}: lower share of the first interval, both shares of the middle bin,
+  // upper share of the second interval
+  float acc[FD_M + 1][4 * NG];
+#pragma unroll
+  for (int q = 0; q <= FD_M; ++q)
+#pragma unroll
+    for (int sl = 0; sl < 4 * NG; ++sl) acc[q][sl] = 0.f;
+
+  // a warp = 8 interval pairs x 4 projections: its 32 pixels of a line lie within ~16 stored
+  // positions, i.e. the LDS.128 touches <= 256 B (2.4 cycles instead of 4, profiles/r02_micro.md)
+  const int jp = (warp & 3) * 8 + (lane >> 2);
+  const int pj = (warp >> 2) * 4 + (lane & 3);
+  const bool active = pj < ck.count;
+  const int m0 = mB + FD_M * jp;
+  const float s = active ? sproj[pj].s : 0.f;
+  const float sig = active ? sproj[pj].sig : 1.f;
+  const int mul = ck.mul16;                    // sgn * 16 (from the table: one IMAD per address)
+
+  for (int k = 0; k < n_bands; ++k) {
+    if (k + 2 < n_bands && warp == ((k + 2) & 15)) produce(k + 2);
+    const int st = k % FD_NSTG;
+    mbar_wait(&full[st], (uint32_t)((k / FD_NSTG) & 1));
+    if (active) {
+      const int origin = sorigin[st];
+      const double w0 = (double)(rg.x + k * FD_RB);
+      const FdProj* sp = &sproj[pj];
+      const double K0 = sp->K0, inv = sp->inv, sD = sp->sD;
+      float afr[FD_M + 1], mg[FD_M + 1];
+#pragma unroll
+      for (int q = 0; q <= FD_M; ++q) {
+        // the boundary's position on the band's first line (double), split; the thread that
+        // shares the boundary evaluates the identical expression
+        const double ks = fma(sD, w0, fma((double)(m0 + q), inv, K0));
+        const double ai = rint(ks);
+        afr[q] = (float)(ks - ai);
+        mg[q] = (float)ai + FD_MAGIC;     // exact: |ai| < 2^22
+      }
+      // byte address of stored position k = sgn * kappa on line 0:  (bias + k - origin) * 16, with
+      // kappa = float_as_int(jm) - 0x4b400000
+      const uint32_t cbase = smem_u32(buf + st * STAGE_F4) + (uint32_t)((bias - origin) * 16) -
+                             (uint32_t)mul * 0x4b400000u;
+#pragma unroll 1
+      for (int r0 = 0; r0 < FD_RB; r0 += FD_UNR) {
+        float ah[FD_M + 1];
+#pragma unroll
+        for (int q = 0; q <= FD_M; ++q) ah[q] = fmaf(s, (float)r0, afr[q]);
+        const uint32_t cb = cbase + (uint32_t)(r0 * FD_PW * 16);
+#pragma unroll
+        for (int r = 0; r < FD_UNR; ++r) {
+          float ksf[FD_M + 1], jm[FD_M + 1];
+#pragma unroll
+          for (int q = 0; q <= FD_M; ++q) {
+            ksf[q] = fmaf(s, (float)r, ah[q]);
+            jm[q] = __fadd_ru(ksf[q], mg[q]);      // ceil(ks) + magic, integer part in the mantissa
+          }
+#pragma unroll
+          for (int q = 0; q < FD_M; ++q) {
+            const float f = sig * ((jm[q] - mg[q]) - ksf[q]);   // t - m of the pixel ceil(ks), in [0, sigma)
+            const float g = 1.f - f;
+            const uint32_t addr = (uint32_t)__float_as_int(jm[q]) * (uint32_t)mul + (cb + r * FD_PW * 16);
+            fd_line<NG>(acc[q], acc[q + 1], jm[q], jm[q + 1], f, g, addr);
+          }
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[st]);
+  }
+
+  // ---- combine the shares through shared memory (the stages are free now) and store -------------
+  __syncthreads();
+  float* lo_s = reinterpret_cast<float*>(buf);                 // [NPJ][NB + 1] lower shares (and complete middle bins)
+  float* up_s = lo_s + FD_NPJ * (FD_NB + 1);                   // [NPJ][NB + 1] upper shares
+#pragma unroll
+  for (int sl = 0; sl < 4 * NG; ++sl) {
+    const int sidx = gA * 4 + sl;
+    if (sidx >= prm.S) break;       // uniform
+    const float a0 = acc[0][sl], a1 = acc[1][sl], a2 = acc[2][sl];
+    // local bin index = bin - mB in [0, NB]
+    lo_s[pj * (FD_NB + 1) + 2 * jp] = a0;
+    lo_s[pj * (FD_NB + 1) + 2 * jp + 1] = a1;
+    up_s[pj * (FD_NB + 1) + 2 * jp + 1] = 0.f;
+    up_s[pj * (FD_NB + 1) + 2 * jp + 2] = a2;
+    __syncthreads();
+    // complete bins: local 1 .. NB - 1
+    for (int e = tid; e < FD_NPJ * (FD_NB - 1); e += FD_NT) {
+      const int q = e / (FD_NB - 1), bl = 1 + e - q * (FD_NB - 1);
+      const int b = mB + bl;
+      if (q < ck.count && b < prm.B) {
+        const int p = sproj[q].p;
+        prm.sino[((int64_t)sidx * prm.P + p) * prm.pitch + b] =
+            prm.scale * (lo_s[q * (FD_NB + 1) + bl] + up_s[q * (FD_NB + 1) + bl]);
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// ---- [S][ny][nx] -> XD, both shears ---------------------------------------------------------------
+// XD[layout][g][w][zpad + k]: one float4 (4 slices of group g) per stored position; line w of layout 0
+// holds the pixels (j = k, i = w - (nx - 1) + k), of layout 1 the pixels (j = k, i = w - k).  Positions
+// that are no pixel (the triangles beside the image, the pads, the spare lines and groups) are zero:
+// they are written once per workspace block and never touched by the repack.
+__global__ void __launch_bounds__(256) repack_diag_kernel(const float* __restrict__ img, int S, int ny, int nx,
+                                                          float4* __restrict__ xd0, float4* __restrict__ xd1,
+                                                          int64_t line_f4, int64_t group_f4, int zpad) {
+  __shared__ float tile[4][32][32];
+  const int g = blockIdx.z;
+  const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+  const int x = threadIdx.x;
+#pragma unroll
+  for (int sl = 0; sl < 4; ++sl) {
+    const int sidx = g * 4 + sl;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+      const int i = by + r, j = bx + x;
+      tile[sl][r][x] = (sidx < S && i < ny && j < nx) ? img[((int64_t)sidx * ny + i) * nx + j] : 0.f;
+    }
+  }
+  __syncthreads();
+  const int j = bx + x;
+  if (j >= nx) return;
+  float4* o0 = xd0 + (int64_t)g * group_f4 + zpad + j;
+  float4* o1 = xd1 + (int64_t)g * group_f4 + zpad + j;
+  // diagonals of the tile: d = i_local - j_local in [-31, 31]; anti-diagonals a = i_local + j_local in [0, 62]
+  for (int d = (int)threadIdx.y - 31; d <= 31; d += blockDim.y) {
+    const int il = x + d;
+    if (il >= 0 && il < 32 && by + il < ny) {
+      const int w = (by + il) - j + (nx - 1);
+      o0[(int64_t)w * line_f4] = make_float4(tile[0][il][x], tile[1][il][x], tile[2][il][x], tile[3][il][x]);
+    }
+  }
+  for (int a = threadIdx.y; a <= 62; a += blockDim.y) {
+    const int il = a - x;
+    if (il >= 0 && il < 32 && by + il < ny) {
+      const int w = (by + il) + j;
+      o1[(int64_t)w * line_f4] = make_float4(tile[0][il][x], tile[1][il][x], tile[2][il][x], tile[3][il][x]);
+    }
+  }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// host: classes, chunks, line ranges and the window width (all in double)
+// ------------------------------------------------------------------------------------------
+namespace {
+
+struct HostProj {
+  FdProj d;
+  int layout, sgn, skew;
+  double a, b, c;      // t = c + a (j - j0) + b (i - i0)
+  double angle;
+};
+
+// range of stored lines w on which the band  tlo <= t <= thi  of projection q meets the image
+// rectangle (widened by one pixel); empty: lo > hi
+void line_range(const HostProj& q, int nx, int ny, double tlo, double thi, double* wlo, double* whi) {
+  const double j0 = 0.5 * (nx - 1), i0 = 0.5 * (ny - 1);
+  const double xl = -1.0, xh = (double)nx, yl = -1.0, yh = (double)ny;   // widened rectangle
+  auto tt = [&](double j, double i) { return q.c + q.a * (j - j0) + q.b * (i - i0); };
+  auto ww = [&](double j, double i) { return q.layout == 0 ? i - j + (double)(nx - 1) : i + j; };
+  double lo = 1e300, hi = -1e300;
+  auto take = [&](double j, double i) {
+    const double w = ww(j, i);
+    lo = std::min(lo, w);
+    hi = std::max(hi, w);
+  };
+  const double cx[4] = {xl, xh, xh, xl}, cy[4] = {yl, yl, yh, yh};
+  for (int v = 0; v < 4; ++v) {
+    const double t = tt(cx[v], cy[v]);
+    if (t >= tlo && t <= thi) take(cx[v], cy[v]);
+  }
+  for (int e = 0; e < 4; ++e) {
+    const double ax = cx[e], ay = cy[e], bx = cx[(e + 1) & 3], by = cy[(e + 1) & 3];
+    const double ta = tt(ax, ay), tb = tt(bx, by);
+    for (double tv : {tlo, thi}) {
+      if ((ta - tv) * (tb - tv) <= 0.0 && ta != tb) {
+        const double u = (tv - ta) / (tb - ta);
+        take(ax + u * (bx - ax), ay + u * (by - ay));
+      }
+    }
+  }
+  *wlo = lo;
+  *whi = hi;
+}
+
+}  // namespace
+
+bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* projs, std::vector<FdChunk>* chunks,
+                     std::vector<int32_t>* ranges, std::vector<int32_t>* legacy) {
+  const int P = g->n_angles, nx = g->nx, ny = g->ny;
+  const double h = g->pixel_size;
+  const double j0 = 0.5 * (nx - 1), i0 = 0.5 * (ny - 1);
+  projs->clear();
+  chunks->clear();
+  ranges->clear();
+  legacy->clear();
+  const int n_bx = (g->n_bins + FD_NB - 2) / (FD_NB - 1);
+  const int n_lines = nx + ny - 1;
+  std::vector<HostProj> cls[12];    // (layout, sgn, skew)
+  for (int p = 0; p < P; ++p) {
+    HostProj q;
+    q.a = h * std::cos(g->angles_rad[p]);
+    q.b = h * std::sin(g->angles_rad[p]);
+    q.c = g->axis_pos[p];
+    q.angle = g->angles_rad[p];
+    q.layout = (q.a * q.b >= 0.0) ? 0 : 1;
+    const double sigma = q.layout == 0 ? q.a + q.b : q.a - q.b;
+    const double as = std::fabs(sigma);
+    // at most one pixel per interval and line, with room for the rounding of the boundaries; and a
+    // window that fits: FD_NB / |sigma| + divergence + skew residue
+    if (!(as >= 1.0 + 1.0 / 4096.0) || as > 8.0) {
+      legacy->push_back(p);
+      continue;
+    }
+    const double T0 = q.layout == 0 ? q.c - q.a * j0 - q.b * ((double)(nx - 1) + i0) : q.c - q.a * j0 - q.b * i0;
+    q.sgn = sigma > 0.0 ? 1 : -1;
+    q.d.inv = 1.0 / as;
+    q.d.K0 = -T0 * q.d.inv;
+    q.d.sD = -q.b * q.d.inv;
+    q.d.s = (float)q.d.sD;
+    q.d.sig = (float)as;
+    q.d.p = p;
+    q.d.pad_ = 0;
+    const double dk = (double)q.sgn * q.d.sD;       // stored positions per line
+    q.skew = dk > 0.5 ? 1 : (dk < -0.5 ? -1 : 0);
+    cls[(q.layout * 2 + (q.sgn > 0 ? 1 : 0)) * 3 + (q.skew + 1)].push_back(q);
+  }
+  plan->n_bx = n_bx;
+  int w_max = 0;
+  // width of the window a set of projections needs for block bx on the band starting at line w0
+  auto width_at = [&](const std::vector<HostProj>& v, size_t i0_, size_t i1_, int bx, double w0) {
+    const int mB = bx * (FD_NB - 1) - 1;
+    double lo = 1e300, hi = -1e300;
+    for (size_t i = i0_; i < i1_; ++i) {
+      const HostProj& q = v[i];
+      for (int mm : {mB, mB + FD_NB})
+        for (int r : {0, FD_RB - 1}) {
+          const double kpos = (double)q.sgn * (q.d.K0 + (double)mm * q.d.inv + q.d.sD * (w0 + r)) - (double)(q.skew * r);
+          lo = std::min(lo, kpos);
+          hi = std::max(hi, kpos);
+        }
+    }
+    return (int)(std::ceil(hi) - (std::floor(lo) - 2.0)) + 3;
+  };
+  for (int c = 0; c < 12; ++c) {
+    std::vector<HostProj>& v = cls[c];
+    if (v.empty()) continue;
+    std::stable_sort(v.begin(), v.end(), [](const HostProj& x, const HostProj& y) { return x.angle < y.angle; });
+    size_t i = 0;
+    while (i < v.size()) {
+      // greedy: add neighbours while the window of every block still fits
+      size_t j = i + 1;
+      std::vector<int32_t> rg_best;
+      int w_best = 0;
+      auto eval = [&](size_t i1_, std::vector<int32_t>* rg_out, int* w_out) {
+        rg_out->assign((size_t)2 * n_bx, 0);
+        int wneed = 0;
+        for (int bx = 0; bx < n_bx; ++bx) {
+          const int mB = bx * (FD_NB - 1) - 1;
+          double lo = 1e300, hi = -1e300;
+          for (size_t t = i; t < i1_; ++t) {
+            double a_, b_;
+            line_range(v[t], nx, ny, (double)mB, (double)(mB + FD_NB), &a_, &b_);
+            lo = std::min(lo, a_);
+            hi = std::max(hi, b_);
+          }
+          int wl = 0, wh = 0;
+          if (lo <= hi) {
+            wl = std::max(0, (int)std::floor(lo) - 1);
+            wh = std::min(n_lines, (int)std::ceil(hi) + 2);
+            if (wh <= wl) wl = wh = 0;
+          }
+          (*rg_out)[2 * bx] = wl;
+          (*rg_out)[2 * bx + 1] = wh;
+          if (wh > wl) {
+            const int nb = (wh - wl + FD_RB - 1) / FD_RB;
+            wneed = std::max(wneed, width_at(v, i, i1_, bx, (double)wl));
+            wneed = std::max(wneed, width_at(v, i, i1_, bx, (double)(wl + (nb - 1) * FD_RB)));
+          }
+        }
+        *w_out = wneed;
+      };
+      eval(j, &rg_best, &w_best);
+      if (w_best > FD_WMAX) {      // one projection alone does not fit: the banded kernel takes it
+        legacy->push_back(v[i].d.p);
+        ++i;
+        continue;
+      }
+      while (j < v.size() && j - i < (size_t)FD_NPJ) {
+        std::vector<int32_t> rg_try;
+        int w_try = 0;
+        eval(j + 1, &rg_try, &w_try);
+        if (w_try > FD_WMAX) break;
+        rg_best.swap(rg_try);
+        w_best = w_try;
+        ++j;
+      }
+      FdChunk ck{};
+      ck.first = (int32_t)projs->size();
+      ck.count = (int32_t)(j - i);
+      ck.layout = v[i].layout;
+      ck.sgn = v[i].sgn;
+      ck.skew = v[i].skew;
+      ck.mul16 = 16 * v[i].sgn;
+      for (size_t t = i; t < j; ++t) projs->push_back(v[t].d);
+      chunks->push_back(ck);
+      ranges->insert(ranges->end(), rg_best.begin(), rg_best.end());
+      w_max = std::max(w_max, w_best);
+      i = j;
+    }
+  }
+  std::sort(legacy->begin(), legacy->end());
+  plan->W = std::max(16, (w_max + 3) & ~3);
+  plan->n_chunks = (int32_t)chunks->size();
+  plan->zpad = FD_WMAX + FD_NB + 2 * FD_RB + 16;
+  plan->n_lines_alloc = n_lines + FD_RB;
+  return plan->n_chunks > 0 && plan->n_chunks <= 65535;
+}
+
+size_t fd_xd_bytes(const FdPlan& plan, const pyhst_geom_t* g, int* n_groups_alloc) {
+  const int ng = (g->n_slices + 3) / 4;
+  const int nga = ng > 1 ? (ng + 1) & ~1 : 1;     // two groups per block: a spare zero group for odd counts
+  if (n_groups_alloc) *n_groups_alloc = nga;
+  const int64_t line_f4 = (int64_t)g->nx + 2 * plan.zpad;
+  return (size_t)2 * nga * plan.n_lines_alloc * line_f4 * 16;
+}
+
+int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch, const pyhst_geom_t* g,
+                                float scale, const FdPlan& plan, cudaStream_t stream) {
+  int nga = 0;
+  const size_t bytes = fd_xd_bytes(plan, g, &nga);
+  const int n_groups = (g->n_slices + 3) / 4;
+  const int64_t line_f4 = (int64_t)g->nx + 2 * plan.zpad;
+  const int64_t group_f4 = line_f4 * plan.n_lines_alloc;
+  void* ws = nullptr;
+  PYHST_TRY(get_workspace(WS_XD, bytes, &ws));
+  float4* xd0 = static_cast<float4*>(ws);
+  float4* xd1 = xd0 + (int64_t)nga * group_f4;
+  // zero positions are written once per (block, layout): see repack_diag_kernel
+  struct Key { size_t k[8]; };
+  static Key seen_all[64];
+  const Key key = {{bytes, (size_t)g->nx, (size_t)g->ny, (size_t)plan.zpad, (size_t)plan.n_lines_alloc, (size_t)nga,
+                    (size_t)workspace_generation(WS_XD), (size_t)reinterpret_cast<uintptr_t>(ws)}};
+  Key& seen = seen_all[std::max(0, current_device()) & 63];
+  {
+    StageScope scope(ST_TRANSPOSE, stream);
+    if (std::memcmp(&seen, &key, sizeof(key)) != 0) {
+      PYHST_CUDA_TRY(cudaMemsetAsync(ws, 0, bytes, stream));
+      seen = key;
+    }
+    dim3 block(32, 8, 1);
+    dim3 grid((g->nx + 31) / 32, (g->ny + 31) / 32, n_groups);
+    if (grid.y > 65535 || grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "image repack: grid too large");
+    scope.kernels();
+    repack_diag_kernel<<<grid, block, 0, stream>>>(d_img, g->n_slices, g->ny, g->nx, xd0, xd1, line_f4, group_f4,
+                                                   plan.zpad);
+    PYHST_CUDA_TRY(cudaGetLastError());
+  }
+  FdParams prm;
+  prm.xd[0] = xd0;
+  prm.xd[1] = xd1;
+  prm.line_f4 = line_f4;
+  prm.group_f4 = group_f4;
+  prm.zpad = plan.zpad;
+  prm.sino = d_sino;
+  prm.pitch = pitch;
+  prm.S = g->n_slices;
+  prm.P = g->n_angles;
+  prm.B = g->n_bins;
+  prm.scale = scale;
+  prm.projs = plan.d_projs;
+  prm.chunks = plan.d_chunks;
+  prm.ranges = reinterpret_cast<const int2*>(plan.d_ranges);
+  prm.n_bx = plan.n_bx;
+  prm.W = plan.W;
+  const bool two = n_groups > 1;
+  static uint64_t configured[2] = {0, 0};
+  if (first_use_on_device(&configured[two ? 1 : 0])) {
+    if (two)
+      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(2)));
+    else
+      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(1)));
+  }
+  dim3 grid(plan.n_bx, plan.n_chunks, two ? nga / 2 : 1);
+  if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
+  StageScope scope(ST_FORWARD, stream);
+  scope.kernels();
+  if (two)
+    fp_diag_kernel<2><<<grid, FD_NT, fd_smem(2), stream>>>(prm);
+  else
+    fp_diag_kernel<1><<<grid, FD_NT, fd_smem(1), stream>>>(prm);
+  PYHST_CUDA_TRY(cudaGetLastError());
+  return PYHST_OK;
+}
+
+}  // namespace pyhst
