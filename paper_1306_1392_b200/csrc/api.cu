@@ -269,7 +269,7 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
   return PYHST_OK;
 }
 
-int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, bool want_diag, const FpPlan** out) {
+int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, int want_diag, const FpPlan** out) {
   DeviceCtx& c = ctx();
   std::lock_guard<std::recursive_mutex> lock(c.mu);
   auto& g_fp_plans = c.fp_plans;
@@ -316,8 +316,18 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, bool want_diag, cons
     std::vector<FdChunk> dchunks;
     std::vector<int32_t> ranges;
     FpPlan probe = pl;
-    if (build_fd_tables(g, &pl.fd, &dprojs, &dchunks, &ranges, &legacy) &&
-        (legacy.empty() || build_fp_tables(g, &probe, &projs, &chunks, &legacy))) {
+    bool use = build_fd_tables(g, &pl.fd, &dprojs, &dchunks, &ranges, &legacy);
+    if (use && want_diag == 1) {
+      // automatic choice: the diagonal-line kernel pays off when its blocks are full (chunks of >= 8
+      // neighbouring projections share a window: dense angle lists) and fill the GPU twice over; sparse
+      // angle lists and small scans stay on the banded kernel
+      const double per_chunk = (double)dprojs.size() / (double)dchunks.size();
+      const int64_t blocks = (int64_t)pl.fd.n_bx * pl.fd.n_chunks * std::max(1, (pl.n_groups + 1) / 2);
+      int n_sm = 148;
+      require_sm100(&n_sm);
+      use = per_chunk >= 8.0 && blocks >= 4 * (int64_t)n_sm;
+    }
+    if (use && (legacy.empty() || build_fp_tables(g, &probe, &projs, &chunks, &legacy))) {
       pl.diag = true;
       pl.n_legacy = (int32_t)legacy.size();
       PYHST_CUDA_TRY(cudaMalloc(&pl.fd.d_projs, dprojs.size() * sizeof(FdProj)));
@@ -647,7 +657,7 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
   PYHST_TRY(get_geom_plan(g, 0.0, g->n_bins, stream, &plan));
   if (g_fp_variant != 1) {
     const FpPlan* fplan = nullptr;
-    PYHST_TRY(get_fp_plan(g, stream, g_fp_variant == 0 || g_fp_variant == 5, &fplan));
+    PYHST_TRY(get_fp_plan(g, stream, g_fp_variant == 5 ? 2 : (g_fp_variant == 0 ? 1 : 0), &fplan));
     if (fplan->diag) {
       PYHST_TRY(launch_forward_project_diag(d_img, d_sino, pitch, g, scale, fplan->fd, stream));
       if (fplan->n_chunks > 0)

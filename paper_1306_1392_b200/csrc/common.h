@@ -215,7 +215,7 @@ struct FpPlan {
   // key
   int32_t n_angles = 0, n_bins = 0, nx = 0, ny = 0, n_groups = 0;
   double pixel_size = 0;
-  bool want_diag = false;
+  int want_diag = 0;
   // diagonal-line kernel: covers every projection except `n_legacy` ones (too close to an image axis,
   // or a window that does not fit), which the banded tables below then hold alone
   bool diag = false;
@@ -223,13 +223,13 @@ struct FpPlan {
   FdPlan fd;
   std::vector<double> angles, axis;
   // product
-  int32_t npj = 0, W = 0, nc = 0, n_chunks = 0;
+  int32_t npj = 0, W = 0, nc = 0, n_chunks = 0, n_tab = 0;   // n_tab: projections in the banded tables
   bool any_rows = false, any_cols = false;
   FpProjD* d_projs = nullptr;
   FpChunk* d_chunks = nullptr;
   uint64_t last_use = 0;
 };
-int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, bool want_diag, const FpPlan** out);  // api.cu
+int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, int want_diag, const FpPlan** out);  // api.cu; want_diag: 0 no, 1 automatic, 2 forced
 // fills the host tables of a plan (for the projections listed in `subset`, all if null); returns false if
 // the banded kernel cannot cover the geometry
 bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* projs,

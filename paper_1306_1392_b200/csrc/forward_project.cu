@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(FB_NT, MINB)
 fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi_cols, XiDims dr,
                XiDims dc, float* __restrict__ sino, int64_t pitch, int S, int P, int B, float scale,
                const FpProjD* __restrict__ projs, const FpChunk* __restrict__ chunks, int W,
-               int n_split, float* __restrict__ part, int64_t part_pitch, int64_t part_stride) {
+               int n_split, float* __restrict__ part, int64_t part_pitch, int64_t part_stride, int n_tab) {
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);        // [2]
   int* sorigin = reinterpret_cast<int*>(smem + 16);          // [2]
@@ -278,22 +278,25 @@ fp_band_kernel(const float4* __restrict__ xi_rows, const float4* __restrict__ xi
         const int s = g * 4 + sl;
         if (s < S) {
           if (!SPLIT || hs == 0) sino[((int64_t)s * P + p) * pitch + b] = scale * acc[m][sl];
-          else part[(int64_t)(hs - 1) * part_stride + ((int64_t)s * P + p) * part_pitch + b] = scale * acc[m][sl];
+          else part[(int64_t)(hs - 1) * part_stride + ((int64_t)s * n_tab + (ck.first + pj)) * part_pitch + b] = scale * acc[m][sl];
         }
       }
     }
   }
 }
 
-// y[row][b] += sum_h part[h][row][b]
+// y[row][b] += sum_h part[h][row][b] for the rows (slice, projection) of the projections in the plan's table
+// (all of them, or the few the diagonal-line kernel leaves to this one)
 __global__ void fp_split_combine_kernel(float* __restrict__ y, int64_t pitch_y, const float* __restrict__ part,
                                         int64_t part_pitch, int64_t part_stride, int n_parts, int B,
-                                        int64_t n_rows) {
+                                        int64_t n_rows_tab, const FpProjD* __restrict__ projs, int n_tab, int P) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
-  const int64_t row = blockIdx.y + (int64_t)blockIdx.z * gridDim.y;
-  if (b >= B || row >= n_rows) return;
+  const int64_t rt = blockIdx.y + (int64_t)blockIdx.z * gridDim.y;
+  if (b >= B || rt >= n_rows_tab) return;
+  const int64_t sl = rt / n_tab;
+  const int64_t row = sl * P + projs[rt - sl * n_tab].p;
   float v = y[row * pitch_y + b];
-  for (int h = 0; h < n_parts; ++h) v += part[(int64_t)h * part_stride + row * part_pitch + b];
+  for (int h = 0; h < n_parts; ++h) v += part[(int64_t)h * part_stride + rt * part_pitch + b];
   y[row * pitch_y + b] = v;
 }
 
@@ -710,6 +713,7 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
     }
   }
   plan->n_chunks = (int32_t)chunks->size();
+  plan->n_tab = (int32_t)projs->size();
   return plan->n_chunks <= 65535;
 }
 
@@ -797,9 +801,8 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
   const int64_t blocks = (int64_t)((g->n_bins + FB_NB - 1) / FB_NB) * plan.n_chunks * n_groups;
   const int64_t slots = (int64_t)n_sm * (four ? 4 : 3);
   const int n_bands_min = (std::min(g->nx, g->ny) + FB_RB - 1) / FB_RB;
-  int n_split = (int)std::max<int64_t>(1, std::min<int64_t>(4, slots / std::max<int64_t>(blocks, 1)));
+  int n_split = (int)std::max<int64_t>(1, std::min<int64_t>(plan.diag ? 8 : 4, slots / std::max<int64_t>(blocks, 1)));
   n_split = std::max(1, std::min(n_split, n_bands_min / 8));
-  if (plan.diag) n_split = 1;   // the tables hold a subset of the projections: the combine pass would touch every row
   static PerDeviceSize configured[5];
   const int vi = four ? 3 : (plan.nc == 3 ? (n_split > 1 ? 4 : 0) : (plan.nc == 4 ? 1 : 2));
   auto kern = four ? fp_band_kernel<3, 4, true>
@@ -811,7 +814,7 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
   }
   const int64_t n_rows = (int64_t)g->n_slices * g->n_angles;
   float* part = nullptr;
-  const int64_t part_pitch = g->n_bins, part_stride = n_rows * part_pitch;
+  const int64_t part_pitch = g->n_bins, part_stride = (int64_t)g->n_slices * plan.n_tab * part_pitch;
   if (n_split > 1) {
     void* wp = nullptr;
     PYHST_TRY(get_workspace(WS_FPL, (size_t)(n_split - 1) * part_stride * 4, &wp));
@@ -823,13 +826,15 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
   scope.kernels(n_split > 1 ? 2 : 1);
   kern<<<grid, FB_NT, smem, stream>>>(xi_r, xi_c, dr, dc, d_sino, pitch, g->n_slices, g->n_angles,
                                       g->n_bins, scale, plan.d_projs, plan.d_chunks, W, n_split, part,
-                                      part_pitch, part_stride);
+                                      part_pitch, part_stride, plan.n_tab);
   PYHST_CUDA_TRY(cudaGetLastError());
   if (n_split > 1) {
-    const unsigned gy = (unsigned)std::min<int64_t>(n_rows, 32768);
-    dim3 grid_c((g->n_bins + 255) / 256, gy, (unsigned)((n_rows + gy - 1) / gy));
+    const int64_t n_rows_tab = (int64_t)g->n_slices * plan.n_tab;
+    const unsigned gy = (unsigned)std::min<int64_t>(n_rows_tab, 32768);
+    dim3 grid_c((g->n_bins + 255) / 256, gy, (unsigned)((n_rows_tab + gy - 1) / gy));
     fp_split_combine_kernel<<<grid_c, 256, 0, stream>>>(d_sino, pitch, part, part_pitch, part_stride,
-                                                        n_split - 1, g->n_bins, n_rows);
+                                                        n_split - 1, g->n_bins, n_rows_tab, plan.d_projs, plan.n_tab,
+                                                        g->n_angles);
   }
   PYHST_CUDA_TRY(cudaGetLastError());
   return PYHST_OK;

@@ -37,14 +37,21 @@ namespace pyhst {
 
 namespace {
 
+#ifndef FD_MIXED
+#define FD_MIXED 0
+#endif
 constexpr int FD_NB = 64;      // intervals per block (FD_NB - 1 complete bins)
 constexpr int FD_NPJ = 16;     // projections per block (at most)
 constexpr int FD_M = 2;        // neighbouring intervals per thread
 constexpr int FD_NT = FD_NB / FD_M * FD_NPJ;   // 512 threads, one (interval pair, projection) each
 constexpr int FD_RB = 8;       // lines per band
 constexpr int FD_UNR = 4;      // lines unrolled together (register budget)
-constexpr int FD_NSTG = 3;     // stages of the band ring
-constexpr int FD_WMAX = 128;   // window capacity (float4 per line)
+constexpr int FD_SB = 4;       // bands per double-precision evaluation of the boundaries
+constexpr int FD_LP = 4;       // projections per warp (lanes of a warp = FD_PPW interval pairs x FD_LP projections)
+constexpr int FD_PPW = 32 / FD_LP;
+constexpr int FD_WPG = FD_NB / FD_M / FD_PPW;   // warps that share a group of FD_LP projections
+constexpr int FD_NSTG = 4;     // stages of the band ring
+constexpr int FD_WMAX = 100;   // window capacity (float4 per line): four stages of two blocks per SM fit in 227 KB
 constexpr int FD_PW = FD_WMAX + FD_RB;   // row pitch of a stage (float4): room for the per-line skew
 constexpr int FD_HDR = 1024;   // mbarriers, origins, FdProj table
 constexpr float FD_MAGIC = 12582912.f;   // 1.5 * 2^23
@@ -67,57 +74,85 @@ struct FdParams {
   int32_t n_bx, W;
 };
 
-// One line of one interval, NG slice groups: predicated on `jlo < jhi` (the interval holds the
-// pixel ceil(ks_lo)), two LDS.128 and 8 NG FFMA.  al / au: accumulators of bins m and m + 1.
+// One line of one interval, NG slice groups: two LDS.128 and 4 NG packed FFMA2 (two slices each).  The
+// accumulators are kept as 64-bit register pairs.  f / g are the weights of the pixel ceil(ks_lo) for
+// bins m + 1 / m, already zeroed when the interval does not hold that pixel (packed instructions cannot
+// be predicated).  An FFMA2 takes one issue slot and holds the FMA pipe for two cycles, so the ALU-pipe
+// and LSU instructions of the line issue in its shadow (profiles/r02_micro.md).
 template <int NG>
-__device__ __forceinline__ void fd_line(float (&al)[4 * NG], float (&au)[4 * NG], float jlo, float jhi,
-                                        float f, float g, uint32_t addr) {
+__device__ __forceinline__ void fd_line(uint64_t (&al)[2 * NG], uint64_t (&au)[2 * NG], float f, float g,
+                                        uint32_t addr) {
   if constexpr (NG == 2) {
+#if FD_MIXED
+    // first slice group packed (FFMA2), second scalar (FFMA on the halves of the 64-bit accumulators):
+    // balances the FMA pipe (an FFMA2 holds it ~3 cycles between scalar FMA-pipe work) against issue slots
     asm volatile("{\n\t"
-        ".reg .pred p;\n\t"
-        ".reg .f32 v<8>;\n\t"
-        "setp.lt.f32 p, %16, %17;\n\t"
-        "ld.shared.v4.f32 {v0, v1, v2, v3}, [%20];\n\t"
-        "ld.shared.v4.f32 {v4, v5, v6, v7}, [%20+%21];\n\t"
-        "@p fma.rn.f32 %0, %19, v0, %0;\n\t"
-        "@p fma.rn.f32 %1, %19, v1, %1;\n\t"
-        "@p fma.rn.f32 %2, %19, v2, %2;\n\t"
-        "@p fma.rn.f32 %3, %19, v3, %3;\n\t"
-        "@p fma.rn.f32 %8, %18, v0, %8;\n\t"
-        "@p fma.rn.f32 %9, %18, v1, %9;\n\t"
-        "@p fma.rn.f32 %10, %18, v2, %10;\n\t"
-        "@p fma.rn.f32 %11, %18, v3, %11;\n\t"
-        "@p fma.rn.f32 %4, %19, v4, %4;\n\t"
-        "@p fma.rn.f32 %5, %19, v5, %5;\n\t"
-        "@p fma.rn.f32 %6, %19, v6, %6;\n\t"
-        "@p fma.rn.f32 %7, %19, v7, %7;\n\t"
-        "@p fma.rn.f32 %12, %18, v4, %12;\n\t"
-        "@p fma.rn.f32 %13, %18, v5, %13;\n\t"
-        "@p fma.rn.f32 %14, %18, v6, %14;\n\t"
-        "@p fma.rn.f32 %15, %18, v7, %15;\n\t"
+        ".reg .b64 v<2>, wf, wg;\n\t"
+        ".reg .f32 x<4>, a<8>;\n\t"
+        "ld.shared.v2.b64 {v0, v1}, [%10];\n\t"
+        "ld.shared.v4.f32 {x0, x1, x2, x3}, [%10+%11];\n\t"
+        "mov.b64 wf, {%8, %8};\n\t"
+        "mov.b64 wg, {%9, %9};\n\t"
+        "mov.b64 {a0, a1}, %2;\n\t"
+        "mov.b64 {a2, a3}, %3;\n\t"
+        "mov.b64 {a4, a5}, %6;\n\t"
+        "mov.b64 {a6, a7}, %7;\n\t"
+        "fma.rn.f32x2 %0, v0, wg, %0;\n\t"
+        "fma.rn.f32x2 %1, v1, wg, %1;\n\t"
+        "fma.rn.f32x2 %4, v0, wf, %4;\n\t"
+        "fma.rn.f32x2 %5, v1, wf, %5;\n\t"
+        "fma.rn.f32 a0, x0, %9, a0;\n\t"
+        "fma.rn.f32 a1, x1, %9, a1;\n\t"
+        "fma.rn.f32 a2, x2, %9, a2;\n\t"
+        "fma.rn.f32 a3, x3, %9, a3;\n\t"
+        "fma.rn.f32 a4, x0, %8, a4;\n\t"
+        "fma.rn.f32 a5, x1, %8, a5;\n\t"
+        "fma.rn.f32 a6, x2, %8, a6;\n\t"
+        "fma.rn.f32 a7, x3, %8, a7;\n\t"
+        "mov.b64 %2, {a0, a1};\n\t"
+        "mov.b64 %3, {a2, a3};\n\t"
+        "mov.b64 %6, {a4, a5};\n\t"
+        "mov.b64 %7, {a6, a7};\n\t"
         "}"
-        : "+f"(al[0]), "+f"(al[1]), "+f"(al[2]), "+f"(al[3]), "+f"(al[4]), "+f"(al[5]), "+f"(al[6]), "+f"(al[7]),
-          "+f"(au[0]), "+f"(au[1]), "+f"(au[2]), "+f"(au[3]), "+f"(au[4]), "+f"(au[5]), "+f"(au[6]), "+f"(au[7])
-        : "f"(jlo), "f"(jhi), "f"(f), "f"(g), "r"(addr), "n"(FD_RB * FD_PW * 16));
+        : "+l"(al[0]), "+l"(al[1]), "+l"(al[2]), "+l"(al[3]), "+l"(au[0]), "+l"(au[1]), "+l"(au[2]), "+l"(au[3])
+        : "f"(f), "f"(g), "r"(addr), "n"(FD_RB * FD_PW * 16));
+#else
+    asm volatile("{\n\t"
+        ".reg .b64 v<4>, wf, wg;\n\t"
+        "ld.shared.v2.b64 {v0, v1}, [%10];\n\t"
+        "ld.shared.v2.b64 {v2, v3}, [%10+%11];\n\t"
+        "mov.b64 wf, {%8, %8};\n\t"
+        "mov.b64 wg, {%9, %9};\n\t"
+        "fma.rn.f32x2 %0, v0, wg, %0;\n\t"
+        "fma.rn.f32x2 %1, v1, wg, %1;\n\t"
+        "fma.rn.f32x2 %4, v0, wf, %4;\n\t"
+        "fma.rn.f32x2 %5, v1, wf, %5;\n\t"
+        "fma.rn.f32x2 %2, v2, wg, %2;\n\t"
+        "fma.rn.f32x2 %3, v3, wg, %3;\n\t"
+        "fma.rn.f32x2 %6, v2, wf, %6;\n\t"
+        "fma.rn.f32x2 %7, v3, wf, %7;\n\t"
+        "}"
+        : "+l"(al[0]), "+l"(al[1]), "+l"(al[2]), "+l"(al[3]), "+l"(au[0]), "+l"(au[1]), "+l"(au[2]), "+l"(au[3])
+        : "f"(f), "f"(g), "r"(addr), "n"(FD_RB * FD_PW * 16));
+#endif
   } else {
     asm volatile("{\n\t"
-        ".reg .pred p;\n\t"
-        ".reg .f32 v<4>;\n\t"
-        "setp.lt.f32 p, %8, %9;\n\t"
-        "ld.shared.v4.f32 {v0, v1, v2, v3}, [%12];\n\t"
-        "@p fma.rn.f32 %0, %11, v0, %0;\n\t"
-        "@p fma.rn.f32 %1, %11, v1, %1;\n\t"
-        "@p fma.rn.f32 %2, %11, v2, %2;\n\t"
-        "@p fma.rn.f32 %3, %11, v3, %3;\n\t"
-        "@p fma.rn.f32 %4, %10, v0, %4;\n\t"
-        "@p fma.rn.f32 %5, %10, v1, %5;\n\t"
-        "@p fma.rn.f32 %6, %10, v2, %6;\n\t"
-        "@p fma.rn.f32 %7, %10, v3, %7;\n\t"
+        ".reg .b64 v<2>, wf, wg;\n\t"
+        "ld.shared.v2.b64 {v0, v1}, [%6];\n\t"
+        "mov.b64 wf, {%4, %4};\n\t"
+        "mov.b64 wg, {%5, %5};\n\t"
+        "fma.rn.f32x2 %0, v0, wg, %0;\n\t"
+        "fma.rn.f32x2 %1, v1, wg, %1;\n\t"
+        "fma.rn.f32x2 %2, v0, wf, %2;\n\t"
+        "fma.rn.f32x2 %3, v1, wf, %3;\n\t"
         "}"
-        : "+f"(al[0]), "+f"(al[1]), "+f"(al[2]), "+f"(al[3]), "+f"(au[0]), "+f"(au[1]), "+f"(au[2]), "+f"(au[3])
-        : "f"(jlo), "f"(jhi), "f"(f), "f"(g), "r"(addr));
+        : "+l"(al[0]), "+l"(al[1]), "+l"(au[0]), "+l"(au[1])
+        : "f"(f), "f"(g), "r"(addr));
   }
 }
+
+__device__ __forceinline__ float fd_lo(uint64_t v) { return __uint_as_float((uint32_t)v); }
+__device__ __forceinline__ float fd_hi(uint64_t v) { return __uint_as_float((uint32_t)(v >> 32)); }
 
 template <int NG>
 __global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
@@ -189,44 +224,51 @@ __global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
 
   if (warp == 0 && n_bands > 0) produce(0);
   if (warp == 1 && n_bands > 1) produce(1);
+  if (warp == 2 && n_bands > 2) produce(2);
 
   // bins mB + 2 jp + {0, 1, 2}: lower share of the first interval, both shares of the middle bin,
   // upper share of the second interval
-  float acc[FD_M + 1][4 * NG];
+  uint64_t acc[FD_M + 1][2 * NG];       // pairs of slices
 #pragma unroll
   for (int q = 0; q <= FD_M; ++q)
 #pragma unroll
-    for (int sl = 0; sl < 4 * NG; ++sl) acc[q][sl] = 0.f;
+    for (int sl = 0; sl < 2 * NG; ++sl) acc[q][sl] = 0ull;
 
   // a warp = 8 interval pairs x 4 projections: its 32 pixels of a line lie within ~16 stored
   // positions, i.e. the LDS.128 touches <= 256 B (2.4 cycles instead of 4, profiles/r02_micro.md)
-  const int jp = (warp & 3) * 8 + (lane >> 2);
-  const int pj = (warp >> 2) * 4 + (lane & 3);
+  const int jp = (warp % FD_WPG) * FD_PPW + lane / FD_LP;
+  const int pj = (warp / FD_WPG) * FD_LP + lane % FD_LP;
   const bool active = pj < ck.count;
   const int m0 = mB + FD_M * jp;
   const float s = active ? sproj[pj].s : 0.f;
   const float sig = active ? sproj[pj].sig : 1.f;
   const int mul = ck.mul16;                    // sgn * 16 (from the table: one IMAD per address)
 
+  float afr[FD_M + 1], mg[FD_M + 1];
+#pragma unroll
+  for (int q = 0; q <= FD_M; ++q) afr[q] = mg[q] = 0.f;
+
   for (int k = 0; k < n_bands; ++k) {
-    if (k + 2 < n_bands && warp == ((k + 2) & 15)) produce(k + 2);
     const int st = k % FD_NSTG;
     mbar_wait(&full[st], (uint32_t)((k / FD_NSTG) & 1));
     if (active) {
       const int origin = sorigin[st];
-      const double w0 = (double)(rg.x + k * FD_RB);
-      const FdProj* sp = &sproj[pj];
-      const double K0 = sp->K0, inv = sp->inv, sD = sp->sD;
-      float afr[FD_M + 1], mg[FD_M + 1];
+      const int kk = k % FD_SB;
+      if (kk == 0) {
+        // every FD_SB bands: the boundaries' positions on the band's first line (double), split into an
+        // integer and a fraction; the thread that shares a boundary evaluates the identical expression
+        const double w0 = (double)(rg.x + k * FD_RB);
+        const FdProj* sp = &sproj[pj];
+        const double K0 = sp->K0, inv = sp->inv, sD = sp->sD;
 #pragma unroll
-      for (int q = 0; q <= FD_M; ++q) {
-        // the boundary's position on the band's first line (double), split; the thread that
-        // shares the boundary evaluates the identical expression
-        const double ks = fma(sD, w0, fma((double)(m0 + q), inv, K0));
-        const double ai = rint(ks);
-        afr[q] = (float)(ks - ai);
-        mg[q] = (float)ai + FD_MAGIC;     // exact: |ai| < 2^22
+        for (int q = 0; q <= FD_M; ++q) {
+          const double ks = fma(sD, w0, fma((double)(m0 + q), inv, K0));
+          const double ai = rint(ks);
+          afr[q] = (float)(ks - ai);
+          mg[q] = (float)ai + FD_MAGIC;     // exact: |ai| < 2^22
+        }
       }
+      const float rk = (float)(kk * FD_RB);
       // byte address of stored position k = sgn * kappa on line 0:  (bias + k - origin) * 16, with
       // kappa = float_as_int(jm) - 0x4b400000
       const uint32_t cbase = smem_u32(buf + st * STAGE_F4) + (uint32_t)((bias - origin) * 16) -
@@ -235,7 +277,7 @@ __global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
       for (int r0 = 0; r0 < FD_RB; r0 += FD_UNR) {
         float ah[FD_M + 1];
 #pragma unroll
-        for (int q = 0; q <= FD_M; ++q) ah[q] = fmaf(s, (float)r0, afr[q]);
+        for (int q = 0; q <= FD_M; ++q) ah[q] = fmaf(s, rk + (float)r0, afr[q]);
         const uint32_t cb = cbase + (uint32_t)(r0 * FD_PW * 16);
 #pragma unroll
         for (int r = 0; r < FD_UNR; ++r) {
@@ -249,14 +291,19 @@ __global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
           for (int q = 0; q < FD_M; ++q) {
             const float f = sig * ((jm[q] - mg[q]) - ksf[q]);   // t - m of the pixel ceil(ks), in [0, sigma)
             const float g = 1.f - f;
-            const uint32_t addr = (uint32_t)__float_as_int(jm[q]) * (uint32_t)mul + (cb + r * FD_PW * 16);
-            fd_line<NG>(acc[q], acc[q + 1], jm[q], jm[q + 1], f, g, addr);
+            const bool in = jm[q] < jm[q + 1];                  // the interval holds that pixel
+            uint32_t addr;
+            asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(addr) : "r"(__float_as_int(jm[q])), "r"(mul), "r"(cb + r * FD_PW * 16));
+            fd_line<NG>(acc[q], acc[q + 1], in ? f : 0.f, in ? g : 0.f, addr);
           }
         }
       }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[st]);
+    // the producer role rotates; a warp produces AFTER its own share of band k, into the stage of band
+    // k - 1, which the other warps have normally left by then: it does not become the straggler
+    if (k + FD_NSTG - 1 < n_bands && warp == (k & 15)) produce(k + FD_NSTG - 1);
   }
 
   // ---- combine the shares through shared memory (the stages are free now) and store -------------
@@ -267,7 +314,9 @@ __global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
   for (int sl = 0; sl < 4 * NG; ++sl) {
     const int sidx = gA * 4 + sl;
     if (sidx >= prm.S) break;       // uniform
-    const float a0 = acc[0][sl], a1 = acc[1][sl], a2 = acc[2][sl];
+    const float a0 = (sl & 1) ? fd_hi(acc[0][sl >> 1]) : fd_lo(acc[0][sl >> 1]);
+    const float a1 = (sl & 1) ? fd_hi(acc[1][sl >> 1]) : fd_lo(acc[1][sl >> 1]);
+    const float a2 = (sl & 1) ? fd_hi(acc[2][sl >> 1]) : fd_lo(acc[2][sl >> 1]);
     // local bin index = bin - mB in [0, NB]
     lo_s[pj * (FD_NB + 1) + 2 * jp] = a0;
     lo_s[pj * (FD_NB + 1) + 2 * jp + 1] = a1;
