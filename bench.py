@@ -297,7 +297,7 @@ def run_b200(args):
                           % (n_sm, f_max / 1e6, peaks_kind)}
         if clocks.get("sm_mhz"):
             r["frac_at_sampled_clock"] = r["frac"] * (f_max / 1e6) / clocks["sm_mhz"]
-        tr = _traffic().get(stage)
+        tr = _traffic().get("config%d" % w.cfg, {}).get(stage) if not args.slices else None
         if tr is not None:
             r["traffic"] = tr
             r["traffic_source"] = "stored: " + str(_traffic().get("_source", "profiles/traffic.json (ncu --set full capture)"))
@@ -305,7 +305,10 @@ def run_b200(args):
 
     calls = n_fista if fista else 1
     r_bp = kernel_roofline("backproject", "bp_run8_kernel<0> + bp_run8_kernel<1>", executed=bp_exec, calls_per_step=calls)
-    r_fp = kernel_roofline("forward_project", "fp_band_kernel", calls_per_step=calls)
+    fp_names = {1: "fp_gather_kernel", 2: "fp_band_kernel", 3: "fp_ivl_kernel", 4: "fp_ivl_kernel (8 slices)",
+                5: "fp_diag_kernel (+ fp_band_kernel for the projections within 2^-12 of an image axis)"}
+    r_fp = kernel_roofline("forward_project", fp_names.get(P.last_forward_project_kernel(), "forward projector"),
+                           calls_per_step=calls)
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     ms_bp = stages["backproject"][0] / args.steps
     ms_fp = (stages["forward_project"][0] + stages["transpose"][0]) / args.steps
@@ -317,7 +320,9 @@ def run_b200(args):
         fbytes = 4.0 * S * NP * (B + (B if w.mode != 2 else P.halfacq_extent(B, float(w.axis.mean()))[0]))
         others.append({"kernel": "ramp filter (a1)", "bound": "hbm", "achieved": fbytes / (ms_filter * 1e-3) / 1e9,
                        "peak": hbm, "unit": "GB/s", "frac": fbytes / (ms_filter * 1e-3) / 1e9 / hbm,
-                       "traffic": None, "avg_ms": ms_filter, "bytes_per_launch": fbytes,
+                       "traffic": _traffic().get("config%d" % w.cfg, {}).get("ramp_filter") if not args.slices else None,
+                       "traffic_source": "stored: " + str(_traffic().get("_source", "")),
+                       "avg_ms": ms_filter, "bytes_per_launch": fbytes,
                        "peak_note": "hbm_gbs of MEASURED_PEAKS.json (%s); algorithmic bytes = 4 (B_in + B_out) per row" % peaks_kind})
     if fista and ms_tv > 0:
         # N1: the dual steps dominate the solver's own kernels; algorithmic bytes of ONE dual step =

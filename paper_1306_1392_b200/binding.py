@@ -27,7 +27,7 @@ _LIBNAME = "libpyhst_b200.so"
 # every symbol include/*.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
            "pyhst_fista_tv", "pyhst_ista_tv", "pyhst_ring_filter", "pyhst_ecohe", "pyhst_cv_distance", "pyhst_patch_grid",
-           "pyhst_patch_gradient", "pyhst_patch_fista", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_set_halfacq_stitch", "pyhst_set_filter_variant", "pyhst_set_patch_gemm_variant",
+           "pyhst_patch_gradient", "pyhst_patch_fista", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_last_forward_project_kernel", "pyhst_set_halfacq_stitch", "pyhst_set_filter_variant", "pyhst_set_patch_gemm_variant",
            "pyhst_last_error", "pyhst_release_cache")
 
 
@@ -378,6 +378,10 @@ def set_patch_gemm_variant(variant: int) -> int:
 
 def set_forward_project_variant(variant: int) -> int:
     return int(_load().pyhst_set_forward_project_variant(int(variant)))
+
+
+def last_forward_project_kernel() -> int:
+    return int(_load().pyhst_last_forward_project_kernel())
 
 
 STAGES = ("ramp_filter", "repack", "backproject", "transpose", "forward_project", "tv_solver")

@@ -75,6 +75,7 @@ std::mutex g_map_mu;
 std::map<int, std::unique_ptr<DeviceCtx>> g_ctx;
 int g_bp_variant = 0;
 int g_fp_variant = 0;
+int g_last_fp_kernel = 0;
 int g_halfacq_stitch = 1;
 int g_filter_variant = 0;
 int g_patch_gemm_variant = 0;
@@ -521,6 +522,8 @@ int pyhst_set_forward_project_variant(int variant) {
   return prev;
 }
 
+int pyhst_last_forward_project_kernel(void) { return g_last_fp_kernel; }
+
 void pyhst_release_cache(void) {
   int prev = current_device();
   std::vector<DeviceCtx*> all;
@@ -659,6 +662,7 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
     const FpPlan* fplan = nullptr;
     PYHST_TRY(get_fp_plan(g, stream, g_fp_variant == 5 ? 2 : (g_fp_variant == 0 ? 1 : 0), &fplan));
     if (fplan->diag) {
+      g_last_fp_kernel = 5;
       PYHST_TRY(launch_forward_project_diag(d_img, d_sino, pitch, g, scale, fplan->fd, stream));
       if (fplan->n_chunks > 0)
         return launch_forward_project_banded(d_img, d_sino, pitch, g, scale, *fplan, 0, stream);
@@ -666,12 +670,15 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
     }
     if (g_fp_variant == 5)
       return set_error(PYHST_ERR_UNSUPPORTED, "diagonal-line forward projector does not cover this geometry");
-    if (fplan->n_chunks > 0)
+    if (fplan->n_chunks > 0) {
+      g_last_fp_kernel = g_fp_variant == 3 || g_fp_variant == 4 ? g_fp_variant : 2;
       return launch_forward_project_banded(d_img, d_sino, pitch, g, scale, *fplan, g_fp_variant == 3 ? 1 : (g_fp_variant == 4 ? 2 : 0), stream);
+    }
     if (g_fp_variant == 2)
       return set_error(PYHST_ERR_UNSUPPORTED, "banded forward projector does not cover pixel_size %g",
                        g->pixel_size);
   }
+  g_last_fp_kernel = 1;
   void* img_t = nullptr;
   PYHST_TRY(get_workspace(WS_IMG_T, (size_t)g->n_slices * g->nx * g->ny * 4, &img_t));
   PYHST_TRY(launch_transpose_images(d_img, static_cast<float*>(img_t), g->n_slices, g->ny, g->nx,

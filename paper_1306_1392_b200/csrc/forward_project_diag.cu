@@ -37,15 +37,21 @@ namespace pyhst {
 
 namespace {
 
-#ifndef FD_MIXED
-#define FD_MIXED 0
+#ifndef FD_PACKED
+#define FD_PACKED 0
+#endif
+#ifndef FD_NG4
+#define FD_NG4 1
 #endif
 constexpr int FD_NB = 64;      // intervals per block (FD_NB - 1 complete bins)
 constexpr int FD_NPJ = 16;     // projections per block (at most)
 constexpr int FD_M = 2;        // neighbouring intervals per thread
 constexpr int FD_NT = FD_NB / FD_M * FD_NPJ;   // 512 threads, one (interval pair, projection) each
 constexpr int FD_RB = 8;       // lines per band
-constexpr int FD_UNR = 4;      // lines unrolled together (register budget)
+#ifndef FD_UNR_
+#define FD_UNR_ 4
+#endif
+constexpr int FD_UNR = FD_UNR_;   // lines unrolled together (register budget)
 constexpr int FD_SB = 4;       // bands per double-precision evaluation of the boundaries
 constexpr int FD_LP = 4;       // projections per warp (lanes of a warp = FD_PPW interval pairs x FD_LP projections)
 constexpr int FD_PPW = 32 / FD_LP;
@@ -80,43 +86,8 @@ struct FdParams {
 // be predicated).  An FFMA2 takes one issue slot and holds the FMA pipe for two cycles, so the ALU-pipe
 // and LSU instructions of the line issue in its shadow (profiles/r02_micro.md).
 template <int NG>
-__device__ __forceinline__ void fd_line(uint64_t (&al)[2 * NG], uint64_t (&au)[2 * NG], float f, float g,
-                                        uint32_t addr) {
-  if constexpr (NG == 2) {
-#if FD_MIXED
-    // first slice group packed (FFMA2), second scalar (FFMA on the halves of the 64-bit accumulators):
-    // balances the FMA pipe (an FFMA2 holds it ~3 cycles between scalar FMA-pipe work) against issue slots
-    asm volatile("{\n\t"
-        ".reg .b64 v<2>, wf, wg;\n\t"
-        ".reg .f32 x<4>, a<8>;\n\t"
-        "ld.shared.v2.b64 {v0, v1}, [%10];\n\t"
-        "ld.shared.v4.f32 {x0, x1, x2, x3}, [%10+%11];\n\t"
-        "mov.b64 wf, {%8, %8};\n\t"
-        "mov.b64 wg, {%9, %9};\n\t"
-        "mov.b64 {a0, a1}, %2;\n\t"
-        "mov.b64 {a2, a3}, %3;\n\t"
-        "mov.b64 {a4, a5}, %6;\n\t"
-        "mov.b64 {a6, a7}, %7;\n\t"
-        "fma.rn.f32x2 %0, v0, wg, %0;\n\t"
-        "fma.rn.f32x2 %1, v1, wg, %1;\n\t"
-        "fma.rn.f32x2 %4, v0, wf, %4;\n\t"
-        "fma.rn.f32x2 %5, v1, wf, %5;\n\t"
-        "fma.rn.f32 a0, x0, %9, a0;\n\t"
-        "fma.rn.f32 a1, x1, %9, a1;\n\t"
-        "fma.rn.f32 a2, x2, %9, a2;\n\t"
-        "fma.rn.f32 a3, x3, %9, a3;\n\t"
-        "fma.rn.f32 a4, x0, %8, a4;\n\t"
-        "fma.rn.f32 a5, x1, %8, a5;\n\t"
-        "fma.rn.f32 a6, x2, %8, a6;\n\t"
-        "fma.rn.f32 a7, x3, %8, a7;\n\t"
-        "mov.b64 %2, {a0, a1};\n\t"
-        "mov.b64 %3, {a2, a3};\n\t"
-        "mov.b64 %6, {a4, a5};\n\t"
-        "mov.b64 %7, {a6, a7};\n\t"
-        "}"
-        : "+l"(al[0]), "+l"(al[1]), "+l"(al[2]), "+l"(al[3]), "+l"(au[0]), "+l"(au[1]), "+l"(au[2]), "+l"(au[3])
-        : "f"(f), "f"(g), "r"(addr), "n"(FD_RB * FD_PW * 16));
-#else
+__device__ __forceinline__ void fd_line(uint64_t* al, uint64_t* au, float f, float g, uint32_t addr) {
+  if constexpr (NG >= 2) {
     asm volatile("{\n\t"
         ".reg .b64 v<4>, wf, wg;\n\t"
         "ld.shared.v2.b64 {v0, v1}, [%10];\n\t"
@@ -134,7 +105,6 @@ __device__ __forceinline__ void fd_line(uint64_t (&al)[2 * NG], uint64_t (&au)[2
         "}"
         : "+l"(al[0]), "+l"(al[1]), "+l"(al[2]), "+l"(al[3]), "+l"(au[0]), "+l"(au[1]), "+l"(au[2]), "+l"(au[3])
         : "f"(f), "f"(g), "r"(addr), "n"(FD_RB * FD_PW * 16));
-#endif
   } else {
     asm volatile("{\n\t"
         ".reg .b64 v<2>, wf, wg;\n\t"
@@ -151,11 +121,51 @@ __device__ __forceinline__ void fd_line(uint64_t (&al)[2 * NG], uint64_t (&au)[2
   }
 }
 
+#if !FD_PACKED
+__device__ __forceinline__ void fd_line_s1(float (&al)[4], float (&au)[4], float f, float g, uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  al[0] = fmaf(g, v.x, al[0]); al[1] = fmaf(g, v.y, al[1]); al[2] = fmaf(g, v.z, al[2]); al[3] = fmaf(g, v.w, al[3]);
+  au[0] = fmaf(f, v.x, au[0]); au[1] = fmaf(f, v.y, au[1]); au[2] = fmaf(f, v.z, au[2]); au[3] = fmaf(f, v.w, au[3]);
+}
+// scalar form: predicated FFMA on float accumulators (one issue slot each; the kernel is then bound by
+// issue slots instead of the FMA pipe -- measured within 2 % of the packed form)
+__device__ __forceinline__ void fd_line_s(float* al, float* au, float jlo, float jhi, float f, float g,
+                                          uint32_t addr) {
+  asm volatile("{\n\t"
+      ".reg .pred p;\n\t"
+      ".reg .f32 v<8>;\n\t"
+      "setp.lt.f32 p, %16, %17;\n\t"
+      "ld.shared.v4.f32 {v0, v1, v2, v3}, [%20];\n\t"
+      "ld.shared.v4.f32 {v4, v5, v6, v7}, [%20+%21];\n\t"
+      "@p fma.rn.f32 %0, %19, v0, %0;\n\t"
+      "@p fma.rn.f32 %1, %19, v1, %1;\n\t"
+      "@p fma.rn.f32 %2, %19, v2, %2;\n\t"
+      "@p fma.rn.f32 %3, %19, v3, %3;\n\t"
+      "@p fma.rn.f32 %8, %18, v0, %8;\n\t"
+      "@p fma.rn.f32 %9, %18, v1, %9;\n\t"
+      "@p fma.rn.f32 %10, %18, v2, %10;\n\t"
+      "@p fma.rn.f32 %11, %18, v3, %11;\n\t"
+      "@p fma.rn.f32 %4, %19, v4, %4;\n\t"
+      "@p fma.rn.f32 %5, %19, v5, %5;\n\t"
+      "@p fma.rn.f32 %6, %19, v6, %6;\n\t"
+      "@p fma.rn.f32 %7, %19, v7, %7;\n\t"
+      "@p fma.rn.f32 %12, %18, v4, %12;\n\t"
+      "@p fma.rn.f32 %13, %18, v5, %13;\n\t"
+      "@p fma.rn.f32 %14, %18, v6, %14;\n\t"
+      "@p fma.rn.f32 %15, %18, v7, %15;\n\t"
+      "}"
+      : "+f"(al[0]), "+f"(al[1]), "+f"(al[2]), "+f"(al[3]), "+f"(al[4]), "+f"(al[5]), "+f"(al[6]), "+f"(al[7]),
+        "+f"(au[0]), "+f"(au[1]), "+f"(au[2]), "+f"(au[3]), "+f"(au[4]), "+f"(au[5]), "+f"(au[6]), "+f"(au[7])
+      : "f"(jlo), "f"(jhi), "f"(f), "f"(g), "r"(addr), "n"(FD_RB * FD_PW * 16));
+}
+#endif
+
 __device__ __forceinline__ float fd_lo(uint64_t v) { return __uint_as_float((uint32_t)v); }
 __device__ __forceinline__ float fd_hi(uint64_t v) { return __uint_as_float((uint32_t)(v >> 32)); }
 
 template <int NG>
-__global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
+__global__ void __launch_bounds__(FD_NT, NG == 4 ? 1 : 2) fp_diag_kernel(const FdParams prm) {
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);              // [NSTG]
   uint64_t* empty = reinterpret_cast<uint64_t*>(smem + 32);        // [NSTG]
@@ -228,11 +238,19 @@ __global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
 
   // bins mB + 2 jp + {0, 1, 2}: lower share of the first interval, both shares of the middle bin,
   // upper share of the second interval
+#if FD_PACKED
   uint64_t acc[FD_M + 1][2 * NG];       // pairs of slices
 #pragma unroll
   for (int q = 0; q <= FD_M; ++q)
 #pragma unroll
     for (int sl = 0; sl < 2 * NG; ++sl) acc[q][sl] = 0ull;
+#else
+  float acc[FD_M + 1][4 * NG];
+#pragma unroll
+  for (int q = 0; q <= FD_M; ++q)
+#pragma unroll
+    for (int sl = 0; sl < 4 * NG; ++sl) acc[q][sl] = 0.f;
+#endif
 
   // a warp = 8 interval pairs x 4 projections: its 32 pixels of a line lie within ~16 stored
   // positions, i.e. the LDS.128 touches <= 256 B (2.4 cycles instead of 4, profiles/r02_micro.md)
@@ -247,14 +265,15 @@ __global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
   float afr[FD_M + 1], mg[FD_M + 1];
 #pragma unroll
   for (int q = 0; q <= FD_M; ++q) afr[q] = mg[q] = 0.f;
+  const uint32_t buf_u32 = smem_u32(buf);
+  const uint32_t magic_off = (uint32_t)mul * 0x4b400000u;
 
   for (int k = 0; k < n_bands; ++k) {
     const int st = k % FD_NSTG;
     mbar_wait(&full[st], (uint32_t)((k / FD_NSTG) & 1));
     if (active) {
       const int origin = sorigin[st];
-      const int kk = k % FD_SB;
-      if (kk == 0) {
+      if ((k % FD_SB) == 0) {
         // every FD_SB bands: the boundaries' positions on the band's first line (double), split into an
         // integer and a fraction; the thread that shares a boundary evaluates the identical expression
         const double w0 = (double)(rg.x + k * FD_RB);
@@ -268,23 +287,19 @@ __global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
           mg[q] = (float)ai + FD_MAGIC;     // exact: |ai| < 2^22
         }
       }
-      const float rk = (float)(kk * FD_RB);
       // byte address of stored position k = sgn * kappa on line 0:  (bias + k - origin) * 16, with
       // kappa = float_as_int(jm) - 0x4b400000
-      const uint32_t cbase = smem_u32(buf + st * STAGE_F4) + (uint32_t)((bias - origin) * 16) -
-                             (uint32_t)mul * 0x4b400000u;
+      const uint32_t cbase = buf_u32 + (uint32_t)(st * STAGE_F4 * 16) + (uint32_t)((bias - origin) * 16) - magic_off;
 #pragma unroll 1
       for (int r0 = 0; r0 < FD_RB; r0 += FD_UNR) {
-        float ah[FD_M + 1];
-#pragma unroll
-        for (int q = 0; q <= FD_M; ++q) ah[q] = fmaf(s, rk + (float)r0, afr[q]);
         const uint32_t cb = cbase + (uint32_t)(r0 * FD_PW * 16);
+        {
 #pragma unroll
         for (int r = 0; r < FD_UNR; ++r) {
           float ksf[FD_M + 1], jm[FD_M + 1];
 #pragma unroll
           for (int q = 0; q <= FD_M; ++q) {
-            ksf[q] = fmaf(s, (float)r, ah[q]);
+            ksf[q] = fmaf(s, (float)r, afr[q]);
             jm[q] = __fadd_ru(ksf[q], mg[q]);      // ceil(ks) + magic, integer part in the mantissa
           }
 #pragma unroll
@@ -294,9 +309,25 @@ __global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
             const bool in = jm[q] < jm[q + 1];                  // the interval holds that pixel
             uint32_t addr;
             asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(addr) : "r"(__float_as_int(jm[q])), "r"(mul), "r"(cb + r * FD_PW * 16));
-            fd_line<NG>(acc[q], acc[q + 1], in ? f : 0.f, in ? g : 0.f, addr);
+#if FD_PACKED
+            const float fz = in ? f : 0.f, gz = in ? g : 0.f;
+            fd_line<NG>(acc[q], acc[q + 1], fz, gz, addr);
+            if constexpr (NG == 4) fd_line<NG>(acc[q] + 4, acc[q + 1] + 4, fz, gz, addr + 2 * FD_RB * FD_PW * 16);
+#else
+            if constexpr (NG >= 2) {
+              fd_line_s(acc[q], acc[q + 1], jm[q], jm[q + 1], f, g, addr);
+              if constexpr (NG == 4) fd_line_s(acc[q] + 8, acc[q + 1] + 8, jm[q], jm[q + 1], f, g, addr + 2 * FD_RB * FD_PW * 16);
+            } else {
+              fd_line_s1(acc[q], acc[q + 1], in ? f : 0.f, in ? g : 0.f, addr);
+            }
+#endif
           }
         }
+        }
+        // the fractions move on by FD_UNR lines (the same FP32 operation in both threads that share a
+        // boundary; re-based in double every FD_SB bands)
+#pragma unroll
+        for (int q = 0; q <= FD_M; ++q) afr[q] = fmaf(s, (float)FD_UNR, afr[q]);
       }
     }
     __syncwarp();
@@ -314,9 +345,13 @@ __global__ void __launch_bounds__(FD_NT, 2) fp_diag_kernel(const FdParams prm) {
   for (int sl = 0; sl < 4 * NG; ++sl) {
     const int sidx = gA * 4 + sl;
     if (sidx >= prm.S) break;       // uniform
+#if FD_PACKED
     const float a0 = (sl & 1) ? fd_hi(acc[0][sl >> 1]) : fd_lo(acc[0][sl >> 1]);
     const float a1 = (sl & 1) ? fd_hi(acc[1][sl >> 1]) : fd_lo(acc[1][sl >> 1]);
     const float a2 = (sl & 1) ? fd_hi(acc[2][sl >> 1]) : fd_lo(acc[2][sl >> 1]);
+#else
+    const float a0 = acc[0][sl], a1 = acc[1][sl], a2 = acc[2][sl];
+#endif
     // local bin index = bin - mB in [0, NB]
     lo_s[pj * (FD_NB + 1) + 2 * jp] = a0;
     lo_s[pj * (FD_NB + 1) + 2 * jp + 1] = a1;
@@ -559,9 +594,20 @@ bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* p
   return plan->n_chunks > 0 && plan->n_chunks <= 65535;
 }
 
+// slice groups (of 4 slices) a block takes: 4 for stacks of >= 13 slices (16 slices per thread: the per-line
+// boundary / weight / address logic is shared by twice the FMAs; one block per SM), 2 from 5 slices on, else 1
+int fd_groups_per_block(int n_slices) {
+  const int ng = (n_slices + 3) / 4;
+#if FD_NG4
+  if (ng >= 4) return 4;
+#endif
+  return ng >= 2 ? 2 : 1;
+}
+
 size_t fd_xd_bytes(const FdPlan& plan, const pyhst_geom_t* g, int* n_groups_alloc) {
   const int ng = (g->n_slices + 3) / 4;
-  const int nga = ng > 1 ? (ng + 1) & ~1 : 1;     // two groups per block: a spare zero group for odd counts
+  const int per = fd_groups_per_block(g->n_slices);
+  const int nga = (ng + per - 1) / per * per;     // whole blocks: spare zero groups for ragged counts
   if (n_groups_alloc) *n_groups_alloc = nga;
   const int64_t line_f4 = (int64_t)g->nx + 2 * plan.zpad;
   return (size_t)2 * nga * plan.n_lines_alloc * line_f4 * 16;
@@ -615,19 +661,23 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
   prm.ranges = reinterpret_cast<const int2*>(plan.d_ranges);
   prm.n_bx = plan.n_bx;
   prm.W = plan.W;
-  const bool two = n_groups > 1;
-  static uint64_t configured[2] = {0, 0};
-  if (first_use_on_device(&configured[two ? 1 : 0])) {
-    if (two)
+  const int ng = fd_groups_per_block(g->n_slices);
+  static uint64_t configured[3] = {0, 0, 0};
+  if (first_use_on_device(&configured[ng == 4 ? 2 : ng - 1])) {
+    if (ng == 4)
+      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(4)));
+    else if (ng == 2)
       PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(2)));
     else
       PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(1)));
   }
-  dim3 grid(plan.n_bx, plan.n_chunks, two ? nga / 2 : 1);
+  dim3 grid(plan.n_bx, plan.n_chunks, nga / ng);
   if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
   StageScope scope(ST_FORWARD, stream);
   scope.kernels();
-  if (two)
+  if (ng == 4)
+    fp_diag_kernel<4><<<grid, FD_NT, fd_smem(4), stream>>>(prm);
+  else if (ng == 2)
     fp_diag_kernel<2><<<grid, FD_NT, fd_smem(2), stream>>>(prm);
   else
     fp_diag_kernel<1><<<grid, FD_NT, fd_smem(1), stream>>>(prm);
