@@ -172,6 +172,78 @@ def test_forward_project_axis_aligned_angles(lib, oracle):
     assert_parity(got, want, "forward_project axis-aligned")
 
 
+def _fp_variant(lib, variant, *args, **kw):
+    prev = lib.set_forward_project_variant(variant)
+    try:
+        return lib.forward_project(*args, **kw).cpu().numpy()
+    finally:
+        lib.set_forward_project_variant(prev)
+
+
+@pytest.mark.parametrize("S", [3, 5, 8, 13, 16, 18])
+def test_forward_project_diag_slice_counts(lib, oracle, S):
+    """The diagonal-line interval kernel takes 1, 2 or 4 slice groups per block (4, 8, 16 slices per thread);
+    ragged stacks leave spare zero groups."""
+    wl = lib.workloads
+    P, B, nx, ny = 40, 140, 120, 100
+    w = wl.custom(S, P, B, nx, ny, drift=1.0, jitter_angles=0.01, seed=S, span=2 * math.pi)
+    x = wl.random_image(S, ny, nx, seed=S)
+    want = oracle.forward_project(x, w.angles, w.axis, B)
+    got = _fp_variant(lib, 5, _dev(x), w.angles, w.axis, B)
+    assert lib.last_forward_project_kernel() == 5
+    assert_parity(got, want, "forward_project diag, %d slices" % S)
+
+
+def test_forward_project_diag_special_angles(lib, oracle):
+    """Angles on and next to the image axes (left to the banded kernel below 2^-12 bins per pixel of slack),
+    the diagonals (largest step, skew boundary) and both detector directions, with an integer-aligned geometry:
+    odd image sizes and an integer axis put pixels exactly on interval boundaries (each must be counted once)."""
+    wl = lib.workloads
+    S, B, nx, ny = 4, 131, 101, 91
+    eps = [0.0, 1e-6, 1e-4, 2.4e-4, 2.5e-4, 1e-3, -1e-6, -1e-4, -1e-3]
+    angles = np.array([q * math.pi / 2 + e for q in range(4) for e in eps] +
+                      [q * math.pi / 4 + e for q in (1, 3, 5, 7) for e in (0.0, 1e-9, -1e-9, 1e-3)] +
+                      list(np.linspace(0.0, 2 * math.pi, 37, endpoint=False) + 0.0123))
+    axis = np.full(angles.size, 65.0)
+    x = wl.random_image(S, ny, nx, seed=5)
+    want = oracle.forward_project(x, angles, axis, B)
+    for variant in (0, 5):
+        got = _fp_variant(lib, variant, _dev(x), angles, axis, B)
+        assert_parity(got, want, "forward_project special angles, variant %d" % variant)
+    # a constant image: every bin of a projection that sees the whole image carries the same mass as the oracle's
+    ones = np.ones((1, ny, nx), dtype=np.float32)
+    got = _fp_variant(lib, 5, _dev(ones), angles, axis, B)
+    want1 = oracle.forward_project(ones, angles, axis, B)
+    assert_parity(got, want1, "forward_project of ones (partition of the pixels)")
+    np.testing.assert_allclose(got.sum(axis=2), want1.sum(axis=2), rtol=2e-6)
+    assert (np.abs(want1.sum(axis=2) - nx * ny) < 1e-6 * nx * ny).sum() >= 40    # K2: whole image on the detector
+
+
+def test_forward_project_diag_sparse_angles_and_wide_detector(lib, oracle):
+    """Few projections far apart (chunks of one or two projections; windows that do not fit go to the banded
+    kernel), a detector much wider than the image (blocks whose strips miss the image write zeros) and a
+    pixel size above one bin."""
+    wl = lib.workloads
+    for (S, P, B, nx, ny, h) in [(8, 7, 700, 300, 260, 1.0), (2, 12, 900, 200, 220, 1.7), (8, 3, 64, 400, 400, 1.0)]:
+        w = wl.custom(S, P, B, nx, ny, pixel_size=h, drift=2.0, jitter_angles=0.3, seed=P + S)
+        x = wl.random_image(S, ny, nx, seed=P)
+        want = oracle.forward_project(x, w.angles, w.axis, B, pixel_size=h)
+        got = _fp_variant(lib, 5, _dev(x), w.angles, w.axis, B, pixel_size=h)
+        assert_parity(got, want, "forward_project diag sparse %r" % ((S, P, B, nx, ny, h),))
+
+
+def test_forward_project_kernels_agree(lib):
+    """Banded, interval and diagonal-line kernels compute the same sums in different orders: FP32 rounding apart."""
+    wl = lib.workloads
+    S, P, B, nx, ny = 16, 96, 300, 256, 256
+    w = wl.custom(S, P, B, nx, ny, drift=1.0, jitter_angles=0.002, seed=9)
+    x = _dev(wl.random_image(S, ny, nx, seed=9))
+    ref = _fp_variant(lib, 2, x, w.angles, w.axis, B)
+    for variant in (0, 4, 5):
+        got = _fp_variant(lib, variant, x, w.angles, w.axis, B)
+        assert_parity(got, ref, "forward_project variant %d vs banded" % variant, rel=3e-6, mabs=3e-5)
+
+
 @pytest.mark.parametrize("B,axis", [(260, None), (120, 75.3)])
 def test_adjoint_identity_on_device(lib, B, axis):
     """K3 in FP32: |<P x, y> - <x, P^T y>| <= 1e-5 ||P x|| ||y||."""
