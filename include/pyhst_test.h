@@ -8,6 +8,8 @@
 #ifndef PYHST_TEST_H_
 #define PYHST_TEST_H_
 
+#include "pyhst.h"
+
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -44,6 +46,14 @@ int pyhst_set_forward_project_variant(int variant);
  * interval forms, 5 diagonal-line interval kernel (plus the banded kernel for the projections it leaves
  * out), 0 none yet.  For bench labels and tests. */
 int pyhst_last_forward_project_kernel(void);
+
+/* Host-only (no device needed): builds the tables of the diagonal-line forward projector for geometry g and reports
+ * info[0] = chunks, info[1] = projections left to the banded kernel, info[2] = staged window width (float4 per line),
+ * info[3] = detector blocks per chunk, info[4] = intervals per block, info[5] = projections per chunk at most,
+ * info[6] = zero pad of a stored line, info[7] = stored lines per slice group.  chunk_of (nullable, [n_angles]) receives
+ * the chunk index of every projection, -1 for those left out; ranges (nullable, [chunks][blocks][2]) the lines each block
+ * walks.  Returns PYHST_OK, or PYHST_ERR_UNSUPPORTED when the kernel covers no projection of g. */
+int pyhst_test_fd_plan(const pyhst_geom_t* g, int32_t* info, int32_t* chunk_of, int32_t* ranges);
 
 /* Selects the ramp-filter implementation: 0 = automatic (default: the fused shared-memory FFT kernel for
  * rows of up to 4096 filtered bins, cuFFT beyond), 1 = the cuFFT path (pad/weight, R2C, x H, C2R, crop:

@@ -27,7 +27,7 @@ _LIBNAME = "libpyhst_b200.so"
 # every symbol include/*.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
            "pyhst_fista_tv", "pyhst_ista_tv", "pyhst_ring_filter", "pyhst_ecohe", "pyhst_cv_distance", "pyhst_patch_grid",
-           "pyhst_patch_gradient", "pyhst_patch_fista", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_last_forward_project_kernel", "pyhst_set_halfacq_stitch", "pyhst_set_filter_variant", "pyhst_set_patch_gemm_variant",
+           "pyhst_patch_gradient", "pyhst_patch_fista", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_last_forward_project_kernel", "pyhst_test_fd_plan", "pyhst_set_halfacq_stitch", "pyhst_set_filter_variant", "pyhst_set_patch_gemm_variant",
            "pyhst_last_error", "pyhst_release_cache")
 
 
@@ -378,6 +378,32 @@ def set_patch_gemm_variant(variant: int) -> int:
 
 def set_forward_project_variant(variant: int) -> int:
     return int(_load().pyhst_set_forward_project_variant(int(variant)))
+
+
+def test_fd_plan(angles, axis, n_bins, nx, ny, pixel_size=1.0, n_slices=1):
+    """Host-only tables of the diagonal-line forward projector (pyhst_test.h): (info dict, chunk index per projection,
+    line ranges [chunks][blocks][2])."""
+    import numpy as np
+    lib = _load()
+    angles = np.ascontiguousarray(angles, dtype=np.float64)
+    axis = np.ascontiguousarray(axis, dtype=np.float64)
+    g = Geom(int(n_slices), int(angles.size), int(n_bins), 0, angles.ctypes.data_as(POINTER(c_double)),
+             axis.ctypes.data_as(POINTER(c_double)), int(nx), int(ny), float(pixel_size))
+    info = np.zeros(8, dtype=np.int32)
+    chunk_of = np.zeros(angles.size, dtype=np.int32)
+    lib.pyhst_test_fd_plan.argtypes = [POINTER(Geom), c_void_p, c_void_p, c_void_p]
+    st = lib.pyhst_test_fd_plan(ctypes.byref(g), info.ctypes.data, chunk_of.ctypes.data, None)
+    names = ("chunks", "left_out", "window", "blocks", "intervals_per_block", "projections_per_chunk", "zpad", "lines")
+    d = dict(zip(names, (int(v) for v in info)))
+    d["status"] = int(st)
+    ranges = None
+    if st == 0:
+        ranges = np.zeros((d["chunks"], d["blocks"], 2), dtype=np.int32)
+        lib.pyhst_test_fd_plan(ctypes.byref(g), info.ctypes.data, chunk_of.ctypes.data, ranges.ctypes.data)
+    return d, chunk_of, ranges
+
+
+test_fd_plan.__test__ = False   # not a pytest test
 
 
 def last_forward_project_kernel() -> int:

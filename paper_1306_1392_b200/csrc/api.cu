@@ -524,6 +524,35 @@ int pyhst_set_forward_project_variant(int variant) {
 
 int pyhst_last_forward_project_kernel(void) { return g_last_fp_kernel; }
 
+int pyhst_test_fd_plan(const pyhst_geom_t* g, int32_t* info, int32_t* chunk_of, int32_t* ranges) {
+  int64_t pitch = 0;
+  PYHST_TRY(check_geom(g, &pitch));
+  if (!info) return set_error(PYHST_ERR_INVALID_ARG, "info is NULL");
+  FdPlan pl;
+  std::vector<FdProj> projs;
+  std::vector<FdChunk> chunks;
+  std::vector<int32_t> rg, legacy;
+  const bool ok = build_fd_tables(g, &pl, &projs, &chunks, &rg, &legacy);
+  int32_t nb = 0, npj = 0;
+  fd_block_shape(&nb, &npj);
+  info[0] = ok ? pl.n_chunks : 0;
+  info[1] = (int32_t)legacy.size();
+  info[2] = pl.W;
+  info[3] = pl.n_bx;
+  info[4] = nb;
+  info[5] = npj;
+  info[6] = pl.zpad;
+  info[7] = pl.n_lines_alloc;
+  if (chunk_of) {
+    for (int p = 0; p < g->n_angles; ++p) chunk_of[p] = -1;
+    for (size_t c = 0; c < chunks.size(); ++c)
+      for (int q = 0; q < chunks[c].count; ++q) chunk_of[projs[chunks[c].first + q].p] = (int32_t)c;
+  }
+  if (ranges && ok) std::memcpy(ranges, rg.data(), rg.size() * sizeof(int32_t));
+  if (!ok) return set_error(PYHST_ERR_UNSUPPORTED, "diagonal-line forward projector covers no projection of this geometry");
+  return PYHST_OK;
+}
+
 void pyhst_release_cache(void) {
   int prev = current_device();
   std::vector<DeviceCtx*> all;

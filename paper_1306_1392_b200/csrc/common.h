@@ -238,6 +238,7 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
 // covers none
 bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* projs, std::vector<FdChunk>* chunks,
                      std::vector<int32_t>* ranges, std::vector<int32_t>* legacy);  // forward_project_diag.cu
+void fd_block_shape(int32_t* nb, int32_t* npj);   // intervals per block, projections per chunk
 int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch, const pyhst_geom_t* g,
                                 float scale, const FdPlan& plan, cudaStream_t stream);
 int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pitch,

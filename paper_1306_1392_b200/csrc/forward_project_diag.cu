@@ -604,6 +604,11 @@ int fd_groups_per_block(int n_slices) {
   return ng >= 2 ? 2 : 1;
 }
 
+void fd_block_shape(int32_t* nb, int32_t* npj) {
+  *nb = FD_NB;
+  *npj = FD_NPJ;
+}
+
 size_t fd_xd_bytes(const FdPlan& plan, const pyhst_geom_t* g, int* n_groups_alloc) {
   const int ng = (g->n_slices + 3) / 4;
   const int per = fd_groups_per_block(g->n_slices);

@@ -4,6 +4,7 @@ multi-GPU plumbing (slice sharding, max-over-ranks, gather) works under gloo wit
 No compute call is made without a GPU.
 """
 import ctypes
+import math
 import os
 import re
 import subprocess
@@ -181,3 +182,73 @@ def test_bench_reference_arm_runs_on_cpu():
               "cpu_baseline", "e2e", "config"):
         assert k in line
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
+
+
+# ------------------------------------------------------------------ diagonal-line forward projector: host tables
+def _fd_plan(angles, axis, B, nx, ny, h=1.0):
+    from paper_1306_1392_b200 import binding
+    return binding.test_fd_plan(angles, axis, B, nx, ny, pixel_size=h)
+
+
+def test_fd_plan_chunks_cover_every_projection_once(cuda_lib):
+    """pyhst_test.h pyhst_test_fd_plan (host only): every projection sits in exactly one chunk of at most 16 neighbours
+    of one walk class, or is left to the banded kernel -- exactly those with fewer than 1 + 2^-12 bins per pixel along
+    an image diagonal (an interval must not hold two pixels of a line)."""
+    P, B, n = 2000, 2048, 2048
+    angles = np.arange(P) * math.pi / P
+    rng = np.random.default_rng(3)
+    axis = 1023.5 + rng.uniform(-1.5, 1.5, P)
+    info, chunk_of, ranges = _fd_plan(angles, axis, B, n, n)
+    assert info["status"] == 0
+    sigma = np.abs(np.cos(angles)) + np.abs(np.sin(angles))
+    left = sigma < 1.0 + 1.0 / 4096.0
+    assert (chunk_of[left] == -1).all() and (chunk_of[~left] >= 0).all()
+    assert info["left_out"] == int(left.sum()) == 2                      # theta = 0 and pi / 2
+    counts = np.bincount(chunk_of[~left], minlength=info["chunks"])
+    assert counts.min() >= 1 and counts.max() <= info["projections_per_chunk"] == 16
+    assert info["chunks"] <= 130                                          # dense list: chunks are full
+    # one walk class per chunk: layout (sign of cos * sin), detector direction, skew (which of |cos|, |sin| is larger)
+    cls = (np.cos(angles) * np.sin(angles) >= 0).astype(int) * 4 + (np.abs(np.sin(angles)) > np.abs(np.cos(angles))) * 2
+    for c in range(info["chunks"]):
+        assert len(set(cls[chunk_of == c])) == 1
+    assert 64 < info["window"] <= 100 and info["zpad"] >= info["window"] + 16
+    assert info["blocks"] == -(-B // (info["intervals_per_block"] - 1))
+    assert ranges.min() >= 0 and ranges[:, :, 1].max() <= info["lines"] - 8
+
+
+def test_fd_plan_line_ranges_contain_every_contributing_pixel(cuda_lib):
+    """Brute force on a small scan: every pixel whose coordinate falls into a block's interval range lies on a stored
+    line inside the range the block walks (layout 0: line = i - j + nx - 1, layout 1: line = i + j)."""
+    rng = np.random.default_rng(5)
+    P, B, nx, ny, h = 37, 150, 70, 50, 1.15
+    angles = np.sort(rng.uniform(0, 2 * math.pi, P))
+    axis = 74.0 + rng.uniform(-20, 20, P)
+    info, chunk_of, ranges = _fd_plan(angles, axis, B, nx, ny, h)
+    assert info["status"] == 0
+    nb = info["intervals_per_block"]
+    j, i = np.meshgrid(np.arange(nx), np.arange(ny))
+    for p in range(P):
+        c = chunk_of[p]
+        if c < 0:
+            continue
+        a, b = h * math.cos(angles[p]), h * math.sin(angles[p])
+        t = axis[p] + a * (j - (nx - 1) / 2) + b * (i - (ny - 1) / 2)
+        w = (i - j + nx - 1) if a * b >= 0 else (i + j)
+        for bx in range(info["blocks"]):
+            mB = bx * (nb - 1) - 1
+            inside = (t >= mB) & (t < mB + nb)
+            if inside.any():
+                lo, hi = ranges[c, bx]
+                assert lo <= w[inside].min() and w[inside].max() < hi, (p, bx)
+
+
+def test_fd_plan_rejects_small_pixels_and_sparse_lists_shrink_chunks(cuda_lib):
+    """Pixel sizes below 1 / sqrt(2) bins leave no projection with >= 1 bin per pixel along a diagonal; a sparse angle
+    list (config 4: 0.9 degrees apart) fans out and fits only a few projections into one staged window."""
+    ang = np.arange(200) * math.pi / 200
+    info, chunk_of, _ = _fd_plan(ang, np.full(200, 511.5), 1024, 1024, 1024, h=0.6)
+    assert info["status"] != 0 and (chunk_of == -1).all()
+    info, chunk_of, _ = _fd_plan(ang, np.full(200, 511.5), 1024, 1024, 1024)
+    assert info["status"] == 0 and info["window"] <= 100
+    per_chunk = (chunk_of >= 0).sum() / info["chunks"]
+    assert 2.0 <= per_chunk <= 8.0
