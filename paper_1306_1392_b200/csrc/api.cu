@@ -318,15 +318,17 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, int want_diag, const
     std::vector<int32_t> ranges;
     FpPlan probe = pl;
     bool use = build_fd_tables(g, &pl.fd, &dprojs, &dchunks, &ranges, &legacy);
+    // sparse angle lists fan out: few projections fit one staged window -- blocks of 8 projections instead of 16
+    if (use && (double)dprojs.size() / (double)dchunks.size() < 8.0 && !std::getenv("PYHST_FD_NPJ16"))
+      use = build_fd_tables(g, &pl.fd, &dprojs, &dchunks, &ranges, &legacy, 8);
     if (use && want_diag == 1) {
-      // automatic choice: the diagonal-line kernel pays off when its blocks are full (chunks of >= 8
-      // neighbouring projections share a window: dense angle lists) and fill the GPU twice over; sparse
-      // angle lists and small scans stay on the banded kernel
+      // automatic choice: the diagonal-line kernel pays off when its blocks are mostly full (neighbouring
+      // projections share a window) and fill the GPU; very sparse lists and small scans stay on the banded kernel
       const double per_chunk = (double)dprojs.size() / (double)dchunks.size();
       const int64_t blocks = (int64_t)pl.fd.n_bx * pl.fd.n_chunks * std::max(1, (pl.n_groups + 1) / 2);
       int n_sm = 148;
       require_sm100(&n_sm);
-      use = per_chunk >= 8.0 && blocks >= 4 * (int64_t)n_sm;
+      use = per_chunk >= 0.55 * pl.fd.npj && blocks >= 4 * (int64_t)n_sm;
     }
     if (use && (legacy.empty() || build_fp_tables(g, &probe, &projs, &chunks, &legacy))) {
       pl.diag = true;

@@ -17,6 +17,9 @@
 //     x) are two launches: pass 0 writes the image, pass 1 adds to it.
 #include "common.h"
 
+#ifndef R8_RELOAD
+#define R8_RELOAD 0
+#endif
 namespace pyhst {
 
 namespace {
@@ -72,6 +75,14 @@ __device__ __forceinline__ void r8_run(float (&acc)[R8_RN][8], uint32_t addr, fl
           "add.rn.f32 %17, %17, %18;\n\t"
           "setp.ge.f32 p, %17, 0f3F800000;\n\t"
           "@p add.rn.f32 %17, %17, 0fBF800000;\n\t"
+#if R8_RELOAD
+          "@p add.u32 %16, %16, 16;\n\t"
+          "@p ld.shared.v4.f32 {%0, %1, %2, %3}, [%16];\n\t"
+          "@p ld.shared.v4.f32 {%4, %5, %6, %7}, [%16+16];\n\t"
+          "@p ld.shared.v4.f32 {%8, %9, %10, %11}, [%16+%20];\n\t"
+          "@p ld.shared.v4.f32 {%12, %13, %14, %15}, [%16+%19];\n\t"
+          "}"
+#else
           "@p mov.f32 %0, %4;\n\t"
           "@p add.rn.f32 %1, %5, 0f80000000;\n\t"
           "@p mov.f32 %2, %6;\n\t"
@@ -84,10 +95,11 @@ __device__ __forceinline__ void r8_run(float (&acc)[R8_RN][8], uint32_t addr, fl
           "@p ld.shared.v4.f32 {%4, %5, %6, %7}, [%16+16];\n\t"
           "@p ld.shared.v4.f32 {%12, %13, %14, %15}, [%16+%19];\n\t"
           "}"
+#endif
           : "+f"(qa.x), "+f"(qa.y), "+f"(qa.z), "+f"(qa.w), "+f"(qb.x), "+f"(qb.y), "+f"(qb.z),
             "+f"(qb.w), "+f"(ra.x), "+f"(ra.y), "+f"(ra.z), "+f"(ra.w), "+f"(rb.x), "+f"(rb.y),
             "+f"(rb.z), "+f"(rb.w), "+r"(addr), "+f"(f)
-          : "f"(dl), "n"(GOFF + 16));
+          : "f"(dl), "n"(GOFF + 16), "n"(GOFF));
     }
   }
 }

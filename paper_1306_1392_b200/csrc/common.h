@@ -121,7 +121,7 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
 
 // Grow-only device workspace slots owned by the library (freed by pyhst_release_cache).
 enum WorkspaceSlot { WS_QI = 0, WS_FFT = 1, WS_WEIGHTS = 2, WS_IMG_T = 3, WS_ROWS = 4,
-                     WS_CHUNKS = 5, WS_XI = 6, WS_FISTA = 7, WS_FPL = 8, WS_STITCH = 9, WS_XD = 10, WS_COUNT = 11 };
+                     WS_CHUNKS = 5, WS_XI = 6, WS_FISTA = 7, WS_FPL = 8, WS_STITCH = 9, WS_XD = 10, WS_FDP = 11, WS_COUNT = 12 };
 int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr);
 // bumped whenever the slot's block is (re)allocated or released: lets a user of the slot remember
 // "I initialised this very block" without being fooled by a recycled address
@@ -205,7 +205,7 @@ struct FdChunk {
   int32_t pad_[2];
 };
 struct FdPlan {
-  int32_t n_chunks = 0, n_bx = 0, W = 0, zpad = 0, n_lines_alloc = 0;
+  int32_t n_chunks = 0, n_bx = 0, W = 0, zpad = 0, n_lines_alloc = 0, npj = 16, n_tab = 0;   // npj: projections per chunk at most (16 or 8); n_tab: projections in the table
   FdProj* d_projs = nullptr;
   FdChunk* d_chunks = nullptr;
   int32_t* d_ranges = nullptr;   // [n_chunks][n_bx][2]
@@ -237,7 +237,7 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
 // diagonal-line kernel: host tables (projections it does not cover are listed in `legacy`); false if it
 // covers none
 bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* projs, std::vector<FdChunk>* chunks,
-                     std::vector<int32_t>* ranges, std::vector<int32_t>* legacy);  // forward_project_diag.cu
+                     std::vector<int32_t>* ranges, std::vector<int32_t>* legacy, int npj = 16);  // forward_project_diag.cu
 void fd_block_shape(int32_t* nb, int32_t* npj);   // intervals per block, projections per chunk
 int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch, const pyhst_geom_t* g,
                                 float scale, const FdPlan& plan, cudaStream_t stream);

@@ -63,7 +63,8 @@ constexpr int FD_HDR = 1024;   // mbarriers, origins, FdProj table
 constexpr float FD_MAGIC = 12582912.f;   // 1.5 * 2^23
 
 // smem bytes of one launch
-constexpr size_t fd_smem(int ng) { return FD_HDR + (size_t)FD_NSTG * FD_RB * ng * FD_PW * 16; }
+constexpr int fd_hdr(int npj) { return npj == 8 ? 512 : FD_HDR; }   // 128 B of barriers / origins + npj x 40 B
+constexpr size_t fd_smem(int ng, int rb, int npj) { return fd_hdr(npj) + (size_t)FD_NSTG * rb * ng * FD_PW * 16; }
 
 struct FdParams {
   const float4* xd[2];     // sheared image, layout 0 (diagonals i - j) and 1 (anti-diagonals i + j)
@@ -78,6 +79,11 @@ struct FdParams {
   const FdChunk* chunks;
   const int2* ranges;      // [n_chunks][n_bx]: lines [x, y) the block walks
   int32_t n_bx, W;
+  // n_seg > 1: blockIdx.z = group block * n_seg + seg; the block walks the seg-th part of its bands and writes its
+  // sums to part[seg] (same row layout, pitch part_pitch); fd_combine_kernel adds the parts (small scans fill the GPU)
+  int32_t n_seg;
+  float* part;
+  int64_t part_pitch, part_stride;
 };
 
 // One line of one interval, NG slice groups: two LDS.128 and 4 NG packed FFMA2 (two slices each).  The
@@ -85,7 +91,7 @@ struct FdParams {
 // bins m + 1 / m, already zeroed when the interval does not hold that pixel (packed instructions cannot
 // be predicated).  An FFMA2 takes one issue slot and holds the FMA pipe for two cycles, so the ALU-pipe
 // and LSU instructions of the line issue in its shadow (profiles/r02_micro.md).
-template <int NG>
+template <int NG, int PLANE>
 __device__ __forceinline__ void fd_line(uint64_t* al, uint64_t* au, float f, float g, uint32_t addr) {
   if constexpr (NG >= 2) {
     asm volatile("{\n\t"
@@ -104,7 +110,7 @@ __device__ __forceinline__ void fd_line(uint64_t* al, uint64_t* au, float f, flo
         "fma.rn.f32x2 %7, v3, wf, %7;\n\t"
         "}"
         : "+l"(al[0]), "+l"(al[1]), "+l"(al[2]), "+l"(al[3]), "+l"(au[0]), "+l"(au[1]), "+l"(au[2]), "+l"(au[3])
-        : "f"(f), "f"(g), "r"(addr), "n"(FD_RB * FD_PW * 16));
+        : "f"(f), "f"(g), "r"(addr), "n"(PLANE));
   } else {
     asm volatile("{\n\t"
         ".reg .b64 v<2>, wf, wg;\n\t"
@@ -130,6 +136,7 @@ __device__ __forceinline__ void fd_line_s1(float (&al)[4], float (&au)[4], float
 }
 // scalar form: predicated FFMA on float accumulators (one issue slot each; the kernel is then bound by
 // issue slots instead of the FMA pipe -- measured within 2 % of the packed form)
+template <int PLANE>
 __device__ __forceinline__ void fd_line_s(float* al, float* au, float jlo, float jhi, float f, float g,
                                           uint32_t addr) {
   asm volatile("{\n\t"
@@ -157,41 +164,52 @@ __device__ __forceinline__ void fd_line_s(float* al, float* au, float jlo, float
       "}"
       : "+f"(al[0]), "+f"(al[1]), "+f"(al[2]), "+f"(al[3]), "+f"(al[4]), "+f"(al[5]), "+f"(al[6]), "+f"(al[7]),
         "+f"(au[0]), "+f"(au[1]), "+f"(au[2]), "+f"(au[3]), "+f"(au[4]), "+f"(au[5]), "+f"(au[6]), "+f"(au[7])
-      : "f"(jlo), "f"(jhi), "f"(f), "f"(g), "r"(addr), "n"(FD_RB * FD_PW * 16));
+      : "f"(jlo), "f"(jhi), "f"(f), "f"(g), "r"(addr), "n"(PLANE));
 }
 #endif
 
 __device__ __forceinline__ float fd_lo(uint64_t v) { return __uint_as_float((uint32_t)v); }
 __device__ __forceinline__ float fd_hi(uint64_t v) { return __uint_as_float((uint32_t)(v >> 32)); }
 
-template <int NG>
-__global__ void __launch_bounds__(FD_NT, NG == 4 ? 1 : 2) fp_diag_kernel(const FdParams prm) {
+// NPJ = projections per block (16: dense angle lists; 8: sparse ones, whose strips fan out so that fewer fit one staged
+// window -- 256-thread blocks with bands of RB = 4 lines, four blocks per SM), NT = 32 NPJ threads.
+template <int NG, int NPJ, int RB>
+__global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ? 2 : 4)) fp_diag_kernel(const FdParams prm) {
+  constexpr int NT = FD_NB / FD_M * NPJ, NWARP = NT / 32, PLANE = RB * FD_PW * 16;
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);              // [NSTG]
   uint64_t* empty = reinterpret_cast<uint64_t*>(smem + 32);        // [NSTG]
   int* sorigin = reinterpret_cast<int*>(smem + 64);                // [NSTG]
-  FdProj* sproj = reinterpret_cast<FdProj*>(smem + 128);           // [FD_NPJ] x 48 B
-  float4* buf = reinterpret_cast<float4*>(smem + FD_HDR);          // [NSTG][NG][RB][PW]
-  constexpr int STAGE_F4 = NG * FD_RB * FD_PW;
+  FdProj* sproj = reinterpret_cast<FdProj*>(smem + 128);           // [NPJ] x 48 B
+  float4* buf = reinterpret_cast<float4*>(smem + (NPJ == 8 ? 512 : FD_HDR));          // [NSTG][NG][RB][PW]
+  constexpr int STAGE_F4 = NG * RB * FD_PW;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const FdChunk ck = prm.chunks[blockIdx.y];
-  const int gA = blockIdx.z * NG;
+  const int seg = blockIdx.z % prm.n_seg;
+  const int gA = (blockIdx.z / prm.n_seg) * NG;
   const int mB = blockIdx.x * (FD_NB - 1) - 1;      // intervals [m, m+1), m in [mB, mB + NB)
-  const int2 rg = prm.ranges[(int64_t)blockIdx.y * prm.n_bx + blockIdx.x];
-  const int n_bands = (rg.y - rg.x + FD_RB - 1) / FD_RB;
+  int2 rg = prm.ranges[(int64_t)blockIdx.y * prm.n_bx + blockIdx.x];
+  if (prm.n_seg > 1) {
+    const int nb_all = (rg.y - rg.x + RB - 1) / RB;
+    const int k0 = seg * nb_all / prm.n_seg, k1 = (seg + 1) * nb_all / prm.n_seg;
+    rg.y = min(rg.y, rg.x + k1 * RB);
+    rg.x = rg.x + k0 * RB;
+    if (rg.y < rg.x) rg.y = rg.x;
+  }
+  const int n_bands = (rg.y - rg.x + RB - 1) / RB;
   const int W = prm.W;
   const uint32_t row_bytes = (uint32_t)W * 16u;
   const float4* xd = (ck.layout ? prm.xd[1] : prm.xd[0]) + (int64_t)gA * prm.group_f4;
   const int sgn = ck.sgn, skew = ck.skew;
-  const int bias = skew < 0 ? FD_RB - 1 : 0;
+  const int bias = skew < 0 ? RB - 1 : 0;
 
   if (tid < ck.count) sproj[tid] = prm.projs[ck.first + tid];
   if (tid == 0) {
 #pragma unroll
     for (int q = 0; q < FD_NSTG; ++q) {
-      mbar_init(&full[q], FD_RB);
-      mbar_init(&empty[q], FD_NT / 32);
+      mbar_init(&full[q], RB);
+      mbar_init(&empty[q], NT / 32);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -205,7 +223,7 @@ __global__ void __launch_bounds__(FD_NT, NG == 4 ? 1 : 2) fp_diag_kernel(const F
   auto produce = [&](int k) {
     const int st = k % FD_NSTG;
     if (k >= FD_NSTG) mbar_wait(&empty[st], (uint32_t)(((k / FD_NSTG) - 1) & 1));
-    const int w0 = rg.x + k * FD_RB;
+    const int w0 = rg.x + k * RB;
     double lo = 1e300;
     if (lane < ck.count) {
       const FdProj pj = sproj[lane];
@@ -215,7 +233,7 @@ __global__ void __launch_bounds__(FD_NT, NG == 4 ? 1 : 2) fp_diag_kernel(const F
       const double ea = sgn > 0 ? e0 : -e1;                      // lowest stored position on line 0
       const double da = (double)sgn * pj.sD;                     // its change per line
       const double a0 = fma(da, (double)w0, ea);
-      const double a1 = fma(da, (double)(w0 + FD_RB - 1), ea) - (double)(skew * (FD_RB - 1));
+      const double a1 = fma(da, (double)(w0 + RB - 1), ea) - (double)(skew * (RB - 1));
       lo = fmin(a0, a1);
     }
 #pragma unroll
@@ -223,12 +241,12 @@ __global__ void __launch_bounds__(FD_NT, NG == 4 ? 1 : 2) fp_diag_kernel(const F
     const int origin = (int)floor(lo) - 2;
     uint64_t* bar = &full[st];
     if (lane == 0) sorigin[st] = origin;
-    if (lane < FD_RB) {
+    if (lane < RB) {
       mbar_arrive_expect_tx(bar, NG * row_bytes);
       const float4* src = xd + (int64_t)(w0 + lane) * prm.line_f4 + (prm.zpad + origin + skew * lane);
       float4* dst = buf + st * STAGE_F4 + lane * FD_PW + bias + skew * lane;
 #pragma unroll
-      for (int q = 0; q < NG; ++q) bulk_g2s(dst + q * FD_RB * FD_PW, src + q * prm.group_f4, row_bytes, bar);
+      for (int q = 0; q < NG; ++q) bulk_g2s(dst + q * RB * FD_PW, src + q * prm.group_f4, row_bytes, bar);
     }
   };
 
@@ -276,7 +294,7 @@ __global__ void __launch_bounds__(FD_NT, NG == 4 ? 1 : 2) fp_diag_kernel(const F
       if ((k % FD_SB) == 0) {
         // every FD_SB bands: the boundaries' positions on the band's first line (double), split into an
         // integer and a fraction; the thread that shares a boundary evaluates the identical expression
-        const double w0 = (double)(rg.x + k * FD_RB);
+        const double w0 = (double)(rg.x + k * RB);
         const FdProj* sp = &sproj[pj];
         const double K0 = sp->K0, inv = sp->inv, sD = sp->sD;
 #pragma unroll
@@ -291,7 +309,7 @@ __global__ void __launch_bounds__(FD_NT, NG == 4 ? 1 : 2) fp_diag_kernel(const F
       // kappa = float_as_int(jm) - 0x4b400000
       const uint32_t cbase = buf_u32 + (uint32_t)(st * STAGE_F4 * 16) + (uint32_t)((bias - origin) * 16) - magic_off;
 #pragma unroll 1
-      for (int r0 = 0; r0 < FD_RB; r0 += FD_UNR) {
+      for (int r0 = 0; r0 < RB; r0 += FD_UNR) {
         const uint32_t cb = cbase + (uint32_t)(r0 * FD_PW * 16);
         {
 #pragma unroll
@@ -311,12 +329,12 @@ __global__ void __launch_bounds__(FD_NT, NG == 4 ? 1 : 2) fp_diag_kernel(const F
             asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(addr) : "r"(__float_as_int(jm[q])), "r"(mul), "r"(cb + r * FD_PW * 16));
 #if FD_PACKED
             const float fz = in ? f : 0.f, gz = in ? g : 0.f;
-            fd_line<NG>(acc[q], acc[q + 1], fz, gz, addr);
-            if constexpr (NG == 4) fd_line<NG>(acc[q] + 4, acc[q + 1] + 4, fz, gz, addr + 2 * FD_RB * FD_PW * 16);
+            fd_line<NG, PLANE>(acc[q], acc[q + 1], fz, gz, addr);
+            if constexpr (NG == 4) fd_line<NG, PLANE>(acc[q] + 4, acc[q + 1] + 4, fz, gz, addr + 2 * PLANE);
 #else
             if constexpr (NG >= 2) {
-              fd_line_s(acc[q], acc[q + 1], jm[q], jm[q + 1], f, g, addr);
-              if constexpr (NG == 4) fd_line_s(acc[q] + 8, acc[q + 1] + 8, jm[q], jm[q + 1], f, g, addr + 2 * FD_RB * FD_PW * 16);
+              fd_line_s<PLANE>(acc[q], acc[q + 1], jm[q], jm[q + 1], f, g, addr);
+              if constexpr (NG == 4) fd_line_s<PLANE>(acc[q] + 8, acc[q + 1] + 8, jm[q], jm[q + 1], f, g, addr + 2 * PLANE);
             } else {
               fd_line_s1(acc[q], acc[q + 1], in ? f : 0.f, in ? g : 0.f, addr);
             }
@@ -334,13 +352,15 @@ __global__ void __launch_bounds__(FD_NT, NG == 4 ? 1 : 2) fp_diag_kernel(const F
     if (lane == 0) mbar_arrive(&empty[st]);
     // the producer role rotates; a warp produces AFTER its own share of band k, into the stage of band
     // k - 1, which the other warps have normally left by then: it does not become the straggler
-    if (k + FD_NSTG - 1 < n_bands && warp == (k & 15)) produce(k + FD_NSTG - 1);
+    if (k + FD_NSTG - 1 < n_bands && warp == (k % NWARP)) produce(k + FD_NSTG - 1);
   }
 
   // ---- combine the shares through shared memory (the stages are free now) and store -------------
   __syncthreads();
+  float* out = prm.n_seg > 1 ? prm.part + (int64_t)seg * prm.part_stride : prm.sino;
+  const int64_t opitch = prm.n_seg > 1 ? prm.part_pitch : prm.pitch;
   float* lo_s = reinterpret_cast<float*>(buf);                 // [NPJ][NB + 1] lower shares (and complete middle bins)
-  float* up_s = lo_s + FD_NPJ * (FD_NB + 1);                   // [NPJ][NB + 1] upper shares
+  float* up_s = lo_s + NPJ * (FD_NB + 1);                   // [NPJ][NB + 1] upper shares
 #pragma unroll
   for (int sl = 0; sl < 4 * NG; ++sl) {
     const int sidx = gA * 4 + sl;
@@ -359,17 +379,31 @@ __global__ void __launch_bounds__(FD_NT, NG == 4 ? 1 : 2) fp_diag_kernel(const F
     up_s[pj * (FD_NB + 1) + 2 * jp + 2] = a2;
     __syncthreads();
     // complete bins: local 1 .. NB - 1
-    for (int e = tid; e < FD_NPJ * (FD_NB - 1); e += FD_NT) {
+    for (int e = tid; e < NPJ * (FD_NB - 1); e += NT) {
       const int q = e / (FD_NB - 1), bl = 1 + e - q * (FD_NB - 1);
       const int b = mB + bl;
       if (q < ck.count && b < prm.B) {
         const int p = sproj[q].p;
-        prm.sino[((int64_t)sidx * prm.P + p) * prm.pitch + b] =
+        out[((int64_t)sidx * prm.P + p) * opitch + b] =
             prm.scale * (lo_s[q * (FD_NB + 1) + bl] + up_s[q * (FD_NB + 1) + bl]);
       }
     }
     __syncthreads();
   }
+}
+
+// y[s][p][b] = sum_seg part[seg][s][p][b] for the projections of the table (fixed order: deterministic)
+__global__ void fd_combine_kernel(float* __restrict__ y, int64_t pitch, const float* __restrict__ part, int64_t part_pitch,
+                                  int64_t part_stride, int n_seg, int B, int P, const FdProj* __restrict__ projs, int n_tab,
+                                  int64_t n_rows_tab) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t rt = blockIdx.y + (int64_t)blockIdx.z * gridDim.y;
+  if (b >= B || rt >= n_rows_tab) return;
+  const int64_t sl = rt / n_tab;
+  const int64_t row = sl * P + projs[rt - sl * n_tab].p;
+  float v = 0.f;
+  for (int h = 0; h < n_seg; ++h) v += part[(int64_t)h * part_stride + row * part_pitch + b];
+  y[row * pitch + b] = v;
 }
 
 // ---- [S][ny][nx] -> XD, both shears ---------------------------------------------------------------
@@ -463,7 +497,9 @@ void line_range(const HostProj& q, int nx, int ny, double tlo, double thi, doubl
 }  // namespace
 
 bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* projs, std::vector<FdChunk>* chunks,
-                     std::vector<int32_t>* ranges, std::vector<int32_t>* legacy) {
+                     std::vector<int32_t>* ranges, std::vector<int32_t>* legacy, int npj) {
+  if (npj != 8) npj = FD_NPJ;
+  plan->npj = npj;
   const int P = g->n_angles, nx = g->nx, ny = g->ny;
   const double h = g->pixel_size;
   const double j0 = 0.5 * (nx - 1), i0 = 0.5 * (ny - 1);
@@ -563,7 +599,7 @@ bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* p
         ++i;
         continue;
       }
-      while (j < v.size() && j - i < (size_t)FD_NPJ) {
+      while (j < v.size() && j - i < (size_t)npj) {
         std::vector<int32_t> rg_try;
         int w_try = 0;
         eval(j + 1, &rg_try, &w_try);
@@ -589,6 +625,7 @@ bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* p
   std::sort(legacy->begin(), legacy->end());
   plan->W = std::max(16, (w_max + 3) & ~3);
   plan->n_chunks = (int32_t)chunks->size();
+  plan->n_tab = (int32_t)projs->size();
   plan->zpad = FD_WMAX + FD_NB + 2 * FD_RB + 16;
   plan->n_lines_alloc = n_lines + FD_RB;
   return plan->n_chunks > 0 && plan->n_chunks <= 65535;
@@ -596,10 +633,10 @@ bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* p
 
 // slice groups (of 4 slices) a block takes: 4 for stacks of >= 13 slices (16 slices per thread: the per-line
 // boundary / weight / address logic is shared by twice the FMAs; one block per SM), 2 from 5 slices on, else 1
-int fd_groups_per_block(int n_slices) {
+int fd_groups_per_block(int n_slices, int npj) {
   const int ng = (n_slices + 3) / 4;
 #if FD_NG4
-  if (ng >= 4) return 4;
+  if (ng >= 4 && npj != 8) return 4;
 #endif
   return ng >= 2 ? 2 : 1;
 }
@@ -611,7 +648,7 @@ void fd_block_shape(int32_t* nb, int32_t* npj) {
 
 size_t fd_xd_bytes(const FdPlan& plan, const pyhst_geom_t* g, int* n_groups_alloc) {
   const int ng = (g->n_slices + 3) / 4;
-  const int per = fd_groups_per_block(g->n_slices);
+  const int per = fd_groups_per_block(g->n_slices, plan.npj);
   const int nga = (ng + per - 1) / per * per;     // whole blocks: spare zero groups for ragged counts
   if (n_groups_alloc) *n_groups_alloc = nga;
   const int64_t line_f4 = (int64_t)g->nx + 2 * plan.zpad;
@@ -666,26 +703,57 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
   prm.ranges = reinterpret_cast<const int2*>(plan.d_ranges);
   prm.n_bx = plan.n_bx;
   prm.W = plan.W;
-  const int ng = fd_groups_per_block(g->n_slices);
-  static uint64_t configured[3] = {0, 0, 0};
-  if (first_use_on_device(&configured[ng == 4 ? 2 : ng - 1])) {
-    if (ng == 4)
-      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(4)));
-    else if (ng == 2)
-      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(2)));
-    else
-      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(1)));
+  const int ng = fd_groups_per_block(g->n_slices, plan.npj);
+  const bool small = plan.npj == 8;     // sparse angle lists: 8 projections per block, 256 threads, bands of 4 lines
+  // small grids are split along the lines so that they fill the block slots a few times over
+  int n_sm = 148;
+  require_sm100(&n_sm);
+  const int64_t blocks = (int64_t)plan.n_bx * plan.n_chunks * (nga / ng);
+  const int64_t slots = (int64_t)n_sm * (ng == 4 ? 1 : (small ? 4 : 2));
+  int n_seg = (int)std::max<int64_t>(1, std::min<int64_t>(4, (3 * slots + blocks - 1) / blocks));
+  n_seg = std::max(1, std::min(n_seg, (g->nx + g->ny) / 256));
+  if (const char* e = std::getenv("PYHST_FD_SEG")) n_seg = std::max(1, std::atoi(e));
+  prm.n_seg = n_seg;
+  prm.part = nullptr;
+  prm.part_pitch = g->n_bins;
+  prm.part_stride = (int64_t)g->n_slices * g->n_angles * prm.part_pitch;
+  if (n_seg > 1) {
+    void* wp = nullptr;
+    PYHST_TRY(get_workspace(WS_FDP, (size_t)n_seg * prm.part_stride * 4, &wp));
+    prm.part = static_cast<float*>(wp);
   }
-  dim3 grid(plan.n_bx, plan.n_chunks, nga / ng);
+  dim3 grid(plan.n_bx, plan.n_chunks, (nga / ng) * n_seg);
   if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
-  StageScope scope(ST_FORWARD, stream);
-  scope.kernels();
-  if (ng == 4)
-    fp_diag_kernel<4><<<grid, FD_NT, fd_smem(4), stream>>>(prm);
-  else if (ng == 2)
-    fp_diag_kernel<2><<<grid, FD_NT, fd_smem(2), stream>>>(prm);
-  else
-    fp_diag_kernel<1><<<grid, FD_NT, fd_smem(1), stream>>>(prm);
+  static uint64_t configured[6] = {0, 0, 0, 0, 0, 0};
+  const int vi = (ng == 4 ? 2 : ng - 1) + (small ? 3 : 0);
+  const bool first = first_use_on_device(&configured[vi]);
+#define FD_LAUNCH(NGV, NPJV, RBV)                                                                                   \
+  do {                                                                                                              \
+    if (first)                                                                                                      \
+      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<NGV, NPJV, RBV>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                          (int)fd_smem(NGV, RBV, NPJV)));                                                \
+    StageScope scope(ST_FORWARD, stream);                                                                           \
+    scope.kernels();                                                                                                \
+    fp_diag_kernel<NGV, NPJV, RBV><<<grid, FD_NB / FD_M * NPJV, fd_smem(NGV, RBV, NPJV), stream>>>(prm);                  \
+  } while (0)
+  if (small) {
+    if (ng == 2) FD_LAUNCH(2, 8, 4);
+    else FD_LAUNCH(1, 8, 4);
+  } else {
+    if (ng == 4) FD_LAUNCH(4, 16, 8);
+    else if (ng == 2) FD_LAUNCH(2, 16, 8);
+    else FD_LAUNCH(1, 16, 8);
+  }
+#undef FD_LAUNCH
+  if (n_seg > 1) {
+    const int64_t n_rows_tab = (int64_t)g->n_slices * plan.n_tab;
+    const unsigned gy = (unsigned)std::min<int64_t>(n_rows_tab, 32768);
+    dim3 grid_c((g->n_bins + 255) / 256, gy, (unsigned)((n_rows_tab + gy - 1) / gy));
+    StageScope scope(ST_FORWARD, stream);
+    scope.kernels();
+    fd_combine_kernel<<<grid_c, 256, 0, stream>>>(d_sino, pitch, prm.part, prm.part_pitch, prm.part_stride, n_seg,
+                                                  g->n_bins, g->n_angles, plan.d_projs, plan.n_tab, n_rows_tab);
+  }
   PYHST_CUDA_TRY(cudaGetLastError());
   return PYHST_OK;
 }
