@@ -30,16 +30,16 @@ int pyhst_set_backproject_variant(int variant);
  * take the general path either way.  Returns the previous value. */
 int pyhst_set_halfacq_stitch(int enable);
 
-/* Selects the forward-projection kernel: 0 = automatic (default: the diagonal-line interval kernel for
- * dense angle lists -- chunks of >= 8 neighbouring projections share a staged window and the grid fills
- * the GPU several times over -- else the banded kernel), 1 = generic gather kernel (one thread per bin
- * and slice, global loads; kept for cross-checks and for pixel sizes the shared-memory kernels do not
- * cover), 2 = banded shared-memory kernel, 3 = interval form of the banded kernel (fewer shared-memory
- * loads, more instructions), 4 = interval form with 8 slices per thread (stacks with an even number of
- * slice groups and 16-projection chunks, else as 3), 5 = diagonal-line interval kernel forced
- * (PYHST_ERR_UNSUPPORTED when no projection has >= 1 + 2^-12 bins per pixel along an image diagonal,
- * i.e. pixel sizes below ~0.71 bins; projections it does not cover -- within 2^-12 of an image axis --
- * run on the banded kernel).  Returns the previous value. */
+/* Selects the forward-projection kernel: 0 = automatic (default: the diagonal-line interval kernel when its
+ * blocks are mostly full -- on average at least 0.55 x 16 (dense angle lists) or 0.55 x 8 (sparser ones)
+ * neighbouring projections share one staged window -- and the grid fills the GPU, else the banded kernel),
+ * 1 = generic gather kernel (one thread per bin and slice, global loads; kept for cross-checks and for pixel
+ * sizes the shared-memory kernels do not cover), 2 = banded shared-memory kernel, 3 = interval form of the
+ * banded kernel (fewer shared-memory loads, more instructions), 4 = interval form with 8 slices per thread
+ * (stacks with an even number of slice groups and 16-projection chunks, else as 3), 5 = diagonal-line interval
+ * kernel forced (PYHST_ERR_UNSUPPORTED when no projection has >= 1 + 2^-12 bins per pixel along an image
+ * diagonal, i.e. pixel sizes below ~0.71 bins; projections it does not cover -- within 2^-12 of an image axis,
+ * or whose window alone does not fit -- run on the banded kernel).  Returns the previous value. */
 int pyhst_set_forward_project_variant(int variant);
 
 /* Which kernel the last pyhst_forward_project of this process ran: 1 generic gather, 2 banded, 3 / 4
