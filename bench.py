@@ -409,8 +409,16 @@ def cpu_baseline(wl_mod, args):
     w, sino = _oracle_sample(wl_mod, args)
     sec = _time_oracle_step(oracle, w, sino)
     upd = w.n_slices * w.nx * w.ny * w.n_angles
+    # the oracle's filter is the direct O(B^2) convolution (its definition, not an FFT): timed alone as well, so
+    # that the projector pair's own share of the baseline can be read off
+    sec_filter = None
+    if w.mode != 2:
+        t0 = time.perf_counter()
+        oracle.ramp_filter(sino, filter=w.filter)
+        sec_filter = time.perf_counter() - t0
     return {"value": 2 * upd / sec / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "seconds": sec,
+            "seconds": sec, "seconds_ramp_filter_alone": sec_filter,
+            "projector_pair_gups": (2 * upd / max(sec - sec_filter, 1e-9) / 1e9) if sec_filter else None,
             "sample": "%d of the config's slices at full size (%dx%d, %d projections x %d bins): oracle FBP "
                       "(direct O(B^2) ramp convolution + backprojection, fp64, OpenMP) + oracle forward "
                       "projection, one pass" % (w.n_slices, w.ny, w.nx, w.n_angles, w.n_bins)}
