@@ -123,28 +123,31 @@ constexpr int FD_TX = 64, FD_TY = 32, FD_KMAX = 5, FD_NT = 256, FD_SEG = 14, FD_
 constexpr int FD_RW = FD_TX + 2 * FD_KMAX, FD_RH = FD_TY + 2 * FD_KMAX;
 static_assert(FD_SEG * FD_NSEG >= FD_RH && FD_RW * FD_NSEG <= FD_NT, "thread map of the fused dual kernel");
 
-__global__ void __launch_bounds__(FD_NT)
-ftv_dual_fused_kernel(const float* __restrict__ z, const float* __restrict__ p1, const float* __restrict__ p2,
-                      float* __restrict__ q1, float* __restrict__ q2, int nx, int ny,
-                      const float* __restrict__ fs, int K, int p_is_zero) {
-  __shared__ float S1[FD_RH][FD_RW];          // p1 as of the last completed step
-  __shared__ float SU[FD_RH][FD_RW];          // u of the current step
-  __shared__ float E2[FD_NSEG][FD_RW];        // p2 of the last row of every segment
+// FAST: the block's staged region lies strictly inside the image and K = FD_KMAX -- every bounds test on image
+// coordinates is dropped and the region's extent is a compile-time constant (the common case: all blocks but
+// those on the image border); the arithmetic per cell is the same.
+template <bool FAST>
+__device__ __forceinline__ void ftv_dual_fused_body(const float* __restrict__ z, const float* __restrict__ p1,
+                                                    const float* __restrict__ p2, float* __restrict__ q1,
+                                                    float* __restrict__ q2, int nx, int ny, float tau, float step, int Kr,
+                                                    int p_is_zero, float (*S1)[FD_RW], float (*SU)[FD_RW],
+                                                    float (*E2)[FD_RW]) {
+  const int K = FAST ? FD_KMAX : Kr;
   const int rw = FD_TX + 2 * K, rh = FD_TY + 2 * K;
   const int col = (int)threadIdx.x % rw, seg = (int)threadIdx.x / rw;
   const bool active = seg < FD_NSEG;
   const int row0 = seg * FD_SEG;
   const int64_t o = (int64_t)blockIdx.z * ny * nx;
   const int gx = blockIdx.x * FD_TX - K + col, gy0 = blockIdx.y * FD_TY - K + row0;
-  const float tau = fs[1], step = fs[2];
-  const bool x_in = gx >= 0 && gx < nx, right_ok = gx + 1 < nx && col + 1 < rw;
+  const bool x_in = FAST || (gx >= 0 && gx < nx);
+  const bool right_ok = (FAST || gx + 1 < nx) && col + 1 < rw;
 
   float vz[FD_SEG], v1[FD_SEG], v2[FD_SEG], vu[FD_SEG];
   if (active) {
 #pragma unroll
     for (int r = 0; r < FD_SEG; ++r) {
       const int gy = gy0 + r;
-      const bool in = x_in && gy >= 0 && gy < ny && row0 + r < rh;
+      const bool in = row0 + r < rh && (FAST || (x_in && gy >= 0 && gy < ny));
       const int64_t k = o + (int64_t)gy * nx + gx;
       vz[r] = in ? z[k] : 0.f;
       v1[r] = (in && !p_is_zero) ? p1[k] : 0.f;
@@ -172,11 +175,11 @@ ftv_dual_fused_kernel(const float* __restrict__ z, const float* __restrict__ p1,
 #pragma unroll
       for (int r = 0; r < FD_SEG; ++r) {
         const int gy = gy0 + r, row = row0 + r;
-        if (row < rh && x_in && gy >= 0 && gy < ny) {
+        if (row < rh && (FAST || (x_in && gy >= 0 && gy < ny))) {
           const float u = vu[r];
           const float ur = right_ok ? SU[row][col + 1] - u : 0.f;
           float ub = 0.f;
-          if (gy + 1 < ny && row + 1 < rh) ub = (r + 1 < FD_SEG ? vu[r + 1] : SU[row + 1][col]) - u;
+          if ((FAST || gy + 1 < ny) && row + 1 < rh) ub = (r + 1 < FD_SEG ? vu[r + 1] : SU[row + 1][col]) - u;
           const float n1 = fmaf(ur, step, v1[r]), n2 = fmaf(ub, step, v2[r]);
           // p = q / max(1, |q|) = q * min(1, 1/|q|)
           const float inv = fminf(1.f, rsqrtf(fmaf(n1, n1, n2 * n2)));
@@ -193,13 +196,30 @@ ftv_dual_fused_kernel(const float* __restrict__ z, const float* __restrict__ p1,
 #pragma unroll
     for (int r = 0; r < FD_SEG; ++r) {
       const int row = row0 + r, gy = gy0 + r;
-      if (row >= K && row < K + FD_TY && gy < ny) {
+      if (row >= K && row < K + FD_TY && (FAST || gy < ny)) {
         const int64_t k = o + (int64_t)gy * nx + gx;
         q1[k] = v1[r];
         q2[k] = v2[r];
       }
     }
   }
+}
+
+__global__ void __launch_bounds__(FD_NT)
+ftv_dual_fused_kernel(const float* __restrict__ z, const float* __restrict__ p1, const float* __restrict__ p2,
+                      float* __restrict__ q1, float* __restrict__ q2, int nx, int ny,
+                      const float* __restrict__ fs, int K, int p_is_zero) {
+  __shared__ float S1[FD_RH][FD_RW];          // p1 as of the last completed step
+  __shared__ float SU[FD_RH][FD_RW];          // u of the current step
+  __shared__ float E2[FD_NSEG][FD_RW];        // p2 of the last row of every segment
+  const float tau = fs[1], step = fs[2];
+  // the staged region [x0 - K, x0 + TX + K) x [y0 - K, y0 + TY + K) and its right / lower neighbours inside the image?
+  const int x0 = blockIdx.x * FD_TX, y0 = blockIdx.y * FD_TY;
+  const bool fast = K == FD_KMAX && x0 - K >= 0 && y0 - K >= 0 && x0 + FD_TX + K < nx && y0 + FD_TY + K < ny;
+  if (fast)
+    ftv_dual_fused_body<true>(z, p1, p2, q1, q2, nx, ny, tau, step, K, p_is_zero, S1, SU, E2);
+  else
+    ftv_dual_fused_body<false>(z, p1, p2, q1, q2, nx, ny, tau, step, K, p_is_zero, S1, SU, E2);
 }
 
 // x+ = z - tau G^T p (tau = 0: x+ = z);  y = x+ + mom (x+ - x);  x = x+
