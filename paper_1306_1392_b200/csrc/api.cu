@@ -319,7 +319,7 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, int want_diag, const
     FpPlan probe = pl;
     bool use = build_fd_tables(g, &pl.fd, &dprojs, &dchunks, &ranges, &legacy);
     // sparse angle lists fan out: few projections fit one staged window -- blocks of 8 projections instead of 16
-    if (use && (double)dprojs.size() / (double)dchunks.size() < 8.0 && !std::getenv("PYHST_FD_NPJ16"))
+    if (use && (double)dprojs.size() / (double)dchunks.size() < 8.0)
       use = build_fd_tables(g, &pl.fd, &dprojs, &dchunks, &ranges, &legacy, 8);
     if (use && want_diag == 1) {
       // automatic choice: the diagonal-line kernel pays off when its blocks are mostly full (neighbouring

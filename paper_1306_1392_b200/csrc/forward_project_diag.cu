@@ -710,9 +710,8 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
   require_sm100(&n_sm);
   const int64_t blocks = (int64_t)plan.n_bx * plan.n_chunks * (nga / ng);
   const int64_t slots = (int64_t)n_sm * (ng == 4 ? 1 : (small ? 4 : 2));
-  int n_seg = (int)std::max<int64_t>(1, std::min<int64_t>(4, (3 * slots + blocks - 1) / blocks));
+  int n_seg = (int)std::max<int64_t>(1, std::min<int64_t>(8, (4 * slots + blocks - 1) / blocks));
   n_seg = std::max(1, std::min(n_seg, (g->nx + g->ny) / 256));
-  if (const char* e = std::getenv("PYHST_FD_SEG")) n_seg = std::max(1, std::atoi(e));
   prm.n_seg = n_seg;
   prm.part = nullptr;
   prm.part_pitch = g->n_bins;
