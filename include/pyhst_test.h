@@ -18,7 +18,10 @@ extern "C" {
  * pixel kernel (global loads; kept for cross-checks), 2 = tiled shared-memory kernel, 3 = run
  * kernel with 4 slices per thread, 4 = run kernel with 8 slices per thread (what 0 picks for
  * pixel sizes below sqrt(2) bins), 6 = the same with the interpolation written as packed FFMA2 (8 fewer
- * warp instructions per step, same time: an FFMA2 costs two issue slots on sm_100a, profiles/r02_micro.md).  A variant that does not cover the geometry makes the next
+ * warp instructions per step, same time: an FFMA2 costs two issue slots on sm_100a, profiles/r02_micro.md), 7 = run kernel
+ * with 16 slices per thread for stacks of >= 13 slices (runs of 4 pixels, one 512-thread block per SM; 11 % fewer
+ * instructions but latency-bound with one run in flight: measured slower, profiles/r02_micro.md sec. C; other stacks
+ * as 4).  A variant that does not cover the geometry makes the next
  * call return PYHST_ERR_UNSUPPORTED.  Returns the previous value.  Test/bench hook; results
  * agree within FP32 rounding. */
 int pyhst_set_backproject_variant(int variant);

@@ -96,6 +96,7 @@ DeviceCtx& ctx() { return *ctx_of(std::max(0, current_device())); }
 int filter_variant() { return g_filter_variant; }
 int patch_gemm_variant() { return g_patch_gemm_variant; }
 bool run8_packed() { return g_bp_variant == 6; }
+int bp_variant() { return g_bp_variant; }
 
 int current_device() {
   int dev = -1;
@@ -454,6 +455,7 @@ static int pick_bp_kernel(double pixel_size, int32_t n_slices) {
     case 3: return run_ok ? 3 : -1;
     case 4: return run8_ok ? 4 : -1;
     case 6: return run8_ok ? 4 : -1;   // run8 with packed FFMA2 interpolation (measured alternative)
+    case 7: return run8_ok ? 4 : -1;   // run16 forced where it covers the stack (else run8)
     // one slice group (<= 4 slices): the 8-slice kernel would spend half of its FMAs on a duplicate
     default: return (run8_ok && n_slices > 4) ? 4 : (run_ok ? 3 : (tiled_ok ? 2 : 1));
   }
@@ -496,7 +498,7 @@ int pyhst_profile_read(double* ms, int64_t* kernels, int64_t* fft_execs, int32_t
 
 int pyhst_set_backproject_variant(int variant) {
   const int prev = g_bp_variant;
-  if (variant >= 0 && variant <= 6 && variant != 5) g_bp_variant = variant;
+  if (variant >= 0 && variant <= 7 && variant != 5) g_bp_variant = variant;
   return prev;
 }
 

@@ -399,6 +399,11 @@ int launch_backproject_run8(const float4* d_qi, const QiLayout& L, const BpArgs&
   const int W = backproject_run8_window(a.pixel_size);
   if (W == 0 || W > L.n_bins + 2 * L.zpad || L.zpad < W + 2)
     return set_error(PYHST_ERR_UNSUPPORTED, "run8 backprojector: window %d does not fit", W);
+  // variant 7: 16 slices per thread where the stack has >= 13 slices (backproject_run16.cu) -- measured slower
+  // (config 2: 19.2 vs 17.9 ms: 11 % fewer instructions, but one run in flight per thread instead of four leaves
+  // the LDS -> FFMA latency exposed: issue slots 71 % instead of 86 %), so not the default
+  if (bp_variant() == 7 && backproject_run16_covers(a.pixel_size, L.n_groups))
+    return launch_backproject_run16(d_qi, L, a, d_run, n_a, n_b, stream);
   // two instantiations: slots of 80 bins, 4 stages (pixel size <= 1.03), or 112 bins, 3 stages
   const bool packed = run8_packed();
   if (W <= 80)

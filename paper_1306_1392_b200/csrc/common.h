@@ -166,6 +166,12 @@ int backproject_run8_window(double pixel_size);
 int launch_backproject_run8(const float4* d_qi, const QiLayout& L, const BpArgs& a,
                             const RunProj* d_run, int32_t n_a, int32_t n_b, cudaStream_t stream);
 
+// run16 kernel (16 slices per thread, stacks of >= 13 slices; backproject_run16.cu)
+bool backproject_run16_covers(double pixel_size, int n_groups);
+int launch_backproject_run16(const float4* d_qi, const QiLayout& L, const BpArgs& a,
+                             const RunProj* d_run, int32_t n_a, int32_t n_b, cudaStream_t stream);
+int bp_variant();   // pyhst_set_backproject_variant value
+
 // ---- interleaved, zero-padded image layout consumed by the banded forward projector -------
 // XI[g][v][zpad + u][sl]: slice group g = s / 4, one float4 per (g, line v, position u); every
 // line carries `zpad` zero float4 on both sides.  Two copies: lines = image rows (u = j, v = i)

@@ -60,7 +60,7 @@ BP_CASES = [
 ]
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 6])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 6, 7])
 @pytest.mark.parametrize("case", BP_CASES)
 def test_backproject_matches_oracle(lib, oracle, case, variant):
     S, P, B, nx, ny, h, axis, drift = case
@@ -103,6 +103,23 @@ def test_backproject_batch_independence(lib):
     finally:
         lib.set_backproject_variant(prev)
     assert (full[2] == one8[0]).all()
+
+
+@pytest.mark.parametrize("S", [13, 16, 18])
+def test_backproject_run16_matches_oracle(lib, oracle, S):
+    """pyhst_test.h variant 7: 16 slices per thread (four slice groups per block, ragged stacks read a duplicate group
+    that is never stored); 360-degree angles exercise both classes and the row reversal."""
+    wl = lib.workloads
+    P, B, nx, ny = 45, 230, 150, 140
+    w = wl.custom(S, P, B, nx, ny, drift=1.5, jitter_angles=0.01, seed=S, span=2 * math.pi)
+    sino = wl.random_sinogram(S, P, B, seed=S)
+    want = oracle.backproject(sino, w.angles, w.axis, nx, ny, scale=0.7)
+    prev = lib.set_backproject_variant(7)
+    try:
+        got = lib.backproject(_dev(sino), w.angles, w.axis, nx, ny, scale=0.7).cpu().numpy()
+    finally:
+        lib.set_backproject_variant(prev)
+    assert_parity(got, want, "backproject run16, %d slices" % S)
 
 
 def test_backproject_affine_rows(lib):
