@@ -43,6 +43,9 @@ namespace {
 #ifndef FD_NG4
 #define FD_NG4 1
 #endif
+#ifndef FD_CHECK
+#define FD_CHECK 0
+#endif
 constexpr int FD_NB = 64;      // intervals per block (FD_NB - 1 complete bins)
 constexpr int FD_NPJ = 16;     // projections per block (at most)
 constexpr int FD_M = 2;        // neighbouring intervals per thread
@@ -327,6 +330,14 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
             const bool in = jm[q] < jm[q + 1];                  // the interval holds that pixel
             uint32_t addr;
             asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(addr) : "r"(__float_as_int(jm[q])), "r"(mul), "r"(cb + r * FD_PW * 16));
+#if FD_CHECK
+            // debug build (-DFD_CHECK=1): a claimed pixel must lie inside the window staged for its line
+            {
+              const int col = (int)(addr - (buf_u32 + (uint32_t)(st * STAGE_F4 * 16) + (uint32_t)((r0 + r) * FD_PW * 16))) / 16;
+              const int lo = bias + skew * (r0 + r);
+              if (in && (col < lo || col >= lo + W)) __trap();
+            }
+#endif
 #if FD_PACKED
             const float fz = in ? f : 0.f, gz = in ? g : 0.f;
             fd_line<NG, PLANE>(acc[q], acc[q + 1], fz, gz, addr);
