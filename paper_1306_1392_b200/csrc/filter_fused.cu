@@ -28,6 +28,9 @@ namespace pyhst {
 
 namespace {
 
+#ifndef FF_SQUARE_TW
+#define FF_SQUARE_TW 1
+#endif
 constexpr int FF_MAX_LOG2 = 13;   // M <= 8192: 2 sequences x 9/8 M x 8 B = 144 KB of shared memory
 
 __device__ __forceinline__ int ff_phys(int i) { return i + (i >> 3); }   // one pad per 8 complex: no bank conflicts
@@ -81,17 +84,19 @@ __device__ __forceinline__ void small_dft(float2 (&v)[R]) {
   }
 }
 
-// powers w^1 .. w^{R-1} of w = tw[k] from three table reads (k, 2k, 4k < M) and products
+// powers w^1 .. w^{R-1} of w = tw[k]: one table read, w^2 and w^4 by squaring (two roundings more on those two
+// factors, ~2e-7 relative: the filter stays at rel-L2 3e-7 against the oracle) -- the three dependent global reads
+// per butterfly were the kernel's top stall (long_scoreboard); FF_SQUARE_TW = 0 restores the table reads
 template <int R>
 __device__ __forceinline__ void twiddle_powers(const float2* __restrict__ tw, int k, float2 (&w)[R]) {
   w[0] = make_float2(1.f, 0.f);
   w[1] = tw[k];
   if (R >= 4) {
-    w[2] = tw[2 * k];
+    w[2] = FF_SQUARE_TW ? cmul(w[1], w[1]) : tw[2 * k];
     w[3] = cmul(w[1], w[2]);
   }
   if (R == 8) {
-    w[4] = tw[4 * k];
+    w[4] = FF_SQUARE_TW ? cmul(w[2], w[2]) : tw[4 * k];
     w[5] = cmul(w[1], w[4]);
     w[6] = cmul(w[2], w[4]);
     w[7] = cmul(w[3], w[4]);
