@@ -116,6 +116,21 @@ def _dev(t, name):
     return c_void_p(t.data_ptr())
 
 
+def _dev_sino(t, name):
+    """(device pointer, sino_pitch) of a float32 CUDA sinogram stack [S, P, B]: contiguous, or rows pitched
+    (stride(2) == 1, stride(1) = pitch >= B, stride(0) == P * pitch -- e.g. a [:, :, :B] view of a wider stack)."""
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.dim() == 3):
+        raise PyhstError("%s must be a float32 CUDA tensor [S, P, B]" % name)
+    if t.is_contiguous():
+        return c_void_p(t.data_ptr()), 0
+    s, p, b = t.shape
+    st = t.stride()
+    if st[2] == 1 and st[1] >= b and (s == 1 or st[0] == p * st[1]):
+        return c_void_p(t.data_ptr()), int(st[1])
+    raise PyhstError("%s must be contiguous or have pitched rows" % name)
+
+
 def _geom(n_slices, n_angles, n_bins, angles, axis, nx, ny, pixel_size, sino_pitch=0):
     angles = np.ascontiguousarray(angles, dtype=np.float64)
     axis = np.ascontiguousarray(axis, dtype=np.float64)
@@ -150,8 +165,9 @@ def backproject(d_sino, angles, axis, nx, ny, pixel_size=1.0, scale=1.0, out=Non
     s, p, b = d_sino.shape
     if out is None:
         out = torch.empty((s, ny, nx), dtype=torch.float32, device=d_sino.device)
-    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size)
-    _check(lib.pyhst_backproject(_dev(d_sino, "d_sino"), _dev(out, "out"), ctypes.byref(g), scale,
+    ptr, pitch = _dev_sino(d_sino, "d_sino")
+    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size, pitch)
+    _check(lib.pyhst_backproject(ptr, _dev(out, "out"), ctypes.byref(g), scale,
                                  _stream(stream)), "pyhst_backproject")
     return out
 
@@ -164,8 +180,9 @@ def forward_project(d_img, angles, axis, n_bins, pixel_size=1.0, scale=1.0, out=
     p = len(angles)
     if out is None:
         out = torch.empty((s, p, n_bins), dtype=torch.float32, device=d_img.device)
-    g = _geom(s, p, n_bins, angles, axis, nx, ny, pixel_size)
-    _check(lib.pyhst_forward_project(_dev(d_img, "d_img"), _dev(out, "out"), ctypes.byref(g), scale,
+    ptr, pitch = _dev_sino(out, "out")
+    g = _geom(s, p, n_bins, angles, axis, nx, ny, pixel_size, pitch)
+    _check(lib.pyhst_forward_project(_dev(d_img, "d_img"), ptr, ctypes.byref(g), scale,
                                      _stream(stream)), "pyhst_forward_project")
     return out
 
@@ -178,8 +195,9 @@ def fbp(d_sino_raw, angles, axis, nx, ny, pixel_size=1.0, filter=FILTER_RAMLAK, 
     s, p, b = d_sino_raw.shape
     if out is None:
         out = torch.empty((s, ny, nx), dtype=torch.float32, device=d_sino_raw.device)
-    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size)
-    _check(lib.pyhst_fbp(_dev(d_sino_raw, "d_sino_raw"), _dev(out, "out"), ctypes.byref(g), filter, mode,
+    ptr, pitch = _dev_sino(d_sino_raw, "d_sino_raw")
+    g = _geom(s, p, b, angles, axis, nx, ny, pixel_size, pitch)
+    _check(lib.pyhst_fbp(ptr, _dev(out, "out"), ctypes.byref(g), filter, mode,
                          _stream(stream)), "pyhst_fbp")
     return out
 

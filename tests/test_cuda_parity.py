@@ -278,6 +278,36 @@ def test_adjoint_identity_on_device(lib, B, axis):
     assert abs(lhs - rhs) <= bound, (lhs, rhs, bound)
 
 
+def test_pitched_sinograms(lib, oracle):
+    """pyhst_geom_t.sino_pitch: rows of the sinogram stack further apart than n_bins (a view of a wider stack), for the
+    input of pyhst_backproject / pyhst_fbp and the output of pyhst_forward_project (every forward kernel); the gap
+    between the rows is neither read nor written."""
+    import torch
+    wl = lib.workloads
+    S, P, B, nx, ny, pitch = 6, 33, 150, 120, 110, 164
+    w = wl.custom(S, P, B, nx, ny, drift=1.0, jitter_angles=0.01, seed=4, span=2 * math.pi)
+    sino = wl.random_sinogram(S, P, B, seed=4)
+    wide = torch.full((S, P, pitch), float("nan"), dtype=torch.float32, device="cuda")
+    wide[:, :, :B] = torch.from_numpy(sino).cuda()
+    view = wide[:, :, :B]
+    assert not view.is_contiguous()
+    assert_parity(lib.backproject(view, w.angles, w.axis, nx, ny).cpu().numpy(),
+                  oracle.backproject(sino, w.angles, w.axis, nx, ny), "backproject, pitched rows")
+    assert_parity(lib.fbp(view, w.angles, w.axis, nx, ny, filter=1).cpu().numpy(),
+                  oracle.fbp(sino, w.angles, w.axis, nx, ny, filter=1), "fbp, pitched rows")
+    x = wl.random_image(S, ny, nx, seed=4)
+    want = oracle.forward_project(x, w.angles, w.axis, B)
+    for variant in (0, 1, 2, 4, 5):
+        out = torch.full((S, P, pitch), -7.0, dtype=torch.float32, device="cuda")
+        prev = lib.set_forward_project_variant(variant)
+        try:
+            lib.forward_project(_dev(x), w.angles, w.axis, B, out=out[:, :, :B])
+        finally:
+            lib.set_forward_project_variant(prev)
+        assert_parity(out[:, :, :B].cpu().numpy(), want, "forward_project variant %d, pitched rows" % variant)
+        assert (out[:, :, B:] == -7.0).all().item(), "variant %d wrote between the rows" % variant
+
+
 # ------------------------------------------------------------------------------ ramp filter
 @pytest.mark.parametrize("f", [0, 1, 2, 3])
 @pytest.mark.parametrize("b_in,b_out,pad,weights", [(367, 367, 0, False), (128, 256, 0, True),
