@@ -211,31 +211,54 @@ patch_residual_kernel(float* __restrict__ r, const float* __restrict__ data, int
   if (part) block_store_sum(acc, part);
 }
 
+// Whether a pixel of a patch is a core pixel of that patch, and how many patches cover it, factorises over the two
+// axes.  tab[axis][idx][off] (32 offsets per patch index; axis 0: rows, na entries; axis 1: columns, nb entries):
+// bit 7 = "the pixel at offset off of patch idx has idx as its core patch along this axis", bits 0..6 = patches
+// that contain it along this axis.  (na + nb) * 32 bytes, rebuilt per call by one small kernel.
+__global__ void patch_axis_tables_kernel(PatchGrid pg, unsigned char* __restrict__ tab) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int total = (pg.na + pg.nb) * 32;
+  if (t >= total) return;
+  const int idx_all = t >> 5, off = t & 31;
+  const int axis = idx_all >= pg.na ? 1 : 0, idx = axis ? idx_all - pg.na : idx_all;
+  unsigned char v = 0;
+  if (off < pg.m) {
+    const int n = axis ? pg.nx : pg.ny, cnt = axis ? pg.nb : pg.na;
+    const int j = pg_origin(idx, n, pg.m, pg.st) + off;
+    int lo, hi;
+    pg_cover_1d(j, n, pg.m, pg.st, cnt, &lo, &hi);
+    v = (unsigned char)((hi - lo + 1) | (pg_core_1d(j, n, pg.m, pg.st, cnt) == idx ? 0x80 : 0));
+  }
+  tab[t] = v;
+}
+
 // Algorithm 1: P'_{p i} = [p == C_j] (R_j + rho (N_v X_j - S_j)) + rho (P_{p i} - X_j), j = r_p + i
+// One thread per element, patches of one slice along blockIdx.x; the core / cover logic comes from the axis tables
+// (2 byte loads instead of 2 m^2-fold evaluated integer routines): the kernel runs at the speed of its two streams
+// (P in, P' out).
 __global__ void __launch_bounds__(256)
 patch_pprime_kernel(const float* __restrict__ Pm, const float* __restrict__ X, const float* __restrict__ S,
-                    const float* __restrict__ R, PatchGrid pg, float rho, float* __restrict__ Pp, int64_t n_total) {
-  const int64_t e = (int64_t)blockIdx.x * 256 + threadIdx.x;
-  if (e >= n_total) return;
-  const int mm = pg.m * pg.m;
-  const int64_t N = (int64_t)pg.na * pg.nb;
-  const int64_t s = e / (N * mm);
-  const int64_t rem = e - s * N * mm;
-  const int p = (int)(rem / mm), i = (int)(rem - (int64_t)p * mm);
-  const int a = p / pg.nb, b = p - a * pg.nb;
-  const int iy = i / pg.m, ix = i - iy * pg.m;
-  const int jy = pg_origin(a, pg.ny, pg.m, pg.st) + iy, jx = pg_origin(b, pg.nx, pg.m, pg.st) + ix;
+                    const float* __restrict__ R, PatchGrid pg, float rho, float* __restrict__ Pp,
+                    const unsigned char* __restrict__ tab) {
+  const int m = pg.m, mm = m * m;
+  const int N = pg.na * pg.nb;
+  const int64_t s = blockIdx.y;
+  const uint32_t e = blockIdx.x * 256u + threadIdx.x;       // element of the slice: patch * mm + i  (< 2^32)
+  if (e >= (uint32_t)N * (uint32_t)mm) return;
+  const uint32_t p = e / (uint32_t)mm, i = e - p * (uint32_t)mm;
+  const uint32_t a = p / (uint32_t)pg.nb, b = p - a * (uint32_t)pg.nb;
+  const uint32_t iy = i / (uint32_t)m, ix = i - iy * (uint32_t)m;
+  const int jy = pg_origin((int)a, pg.ny, m, pg.st) + (int)iy, jx = pg_origin((int)b, pg.nx, m, pg.st) + (int)ix;
   const int64_t j = s * (int64_t)pg.ny * pg.nx + (int64_t)jy * pg.nx + jx;
+  const int64_t k = s * (int64_t)N * mm + e;
   const float x = X[j];
-  float v = rho * (Pm[e] - x);
-  if (pg_core_1d(jy, pg.ny, pg.m, pg.st, pg.na) == a && pg_core_1d(jx, pg.nx, pg.m, pg.st, pg.nb) == b) {
-    int alo, ahi, blo, bhi;
-    pg_cover_1d(jy, pg.ny, pg.m, pg.st, pg.na, &alo, &ahi);
-    pg_cover_1d(jx, pg.nx, pg.m, pg.st, pg.nb, &blo, &bhi);
-    const float nv = (float)((ahi - alo + 1) * (bhi - blo + 1));
+  float v = rho * (Pm[k] - x);
+  const unsigned ty = tab[a * 32u + iy], tx = tab[(pg.na + b) * 32u + ix];
+  if (ty & tx & 0x80u) {
+    const float nv = (float)((ty & 0x7fu) * (tx & 0x7fu));
     v += R[j] + rho * fmaf(nv, x, -S[j]);
   }
-  Pp[e] = v;
+  Pp[k] = v;
 }
 
 // FISTA on the coefficients: u = v - g / Lw; w+ = shrink(u, beta / Lw); v = w+ + mom (w+ - w); w = w+
@@ -300,6 +323,7 @@ int patch_gemm(const float* A, const float* Bm, float* C, int64_t M, int N, int 
 struct PatchWs {
   float *P, *Pp, *X, *S, *R, *r;
   double* part;
+  unsigned char* tab;   // axis tables of patch_pprime_kernel, (na + nb) * 32 bytes
   int64_t n_part;
   size_t bytes;
 };
@@ -322,6 +346,7 @@ PatchWs carve(char* base, int S, const PatchGrid& pg, int n_angles, int n_bins) 
   const int64_t g_res = (int64_t)((n_bins + 31) / 32) * std::min<int64_t>(((int64_t)S * n_angles + 7) / 8, 4096);
   w.n_part = std::max<int64_t>(std::max(g_img, g_res), 1024);
   w.part = reinterpret_cast<double*>(take((size_t)w.n_part * 8));
+  w.tab = reinterpret_cast<unsigned char*>(take((size_t)(pg.na + pg.nb) * 32));
   w.bytes = off;
   return w;
 }
@@ -354,8 +379,10 @@ int patch_gradient_device(const float* d_W, const float* d_D, const float* d_dat
   if (!d_G) return PYHST_OK;
   PYHST_TRY(pyhst_backproject(w.r, w.R, &gs, 1.f, stream));
   // P' and G <- 2 P' D^T
-  const int64_t n_total = (int64_t)S * N * mm;
-  patch_pprime_kernel<<<(unsigned)((n_total + 255) / 256), 256, 0, stream>>>(w.P, w.X, w.S, w.R, pg, rho, w.Pp, n_total);
+  if (N * mm >= ((int64_t)1 << 32) || N >= ((int64_t)1 << 31))
+    return set_error(PYHST_ERR_UNSUPPORTED, "patch: more than 2^32 patch elements per slice");
+  patch_axis_tables_kernel<<<((pg.na + pg.nb) * 32 + 255) / 256, 256, 0, stream>>>(pg, w.tab);
+  patch_pprime_kernel<<<dim3((unsigned)((N * mm + 255) / 256), (unsigned)S), 256, 0, stream>>>(w.P, w.X, w.S, w.R, pg, rho, w.Pp, w.tab);
   PYHST_TRY(patch_gemm(w.Pp, d_D, d_G, N, n_atoms, mm, 2.f, true, S, stream));
   PYHST_CUDA_TRY(cudaGetLastError());
   return PYHST_OK;
