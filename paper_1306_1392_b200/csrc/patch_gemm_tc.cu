@@ -20,6 +20,8 @@
 //     and writes its row with 16-byte stores.
 // The FP32 SIMT kernel of patches.cu remains the fall-back for shapes this kernel does not cover
 // (K % 32 != 0, N % 16 != 0, N > 256, operands that do not fit in shared memory) and the cross-check.
+#include <algorithm>
+
 #include "common.h"
 
 namespace pyhst {
@@ -79,15 +81,13 @@ __device__ __forceinline__ uint32_t core_offset_f(int r, int kc4, int sbo_f) {  
 template <bool TRANS_B, int TMEM_COLS>
 __global__ void __launch_bounds__(TC_NT)
 patch_gemm_tc_kernel(const float* __restrict__ A, const float* __restrict__ Bm, float* __restrict__ C, int64_t M,
-                     int N, int K, float alpha, int tiles_per_slice) {
+                     int N, int K, float alpha, int tiles_per_slice, int64_t n_tiles_total) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   __shared__ uint64_t mma_bar;
   __shared__ uint32_t tmem_base_smem;
   const int tid = threadIdx.x, warp = tid >> 5;
-  const int z = blockIdx.x / tiles_per_slice;
-  const int64_t m0 = (int64_t)(blockIdx.x - z * tiles_per_slice) * TC_BM;
-  A += (int64_t)z * M * K;
-  C += (int64_t)z * M * N;
+  const float* const A_all = A;
+  float* const C_all = C;
 
   // shared memory: B hi, B lo [N x K]; A chunk hi, lo [128 x 32]
   const int b_floats = N * K;
@@ -140,18 +140,41 @@ patch_gemm_tc_kernel(const float* __restrict__ A, const float* __restrict__ Bm, 
 
   const int n_chunks = K / TC_KC;
   uint32_t phase = 0;
+  // persistent CTA: B (hi / lo) is staged once and serves every 128-row tile this CTA takes.  The A chunk that is
+  // staged next is always already on its way: its eight 16-byte loads per thread are issued right after the MMAs of
+  // the chunk before it (software pipelining through registers), so the global latency overlaps the MMAs, the
+  // barrier and the epilogue.
+  constexpr int A_PER_THREAD = TC_BM * (TC_KC / 4) / TC_NT;
+  float4 av[A_PER_THREAD];
+  auto load_chunk = [&](int64_t tl, int c) {   // 128 rows x 8 groups; a warp reads 4 rows x 128 contiguous bytes
+    const int zz = (int)(tl / tiles_per_slice);
+    const int64_t mm0 = (tl - (int64_t)zz * tiles_per_slice) * TC_BM;
+    const float* Az = A_all + (int64_t)zz * M * K;
+#pragma unroll
+    for (int q = 0; q < A_PER_THREAD; ++q) {
+      const int e = tid + q * TC_NT;
+      const int r = ((e >> 6) << 3) | (e & 7), k4 = (e >> 3) & 7;   // 8 rows x 4 groups per warp: contiguous stores
+      av[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (mm0 + r < M) av[q] = __ldg(reinterpret_cast<const float4*>(Az + (mm0 + r) * K + c * TC_KC + 4 * k4));
+    }
+  };
+  if ((int64_t)blockIdx.x < n_tiles_total) load_chunk(blockIdx.x, 0);
+  for (int64_t tile = blockIdx.x; tile < n_tiles_total; tile += gridDim.x) {
+  const int z = (int)(tile / tiles_per_slice);
+  const int64_t m0 = (tile - (int64_t)z * tiles_per_slice) * TC_BM;
+  C = C_all + (int64_t)z * M * N;
   for (int c = 0; c < n_chunks; ++c) {
     if (c > 0) {   // the MMAs of the previous chunk have read the A buffers
       mbar_wait(&mma_bar, phase);
       phase ^= 1;
     }
-    // ---- stage the A chunk: 128 rows x 8 groups; a warp reads 4 rows x 128 contiguous bytes
-    for (int e = tid; e < TC_BM * (TC_KC / 4); e += TC_NT) {
-      const int r = ((e >> 6) << 3) | (e & 7), k4 = (e >> 3) & 7;   // 8 rows x 4 groups per warp: contiguous stores
-      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (m0 + r < M) v = *reinterpret_cast<const float4*>(A + (m0 + r) * K + c * TC_KC + 4 * k4);
+    // ---- stage the A chunk from the registers
+#pragma unroll
+    for (int q = 0; q < A_PER_THREAD; ++q) {
+      const int e = tid + q * TC_NT;
+      const int r = ((e >> 6) << 3) | (e & 7), k4 = (e >> 3) & 7;
       const uint32_t o = core_offset_f(r, k4, sbo_a_f);
-      store_hi_lo(a_hi + o, a_lo + o, v);
+      store_hi_lo(a_hi + o, a_lo + o, av[q]);
     }
     // generic-proxy writes -> visible to the tensor core (async proxy), then hand over to the issuing thread
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -167,7 +190,7 @@ patch_gemm_tc_kernel(const float* __restrict__ A, const float* __restrict__ Bm, 
         const uint64_t da_lo = umma_desc(a_lo_s + a_off, 128u, (uint32_t)sbo_a_f * 4u);
         const uint64_t db_hi = umma_desc(b_hi_s + b_off, 128u, (uint32_t)sbo_b_f * 4u);
         const uint64_t db_lo = umma_desc(b_lo_s + b_off, 128u, (uint32_t)sbo_b_f * 4u);
-        umma_tf32(tmem_d, da_lo, db_hi, idesc, (c | j) ? 1u : 0u);   // small terms first
+        umma_tf32(tmem_d, da_lo, db_hi, idesc, (c | j) ? 1u : 0u);   // small terms first; a new tile starts a new sum
         umma_tf32(tmem_d, da_hi, db_lo, idesc, 1u);
         umma_tf32(tmem_d, da_hi, db_hi, idesc, 1u);
       }
@@ -176,8 +199,12 @@ patch_gemm_tc_kernel(const float* __restrict__ A, const float* __restrict__ Bm, 
                        smem_u32(&mma_bar))
                    : "memory");
     }
+    // the next chunk (of this tile or of the CTA's next tile) goes on its way
+    if (c + 1 < n_chunks) load_chunk(tile, c + 1);
+    else if (tile + gridDim.x < n_tiles_total) load_chunk(tile + gridDim.x, 0);
   }
   mbar_wait(&mma_bar, phase);
+  phase ^= 1;
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
   // ---- epilogue: thread = TMEM lane = tile row
@@ -202,8 +229,11 @@ patch_gemm_tc_kernel(const float* __restrict__ A, const float* __restrict__ Bm, 
                         alpha * __uint_as_float(v[4 * q + 2]), alpha * __uint_as_float(v[4 * q + 3]));
     }
   }
+  // the accumulator has been read: the next tile's MMAs may overwrite it
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  }   // tiles
   if (warp == 0)
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"((uint32_t)TMEM_COLS) : "memory");
 }
@@ -214,7 +244,10 @@ int launch_tc(const float* A, const float* Bm, float* C, int64_t M, int N, int K
   const size_t smem = ((size_t)2 * N * K + (size_t)2 * TC_BM * TC_KC) * sizeof(float);
   const int64_t tiles = (M + TC_BM - 1) / TC_BM;
   if (tiles * n_slices > 0x7fffffff) return set_error(PYHST_ERR_UNSUPPORTED, "patch GEMM: too many tiles");
-  const unsigned grid = (unsigned)(tiles * n_slices);
+  int n_sm = 148;
+  require_sm100(&n_sm);
+  // persistent CTAs, two per SM (their loads and MMAs overlap one another); B is staged once per CTA
+  const unsigned grid = (unsigned)std::min<int64_t>(tiles * n_slices, (int64_t)2 * n_sm);
 #define PYHST_TC_LAUNCH(COLS)                                                                                     \
   do {                                                                                                            \
     static PerDeviceSize configured;                                                                              \
@@ -223,7 +256,7 @@ int launch_tc(const float* A, const float* Bm, float* C, int64_t M, int N, int K
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));               \
       configured.here() = smem;                                                                                   \
     }                                                                                                             \
-    patch_gemm_tc_kernel<TRANS_B, COLS><<<grid, TC_NT, smem, stream>>>(A, Bm, C, M, N, K, alpha, (int)tiles);     \
+    patch_gemm_tc_kernel<TRANS_B, COLS><<<grid, TC_NT, smem, stream>>>(A, Bm, C, M, N, K, alpha, (int)tiles, tiles * n_slices);     \
   } while (0)
   if (N <= 32) PYHST_TC_LAUNCH(32);
   else if (N <= 64) PYHST_TC_LAUNCH(64);
