@@ -165,23 +165,22 @@ __global__ void __launch_bounds__(1024) sum_partials_kernel(const double* __rest
 // part = sum_j sum_{p covers j} (X_j - P_p(j))^2   (the similarity term of eq. 8)
 __global__ void __launch_bounds__(256)
 patch_compose_kernel(const float* __restrict__ Pm, PatchGrid pg, float* __restrict__ X, float* __restrict__ S,
-                     double* __restrict__ part) {
+                     double* __restrict__ part, const short4* __restrict__ pix) {
   const int jx = blockIdx.x * 32 + threadIdx.x, jy = blockIdx.y * 8 + threadIdx.y;
   const int64_t s = blockIdx.z;
   const int mm = pg.m * pg.m;
   const float* Ps = Pm + s * (int64_t)pg.na * pg.nb * mm;
   double sim = 0.0;
   if (jx < pg.nx && jy < pg.ny) {
-    const int ca = pg_core_1d(jy, pg.ny, pg.m, pg.st, pg.na), cb = pg_core_1d(jx, pg.nx, pg.m, pg.st, pg.nb);
+    // per-axis pixel tables (patch_axis_tables_kernel): x = core patch, y / z = first / last covering patch
+    const short4 ty = pix[jy], tx = pix[pg.ny + jx];
+    const int ca = ty.x, cb = tx.x;
     const int coy = pg_origin(ca, pg.ny, pg.m, pg.st), cox = pg_origin(cb, pg.nx, pg.m, pg.st);
     const float x = Ps[(int64_t)(ca * pg.nb + cb) * mm + (jy - coy) * pg.m + (jx - cox)];
-    int alo, ahi, blo, bhi;
-    pg_cover_1d(jy, pg.ny, pg.m, pg.st, pg.na, &alo, &ahi);
-    pg_cover_1d(jx, pg.nx, pg.m, pg.st, pg.nb, &blo, &bhi);
     float sum = 0.f;
-    for (int a = alo; a <= ahi; ++a) {
+    for (int a = ty.y; a <= ty.z; ++a) {
       const int oy = pg_origin(a, pg.ny, pg.m, pg.st);
-      for (int b = blo; b <= bhi; ++b) {
+      for (int b = tx.y; b <= tx.z; ++b) {
         const int ox = pg_origin(b, pg.nx, pg.m, pg.st);
         const float v = Ps[(int64_t)(a * pg.nb + b) * mm + (jy - oy) * pg.m + (jx - ox)];
         sum += v;
@@ -215,9 +214,16 @@ patch_residual_kernel(float* __restrict__ r, const float* __restrict__ data, int
 // axes.  tab[axis][idx][off] (32 offsets per patch index; axis 0: rows, na entries; axis 1: columns, nb entries):
 // bit 7 = "the pixel at offset off of patch idx has idx as its core patch along this axis", bits 0..6 = patches
 // that contain it along this axis.  (na + nb) * 32 bytes, rebuilt per call by one small kernel.
-__global__ void patch_axis_tables_kernel(PatchGrid pg, unsigned char* __restrict__ tab) {
+__global__ void patch_axis_tables_kernel(PatchGrid pg, unsigned char* __restrict__ tab, short4* __restrict__ pix) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   const int total = (pg.na + pg.nb) * 32;
+  if (t < pg.ny + pg.nx) {   // per pixel and axis: core patch, first and last covering patch (patch_compose_kernel)
+    const int axis = t >= pg.ny ? 1 : 0, j = axis ? t - pg.ny : t;
+    const int n = axis ? pg.nx : pg.ny, cnt = axis ? pg.nb : pg.na;
+    int lo, hi;
+    pg_cover_1d(j, n, pg.m, pg.st, cnt, &lo, &hi);
+    pix[t] = make_short4((short)pg_core_1d(j, n, pg.m, pg.st, cnt), (short)lo, (short)hi, 0);
+  }
   if (t >= total) return;
   const int idx_all = t >> 5, off = t & 31;
   const int axis = idx_all >= pg.na ? 1 : 0, idx = axis ? idx_all - pg.na : idx_all;
@@ -324,6 +330,7 @@ struct PatchWs {
   float *P, *Pp, *X, *S, *R, *r;
   double* part;
   unsigned char* tab;   // axis tables of patch_pprime_kernel, (na + nb) * 32 bytes
+  short4* pix;          // per-pixel axis tables of patch_compose_kernel, ny + nx entries
   int64_t n_part;
   size_t bytes;
 };
@@ -347,6 +354,7 @@ PatchWs carve(char* base, int S, const PatchGrid& pg, int n_angles, int n_bins) 
   w.n_part = std::max<int64_t>(std::max(g_img, g_res), 1024);
   w.part = reinterpret_cast<double*>(take((size_t)w.n_part * 8));
   w.tab = reinterpret_cast<unsigned char*>(take((size_t)(pg.na + pg.nb) * 32));
+  w.pix = reinterpret_cast<short4*>(take((size_t)(pg.ny + pg.nx) * sizeof(short4)));
   w.bytes = off;
   return w;
 }
@@ -365,7 +373,11 @@ int patch_gradient_device(const float* d_W, const float* d_D, const float* d_dat
   PYHST_TRY(patch_gemm(d_W, d_D, w.P, N, mm, n_atoms, 1.f, false, S, stream));
   // X, S, similarity
   const dim3 blk(32, 8, 1), grid_img((pg.nx + 31) / 32, (pg.ny + 7) / 8, S);
-  patch_compose_kernel<<<grid_img, blk, 0, stream>>>(w.P, pg, w.X, w.S, d_f ? w.part : nullptr);
+  {
+    const int n_tab = std::max((pg.na + pg.nb) * 32, pg.ny + pg.nx);
+    patch_axis_tables_kernel<<<(n_tab + 255) / 256, 256, 0, stream>>>(pg, w.tab, w.pix);
+  }
+  patch_compose_kernel<<<grid_img, blk, 0, stream>>>(w.P, pg, w.X, w.S, d_f ? w.part : nullptr, w.pix);
   if (d_f) sum_partials_kernel<<<1, 1024, 0, stream>>>(w.part, (int)(grid_img.x * grid_img.y * grid_img.z), (double)rho, d_f);
   PYHST_CUDA_TRY(cudaGetLastError());
   // R <- Pi^T (Pi X - y)
@@ -381,7 +393,6 @@ int patch_gradient_device(const float* d_W, const float* d_D, const float* d_dat
   // P' and G <- 2 P' D^T
   if (N * mm >= ((int64_t)1 << 32) || N >= ((int64_t)1 << 31))
     return set_error(PYHST_ERR_UNSUPPORTED, "patch: more than 2^32 patch elements per slice");
-  patch_axis_tables_kernel<<<((pg.na + pg.nb) * 32 + 255) / 256, 256, 0, stream>>>(pg, w.tab);
   patch_pprime_kernel<<<dim3((unsigned)((N * mm + 255) / 256), (unsigned)S), 256, 0, stream>>>(w.P, w.X, w.S, w.R, pg, rho, w.Pp, w.tab);
   PYHST_TRY(patch_gemm(w.Pp, d_D, d_G, N, n_atoms, mm, 2.f, true, S, stream));
   PYHST_CUDA_TRY(cudaGetLastError());
@@ -505,8 +516,12 @@ extern "C" int pyhst_patch_fista(const float* d_D, const float* d_data, const py
   }
   if (d_X) {  // the image of eq. 7 at the final coefficients
     PYHST_TRY(patch_gemm(d_W, d_D, w.P, (int64_t)pg.na * pg.nb, pg.m * pg.m, pp->n_atoms, 1.f, false, S, stream));
+    {
+      const int n_tab = std::max((pg.na + pg.nb) * 32, pg.ny + pg.nx);
+      patch_axis_tables_kernel<<<(n_tab + 255) / 256, 256, 0, stream>>>(pg, w.tab, w.pix);
+    }
     patch_compose_kernel<<<dim3((pg.nx + 31) / 32, (pg.ny + 7) / 8, S), dim3(32, 8, 1), 0, stream>>>(w.P, pg, d_X, w.S,
-                                                                                                    nullptr);
+                                                                                                    nullptr, w.pix);
     PYHST_CUDA_TRY(cudaGetLastError());
   }
   if (energy || lipschitz) {
