@@ -221,13 +221,17 @@ def run_b200(args):
         h_img = torch.empty((S, ny, nx), dtype=torch.float32, pin_memory=True)
         h_proj = torch.empty((S, NP, B), dtype=torch.float32, pin_memory=True)
 
+        # chunks of the host pipeline: copies of one chunk overlap the kernels of another; 16-slice chunks (the
+        # 16-slices-per-thread forward kernel) once the stack has at least two of them
+        chunk = 16 if S >= 32 else 8
+
         def e2e_fbp():
             P.fbp_host(h_sino, w.angles, w.axis, nx, ny, w.pixel_size, filter=w.filter, mode=w.mode,
-                       out=h_img, max_slices_per_chunk=8)
+                       out=h_img, max_slices_per_chunk=chunk)
 
         def e2e_fp():
             P.forward_project_host(h_img, w.angles, w.axis, B, w.pixel_size, out=h_proj,
-                                   max_slices_per_chunk=8)
+                                   max_slices_per_chunk=chunk)
 
         for _ in range(min(args.warmup, 2) or 1):
             e2e_fbp()
@@ -258,8 +262,8 @@ def run_b200(args):
                "steps": n_e2e,
                "h2d_bytes_per_step": int(h_sino.numel() * 4 + h_img.numel() * 4),
                "d2h_bytes_per_step": int(h_img.numel() * 4 + h_proj.numel() * 4),
-               "api": "pyhst_fbp_host + pyhst_forward_project_host (pinned host buffers, 8-slice chunks, "
-                      "copies overlapped with kernels)"}
+               "api": "pyhst_fbp_host + pyhst_forward_project_host (pinned host buffers, %d-slice chunks, "
+                      "copies overlapped with kernels)" % chunk}
         P.profile_read(reset=True)
         del h_sino, h_img, h_proj
 
