@@ -35,7 +35,7 @@ int pyhst_set_halfacq_stitch(int enable);
 
 /* Selects the forward-projection kernel: 0 = automatic (default: the diagonal-line interval kernel when its
  * blocks are mostly full -- on average at least 0.55 x 16 (dense angle lists) or 0.55 x 8 (sparser ones)
- * neighbouring projections share one staged window -- and the grid fills the GPU, else the banded kernel),
+ * neighbouring projections share one staged window -- and the grid has at least one block per SM, else the banded kernel),
  * 1 = generic gather kernel (one thread per bin and slice, global loads; kept for cross-checks and for pixel
  * sizes the shared-memory kernels do not cover), 2 = banded shared-memory kernel, 3 = interval form of the
  * banded kernel (fewer shared-memory loads, more instructions), 4 = interval form with 8 slices per thread

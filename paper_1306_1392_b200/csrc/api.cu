@@ -329,7 +329,9 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, int want_diag, const
       const int64_t blocks = (int64_t)pl.fd.n_bx * pl.fd.n_chunks * std::max(1, (pl.n_groups + 1) / 2);
       int n_sm = 148;
       require_sm100(&n_sm);
-      use = per_chunk >= 0.55 * pl.fd.npj && blocks >= 4 * (int64_t)n_sm;
+      // (grids of fewer blocks than 4 per SM are split along the lines by the launcher; below one block per SM the
+      // banded kernel's smaller blocks win)
+      use = per_chunk >= 0.55 * pl.fd.npj && blocks >= (int64_t)n_sm;
     }
     if (use && (legacy.empty() || build_fp_tables(g, &probe, &projs, &chunks, &legacy))) {
       pl.diag = true;
