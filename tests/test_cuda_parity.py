@@ -105,6 +105,19 @@ def test_backproject_batch_independence(lib):
     assert (full[2] == one8[0]).all()
 
 
+@pytest.mark.parametrize("S", [4, 7, 9, 12, 20])
+def test_backproject_default_kernel_choice(lib, oracle, S):
+    """Automatic kernel choice: <= 4 slices the 4-slice run kernel, pairs of slice groups the 8-slice kernel, and the
+    last group of an odd number (>= 3) of groups the 4-slice kernel again (no duplicate group)."""
+    wl = lib.workloads
+    P, B, nx, ny = 40, 210, 140, 130
+    w = wl.custom(S, P, B, nx, ny, drift=1.0, jitter_angles=0.01, seed=S, span=2 * math.pi)
+    sino = wl.random_sinogram(S, P, B, seed=S)
+    want = oracle.backproject(sino, w.angles, w.axis, nx, ny, scale=1.3)
+    got = lib.backproject(_dev(sino), w.angles, w.axis, nx, ny, scale=1.3).cpu().numpy()
+    assert_parity(got, want, "backproject, default kernels, %d slices" % S)
+
+
 @pytest.mark.parametrize("S", [13, 16, 18])
 def test_backproject_run16_matches_oracle(lib, oracle, S):
     """pyhst_test.h variant 7: 16 slices per thread (four slice groups per block, ragged stacks read a duplicate group
