@@ -85,6 +85,7 @@ struct FdParams {
   // n_seg > 1: blockIdx.z = group block * n_seg + seg; the block walks the seg-th part of its bands and writes its
   // sums to part[seg] (same row layout, pitch part_pitch); fd_combine_kernel adds the parts (small scans fill the GPU)
   int32_t n_seg;
+  int32_t g_off;           // first slice group of this launch (a stack is covered by launches of 4, 2 and 1 groups per block)
   float* part;
   int64_t part_pitch, part_stride;
 };
@@ -190,7 +191,7 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const FdChunk ck = prm.chunks[blockIdx.y];
   const int seg = blockIdx.z % prm.n_seg;
-  const int gA = (blockIdx.z / prm.n_seg) * NG;
+  const int gA = prm.g_off + (blockIdx.z / prm.n_seg) * NG;
   const int mB = blockIdx.x * (FD_NB - 1) - 1;      // intervals [m, m+1), m in [mB, mB + NB)
   int2 rg = prm.ranges[(int64_t)blockIdx.y * prm.n_bx + blockIdx.x];
   if (prm.n_seg > 1) {
@@ -642,14 +643,17 @@ bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* p
   return plan->n_chunks > 0 && plan->n_chunks <= 65535;
 }
 
-// slice groups (of 4 slices) a block takes: 4 for stacks of >= 13 slices (16 slices per thread: the per-line
-// boundary / weight / address logic is shared by twice the FMAs; one block per SM), 2 from 5 slices on, else 1
-int fd_groups_per_block(int n_slices, int npj) {
-  const int ng = (n_slices + 3) / 4;
+// A stack of n groups (of 4 slices) is covered by launches with 4 groups per block (16 slices per thread: the per-line
+// boundary / weight / address logic is shared by twice the FMAs; one block per SM; dense angle lists only), then 2, then 1:
+// no block works on a spare group.  Returns the number of launches; ng[i] groups per block, cnt[i] blocks along z.
+int fd_group_launches(int n_groups, int npj, int ng[3], int cnt[3]) {
+  int n = 0, left = n_groups;
 #if FD_NG4
-  if (ng >= 4 && npj != 8) return 4;
+  if (npj != 8 && left >= 4) { ng[n] = 4; cnt[n] = left / 4; left -= 4 * cnt[n]; ++n; }
 #endif
-  return ng >= 2 ? 2 : 1;
+  if (left >= 2) { ng[n] = 2; cnt[n] = left / 2; left -= 2 * cnt[n]; ++n; }
+  if (left >= 1) { ng[n] = 1; cnt[n] = 1; ++n; }
+  return n;
 }
 
 void fd_block_shape(int32_t* nb, int32_t* npj) {
@@ -659,11 +663,9 @@ void fd_block_shape(int32_t* nb, int32_t* npj) {
 
 size_t fd_xd_bytes(const FdPlan& plan, const pyhst_geom_t* g, int* n_groups_alloc) {
   const int ng = (g->n_slices + 3) / 4;
-  const int per = fd_groups_per_block(g->n_slices, plan.npj);
-  const int nga = (ng + per - 1) / per * per;     // whole blocks: spare zero groups for ragged counts
-  if (n_groups_alloc) *n_groups_alloc = nga;
+  if (n_groups_alloc) *n_groups_alloc = ng;
   const int64_t line_f4 = (int64_t)g->nx + 2 * plan.zpad;
-  return (size_t)2 * nga * plan.n_lines_alloc * line_f4 * 16;
+  return (size_t)2 * ng * plan.n_lines_alloc * line_f4 * 16;
 }
 
 int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch, const pyhst_geom_t* g,
@@ -714,14 +716,16 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
   prm.ranges = reinterpret_cast<const int2*>(plan.d_ranges);
   prm.n_bx = plan.n_bx;
   prm.W = plan.W;
-  const int ng = fd_groups_per_block(g->n_slices, plan.npj);
   const bool small = plan.npj == 8;     // sparse angle lists: 8 projections per block, 256 threads, bands of 4 lines
+  int ngl[3], cntl[3];
+  const int n_launch = fd_group_launches(n_groups, plan.npj, ngl, cntl);
   // small grids are split along the lines so that they fill the block slots a few times over
   int n_sm = 148;
   require_sm100(&n_sm);
-  const int64_t blocks = (int64_t)plan.n_bx * plan.n_chunks * (nga / ng);
-  const int64_t slots = (int64_t)n_sm * (ng == 4 ? 1 : (small ? 4 : 2));
-  int n_seg = (int)std::max<int64_t>(1, std::min<int64_t>(8, (4 * slots + blocks - 1) / blocks));
+  double waves = 0.0;   // of the block slots, over all launches, unsplit
+  for (int i = 0; i < n_launch; ++i)
+    waves += (double)plan.n_bx * plan.n_chunks * cntl[i] / (double)(n_sm * (ngl[i] == 4 ? 1 : (small ? 4 : 2)));
+  int n_seg = (int)std::max(1.0, std::min(8.0, std::ceil(4.0 / std::max(waves, 1e-9))));
   n_seg = std::max(1, std::min(n_seg, (g->nx + g->ny) / 256));
   prm.n_seg = n_seg;
   prm.part = nullptr;
@@ -732,27 +736,34 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
     PYHST_TRY(get_workspace(WS_FDP, (size_t)n_seg * prm.part_stride * 4, &wp));
     prm.part = static_cast<float*>(wp);
   }
-  dim3 grid(plan.n_bx, plan.n_chunks, (nga / ng) * n_seg);
-  if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
   static uint64_t configured[6] = {0, 0, 0, 0, 0, 0};
-  const int vi = (ng == 4 ? 2 : ng - 1) + (small ? 3 : 0);
-  const bool first = first_use_on_device(&configured[vi]);
 #define FD_LAUNCH(NGV, NPJV, RBV)                                                                                   \
   do {                                                                                                              \
     if (first)                                                                                                      \
       PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<NGV, NPJV, RBV>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                          (int)fd_smem(NGV, RBV, NPJV)));                                                \
+                                          (int)fd_smem(NGV, RBV, NPJV)));                                           \
     StageScope scope(ST_FORWARD, stream);                                                                           \
     scope.kernels();                                                                                                \
-    fp_diag_kernel<NGV, NPJV, RBV><<<grid, FD_NB / FD_M * NPJV, fd_smem(NGV, RBV, NPJV), stream>>>(prm);                  \
+    fp_diag_kernel<NGV, NPJV, RBV><<<grid, FD_NB / FD_M * NPJV, fd_smem(NGV, RBV, NPJV), stream>>>(prm);            \
   } while (0)
-  if (small) {
-    if (ng == 2) FD_LAUNCH(2, 8, 4);
-    else FD_LAUNCH(1, 8, 4);
-  } else {
-    if (ng == 4) FD_LAUNCH(4, 16, 8);
-    else if (ng == 2) FD_LAUNCH(2, 16, 8);
-    else FD_LAUNCH(1, 16, 8);
+  int g_off = 0;
+  for (int i = 0; i < n_launch; ++i) {
+    const int ng = ngl[i];
+    prm.g_off = g_off;
+    g_off += ng * cntl[i];
+    dim3 grid(plan.n_bx, plan.n_chunks, cntl[i] * n_seg);
+    if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
+    const int vi = (ng == 4 ? 2 : ng - 1) + (small ? 3 : 0);
+    const bool first = first_use_on_device(&configured[vi]);
+    if (small) {
+      if (ng == 2) FD_LAUNCH(2, 8, 4);
+      else FD_LAUNCH(1, 8, 4);
+    } else {
+      if (ng == 4) FD_LAUNCH(4, 16, 8);
+      else if (ng == 2) FD_LAUNCH(2, 16, 8);
+      else FD_LAUNCH(1, 16, 8);
+    }
+    PYHST_CUDA_TRY(cudaGetLastError());
   }
 #undef FD_LAUNCH
   if (n_seg > 1) {
