@@ -310,7 +310,7 @@ def run_b200(args):
     calls = n_fista if fista else 1
     r_bp = kernel_roofline("backproject", "bp_run8_kernel<0> + bp_run8_kernel<1>", executed=bp_exec, calls_per_step=calls)
     fp_names = {1: "fp_gather_kernel", 2: "fp_band_kernel", 3: "fp_ivl_kernel", 4: "fp_ivl_kernel (8 slices)",
-                5: "fp_diag_kernel (+ fp_band_kernel for the projections within 2^-12 of an image axis)"}
+                5: "fp_diag_kernel"}
     r_fp = kernel_roofline("forward_project", fp_names.get(P.last_forward_project_kernel(), "forward projector"),
                            calls_per_step=calls)
     hbm = float(peaks.get("hbm_gbs", 6650.0))

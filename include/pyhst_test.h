@@ -41,8 +41,8 @@ int pyhst_set_halfacq_stitch(int enable);
  * banded kernel (fewer shared-memory loads, more instructions), 4 = interval form with 8 slices per thread
  * (stacks with an even number of slice groups and 16-projection chunks, else as 3), 5 = diagonal-line interval
  * kernel forced (PYHST_ERR_UNSUPPORTED when no projection has >= 1 + 2^-12 bins per pixel along an image
- * diagonal, i.e. pixel sizes below ~0.71 bins; projections it does not cover -- within 2^-12 of an image axis,
- * or whose window alone does not fit -- run on the banded kernel).  Returns the previous value. */
+ * diagonal, i.e. pixel sizes below ~0.71 bins; projections it does not cover -- fewer than 1 - 1e-6 bins per pixel
+ * along the diagonal, or a window that alone does not fit -- run on the banded kernel).  Returns the previous value. */
 int pyhst_set_forward_project_variant(int variant);
 
 /* Which kernel the last pyhst_forward_project of this process ran: 1 generic gather, 2 banded, 3 / 4

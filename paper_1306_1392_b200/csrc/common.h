@@ -211,7 +211,7 @@ struct FdChunk {
   int32_t pad_[2];
 };
 struct FdPlan {
-  int32_t n_chunks = 0, n_bx = 0, W = 0, zpad = 0, n_lines_alloc = 0, npj = 16, n_tab = 0;   // npj: projections per chunk at most (16 or 8); n_tab: projections in the table
+  int32_t n_chunks = 0, n_bx = 0, W = 0, zpad = 0, n_lines_alloc = 0, npj = 16, n_tab = 0, n_chunks_one = 0, n_tab_one = 0;   // npj: projections per chunk at most (16 or 8); n_tab: projections in the table; chunks [n_chunks_one, n_chunks) hold the near-axis projections (two pixels per interval possible)
   FdProj* d_projs = nullptr;
   FdChunk* d_chunks = nullptr;
   int32_t* d_ranges = nullptr;   // [n_chunks][n_bx][2]

@@ -23,8 +23,11 @@
 //     double per (boundary, band), split into an integer and a float fraction, then
 //     fmaf(s, r, fraction) per line and a round-up add of 1.5 * 2^23 + integer -- so the sets
 //     [ceil(ks(m)), ceil(ks(m+1))) partition the line whatever the rounding.  With
-//     |sigma| >= 1 + 2^-12 such a set has at most one element; projections closer to an image
-//     axis than that (and pixel sizes below 1 bin) go to the banded kernel (forward_project.cu).
+//     |sigma| >= 1 + 2^-12 such a set has at most one element.  Projections on or next to an image
+//     axis (1 - 1e-6 <= |sigma| < 1 + 2^-12 at pixel size 1: theta = 0, pi/2 of every scan) may
+//     get two: they form chunks of their own, run by the TWO form of the kernel, which also takes
+//     the next pixel of the line when the computed boundaries enclose it.  Pixel sizes with
+//     |sigma| < 1 - 1e-6 go to the banded kernel (forward_project.cu).
 //   * The weight f = |sigma| (ceil(ks) - ks) uses the continuous position (R11: double per band,
 //     FP32 only for the in-band offset).
 #include <algorithm>
@@ -85,9 +88,11 @@ struct FdParams {
   // n_seg > 1: blockIdx.z = group block * n_seg + seg; the block walks the seg-th part of its bands and writes its
   // sums to part[seg] (same row layout, pitch part_pitch); fd_combine_kernel adds the parts (small scans fill the GPU)
   int32_t n_seg;
+  int32_t chunk_off;       // first chunk of this launch
   int32_t g_off;           // first slice group of this launch (a stack is covered by launches of 4, 2 and 1 groups per block)
-  float* part;
+  float* part;             // [n_seg][S][part_nt][part_pitch]: rows of the pass's projections only
   int64_t part_pitch, part_stride;
+  int32_t part_t0, part_nt;   // the pass's range of the projection table
 };
 
 // One line of one interval, NG slice groups: two LDS.128 and 4 NG packed FFMA2 (two slices each).  The
@@ -177,7 +182,9 @@ __device__ __forceinline__ float fd_hi(uint64_t v) { return __uint_as_float((uin
 
 // NPJ = projections per block (16: dense angle lists; 8: sparse ones, whose strips fan out so that fewer fit one staged
 // window -- 256-thread blocks with bands of RB = 4 lines, four blocks per SM), NT = 32 NPJ threads.
-template <int NG, int NPJ, int RB>
+// TWO: chunks of projections with 1 - 1e-6 <= |sigma| < 1 + 2^-12 (on or next to an image axis at pixel size 1): the
+// computed boundaries of an interval may then enclose two pixels of a line, and the second one is taken as well.
+template <int NG, int NPJ, int RB, bool TWO>
 __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ? 2 : 4)) fp_diag_kernel(const FdParams prm) {
   constexpr int NT = FD_NB / FD_M * NPJ, NWARP = NT / 32, PLANE = RB * FD_PW * 16;
   extern __shared__ __align__(128) unsigned char smem[];
@@ -189,11 +196,12 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
   constexpr int STAGE_F4 = NG * RB * FD_PW;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const FdChunk ck = prm.chunks[blockIdx.y];
+  const int chunk = prm.chunk_off + blockIdx.y;
+  const FdChunk ck = prm.chunks[chunk];
   const int seg = blockIdx.z % prm.n_seg;
   const int gA = prm.g_off + (blockIdx.z / prm.n_seg) * NG;
   const int mB = blockIdx.x * (FD_NB - 1) - 1;      // intervals [m, m+1), m in [mB, mB + NB)
-  int2 rg = prm.ranges[(int64_t)blockIdx.y * prm.n_bx + blockIdx.x];
+  int2 rg = prm.ranges[(int64_t)chunk * prm.n_bx + blockIdx.x];
   if (prm.n_seg > 1) {
     const int nb_all = (rg.y - rg.x + RB - 1) / RB;
     const int k0 = seg * nb_all / prm.n_seg, k1 = (seg + 1) * nb_all / prm.n_seg;
@@ -351,6 +359,24 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
               fd_line_s1(acc[q], acc[q + 1], in ? f : 0.f, in ? g : 0.f, addr);
             }
 #endif
+            if constexpr (TWO) {   // the next pixel of the line, if the interval's computed boundaries enclose it too
+              const float j2 = jm[q] + 1.f, f2 = f + sig, g2 = 1.f - f2;
+              const uint32_t addr2 = addr + (uint32_t)mul;
+#if FD_PACKED
+              const bool in2 = j2 < jm[q + 1];
+              const float fz2 = in2 ? f2 : 0.f, gz2 = in2 ? g2 : 0.f;
+              fd_line<NG, PLANE>(acc[q], acc[q + 1], fz2, gz2, addr2);
+              if constexpr (NG == 4) fd_line<NG, PLANE>(acc[q] + 4, acc[q + 1] + 4, fz2, gz2, addr2 + 2 * PLANE);
+#else
+              if constexpr (NG >= 2) {
+                fd_line_s<PLANE>(acc[q], acc[q + 1], j2, jm[q + 1], f2, g2, addr2);
+                if constexpr (NG == 4) fd_line_s<PLANE>(acc[q] + 8, acc[q + 1] + 8, j2, jm[q + 1], f2, g2, addr2 + 2 * PLANE);
+              } else {
+                const bool in2 = j2 < jm[q + 1];
+                fd_line_s1(acc[q], acc[q + 1], in2 ? f2 : 0.f, in2 ? g2 : 0.f, addr2);
+              }
+#endif
+            }
           }
         }
         }
@@ -396,7 +422,9 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
       const int b = mB + bl;
       if (q < ck.count && b < prm.B) {
         const int p = sproj[q].p;
-        out[((int64_t)sidx * prm.P + p) * opitch + b] =
+        const int64_t orow = prm.n_seg > 1 ? (int64_t)sidx * prm.part_nt + (ck.first + q - prm.part_t0)
+                                           : (int64_t)sidx * prm.P + p;
+        out[orow * opitch + b] =
             prm.scale * (lo_s[q * (FD_NB + 1) + bl] + up_s[q * (FD_NB + 1) + bl]);
       }
     }
@@ -414,7 +442,7 @@ __global__ void fd_combine_kernel(float* __restrict__ y, int64_t pitch, const fl
   const int64_t sl = rt / n_tab;
   const int64_t row = sl * P + projs[rt - sl * n_tab].p;
   float v = 0.f;
-  for (int h = 0; h < n_seg; ++h) v += part[(int64_t)h * part_stride + row * part_pitch + b];
+  for (int h = 0; h < n_seg; ++h) v += part[(int64_t)h * part_stride + rt * part_pitch + b];
   y[row * pitch + b] = v;
 }
 
@@ -521,7 +549,7 @@ bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* p
   legacy->clear();
   const int n_bx = (g->n_bins + FD_NB - 2) / (FD_NB - 1);
   const int n_lines = nx + ny - 1;
-  std::vector<HostProj> cls[12];    // (layout, sgn, skew)
+  std::vector<HostProj> cls[24];    // (two, layout, sgn, skew)
   for (int p = 0; p < P; ++p) {
     HostProj q;
     q.a = h * std::cos(g->angles_rad[p]);
@@ -533,10 +561,14 @@ bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* p
     const double as = std::fabs(sigma);
     // at most one pixel per interval and line, with room for the rounding of the boundaries; and a
     // window that fits: FD_NB / |sigma| + divergence + skew residue
-    if (!(as >= 1.0 + 1.0 / 4096.0) || as > 8.0) {
+    // |sigma| >= 1 + 2^-12: at most one pixel per interval and line, with room for the rounding of the boundaries.
+    // 1 - 1e-6 <= |sigma| < 1 + 2^-12 (theta on or next to an image axis at pixel size 1): at most two -- chunks of
+    // their own, run by the TWO form of the kernel.  Anything finer goes to the banded kernel.
+    if (!(as >= 1.0 - 1e-6) || as > 8.0) {
       legacy->push_back(p);
       continue;
     }
+    const int two = as < 1.0 + 1.0 / 4096.0 ? 1 : 0;
     const double T0 = q.layout == 0 ? q.c - q.a * j0 - q.b * ((double)(nx - 1) + i0) : q.c - q.a * j0 - q.b * i0;
     q.sgn = sigma > 0.0 ? 1 : -1;
     q.d.inv = 1.0 / as;
@@ -548,7 +580,7 @@ bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* p
     q.d.pad_ = 0;
     const double dk = (double)q.sgn * q.d.sD;       // stored positions per line
     q.skew = dk > 0.5 ? 1 : (dk < -0.5 ? -1 : 0);
-    cls[(q.layout * 2 + (q.sgn > 0 ? 1 : 0)) * 3 + (q.skew + 1)].push_back(q);
+    cls[two * 12 + (q.layout * 2 + (q.sgn > 0 ? 1 : 0)) * 3 + (q.skew + 1)].push_back(q);
   }
   plan->n_bx = n_bx;
   int w_max = 0;
@@ -567,7 +599,12 @@ bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* p
     }
     return (int)(std::ceil(hi) - (std::floor(lo) - 2.0)) + 3;
   };
-  for (int c = 0; c < 12; ++c) {
+  plan->n_chunks_one = -1;
+  for (int c = 0; c < 24; ++c) {
+    if (c == 12) {   // chunks of the TWO form follow
+      plan->n_chunks_one = (int32_t)chunks->size();
+      plan->n_tab_one = (int32_t)projs->size();
+    }
     std::vector<HostProj>& v = cls[c];
     if (v.empty()) continue;
     std::stable_sort(v.begin(), v.end(), [](const HostProj& x, const HostProj& y) { return x.angle < y.angle; });
@@ -719,62 +756,75 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
   const bool small = plan.npj == 8;     // sparse angle lists: 8 projections per block, 256 threads, bands of 4 lines
   int ngl[3], cntl[3];
   const int n_launch = fd_group_launches(n_groups, plan.npj, ngl, cntl);
-  // small grids are split along the lines so that they fill the block slots a few times over
   int n_sm = 148;
   require_sm100(&n_sm);
-  double waves = 0.0;   // of the block slots, over all launches, unsplit
-  for (int i = 0; i < n_launch; ++i)
-    waves += (double)plan.n_bx * plan.n_chunks * cntl[i] / (double)(n_sm * (ngl[i] == 4 ? 1 : (small ? 4 : 2)));
-  int n_seg = (int)std::max(1.0, std::min(8.0, std::ceil(4.0 / std::max(waves, 1e-9))));
-  n_seg = std::max(1, std::min(n_seg, (g->nx + g->ny) / 256));
-  prm.n_seg = n_seg;
   prm.part = nullptr;
   prm.part_pitch = g->n_bins;
-  prm.part_stride = (int64_t)g->n_slices * g->n_angles * prm.part_pitch;
-  if (n_seg > 1) {
-    void* wp = nullptr;
-    PYHST_TRY(get_workspace(WS_FDP, (size_t)n_seg * prm.part_stride * 4, &wp));
-    prm.part = static_cast<float*>(wp);
-  }
-  static uint64_t configured[6] = {0, 0, 0, 0, 0, 0};
-#define FD_LAUNCH(NGV, NPJV, RBV)                                                                                   \
+  prm.part_stride = 0;
+  static uint64_t configured[12] = {0};
+#define FD_LAUNCH(NGV, NPJV, RBV, TWOV)                                                                             \
   do {                                                                                                              \
     if (first)                                                                                                      \
-      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<NGV, NPJV, RBV>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                          (int)fd_smem(NGV, RBV, NPJV)));                                           \
+      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<NGV, NPJV, RBV, TWOV>,                                     \
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(NGV, RBV, NPJV))); \
     StageScope scope(ST_FORWARD, stream);                                                                           \
     scope.kernels();                                                                                                \
-    fp_diag_kernel<NGV, NPJV, RBV><<<grid, FD_NB / FD_M * NPJV, fd_smem(NGV, RBV, NPJV), stream>>>(prm);            \
+    fp_diag_kernel<NGV, NPJV, RBV, TWOV><<<grid, FD_NB / FD_M * NPJV, fd_smem(NGV, RBV, NPJV), stream>>>(prm);      \
   } while (0)
-  int g_off = 0;
-  for (int i = 0; i < n_launch; ++i) {
-    const int ng = ngl[i];
-    prm.g_off = g_off;
-    g_off += ng * cntl[i];
-    dim3 grid(plan.n_bx, plan.n_chunks, cntl[i] * n_seg);
-    if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
-    const int vi = (ng == 4 ? 2 : ng - 1) + (small ? 3 : 0);
-    const bool first = first_use_on_device(&configured[vi]);
-    if (small) {
-      if (ng == 2) FD_LAUNCH(2, 8, 4);
-      else FD_LAUNCH(1, 8, 4);
-    } else {
-      if (ng == 4) FD_LAUNCH(4, 16, 8);
-      else if (ng == 2) FD_LAUNCH(2, 16, 8);
-      else FD_LAUNCH(1, 16, 8);
+  const int n_one = plan.n_chunks_one < 0 ? plan.n_chunks : plan.n_chunks_one;
+  // two passes: the chunks of the generic projections, then those of the near-axis projections (TWO form).  Each pass
+  // splits the line range of its blocks into n_seg segments when its grid would not fill the block slots about four
+  // times over (small scans; the one or two near-axis projections of a scan) and adds the partial sums afterwards.
+  for (int two = 0; two < 2; ++two) {
+    const int n_ck = two ? plan.n_chunks - n_one : n_one;
+    if (n_ck <= 0) continue;
+    double waves = 0.0;   // of the block slots, over the pass's launches, unsplit
+    for (int i = 0; i < n_launch; ++i)
+      waves += (double)plan.n_bx * n_ck * cntl[i] / (double)(n_sm * (ngl[i] == 4 ? 1 : (small ? 4 : 2)));
+    int n_seg = (int)std::max(1.0, std::min(8.0, std::ceil(4.0 / std::max(waves, 1e-9))));
+    n_seg = std::max(1, std::min(n_seg, (g->nx + g->ny) / 256));
+    prm.n_seg = n_seg;
+    prm.part_t0 = two ? plan.n_tab_one : 0;
+    prm.part_nt = two ? plan.n_tab - plan.n_tab_one : plan.n_tab_one;
+    prm.part_stride = (int64_t)g->n_slices * prm.part_nt * prm.part_pitch;
+    if (n_seg > 1) {
+      // (the two passes use the block one after the other on the stream; a regrowth synchronises the device)
+      void* wp = nullptr;
+      PYHST_TRY(get_workspace(WS_FDP, (size_t)n_seg * prm.part_stride * 4, &wp));
+      prm.part = static_cast<float*>(wp);
     }
-    PYHST_CUDA_TRY(cudaGetLastError());
+    prm.chunk_off = two ? n_one : 0;
+    int g_off = 0;
+    for (int i = 0; i < n_launch; ++i) {
+      const int ng = ngl[i];
+      prm.g_off = g_off;
+      g_off += ng * cntl[i];
+      dim3 grid(plan.n_bx, n_ck, cntl[i] * n_seg);
+      if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
+      const int vi = ((ng == 4 ? 2 : ng - 1) + (small ? 3 : 0)) * 2 + two;
+      const bool first = first_use_on_device(&configured[vi]);
+      if (small) {
+        if (ng == 2) { if (two) FD_LAUNCH(2, 8, 4, true); else FD_LAUNCH(2, 8, 4, false); }
+        else { if (two) FD_LAUNCH(1, 8, 4, true); else FD_LAUNCH(1, 8, 4, false); }
+      } else {
+        if (ng == 4) { if (two) FD_LAUNCH(4, 16, 8, true); else FD_LAUNCH(4, 16, 8, false); }
+        else if (ng == 2) { if (two) FD_LAUNCH(2, 16, 8, true); else FD_LAUNCH(2, 16, 8, false); }
+        else { if (two) FD_LAUNCH(1, 16, 8, true); else FD_LAUNCH(1, 16, 8, false); }
+      }
+      PYHST_CUDA_TRY(cudaGetLastError());
+    }
+    if (n_seg > 1) {   // the pass's projections: [0, n_tab_one) or [n_tab_one, n_tab) of the table
+      const int t0 = prm.part_t0, nt = prm.part_nt;
+      const int64_t n_rows_tab = (int64_t)g->n_slices * nt;
+      const unsigned gy = (unsigned)std::min<int64_t>(n_rows_tab, 32768);
+      dim3 grid_c((g->n_bins + 255) / 256, gy, (unsigned)((n_rows_tab + gy - 1) / gy));
+      StageScope scope(ST_FORWARD, stream);
+      scope.kernels();
+      fd_combine_kernel<<<grid_c, 256, 0, stream>>>(d_sino, pitch, prm.part, prm.part_pitch, prm.part_stride, n_seg,
+                                                    g->n_bins, g->n_angles, plan.d_projs + t0, nt, n_rows_tab);
+    }
   }
 #undef FD_LAUNCH
-  if (n_seg > 1) {
-    const int64_t n_rows_tab = (int64_t)g->n_slices * plan.n_tab;
-    const unsigned gy = (unsigned)std::min<int64_t>(n_rows_tab, 32768);
-    dim3 grid_c((g->n_bins + 255) / 256, gy, (unsigned)((n_rows_tab + gy - 1) / gy));
-    StageScope scope(ST_FORWARD, stream);
-    scope.kernels();
-    fd_combine_kernel<<<grid_c, 256, 0, stream>>>(d_sino, pitch, prm.part, prm.part_pitch, prm.part_stride, n_seg,
-                                                  g->n_bins, g->n_angles, plan.d_projs, plan.n_tab, n_rows_tab);
-  }
   PYHST_CUDA_TRY(cudaGetLastError());
   return PYHST_OK;
 }
