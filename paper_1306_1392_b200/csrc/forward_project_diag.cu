@@ -49,6 +49,12 @@ namespace {
 #ifndef FD_CHECK
 #define FD_CHECK 0
 #endif
+// block order: chunk index fastest (1) -- the blocks resident together are the same detector range at neighbouring
+// angles, whose staged bands overlap: L2 hit rate 29 % -> 74 %, DRAM reads 42 -> 10.6 GB per config-2 call -- or
+// detector block fastest (0)
+#ifndef FD_SWAP
+#define FD_SWAP 1
+#endif
 constexpr int FD_NB = 64;      // intervals per block (FD_NB - 1 complete bins)
 constexpr int FD_NPJ = 16;     // projections per block (at most)
 constexpr int FD_M = 2;        // neighbouring intervals per thread
@@ -196,12 +202,17 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
   constexpr int STAGE_F4 = NG * RB * FD_PW;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int chunk = prm.chunk_off + blockIdx.y;
+#if FD_SWAP
+  const int bxi = blockIdx.y, cki = blockIdx.x;
+#else
+  const int bxi = blockIdx.x, cki = blockIdx.y;
+#endif
+  const int chunk = prm.chunk_off + cki;
   const FdChunk ck = prm.chunks[chunk];
   const int seg = blockIdx.z % prm.n_seg;
   const int gA = prm.g_off + (blockIdx.z / prm.n_seg) * NG;
-  const int mB = blockIdx.x * (FD_NB - 1) - 1;      // intervals [m, m+1), m in [mB, mB + NB)
-  int2 rg = prm.ranges[(int64_t)chunk * prm.n_bx + blockIdx.x];
+  const int mB = bxi * (FD_NB - 1) - 1;      // intervals [m, m+1), m in [mB, mB + NB)
+  int2 rg = prm.ranges[(int64_t)chunk * prm.n_bx + bxi];
   if (prm.n_seg > 1) {
     const int nb_all = (rg.y - rg.x + RB - 1) / RB;
     const int k0 = seg * nb_all / prm.n_seg, k1 = (seg + 1) * nb_all / prm.n_seg;
@@ -799,7 +810,11 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
       const int ng = ngl[i];
       prm.g_off = g_off;
       g_off += ng * cntl[i];
+#if FD_SWAP
+      dim3 grid(n_ck, plan.n_bx, cntl[i] * n_seg);
+#else
       dim3 grid(plan.n_bx, n_ck, cntl[i] * n_seg);
+#endif
       if (grid.z > 65535) return set_error(PYHST_ERR_UNSUPPORTED, "forward projector: too many slice groups");
       const int vi = ((ng == 4 ? 2 : ng - 1) + (small ? 3 : 0)) * 2 + two;
       const bool first = first_use_on_device(&configured[vi]);
