@@ -63,6 +63,19 @@ def test_library_has_sm100a_code_and_tma():
     assert "sm_100a" in out
     sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True).stdout
     assert "UBLKCP" in sass
+    # per kernel: the product projectors stage by TMA bulk copy and synchronise through mbarriers (SYNCS); the GEMM of
+    # Algorithm 1 runs on the 5th-generation tensor cores (UTCMMA = tcgen05.mma, LDTM = tcgen05.ld)
+    chunks = sass.split("Function : ")
+    def body(name):
+        hits = [c for c in chunks if name in c.split("\n", 1)[0]]
+        assert hits, name
+        return "\n".join(hits)
+    for name in ("bp_run8_kernel", "fp_diag_kernel"):
+        k = body(name)
+        assert "UBLKCP" in k and "SYNCS" in k and "FFMA" in k, name
+    g = body("patch_gemm_tc_kernel")
+    assert "UTCMMA" in g or "UTCHMMA" in g or "UTCQMMA" in g, "no tcgen05.mma in the tensor-core GEMM"
+    assert "LDTM" in g, "no tcgen05.ld in the tensor-core GEMM"
 
 
 def test_halfacq_extent_host_logic(cuda_lib, oracle):
