@@ -274,6 +274,51 @@ def test_forward_project_kernels_agree(lib):
         assert_parity(got, ref, "forward_project variant %d vs banded" % variant, rel=3e-6, mabs=3e-5)
 
 
+def _fuzz_geometry(rng):
+    """A random small scan: slice counts around the group sizes, random / regular / near-special angle lists, random
+    pixel sizes, integer-aligned geometries (pixels exactly on bin centres and interval boundaries)."""
+    S = int(rng.choice([1, 2, 4, 5, 8, 9, 12, 13, 16, 17]))
+    nx, ny = int(rng.integers(20, 180)), int(rng.integers(20, 180))
+    B, NP = int(rng.integers(16, 300)), int(rng.integers(1, 70))
+    h = float(rng.choice([1.0, 1.0, 1.0, rng.uniform(0.72, 2.5)]))
+    kind = int(rng.integers(0, 3))
+    if kind == 0:
+        ang = np.sort(rng.uniform(0, 2 * math.pi, NP))
+    elif kind == 1:
+        ang = np.arange(NP) * math.pi / NP
+    else:
+        base = rng.choice([0, math.pi / 4, math.pi / 2, 3 * math.pi / 4, math.pi, 1.5 * math.pi], NP)
+        ang = base + rng.choice([0, 1e-9, 1e-6, 1e-4, 2.44e-4, 1e-3, -1e-7, -1e-4], NP)
+    if rng.random() < 0.3:
+        nx |= 1
+        ny |= 1
+        axis = np.full(NP, float(rng.integers(0, B)))
+    else:
+        axis = rng.uniform(-5, B + 5) + rng.uniform(-2, 2, NP)
+    return S, NP, B, nx, ny, h, ang, axis
+
+
+def test_projector_pair_fuzz(lib, oracle):
+    """40 seeded random scans through the automatic kernel choices of both projectors and through the forced
+    diagonal-line forward kernel (400 such cases were run once while it was written: worst rel-L2 3e-6)."""
+    rng = np.random.default_rng(20241105)
+    for case in range(40):
+        S, NP, B, nx, ny, h, ang, axis = _fuzz_geometry(rng)
+        x = rng.normal(size=(S, ny, nx)).astype(np.float32)
+        want = oracle.forward_project(x, ang, axis, B, pixel_size=h)
+        for variant in (0, 5):
+            prev = lib.set_forward_project_variant(variant)
+            try:
+                got = lib.forward_project(_dev(x), ang, axis, B, pixel_size=h).cpu().numpy()
+            finally:
+                lib.set_forward_project_variant(prev)
+            assert_parity(got, want, "fuzz case %d forward variant %d %r" % (case, variant, (S, NP, B, nx, ny, h)))
+        q = rng.normal(size=(S, NP, B)).astype(np.float32)
+        assert_parity(lib.backproject(_dev(q), ang, axis, nx, ny, pixel_size=h).cpu().numpy(),
+                      oracle.backproject(q, ang, axis, nx, ny, pixel_size=h),
+                      "fuzz case %d backproject %r" % (case, (S, NP, B, nx, ny, h)))
+
+
 @pytest.mark.parametrize("B,axis", [(260, None), (120, 75.3)])
 def test_adjoint_identity_on_device(lib, B, axis):
     """K3 in FP32: |<P x, y> - <x, P^T y>| <= 1e-5 ||P x|| ||y||."""
