@@ -457,6 +457,59 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_extra(args):
+    """Timings of the NEXT-row entry points that are not part of the hot-path step (profiles/r02_ncu_kernels.md
+    sec. 5, 6): `--extra patch` = pyhst_patch_gradient on a config-4-sized problem (8 x 1024^2, 200 x 1024, 8 x 8 patches
+    at stride 4, 128 atoms) with both GEMM kernels; `--extra estimators` = pyhst_ring_filter / pyhst_ecohe on
+    config-2-sized operands.  One JSON line; CUDA events, `--steps` timed calls after `--warmup`."""
+    import torch
+    import paper_1306_1392_b200 as P
+    wl = P.workloads
+
+    def timeit(f):
+        for _ in range(max(args.warmup, 1)):
+            f()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            f()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps
+
+    out = {"extra": args.extra, "steps": args.steps, "warmup": args.warmup, "data": "synthetic"}
+    if args.extra == "patch":
+        w = wl.config(4)
+        S, n, m, st, n_atoms = w.n_slices, w.nx, 8, 4, 128
+        wl.set_device("cuda")
+        data = w.sinogram_tensor(range(S)).contiguous()
+        wl.set_device("cpu")
+        D = torch.from_numpy(wl.dct_dictionary(m, n_atoms, seed=1)).cuda()
+        na, nb = P.patch_grid(n, n, m, st)
+        torch.manual_seed(0)
+        W = (torch.randn((S, na * nb, n_atoms), device="cuda") * 0.01).contiguous()
+        out["workload"] = "pyhst_patch_gradient: %d slices of %dx%d, %d x %d sinograms, %d patches of %dx%d per slice, %d atoms" \
+                          % (S, n, n, w.n_angles, w.n_bins, na * nb, m, m, n_atoms)
+        for variant, name in ((1, "ms_fp32_simt_gemm"), (2, "ms_tcgen05_3xtf32_gemm")):
+            prev = P.set_patch_gemm_variant(variant)
+            try:
+                out[name] = timeit(lambda: P.patch_gradient(W, D, data, w.angles, w.axis, n, n, m, st, 0.8, want_f=False))
+            finally:
+                P.set_patch_gemm_variant(prev)
+    else:
+        S, NP, B, n = 16, 2000, 2048, 2048
+        sino = torch.rand((S, NP, B), device="cuda")
+        res = torch.empty_like(sino)
+        a, b = torch.rand((S, n, n), device="cuda"), torch.rand((S, n, n), device="cuda")
+        out["workload"] = "config-2-sized operands: %d x %d x %d sinogram stack, two %d x %dx%d image stacks" % (S, NP, B, S, n, n)
+        t = timeit(lambda: P.ring_filter(sino, 8, out=res))
+        out["ring_filter"] = {"ms": t, "gb_per_s": 3 * sino.numel() * 4 / t / 1e6, "bytes_counted": "3 x stack (mean pass, subtract pass in + out)"}
+        t = timeit(lambda: P.ecohe(a, b))
+        out["ecohe"] = {"ms": t, "gb_per_s": 2 * a.numel() * 4 / t / 1e6, "bytes_counted": "2 x stack; time includes the D2H of the results"}
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -470,12 +523,16 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fista", action="store_true",
                     help="config 4: time FBP + forward projection instead of the 100-iteration TV-FISTA")
+    ap.add_argument("--extra", default="", choices=["", "patch", "estimators"],
+                    help="time pyhst_patch_gradient / the estimators instead of the hot-path step (see run_extra)")
     ap.add_argument("--warmup-ref", type=int, default=0)
     ap.add_argument("--max-ref-steps", type=int, default=2)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         sys.stderr.write("note: fewer than 3 warm-up steps; the number is not a valid bench value\n")
-    if args.impl == "reference":
+    if args.extra:
+        run_extra(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_b200(args)
