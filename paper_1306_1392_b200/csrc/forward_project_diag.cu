@@ -52,6 +52,9 @@ namespace {
 // block order: chunk index fastest (1) -- the blocks resident together are the same detector range at neighbouring
 // angles, whose staged bands overlap: L2 hit rate 29 % -> 74 %, DRAM reads 42 -> 10.6 GB per config-2 call -- or
 // detector block fastest (0)
+#ifndef FD_M1
+#define FD_M1 0
+#endif
 #ifndef FD_SWAP
 #define FD_SWAP 1
 #endif
@@ -67,7 +70,6 @@ constexpr int FD_UNR = FD_UNR_;   // lines unrolled together (register budget)
 constexpr int FD_SB = 4;       // bands per double-precision evaluation of the boundaries
 constexpr int FD_LP = 4;       // projections per warp (lanes of a warp = FD_PPW interval pairs x FD_LP projections)
 constexpr int FD_PPW = 32 / FD_LP;
-constexpr int FD_WPG = FD_NB / FD_M / FD_PPW;   // warps that share a group of FD_LP projections
 constexpr int FD_NSTG = 4;     // stages of the band ring
 constexpr int FD_WMAX = 100;   // window capacity (float4 per line): four stages of two blocks per SM fit in 227 KB
 constexpr int FD_PW = FD_WMAX + FD_RB;   // row pitch of a stage (float4): room for the per-line skew
@@ -190,9 +192,11 @@ __device__ __forceinline__ float fd_hi(uint64_t v) { return __uint_as_float((uin
 // window -- 256-thread blocks with bands of RB = 4 lines, four blocks per SM), NT = 32 NPJ threads.
 // TWO: chunks of projections with 1 - 1e-6 <= |sigma| < 1 + 2^-12 (on or next to an image axis at pixel size 1): the
 // computed boundaries of an interval may then enclose two pixels of a line, and the second one is taken as well.
-template <int NG, int NPJ, int RB, bool TWO>
-__global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ? 2 : 4)) fp_diag_kernel(const FdParams prm) {
-  constexpr int NT = FD_NB / FD_M * NPJ, NWARP = NT / 32, PLANE = RB * FD_PW * 16;
+// M = neighbouring intervals per thread (2; 1 is a measured alternative for NG = 4: 1024 threads per block).
+template <int NG, int NPJ, int RB, bool TWO, int M>
+__global__ void __launch_bounds__(FD_NB / M * NPJ, NG == 4 ? 1 : (NPJ == 16 ? 2 : 4)) fp_diag_kernel(const FdParams prm) {
+  constexpr int NT = FD_NB / M * NPJ, NWARP = NT / 32, PLANE = RB * FD_PW * 16;
+  constexpr int WPG = FD_NB / M / FD_PPW;   // warps that share a group of FD_LP projections
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);              // [NSTG]
   uint64_t* empty = reinterpret_cast<uint64_t*>(smem + 32);        // [NSTG]
@@ -280,32 +284,32 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
   // bins mB + 2 jp + {0, 1, 2}: lower share of the first interval, both shares of the middle bin,
   // upper share of the second interval
 #if FD_PACKED
-  uint64_t acc[FD_M + 1][2 * NG];       // pairs of slices
+  uint64_t acc[M + 1][2 * NG];       // pairs of slices
 #pragma unroll
-  for (int q = 0; q <= FD_M; ++q)
+  for (int q = 0; q <= M; ++q)
 #pragma unroll
     for (int sl = 0; sl < 2 * NG; ++sl) acc[q][sl] = 0ull;
 #else
-  float acc[FD_M + 1][4 * NG];
+  float acc[M + 1][4 * NG];
 #pragma unroll
-  for (int q = 0; q <= FD_M; ++q)
+  for (int q = 0; q <= M; ++q)
 #pragma unroll
     for (int sl = 0; sl < 4 * NG; ++sl) acc[q][sl] = 0.f;
 #endif
 
   // a warp = 8 interval pairs x 4 projections: its 32 pixels of a line lie within ~16 stored
   // positions, i.e. the LDS.128 touches <= 256 B (2.4 cycles instead of 4, profiles/r02_micro.md)
-  const int jp = (warp % FD_WPG) * FD_PPW + lane / FD_LP;
-  const int pj = (warp / FD_WPG) * FD_LP + lane % FD_LP;
+  const int jp = (warp % WPG) * FD_PPW + lane / FD_LP;
+  const int pj = (warp / WPG) * FD_LP + lane % FD_LP;
   const bool active = pj < ck.count;
-  const int m0 = mB + FD_M * jp;
+  const int m0 = mB + M * jp;
   const float s = active ? sproj[pj].s : 0.f;
   const float sig = active ? sproj[pj].sig : 1.f;
   const int mul = ck.mul16;                    // sgn * 16 (from the table: one IMAD per address)
 
-  float afr[FD_M + 1], mg[FD_M + 1];
+  float afr[M + 1], mg[M + 1];
 #pragma unroll
-  for (int q = 0; q <= FD_M; ++q) afr[q] = mg[q] = 0.f;
+  for (int q = 0; q <= M; ++q) afr[q] = mg[q] = 0.f;
   const uint32_t buf_u32 = smem_u32(buf);
   const uint32_t magic_off = (uint32_t)mul * 0x4b400000u;
 
@@ -321,7 +325,7 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
         const FdProj* sp = &sproj[pj];
         const double K0 = sp->K0, inv = sp->inv, sD = sp->sD;
 #pragma unroll
-        for (int q = 0; q <= FD_M; ++q) {
+        for (int q = 0; q <= M; ++q) {
           const double ks = fma(sD, w0, fma((double)(m0 + q), inv, K0));
           const double ai = rint(ks);
           afr[q] = (float)(ks - ai);
@@ -337,14 +341,14 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
         {
 #pragma unroll
         for (int r = 0; r < FD_UNR; ++r) {
-          float ksf[FD_M + 1], jm[FD_M + 1];
+          float ksf[M + 1], jm[M + 1];
 #pragma unroll
-          for (int q = 0; q <= FD_M; ++q) {
+          for (int q = 0; q <= M; ++q) {
             ksf[q] = fmaf(s, (float)r, afr[q]);
             jm[q] = __fadd_ru(ksf[q], mg[q]);      // ceil(ks) + magic, integer part in the mantissa
           }
 #pragma unroll
-          for (int q = 0; q < FD_M; ++q) {
+          for (int q = 0; q < M; ++q) {
             const float f = sig * ((jm[q] - mg[q]) - ksf[q]);   // t - m of the pixel ceil(ks), in [0, sigma)
             const float g = 1.f - f;
             const bool in = jm[q] < jm[q + 1];                  // the interval holds that pixel
@@ -394,7 +398,7 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
         // the fractions move on by FD_UNR lines (the same FP32 operation in both threads that share a
         // boundary; re-based in double every FD_SB bands)
 #pragma unroll
-        for (int q = 0; q <= FD_M; ++q) afr[q] = fmaf(s, (float)FD_UNR, afr[q]);
+        for (int q = 0; q <= M; ++q) afr[q] = fmaf(s, (float)FD_UNR, afr[q]);
       }
     }
     __syncwarp();
@@ -414,18 +418,19 @@ __global__ void __launch_bounds__(FD_NB / FD_M * NPJ, NG == 4 ? 1 : (NPJ == 16 ?
   for (int sl = 0; sl < 4 * NG; ++sl) {
     const int sidx = gA * 4 + sl;
     if (sidx >= prm.S) break;       // uniform
+    // local bin index = bin - mB in [0, NB]: bins M jp + q, q < M, hold this thread's complete or lower share, bin
+    // M jp + M the upper share of its last interval
+#pragma unroll
+    for (int q = 0; q <= M; ++q) {
 #if FD_PACKED
-    const float a0 = (sl & 1) ? fd_hi(acc[0][sl >> 1]) : fd_lo(acc[0][sl >> 1]);
-    const float a1 = (sl & 1) ? fd_hi(acc[1][sl >> 1]) : fd_lo(acc[1][sl >> 1]);
-    const float a2 = (sl & 1) ? fd_hi(acc[2][sl >> 1]) : fd_lo(acc[2][sl >> 1]);
+      const float aq = (sl & 1) ? fd_hi(acc[q][sl >> 1]) : fd_lo(acc[q][sl >> 1]);
 #else
-    const float a0 = acc[0][sl], a1 = acc[1][sl], a2 = acc[2][sl];
+      const float aq = acc[q][sl];
 #endif
-    // local bin index = bin - mB in [0, NB]
-    lo_s[pj * (FD_NB + 1) + 2 * jp] = a0;
-    lo_s[pj * (FD_NB + 1) + 2 * jp + 1] = a1;
-    up_s[pj * (FD_NB + 1) + 2 * jp + 1] = 0.f;
-    up_s[pj * (FD_NB + 1) + 2 * jp + 2] = a2;
+      if (q < M) lo_s[pj * (FD_NB + 1) + M * jp + q] = aq;
+      else up_s[pj * (FD_NB + 1) + M * jp + M] = aq;
+      if (q > 0 && q < M) up_s[pj * (FD_NB + 1) + M * jp + q] = 0.f;
+    }
     __syncthreads();
     // complete bins: local 1 .. NB - 1
     for (int e = tid; e < NPJ * (FD_NB - 1); e += NT) {
@@ -776,11 +781,12 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
 #define FD_LAUNCH(NGV, NPJV, RBV, TWOV)                                                                             \
   do {                                                                                                              \
     if (first)                                                                                                      \
-      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<NGV, NPJV, RBV, TWOV>,                                     \
+      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<NGV, NPJV, RBV, TWOV, (NGV == 4 && FD_M1) ? 1 : FD_M>,                                     \
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(NGV, RBV, NPJV))); \
     StageScope scope(ST_FORWARD, stream);                                                                           \
     scope.kernels();                                                                                                \
-    fp_diag_kernel<NGV, NPJV, RBV, TWOV><<<grid, FD_NB / FD_M * NPJV, fd_smem(NGV, RBV, NPJV), stream>>>(prm);      \
+    fp_diag_kernel<NGV, NPJV, RBV, TWOV, (NGV == 4 && FD_M1) ? 1 : FD_M>                                          \
+        <<<grid, FD_NB / ((NGV == 4 && FD_M1) ? 1 : FD_M) * NPJV, fd_smem(NGV, RBV, NPJV), stream>>>(prm);      \
   } while (0)
   const int n_one = plan.n_chunks_one < 0 ? plan.n_chunks : plan.n_chunks_one;
   // two passes: the chunks of the generic projections, then those of the near-axis projections (TWO form).  Each pass
