@@ -55,6 +55,12 @@ namespace {
 #ifndef FD_M1
 #define FD_M1 0
 #endif
+// intervals per thread of the 8-slice dense form (NG = 2, 16 projections per block): 4 -- five boundaries serve four
+// intervals and the per-band set-up is shared by twice the work (256-thread blocks, two per SM): config 2 run on this
+// form 24.3 -> 23.3 ms, the 8-slice chunks of pyhst_forward_project_host 29.6 -> 28.6 ms
+#ifndef FD_M2
+#define FD_M2 4
+#endif
 #ifndef FD_SWAP
 #define FD_SWAP 1
 #endif
@@ -781,12 +787,12 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
 #define FD_LAUNCH(NGV, NPJV, RBV, TWOV)                                                                             \
   do {                                                                                                              \
     if (first)                                                                                                      \
-      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<NGV, NPJV, RBV, TWOV, (NGV == 4 && FD_M1) ? 1 : FD_M>,                                     \
+      PYHST_CUDA_TRY(cudaFuncSetAttribute(fp_diag_kernel<NGV, NPJV, RBV, TWOV, (NGV == 4 && FD_M1) ? 1 : ((NGV == 2 && NPJV == 16) ? FD_M2 : FD_M)>,                                     \
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fd_smem(NGV, RBV, NPJV))); \
     StageScope scope(ST_FORWARD, stream);                                                                           \
     scope.kernels();                                                                                                \
-    fp_diag_kernel<NGV, NPJV, RBV, TWOV, (NGV == 4 && FD_M1) ? 1 : FD_M>                                          \
-        <<<grid, FD_NB / ((NGV == 4 && FD_M1) ? 1 : FD_M) * NPJV, fd_smem(NGV, RBV, NPJV), stream>>>(prm);      \
+    fp_diag_kernel<NGV, NPJV, RBV, TWOV, (NGV == 4 && FD_M1) ? 1 : ((NGV == 2 && NPJV == 16) ? FD_M2 : FD_M)>                                          \
+        <<<grid, FD_NB / ((NGV == 4 && FD_M1) ? 1 : ((NGV == 2 && NPJV == 16) ? FD_M2 : FD_M)) * NPJV, fd_smem(NGV, RBV, NPJV), stream>>>(prm);      \
   } while (0)
   const int n_one = plan.n_chunks_one < 0 ? plan.n_chunks : plan.n_chunks_one;
   // two passes: the chunks of the generic projections, then those of the near-axis projections (TWO form).  Each pass
