@@ -186,6 +186,43 @@ int pyhst_ista_tv(const float* d_data, float* d_img, const pyhst_geom_t* g, floa
 int pyhst_ring_filter(const float* d_sino, const float* d_model, float* d_out, int32_t n_slices,
                       int32_t n_angles, int32_t n_bins, int64_t pitch, int32_t half_width, void* stream);
 
+/* The same ring filter for callers that cannot let the library allocate device memory.
+ *
+ * pyhst_ring_filter keeps two intermediates in the library's grow-on-demand workspace: the per-chunk
+ * column sums (double [n_slices][<= 32][n_bins]) and the high-pass row (float [n_slices][n_bins]).  Its first
+ * call with a new shape therefore runs cudaMalloc (and cudaFree of the outgrown block), which synchronises
+ * the device and can fail.  That rules it out for code running where allocation is forbidden or impossible:
+ * a host application that has carved the whole device memory up in advance into pools of its own (nothing
+ * is left for a library to claim), a latency-bound acquisition loop in which the device-wide
+ * synchronisation of cudaMalloc / cudaFree is not acceptable, or a process that has to keep correcting
+ * sinograms after the device ran out of memory.
+ *
+ * pyhst_ring_filter_static computes exactly the same result with exactly the same kernels, in the same
+ * summation order (bit-identical output), but keeps the two intermediates in a fixed array compiled into
+ * the library.  It calls no cudaMalloc / cudaFree / cudaMallocAsync, creates no stream, event or plan, and
+ * uses none of the library's cached workspace; the caller supplies the input and output buffers as before.
+ *
+ * Limit and cost: n_slices * n_bins <= PYHST_RING_STATIC_MAX_CELLS (32768 -- e.g. 16 slices of 2048 bins,
+ * any number of projections).  Larger requests are refused with PYHST_ERR_UNSUPPORTED and an explanatory
+ * pyhst_last_error(); split the stack by slices (slices are independent).  The array takes
+ * 32768 * (32 * 8 + 4) = 8 519 680 bytes of device memory on EVERY GPU on which this library is loaded,
+ * from load until the process exits, whether or not this entry point is ever called.
+ *
+ * First call on a device: it looks the array's device address up (cudaGetSymbolAddress) and raises the
+ * shared-memory limit of one kernel (cudaFuncSetAttribute), with that device current.  Neither allocates,
+ * but make this first call once per device during set-up, and before any stream capture is started.  Every
+ * later call only enqueues three kernels on `stream`.
+ *
+ * Sharing: all calls on one device use the same array, and it is NOT covered by the library's
+ * one-call-in-flight serialisation.  Two calls whose kernels can overlap on the GPU (different streams
+ * without an ordering between them, or different host threads on different streams) race on it and give
+ * wrong results; order them on one stream or with events.  The array keeps whatever the last call wrote;
+ * nothing in it needs to start at zero, because each call writes every element before reading it.
+ * Arguments, layouts and the remaining errors are those of pyhst_ring_filter (d_out may be d_sino). */
+#define PYHST_RING_STATIC_MAX_CELLS 32768
+int pyhst_ring_filter_static(const float* d_sino, const float* d_model, float* d_out, int32_t n_slices,
+                             int32_t n_angles, int32_t n_bins, int64_t pitch, int32_t half_width, void* stream);
+
 /* NEXT row N4 -- decoherence-maximising estimator, eq. 11:
  *   E_cohe[s] = Cos(I(beta) - I(0+), I(beta)) = <a - b, a> / (||a - b|| ||a||),  a = d_img_beta[s], b = d_img_0[s]
  * one fused pass over the two stacks, sums in double, fixed summation order (deterministic).

@@ -26,7 +26,7 @@ _LIBNAME = "libpyhst_b200.so"
 
 # every symbol include/*.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
-           "pyhst_fista_tv", "pyhst_ista_tv", "pyhst_ring_filter", "pyhst_ecohe", "pyhst_cv_distance", "pyhst_patch_grid",
+           "pyhst_fista_tv", "pyhst_ista_tv", "pyhst_ring_filter", "pyhst_ring_filter_static", "pyhst_ecohe", "pyhst_cv_distance", "pyhst_patch_grid",
            "pyhst_patch_gradient", "pyhst_patch_fista", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_last_forward_project_kernel", "pyhst_test_fd_plan", "pyhst_set_halfacq_stitch", "pyhst_set_filter_variant", "pyhst_set_patch_gemm_variant",
            "pyhst_last_error", "pyhst_release_cache")
 
@@ -71,6 +71,7 @@ def _load():
     lib.pyhst_ista_tv.argtypes = lib.pyhst_fista_tv.argtypes
     lib.pyhst_ring_filter.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int64, c_int32,
                                       c_void_p]
+    lib.pyhst_ring_filter_static.argtypes = lib.pyhst_ring_filter.argtypes
     lib.pyhst_ecohe.argtypes = [c_void_p, c_void_p, c_int32, c_int64, POINTER(c_double), c_void_p]
     lib.pyhst_cv_distance.argtypes = [c_void_p, c_void_p, POINTER(Geom), POINTER(c_double), c_void_p]
     lib.pyhst_patch_grid.argtypes = [c_int32, c_int32, c_int32, c_int32, POINTER(c_int32), POINTER(c_int32)]
@@ -239,6 +240,35 @@ def ring_filter(d_sino, half_width, model=None, out=None, stream=None):
     _check(lib.pyhst_ring_filter(_dev(d_sino, "d_sino"), None if model is None else _dev(model, "model"),
                                  _dev(out, "out"), s, p, b, c_int64(b), int(half_width), _stream(stream)),
            "pyhst_ring_filter")
+    return out
+
+
+RING_STATIC_MAX_CELLS = 32768   # PYHST_RING_STATIC_MAX_CELLS of include/pyhst.h
+
+
+def ring_filter_static(d_sino, half_width, model=None, out=None, stream=None):
+    """pyhst_ring_filter_static: ``ring_filter`` for programs in which the library may not allocate.
+
+    ``ring_filter`` parks its column sums in a workspace the library grows with cudaMalloc on the first
+    call of a shape.  Some programs cannot have that: they have given all device memory to their own
+    pools, cannot afford the device-wide stall of cudaMalloc / cudaFree inside an acquisition loop, or
+    have to go on after an out-of-memory condition.  This variant keeps the same intermediates in a fixed
+    8.5 MB array inside the library, allocates nothing, and returns bit-identical output.
+
+    Limit: ``S * B <= RING_STATIC_MAX_CELLS`` (32768), otherwise ``PyhstError`` -- split the stack by
+    slices.  Pass ``out`` if this wrapper must not allocate either (without it the result tensor comes
+    from torch's allocator).  All calls on a device share the one array: keep them ordered on one stream
+    (or by events); calls that overlap on the GPU corrupt each other.  The first call on a device looks
+    the array's address up -- make it during set-up, before any stream capture.
+    """
+    import torch
+    lib = _load()
+    s, p, b = d_sino.shape
+    if out is None:
+        out = torch.empty_like(d_sino)
+    _check(lib.pyhst_ring_filter_static(_dev(d_sino, "d_sino"), None if model is None else _dev(model, "model"),
+                                        _dev(out, "out"), s, p, b, c_int64(b), int(half_width), _stream(stream)),
+           "pyhst_ring_filter_static")
     return out
 
 

@@ -5,6 +5,7 @@
 // reductions in a fixed order (no atomics: results are bit-reproducible).
 #include <algorithm>
 #include <cmath>
+#include <mutex>
 #include <vector>
 
 #include "common.h"
@@ -230,5 +231,84 @@ extern "C" int pyhst_cv_distance(const float* d_img, const float* d_data_excl, c
   PYHST_CUDA_TRY(cudaGetLastError());
   PYHST_CUDA_TRY(cudaMemcpyAsync(h_out, d_out, (size_t)S * 8, cudaMemcpyDeviceToHost, stream));
   PYHST_CUDA_TRY(cudaStreamSynchronize(stream));
+  return PYHST_OK;
+}
+
+// ---- pyhst_ring_filter_static: the ring filter for callers that must not allocate -----------------
+// Same three kernels as pyhst_ring_filter, but the column sums `part` and the high-pass row `hp` live in
+// a fixed array that is part of the library image instead of the grow-on-demand workspace.  See
+// include/pyhst.h for who needs this and what it costs.
+namespace pyhst {
+namespace {
+
+// bytes per (slice, bin) cell: RG_PY partial column sums in double + one float of hp
+constexpr size_t RG_STATIC_CELL_BYTES = (size_t)RG_PY * sizeof(double) + sizeof(float);
+constexpr size_t RG_STATIC_BYTES = (size_t)PYHST_RING_STATIC_MAX_CELLS * RG_STATIC_CELL_BYTES;   // 8 519 680
+
+// One copy per GPU that loads the library, resident from module load until the process exits.
+// In HOST code this name is only a handle for cudaGetSymbolAddress -- it is not a device address and
+// must never be handed to a kernel as a pointer.
+static __device__ __align__(256) unsigned char g_ring_static_scratch[RG_STATIC_BYTES];
+
+constexpr int RG_STATIC_MAX_DEVICES = 64;
+std::mutex g_ring_static_mu;
+void* g_ring_static_ptr[RG_STATIC_MAX_DEVICES] = {nullptr};   // device address of the array, per device
+
+// First call on the current device: look the array's device address up and raise the shared-memory limit
+// of the high-pass kernel.  Neither step allocates.  Later calls return the remembered address.
+int ring_static_setup(void** scratch) {
+  const int dev = current_device();
+  if (dev < 0 || dev >= RG_STATIC_MAX_DEVICES)
+    return set_error(PYHST_ERR_UNSUPPORTED, "pyhst_ring_filter_static: device index %d outside 0..%d", dev,
+                     RG_STATIC_MAX_DEVICES - 1);
+  std::lock_guard<std::mutex> lock(g_ring_static_mu);
+  if (!g_ring_static_ptr[dev]) {
+    void* p = nullptr;
+    PYHST_CUDA_TRY(cudaGetSymbolAddress(&p, g_ring_static_scratch));
+    PYHST_CUDA_TRY(cudaFuncSetAttribute(ring_highpass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * 8));
+    g_ring_static_ptr[dev] = p;
+  }
+  *scratch = g_ring_static_ptr[dev];
+  return PYHST_OK;
+}
+
+}  // namespace
+}  // namespace pyhst
+
+extern "C" int pyhst_ring_filter_static(const float* d_sino, const float* d_model, float* d_out, int32_t n_slices,
+                                        int32_t n_angles, int32_t n_bins, int64_t pitch, int32_t half_width,
+                                        void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!d_sino || !d_out) return set_error(PYHST_ERR_INVALID_ARG, "pyhst_ring_filter_static: null pointer");
+  if (n_slices <= 0 || n_angles <= 0 || n_bins <= 0 || half_width < 1)
+    return set_error(PYHST_ERR_INVALID_ARG, "pyhst_ring_filter_static: S=%d P=%d B=%d half_width=%d", n_slices,
+                     n_angles, n_bins, half_width);
+  if (pitch == 0) pitch = n_bins;
+  if (pitch < n_bins) return set_error(PYHST_ERR_INVALID_ARG, "pyhst_ring_filter_static: pitch %lld < n_bins %d",
+                                       (long long)pitch, n_bins);
+  if (n_bins > 16384 || n_slices > 65535)
+    return set_error(PYHST_ERR_UNSUPPORTED, "pyhst_ring_filter_static: more than 16384 bins or 65535 slices");
+  if ((int64_t)n_slices * n_bins > PYHST_RING_STATIC_MAX_CELLS)
+    return set_error(PYHST_ERR_UNSUPPORTED,
+                     "pyhst_ring_filter_static: n_slices * n_bins = %lld exceeds the fixed scratch of %d cells "
+                     "(PYHST_RING_STATIC_MAX_CELLS); filter fewer slices per call or use pyhst_ring_filter",
+                     (long long)n_slices * n_bins, (int)PYHST_RING_STATIC_MAX_CELLS);
+  PYHST_TRY(require_sm100(nullptr));
+  void* scratch = nullptr;
+  PYHST_TRY(ring_static_setup(&scratch));
+  const int n_chunks = std::min(RG_PY, n_angles);
+  const int rows_per_chunk = (n_angles + n_chunks - 1) / n_chunks;
+  const size_t part_bytes = (size_t)n_slices * n_chunks * n_bins * sizeof(double);
+  double* part = static_cast<double*>(scratch);
+  float* hp = reinterpret_cast<float*>(static_cast<char*>(scratch) + part_bytes);
+  // Nothing has to be cleared: ring_colsum_kernel writes every part[s][c][b] (an empty chunk writes 0) and
+  // ring_highpass_kernel every hp[s][b] before the next kernel reads them; what the previous call left in
+  // the array is never read.
+  ring_colsum_kernel<<<dim3((n_bins + RG_BX - 1) / RG_BX, n_chunks, n_slices), RG_BX, 0, stream>>>(
+      d_sino, d_model, pitch, n_angles, n_bins, rows_per_chunk, part);
+  ring_highpass_kernel<<<n_slices, 256, (size_t)n_bins * 8, stream>>>(part, n_chunks, n_angles, n_bins, half_width, hp);
+  ring_subtract_kernel<<<dim3((n_bins + 255) / 256, std::min(n_angles, 64), n_slices), 256, 0, stream>>>(
+      d_sino, hp, d_out, pitch, n_angles, n_bins);
+  PYHST_CUDA_TRY(cudaGetLastError());
   return PYHST_OK;
 }
