@@ -33,7 +33,12 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "backprojection GUPS (pixel*projection*slice updates/s of the backprojection stage; FBP slices/s in metrics)"
+METRIC = ("backprojection GUPS (nominal S*nx*ny*P pixel*projection*slice updates / time of the backprojection stage; "
+          "executed updates and FBP slices/s in metrics)")
+# 1 (round 1): updates of the whole step / step time.  2 (round 2): backprojection updates / backprojection-stage time.
+# 3: as 2, and the reference arm prints the same quantity (oracle backprojection alone); nominal counting stated.
+METRIC_VERSION = 3
+N_INNER_TV = 20                  # dual steps per FISTA iteration of the config-4 solve
 METRIC_STEP = "projector updates/s over one hot-path step (ramp filter + backprojection + forward projection)"
 UNIT = "GUPS"
 FP32_LANES_PER_SM = 128          # FP32 FMA lanes per SM per clock (4 SMSP x 32)
@@ -183,7 +188,7 @@ def run_b200(args):
 
     def step():
         if fista:
-            P.fista_tv(sino, w.angles, w.axis, nx, ny, 0.01, n_fista, n_inner=20, n_power=8,
+            P.fista_tv(sino, w.angles, w.axis, nx, ny, 0.01, n_fista, n_inner=N_INNER_TV, n_power=8,
                        pixel_size=w.pixel_size, out=img, want_energy=False)
             return
         P.fbp(sino, w.angles, w.axis, nx, ny, w.pixel_size, filter=w.filter, mode=w.mode, out=img)
@@ -303,8 +308,13 @@ def run_b200(args):
             r["frac_at_sampled_clock"] = r["frac"] * (f_max / 1e6) / clocks["sm_mhz"]
         tr = _traffic().get("config%d" % w.cfg, {}).get(stage) if not args.slices else None
         if tr is not None:
-            r["traffic"] = tr
-            r["traffic_source"] = "stored: " + str(_traffic().get("_source", "profiles/traffic.json (ncu --set full capture)"))
+            # a stored number (one ncu --set full capture, not this run): only valid for the kernel it was taken on
+            captured = str(_traffic().get("_kernels", {}).get(stage, ""))
+            if captured and captured in name:
+                r["traffic"] = tr
+                r["traffic_source"] = _traffic_source()
+            else:
+                r["traffic_source"] = "none: the stored capture is of '%s', this run used '%s'" % (captured, name)
         return r
 
     calls = n_fista if fista else 1
@@ -325,14 +335,14 @@ def run_b200(args):
         others.append({"kernel": "ramp filter (a1)", "bound": "hbm", "achieved": fbytes / (ms_filter * 1e-3) / 1e9,
                        "peak": hbm, "unit": "GB/s", "frac": fbytes / (ms_filter * 1e-3) / 1e9 / hbm,
                        "traffic": _traffic().get("config%d" % w.cfg, {}).get("ramp_filter") if not args.slices else None,
-                       "traffic_source": "stored: " + str(_traffic().get("_source", "")),
+                       "traffic_source": _traffic_source(),
                        "avg_ms": ms_filter, "bytes_per_launch": fbytes,
                        "peak_note": "hbm_gbs of MEASURED_PEAKS.json (%s); algorithmic bytes = 4 (B_in + B_out) per row" % peaks_kind})
     if fista and ms_tv > 0:
         # N1: the dual steps dominate the solver's own kernels; algorithmic bytes of ONE dual step =
         # read z, p1, p2 + write p1', p2' = 5 image stacks
         dbytes = 5.0 * 4.0 * S * nx * ny
-        n_dual = n_fista * 20
+        n_dual = n_fista * N_INNER_TV
         others.append({"kernel": "ftv_dual_fused_kernel (+ residual / step / finish kernels of pyhst_fista_tv)",
                        "bound": "hbm", "achieved": dbytes * n_dual / (ms_tv * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
                        "frac": dbytes * n_dual / (ms_tv * 1e-3) / 1e9 / hbm, "traffic": None,
@@ -349,7 +359,7 @@ def run_b200(args):
         roofs = [x for x in (r_bp, r_fp) if x]       # the stated metric is the backprojector's: it leads
         metric, value = METRIC, bp_gups
     line = {
-        "metric": metric, "value": value, "unit": UNIT,
+        "metric": metric, "metric_version": METRIC_VERSION, "value": value, "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "impl": "b200",
@@ -389,6 +399,12 @@ def _traffic():
         return {}
 
 
+def _traffic_source():
+    t = _traffic()
+    return "stored: %s; captured at commit %s on %s" % (t.get("_source", "profiles/traffic.json"), t.get("_head", "?"),
+                                                       t.get("_date", "?"))
+
+
 def _oracle_sample(wl_mod, args):
     """One bounded sample of the workload for the oracle: the first `cpu_slices` slices (default 1) at
     full size -- all projections, bins and pixels, so every inner loop has the workload's own length."""
@@ -398,37 +414,51 @@ def _oracle_sample(wl_mod, args):
 
 
 def _time_oracle_step(oracle, w, sino):
-    """One hot-path step in the oracle, as it stands: FBP (direct-convolution filter + BP, fp64) then
-    forward projection of the float32-rounded result."""
+    """One hot-path step in the oracle, as it stands, stage by stage: ramp filter (direct convolution, fp64),
+    backprojection of the filtered rows (scale pi / P), forward projection of the float32-rounded result.
+    oracle.fbp is exactly filter then backprojection (pin K12); the half-acquisition mode has no separate
+    stages in the oracle and is timed as one FBP.  Returns (total, filter, backprojection, forward) seconds."""
+    import math
     import numpy as np
     t0 = time.perf_counter()
-    img = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, pixel_size=w.pixel_size, filter=w.filter, mode=w.mode)
+    if w.mode != 2:
+        q = oracle.ramp_filter(sino, filter=w.filter)
+        t1 = time.perf_counter()
+        scale = (math.pi if w.mode == 0 else 2.0 * math.pi) / w.n_angles
+        img = oracle.backproject(q, w.angles, w.axis, w.nx, w.ny, pixel_size=w.pixel_size, scale=scale)
+    else:
+        t1 = t0
+        img = oracle.fbp(sino, w.angles, w.axis, w.nx, w.ny, pixel_size=w.pixel_size, filter=w.filter, mode=w.mode)
+    t2 = time.perf_counter()
     oracle.forward_project(img.astype(np.float32), w.angles, w.axis, w.n_bins, pixel_size=w.pixel_size)
-    return time.perf_counter() - t0
+    t3 = time.perf_counter()
+    return t3 - t0, t1 - t0, t2 - t1, t3 - t2
 
 
 def cpu_baseline(wl_mod, args):
     import oracle
     oracle.build()
     w, sino = _oracle_sample(wl_mod, args)
-    sec = _time_oracle_step(oracle, w, sino)
+    sec, sec_filter, sec_bp, sec_fp = _time_oracle_step(oracle, w, sino)
     upd = w.n_slices * w.nx * w.ny * w.n_angles
-    # the oracle's filter is the direct O(B^2) convolution (its definition, not an FFT): timed alone as well, so
-    # that the projector pair's own share of the baseline can be read off (ADVICE.md round 1)
-    sec_filter = None
-    if w.mode != 2:
-        t0 = time.perf_counter()
-        oracle.ramp_filter(sino, filter=w.filter)
-        sec_filter = time.perf_counter() - t0
-    return {"value": 2 * upd / sec / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "seconds": sec, "seconds_ramp_filter_alone": sec_filter,
-            "projector_pair_gups": (2 * upd / max(sec - sec_filter, 1e-9) / 1e9) if sec_filter else None,
-            "sample": "%d of the config's slices at full size (%dx%d, %d projections x %d bins): oracle FBP "
-                      "(direct O(B^2) ramp convolution + backprojection, fp64, OpenMP) + oracle forward "
-                      "projection, one pass" % (w.n_slices, w.ny, w.nx, w.n_angles, w.n_bins)}
+    # value = the metric's own quantity (backprojection updates / time of the oracle's backprojection); the oracle's
+    # filter is the direct O(B^2) convolution (its definition, not an FFT), so the stages are listed one by one
+    return {"value": upd / sec_bp / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "seconds": sec, "seconds_ramp_filter": sec_filter, "seconds_backproject": sec_bp,
+            "seconds_forward_project": sec_fp, "step_gups": 2 * upd / sec / 1e9,
+            "projector_pair_gups": 2 * upd / max(sec_bp + sec_fp, 1e-9) / 1e9,
+            "sample": "%d of the config's slices at full size (%dx%d, %d projections x %d bins): oracle ramp filter "
+                      "(direct O(B^2) convolution), backprojection and forward projection (fp64, OpenMP), one pass; "
+                      "value = updates / backprojection seconds%s"
+                      % (w.n_slices, w.ny, w.nx, w.n_angles, w.n_bins,
+                         " (half acquisition: filter included, the oracle has one FBP routine for it)" if w.mode == 2 else "")}
 
 
 def run_reference(args):
+    """The oracle as it stands on the host cores, printing the SAME quantity as the b200 arm: backprojection updates
+    per second of the backprojection stage.  config / metric / unit are the b200 arm's; each step is a bounded sample
+    of that workload (cpu_baseline.sample says which).  --steps / --warmup are honoured as long as the run stays
+    within --ref-seconds (default 200 s; estimated from the first step), else fewer steps are run and reported."""
     rank, world = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1)
     if rank != 0:
         return
@@ -437,19 +467,30 @@ def run_reference(args):
     oracle.build()
     w, sino = _oracle_sample(wl_mod, args)
     full = wl_mod.config(args.config, n_slices=args.slices or None)
-    for _ in range(args.warmup_ref):
+    first = _time_oracle_step(oracle, w, sino)           # warm-up step 1 (or, with --warmup 0, timed step 1)
+    fit = max(1, int(args.ref_seconds / max(first[0], 1e-9)))
+    warmup = min(args.warmup, max(0, fit - 1))
+    steps = max(1, min(args.steps, fit - warmup))
+    runs = [first] if warmup == 0 else []
+    for _ in range(max(0, warmup - 1)):
         _time_oracle_step(oracle, w, sino)
-    steps = max(1, min(args.steps, args.max_ref_steps))
-    secs = [_time_oracle_step(oracle, w, sino) for _ in range(steps)]
-    sec = sum(secs) / len(secs)
+    while len(runs) < steps:
+        runs.append(_time_oracle_step(oracle, w, sino))
+    sec, sec_filter, sec_bp, sec_fp = [sum(r[k] for r in runs) / len(runs) for k in range(4)]
     upd = w.n_slices * w.nx * w.ny * w.n_angles
-    val = 2 * upd / sec / 1e9
-    sample = ("each step = %d of %d slices of the config at full size, oracle FBP + forward projection"
+    val = upd / sec_bp / 1e9
+    sample = ("each step = %d of %d slices of the config at full size: oracle ramp filter, backprojection, forward "
+              "projection; value = that sample's backprojection updates / its backprojection seconds"
               % (w.n_slices, full.n_slices))
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": steps, "warmup": args.warmup_ref, "ms_per_step": sec * 1e3, "higher_is_better": True,
+    line = {"impl": "reference", "metric": METRIC, "metric_version": METRIC_VERSION, "value": val, "unit": UNIT,
+            "n_gpus": args.gpus, "steps": steps, "warmup": warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": _config_dict(full, 1, {"reference": "oracle/ (fp64 CPU, OpenMP) on the host cores; " + sample}),
+            "config": _config_dict(full, 1),
+            "reference": "oracle/ (fp64 CPU, OpenMP) on the host cores; " + sample,
+            "metrics": {"backprojection_gups": val, "step_gups": 2 * upd / sec / 1e9,
+                        "projector_pair_gups": 2 * upd / max(sec_bp + sec_fp, 1e-9) / 1e9,
+                        "ms_ramp_filter": sec_filter * 1e3, "ms_backproject": sec_bp * 1e3,
+                        "ms_forward_project": sec_fp * 1e3, "slices_timed_per_step": w.n_slices},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -525,8 +566,8 @@ def main():
                     help="config 4: time FBP + forward projection instead of the 100-iteration TV-FISTA")
     ap.add_argument("--extra", default="", choices=["", "patch", "estimators"],
                     help="time pyhst_patch_gradient / the estimators instead of the hot-path step (see run_extra)")
-    ap.add_argument("--warmup-ref", type=int, default=0)
-    ap.add_argument("--max-ref-steps", type=int, default=2)
+    ap.add_argument("--ref-seconds", type=float, default=200.0,
+                    help="--impl reference: time budget within which --steps / --warmup are honoured")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         sys.stderr.write("note: fewer than 3 warm-up steps; the number is not a valid bench value\n")
