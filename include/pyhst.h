@@ -114,7 +114,14 @@ int pyhst_backproject(const float* d_sino, float* d_img, const pyhst_geom_t* g, 
  *   Lambda(u) = max(0, 1 - |u|).  Computed as a gather over detector bins (no atomics), so
  *   <P x, y> = <x, P^T y> holds up to FP32 rounding for the same `g`.
  *   d_img   [n_slices][ny][nx]               float32 (device, read)
- *   d_sino  [n_slices][n_angles][sino_pitch] float32 (device, columns < n_bins overwritten) */
+ *   d_sino  [n_slices][n_angles][sino_pitch] float32 (device, columns < n_bins overwritten)
+ * Workspace (cached per device, released by pyhst_release_cache): the diagonal-line kernel, which the library
+ * chooses for dense angle lists, keeps two sheared copies of the image stack,
+ *   2 * ceil(n_slices / 4) * (nx + ny + 7) lines * (nx + 392) * 16 bytes
+ * -- about 4.8x the stack: 1.3 GB for 16 slices of 2048^2, 7.7 GB for 64 slices of 2560^2.  The banded kernel
+ * (sparse lists, or when that block cannot be allocated: the library then falls back to it by itself) keeps
+ * about 2x the stack.  Stacks too large for either are projected in slice chunks by the caller
+ * (pyhst_forward_project_host does so). */
 int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t* g, float scale,
                           void* stream);
 

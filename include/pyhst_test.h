@@ -69,6 +69,12 @@ int pyhst_set_filter_variant(int variant);
  * kernel (UNSUPPORTED for other shapes).  Returns the previous value. */
 int pyhst_set_patch_gemm_variant(int variant);
 
+/* Makes every growth of an internal workspace block beyond `max_bytes` fail with PYHST_ERR_NOMEM, as if
+ * cudaMalloc had (0 = no limit, the default; blocks that are already large enough are not affected).  Lets a
+ * test exercise the out-of-memory paths -- e.g. the forward projector's fall-back from the diagonal-line to the
+ * banded kernel -- without exhausting the device.  Returns the previous limit. */
+int64_t pyhst_test_set_workspace_limit(int64_t max_bytes);
+
 #ifdef __cplusplus
 }
 #endif

@@ -9,5 +9,5 @@ from . import workloads  # noqa: F401
 from .binding import (  # noqa: F401
     FILTER_RAMLAK, FILTER_SHEPP_LOGAN, FILTER_HANN, FILTER_HAMMING, FILTER_COSINE, SCAN_180, SCAN_360, SCAN_360_HALF, PyhstError,
     backproject, backproject_host, fbp, fbp_host, fista_tv, ista_tv, ring_filter, ring_filter_static, ecohe, cv_distance, patch_grid, patch_gradient, patch_fista, forward_project_host, forward_project, halfacq_extent, last_error, library_path, profile_enable, profile_read,
-    ramp_filter, release_cache, set_backproject_variant, set_forward_project_variant, last_forward_project_kernel, set_halfacq_stitch, set_filter_variant, set_patch_gemm_variant,
+    ramp_filter, release_cache, set_backproject_variant, set_forward_project_variant, last_forward_project_kernel, set_halfacq_stitch, set_filter_variant, set_patch_gemm_variant, set_test_workspace_limit,
 )

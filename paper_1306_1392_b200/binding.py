@@ -27,7 +27,7 @@ _LIBNAME = "libpyhst_b200.so"
 # every symbol include/*.h declares
 EXPORTS = ("pyhst_ramp_filter", "pyhst_backproject", "pyhst_forward_project", "pyhst_fbp",
            "pyhst_fista_tv", "pyhst_ista_tv", "pyhst_ring_filter", "pyhst_ring_filter_static", "pyhst_ecohe", "pyhst_cv_distance", "pyhst_patch_grid",
-           "pyhst_patch_gradient", "pyhst_patch_fista", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_last_forward_project_kernel", "pyhst_test_fd_plan", "pyhst_set_halfacq_stitch", "pyhst_set_filter_variant", "pyhst_set_patch_gemm_variant",
+           "pyhst_patch_gradient", "pyhst_patch_fista", "pyhst_fbp_host", "pyhst_backproject_host", "pyhst_forward_project_host", "pyhst_halfacq_extent", "pyhst_profile_enable", "pyhst_profile_read", "pyhst_set_backproject_variant", "pyhst_set_forward_project_variant", "pyhst_last_forward_project_kernel", "pyhst_test_fd_plan", "pyhst_set_halfacq_stitch", "pyhst_set_filter_variant", "pyhst_set_patch_gemm_variant", "pyhst_test_set_workspace_limit",
            "pyhst_last_error", "pyhst_release_cache")
 
 
@@ -84,6 +84,8 @@ def _load():
     lib.pyhst_set_forward_project_variant.argtypes = [c_int]
     lib.pyhst_set_halfacq_stitch.argtypes = [c_int]
     lib.pyhst_set_filter_variant.argtypes = [c_int]
+    lib.pyhst_test_set_workspace_limit.argtypes = [c_int64]
+    lib.pyhst_test_set_workspace_limit.restype = c_int64
     lib.pyhst_set_patch_gemm_variant.argtypes = [c_int]
     lib.pyhst_profile_enable.argtypes = [c_int]
     lib.pyhst_profile_read.argtypes = [POINTER(c_double), POINTER(c_int64), POINTER(c_int64), c_int32]
@@ -452,6 +454,13 @@ def test_fd_plan(angles, axis, n_bins, nx, ny, pixel_size=1.0, n_slices=1):
 
 
 test_fd_plan.__test__ = False   # not a pytest test
+
+
+def set_test_workspace_limit(max_bytes: int) -> int:
+    """pyhst_test_set_workspace_limit (pyhst_test.h): workspace growth beyond max_bytes fails with NOMEM; 0 = off."""
+    return int(_load().pyhst_test_set_workspace_limit(int(max_bytes)))
+
+
 
 
 def last_forward_project_kernel() -> int:

@@ -79,6 +79,7 @@ int g_last_fp_kernel = 0;
 int g_halfacq_stitch = 1;
 int g_filter_variant = 0;
 int g_patch_gemm_variant = 0;
+std::atomic<int64_t> g_ws_limit{0};   // pyhst_test_set_workspace_limit
 
 DeviceCtx* ctx_of(int dev) {
   std::lock_guard<std::mutex> lock(g_map_mu);
@@ -107,18 +108,22 @@ int current_device() {
   return dev;
 }
 
-bool first_use_on_device(uint64_t* mask) {
-  const int dev = std::max(0, current_device()) & 63;
-  if ((*mask >> dev) & 1) return false;
-  *mask |= (uint64_t)1 << dev;
-  return true;
+// (device indices >= PYHST_MAX_DEVICES never get here: CallScope refuses them)
+bool first_use_on_device(DeviceMask* mask) {
+  const uint64_t bit = (uint64_t)1 << (std::max(0, current_device()) % PYHST_MAX_DEVICES);
+  return (mask->fetch_or(bit, std::memory_order_acq_rel) & bit) == 0;
 }
 
-size_t& PerDeviceSize::here() { return v[std::max(0, current_device()) & 63]; }
+size_t& PerDeviceSize::here() { return v[std::max(0, current_device()) % PYHST_MAX_DEVICES]; }
 
 CallScope::CallScope(cudaStream_t stream_) : stream(stream_) {
   const int dev = current_device();
   if (dev < 0) return;   // no device: the entry point's require_sm100() reports it
+  if (dev >= PYHST_MAX_DEVICES) {   // the per-device tables (first-use masks, PerDeviceSize) have one entry per index
+    status = set_error(PYHST_ERR_UNSUPPORTED, "device index %d: this library keeps state for devices 0..%d only", dev,
+                       PYHST_MAX_DEVICES - 1);
+    return;
+  }
   ctx = ctx_of(dev);
   ctx->mu.lock();
   if (ctx->depth++ == 0 && ctx->have_last && ctx->last_stream != stream) {
@@ -146,18 +151,19 @@ CallScope::~CallScope() {
 
 // ---- stage accounting --------------------------------------------------------------------
 namespace {
-struct StageEvents { Stage st; cudaEvent_t a, b; };
+struct StageEvents { Stage st; cudaEvent_t a, b; int dev; };
 std::mutex g_prof_mu;
 bool g_prof_on = false;
 std::vector<StageEvents> g_prof_pending;
-std::vector<cudaEvent_t> g_prof_pool;
+std::map<int, std::vector<cudaEvent_t>> g_prof_pool;   // per device: an event can only be recorded on a stream of the device it was created on
 double g_prof_ms[ST_COUNT] = {0};
 int64_t g_prof_kernels[ST_COUNT] = {0}, g_prof_fft[ST_COUNT] = {0};
 
-cudaEvent_t prof_event() {
-  if (!g_prof_pool.empty()) {
-    cudaEvent_t e = g_prof_pool.back();
-    g_prof_pool.pop_back();
+cudaEvent_t prof_event(int dev) {
+  auto& pool = g_prof_pool[dev];
+  if (!pool.empty()) {
+    cudaEvent_t e = pool.back();
+    pool.pop_back();
     return e;
   }
   cudaEvent_t e = nullptr;
@@ -169,7 +175,9 @@ cudaEvent_t prof_event() {
 StageScope::StageScope(Stage st_, cudaStream_t stream_) : st(st_), stream(stream_), slot(-1) {
   std::lock_guard<std::mutex> lock(g_prof_mu);
   if (!g_prof_on) return;
-  StageEvents ev{st, prof_event(), prof_event()};
+  const int dev = current_device();
+  if (dev < 0) return;
+  StageEvents ev{st, prof_event(dev), prof_event(dev), dev};
   if (!ev.a || !ev.b) return;
   cudaEventRecord(ev.a, stream);
   slot = (int)g_prof_pending.size();
@@ -217,6 +225,18 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
     g_geom.erase(lru);
   }
   GeomPlan pl;
+  // an early return below (PYHST_CUDA_TRY) must not leak what the plan already owns
+  struct GeomGuard {
+    GeomPlan* pl;
+    bool keep = false;
+    ~GeomGuard() {
+      if (keep) return;
+      cudaFree(pl->d_proj);
+      cudaFree(pl->d_run);
+      cudaFree(pl->d_flip);
+      cudaFreeHost(pl->h_pinned);
+    }
+  } guard{&pl};
   pl.n_angles = g->n_angles;
   pl.n_bins = n_bins;
   pl.pixel_size = g->pixel_size;
@@ -226,7 +246,6 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
   PYHST_CUDA_TRY(cudaMallocHost(&pl.h_pinned, n * sizeof(ProjGeom)));
   cudaError_t e = cudaMalloc(&pl.d_proj, n * sizeof(ProjGeom));
   if (e != cudaSuccess) {
-    cudaFreeHost(pl.h_pinned);
     return set_error(PYHST_ERR_NOMEM, "cudaMalloc of the geometry table failed: %s",
                      cudaGetErrorString(e));
   }
@@ -266,6 +285,7 @@ int get_geom_plan(const pyhst_geom_t* g, double axis_shift, int32_t n_bins, cuda
     PYHST_CUDA_TRY(cudaMemcpyAsync(pl.d_flip, flip.data(), n, cudaMemcpyHostToDevice, stream));
   }
   pl.last_use = ++g_tick;
+  guard.keep = true;
   g_geom.push_back(std::move(pl));
   *out = &g_geom.back();
   return PYHST_OK;
@@ -299,6 +319,18 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, int want_diag, const
     g_fp_plans.erase(lru);
   }
   FpPlan pl;
+  struct FpGuard {   // frees the device tables of a plan that an early return abandons
+    FpPlan* pl;
+    bool keep = false;
+    ~FpGuard() {
+      if (keep) return;
+      cudaFree(pl->d_projs);
+      cudaFree(pl->d_chunks);
+      cudaFree(pl->fd.d_projs);
+      cudaFree(pl->fd.d_chunks);
+      cudaFree(pl->fd.d_ranges);
+    }
+  } guard{&pl};
   pl.n_angles = g->n_angles;
   pl.n_bins = g->n_bins;
   pl.nx = g->nx;
@@ -311,6 +343,7 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, int want_diag, const
   std::vector<FpProjD> projs;
   std::vector<FpChunk> chunks;
   std::vector<int32_t> legacy;
+  bool banded_built = false;   // projs / chunks already hold the banded tables of the `legacy` projections
   if (want_diag) {
     // diagonal-line interval kernel for every projection it covers; the banded tables then hold
     // only the rest (projections within 2^-12 rad of an image axis, windows that do not fit)
@@ -333,8 +366,13 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, int want_diag, const
       // banded kernel's smaller blocks win)
       use = per_chunk >= 0.55 * pl.fd.npj && blocks >= (int64_t)n_sm;
     }
-    if (use && (legacy.empty() || build_fp_tables(g, &probe, &projs, &chunks, &legacy))) {
+    if (use && !legacy.empty()) banded_built = build_fp_tables(g, &probe, &projs, &chunks, &legacy);
+    if (use && (legacy.empty() || banded_built)) {
       pl.diag = true;
+      if (banded_built) {   // keep the probe's tables: the banded part of the plan is exactly what it built
+        pl.nc = probe.nc; pl.W = probe.W; pl.npj = probe.npj; pl.n_chunks = probe.n_chunks; pl.n_tab = probe.n_tab;
+        pl.any_rows = probe.any_rows; pl.any_cols = probe.any_cols;
+      }
       pl.n_legacy = (int32_t)legacy.size();
       PYHST_CUDA_TRY(cudaMalloc(&pl.fd.d_projs, dprojs.size() * sizeof(FdProj)));
       PYHST_CUDA_TRY(cudaMalloc(&pl.fd.d_chunks, dchunks.size() * sizeof(FdChunk)));
@@ -350,12 +388,15 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, int want_diag, const
                 g->n_angles, g->n_bins, g->nx, g->ny, g->pixel_size, pl.fd.W, pl.fd.n_chunks, pl.fd.n_bx,
                 pl.n_legacy);
     }
-    projs.clear();
-    chunks.clear();
+    banded_built = banded_built && pl.diag;
+    if (!banded_built) {
+      projs.clear();
+      chunks.clear();
+    }
   }
   if (pl.diag && legacy.empty()) {
     pl.n_chunks = 0;
-  } else if (build_fp_tables(g, &pl, &projs, &chunks, pl.diag ? &legacy : nullptr)) {
+  } else if (banded_built || build_fp_tables(g, &pl, &projs, &chunks, pl.diag ? &legacy : nullptr)) {
     PYHST_CUDA_TRY(cudaMalloc(&pl.d_projs, projs.size() * sizeof(FpProjD)));
     PYHST_CUDA_TRY(cudaMalloc(&pl.d_chunks, chunks.size() * sizeof(FpChunk)));
     // pageable sources: the copies are complete (staged) when the calls return
@@ -371,6 +412,7 @@ int get_fp_plan(const pyhst_geom_t* g, cudaStream_t stream, int want_diag, const
     pl.n_chunks = 0;  // geometry not covered by the banded kernel: the generic gather kernel runs
   }
   pl.last_use = ++g_tick;
+  guard.keep = true;
   g_fp_plans.push_back(std::move(pl));
   *out = &g_fp_plans.back();
   return PYHST_OK;
@@ -387,6 +429,10 @@ int get_workspace(WorkspaceSlot slot, size_t bytes, void** ptr) {
       w.bytes = 0;
     }
     ++w.gen;
+    const int64_t limit = g_ws_limit.load();
+    if (limit > 0 && bytes > (size_t)limit)
+      return set_error(PYHST_ERR_NOMEM, "workspace allocation of %zu bytes refused (test limit %lld)", bytes,
+                       (long long)limit);
     cudaError_t e = cudaMalloc(&w.p, bytes);
     if (e != cudaSuccess) {
       cudaGetLastError();
@@ -506,8 +552,8 @@ int pyhst_profile_read(double* ms, int64_t* kernels, int64_t* fft_execs, int32_t
     float t = 0.f;
     PYHST_CUDA_TRY(cudaEventElapsedTime(&t, ev.a, ev.b));
     g_prof_ms[ev.st] += (double)t;
-    g_prof_pool.push_back(ev.a);
-    g_prof_pool.push_back(ev.b);
+    g_prof_pool[ev.dev].push_back(ev.a);
+    g_prof_pool[ev.dev].push_back(ev.b);
   }
   g_prof_pending.clear();
   for (int i = 0; i < ST_COUNT; ++i) {
@@ -524,6 +570,8 @@ int pyhst_set_backproject_variant(int variant) {
   if (variant >= 0 && variant <= 7 && variant != 5) g_bp_variant = variant;
   return prev;
 }
+
+int64_t pyhst_test_set_workspace_limit(int64_t max_bytes) { return g_ws_limit.exchange(max_bytes < 0 ? 0 : max_bytes); }
 
 int pyhst_set_halfacq_stitch(int enable) {
   const int prev = g_halfacq_stitch;
@@ -616,8 +664,10 @@ void pyhst_release_cache(void) {
     for (auto& e : c->events) if (e) { cudaEventDestroy(e); e = nullptr; }
     if (c->last_done) { cudaEventDestroy(c->last_done); c->last_done = nullptr; }
     c->have_last = false;
+    // while c->mu is still held: a call in flight on another thread may have copied a table pointer or a
+    // cuFFT handle out of the maps and be about to launch with it
+    release_filter_plans(c->device);
   }
-  release_filter_plans();
   if (prev >= 0) cudaSetDevice(prev);
   cudaGetLastError();
 }
@@ -715,6 +765,13 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
   if (g_fp_variant != 1) {
     const FpPlan* fplan = nullptr;
     PYHST_TRY(get_fp_plan(g, stream, g_fp_variant == 5 ? 2 : (g_fp_variant == 0 ? 1 : 0), &fplan));
+    if (fplan->diag && g_fp_variant == 0) {
+      // automatic choice: the diagonal-line kernel needs two sheared copies of the stack (about 4.6x its size,
+      // see pyhst.h).  If that block cannot be had, the banded kernel (about 2x) still can run: take its plan.
+      void* xd = nullptr;
+      if (get_workspace(WS_XD, fd_xd_bytes(fplan->fd, g, nullptr), &xd) == PYHST_ERR_NOMEM)
+        PYHST_TRY(get_fp_plan(g, stream, 0, &fplan));
+    }
     if (fplan->diag) {
       g_last_fp_kernel = 5;
       PYHST_TRY(launch_forward_project_diag(d_img, d_sino, pitch, g, scale, fplan->fd, stream));

@@ -249,7 +249,7 @@ template <int WS, int NS>
 int launch_run16(const float4* d_qi, const QiLayout& L, const BpArgs& a, const RunProj* d_run, int32_t n_a,
                  int32_t n_b, int W, cudaStream_t stream) {
   const size_t smem = R16_HDR + (size_t)NS * R16_NA * R16_NG * WS * 16;
-  static uint64_t configured = 0;   // one bit per device (cudaFuncSetAttribute is per device)
+  static DeviceMask configured{0};   // one bit per device (cudaFuncSetAttribute is per device)
   if (first_use_on_device(&configured)) {
     PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run16_kernel<0, WS, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)smem));

@@ -362,7 +362,7 @@ template <int WS, int NS, bool PACKED>
 int launch_run8(const float4* d_qi, const QiLayout& L, const BpArgs& a, const RunProj* d_run,
                 int32_t n_a, int32_t n_b, int W, cudaStream_t stream) {
   const size_t smem = R8_HDR + (size_t)NS * R8_NA * 2 * WS * 16;
-  static uint64_t configured = 0;   // one bit per device (cudaFuncSetAttribute is per device)
+  static DeviceMask configured{0};   // one bit per device (cudaFuncSetAttribute is per device)
   if (first_use_on_device(&configured)) {
     PYHST_CUDA_TRY(cudaFuncSetAttribute(bp_run8_kernel<0, WS, NS, PACKED>,
                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

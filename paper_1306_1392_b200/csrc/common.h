@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <cstdarg>
 #include <cstdio>
 #include <vector>
@@ -74,13 +75,16 @@ struct CallScope {
   if (_call_scope.status != PYHST_OK) return _call_scope.status
 
 int current_device();  // cudaGetDevice, -1 on failure
-// true exactly once per (mask, device): cudaFuncSetAttribute and friends are per device.
-// Call inside a CallScope (the device lock makes it race-free).
-bool first_use_on_device(uint64_t* mask);
+// true exactly once per (mask, device): cudaFuncSetAttribute and friends are per device.  The mask is
+// shared by all devices (one bit each, device index < PYHST_MAX_DEVICES), hence atomic: threads working
+// on different devices hold different device locks.
+constexpr int PYHST_MAX_DEVICES = 64;
+using DeviceMask = std::atomic<uint64_t>;
+bool first_use_on_device(DeviceMask* mask);
 // per-device table of sizes already configured (index = device), for kernels whose dynamic
 // shared-memory limit grows with the geometry
 struct PerDeviceSize {
-  size_t v[64] = {0};
+  size_t v[PYHST_MAX_DEVICES] = {0};   // one element per device: written under that device's lock only
   size_t& here();
 };
 
@@ -244,6 +248,7 @@ bool build_fp_tables(const pyhst_geom_t* g, FpPlan* plan, std::vector<FpProjD>* 
 // covers none
 bool build_fd_tables(const pyhst_geom_t* g, FdPlan* plan, std::vector<FdProj>* projs, std::vector<FdChunk>* chunks,
                      std::vector<int32_t>* ranges, std::vector<int32_t>* legacy, int npj = 16);  // forward_project_diag.cu
+size_t fd_xd_bytes(const FdPlan& plan, const pyhst_geom_t* g, int* n_groups_alloc);   // bytes of the WS_XD block
 void fd_block_shape(int32_t* nb, int32_t* npj);   // intervals per block, projections per chunk
 int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch, const pyhst_geom_t* g,
                                 float scale, const FdPlan& plan, cudaStream_t stream);
@@ -280,7 +285,8 @@ int launch_ramp_filter_fused(const float* d_in, int64_t in_pitch, int64_t n_rows
                              int32_t n_bins_out, int32_t pad_left, int filter, const float* d_col_weights,
                              float* d_out, int64_t out_pitch, float4* d_qi, const QiLayout* L, int32_t n_slices_in,
                              const uint8_t* d_flip, cudaStream_t stream);
-void release_fused_filter_tables();
+// frees the tables of `device` (current, idle, and with its DeviceCtx lock held by the caller)
+void release_fused_filter_tables(int device);
 int filter_variant();   // 0 automatic, 1 cuFFT path, 2 fused kernel (pyhst_test.h)
 // tensor-core GEMM of Algorithm 1 (patch_gemm_tc.cu): C[M x N] = alpha A[M x K] B, per slice of a stack
 bool patch_gemm_tc_covers(int N, int K);
@@ -291,7 +297,8 @@ int patch_gemm_variant();   // 0 automatic, 1 FP32 SIMT kernel, 2 tcgen05 3xTF32
 int launch_halfacq_weights(float* d_w, int32_t n_bins, double cbar, cudaStream_t stream);
 int launch_halfacq_fold(const float* d_rows, float* d_out, int32_t n_slices, int32_t half_angles,
                         int32_t b_out, int32_t b_st, int32_t off, const int* d_two_c, cudaStream_t stream);
-void release_filter_plans();
+// frees the cuFFT plans, spectra and fused-filter tables of `device` (same conditions)
+void release_filter_plans(int device);
 
 // ---- device helpers: mbarrier + TMA bulk copy (inline PTX) -----------------------------------
 #ifdef __CUDACC__

@@ -167,7 +167,7 @@ extern "C" int pyhst_ring_filter(const float* d_sino, const float* d_model, floa
   PYHST_TRY(get_workspace(WS_FPL, part_bytes + (size_t)n_slices * n_bins * 4, &ws));
   double* part = static_cast<double*>(ws);
   float* hp = reinterpret_cast<float*>(static_cast<char*>(ws) + part_bytes);
-  static uint64_t configured = 0;
+  static DeviceMask configured{0};
   if (first_use_on_device(&configured))
     PYHST_CUDA_TRY(cudaFuncSetAttribute(ring_highpass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * 8));
   StageScope scope(ST_FILTER, stream);

@@ -276,16 +276,20 @@ int launch_ramp_filter(const float* d_in, int64_t in_pitch, int64_t n_rows, int3
   return PYHST_OK;
 }
 
-void release_filter_plans() {
-  release_fused_filter_tables();
+void release_filter_plans(int device) {
+  release_fused_filter_tables(device);
   std::lock_guard<std::mutex> lock(g_mu);
-  for (auto& kv : g_plans) {
-    cufftDestroy(kv.second.r2c);
-    cufftDestroy(kv.second.c2r);
+  for (auto it = g_plans.begin(); it != g_plans.end();) {
+    if (std::get<0>(it->first) != device) { ++it; continue; }
+    cufftDestroy(it->second.r2c);
+    cufftDestroy(it->second.c2r);
+    it = g_plans.erase(it);
   }
-  g_plans.clear();
-  for (auto& kv : g_spectra) cudaFree(kv.second.d_H);
-  g_spectra.clear();
+  for (auto it = g_spectra.begin(); it != g_spectra.end();) {
+    if (std::get<0>(it->first) != device) { ++it; continue; }
+    cudaFree(it->second.d_H);
+    it = g_spectra.erase(it);
+  }
 }
 
 // ---- stitched half acquisition (NEXT row N2; reading R10) -------------------------

@@ -406,12 +406,18 @@ int launch_ramp_filter_fused(const float* d_in, int64_t in_pitch, int64_t n_rows
   return PYHST_OK;
 }
 
-void release_fused_filter_tables() {
+void release_fused_filter_tables(int device) {
   std::lock_guard<std::mutex> lock(g_mu);
-  for (auto& kv : g_tables) cudaFree(kv.second.d_Hq);
-  g_tables.clear();
-  for (auto& kv : g_twiddles) cudaFree(kv.second);
-  g_twiddles.clear();
+  for (auto it = g_tables.begin(); it != g_tables.end();) {
+    if (std::get<0>(it->first) != device) { ++it; continue; }
+    cudaFree(it->second.d_Hq);
+    it = g_tables.erase(it);
+  }
+  for (auto it = g_twiddles.begin(); it != g_twiddles.end();) {
+    if (it->first.first != device) { ++it; continue; }
+    cudaFree(it->second);
+    it = g_twiddles.erase(it);
+  }
 }
 
 }  // namespace pyhst

@@ -729,22 +729,30 @@ int launch_forward_project_banded(const float* d_img, float* d_sino, int64_t pit
   const int n_groups = (g->n_slices + 3) / 4;
   const int W = plan.W;
   XiLayout Lr{n_groups, g->ny, g->nx, W}, Lc{n_groups, g->nx, g->ny, W};
-  const size_t bytes_r = plan.any_rows ? Lr.bytes() : 0, bytes_c = plan.any_cols ? Lc.bytes() : 0;
+  size_t bytes_r = plan.any_rows ? Lr.bytes() : 0, bytes_c = plan.any_cols ? Lc.bytes() : 0;
   void* ws = nullptr;
   PYHST_TRY(get_workspace(WS_XI, bytes_r + bytes_c, &ws));
-  float4* xi_r = plan.any_rows ? static_cast<float4*>(ws) : nullptr;
-  float4* xi_c = plan.any_cols ? reinterpret_cast<float4*>(static_cast<char*>(ws) + bytes_r) : nullptr;
   // the zero pads are written once per (block, layout); the repack only touches the interior
   // ("this very block": device + the slot's allocation generation, so that a block freed by
-  // pyhst_release_cache or regrown and handed back at the same address is zeroed again)
+  // pyhst_release_cache or regrown and handed back at the same address is zeroed again).
+  // A stack of FEWER slice groups than the one the block was zeroed for (the last chunk of a host
+  // pipeline) is laid out as that larger stack -- the column copy keeps its place -- so that it finds
+  // the pads already zero instead of clearing the block on every call; groups >= n_groups are not read.
   struct PadsKey { size_t k[8]; };
-  static PadsKey pads[64];
-  const PadsKey key = {{bytes_r, bytes_c, (size_t)g->nx, (size_t)g->ny, (size_t)W, (size_t)n_groups,
-                        (size_t)workspace_generation(WS_XI), (size_t)reinterpret_cast<uintptr_t>(ws)}};
-  PadsKey& seen = pads[std::max(0, current_device()) & 63];
+  static PadsKey pads[PYHST_MAX_DEVICES];
+  PadsKey key = {{(size_t)plan.any_rows, (size_t)plan.any_cols, (size_t)g->nx, (size_t)g->ny, (size_t)W,
+                  (size_t)n_groups, (size_t)workspace_generation(WS_XI), (size_t)reinterpret_cast<uintptr_t>(ws)}};
+  PadsKey& seen = pads[std::max(0, current_device()) % PYHST_MAX_DEVICES];
+  const size_t seen_groups = seen.k[5];
+  key.k[5] = seen_groups;
+  const bool pads_zero = std::memcmp(&seen, &key, sizeof(key)) == 0 && seen_groups >= (size_t)n_groups;
+  key.k[5] = (size_t)n_groups;
+  if (pads_zero && plan.any_rows) bytes_r = XiLayout{(int32_t)seen_groups, g->ny, g->nx, W}.bytes();
+  float4* xi_r = plan.any_rows ? static_cast<float4*>(ws) : nullptr;
+  float4* xi_c = plan.any_cols ? reinterpret_cast<float4*>(static_cast<char*>(ws) + bytes_r) : nullptr;
   {
     StageScope scope(ST_TRANSPOSE, stream);
-    if (std::memcmp(&seen, &key, sizeof(key)) != 0) {
+    if (!pads_zero) {
       PYHST_CUDA_TRY(cudaMemsetAsync(ws, 0, bytes_r + bytes_c, stream));
       seen = key;
     }

@@ -738,15 +738,23 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
   PYHST_TRY(get_workspace(WS_XD, bytes, &ws));
   float4* xd0 = static_cast<float4*>(ws);
   float4* xd1 = xd0 + (int64_t)nga * group_f4;
-  // zero positions are written once per (block, layout): see repack_diag_kernel
+  // zero positions are written once per (block, layout): see repack_diag_kernel.  A stack of FEWER slice groups
+  // than the one the block was zeroed for (the last chunk of a host pipeline) is laid out as that larger stack
+  // -- the second sheared copy keeps its place -- and finds its zeros in place instead of clearing the block on
+  // every call; the kernels read groups < n_groups only.
   struct Key { size_t k[8]; };
-  static Key seen_all[64];
-  const Key key = {{bytes, (size_t)g->nx, (size_t)g->ny, (size_t)plan.zpad, (size_t)plan.n_lines_alloc, (size_t)nga,
-                    (size_t)workspace_generation(WS_XD), (size_t)reinterpret_cast<uintptr_t>(ws)}};
-  Key& seen = seen_all[std::max(0, current_device()) & 63];
+  static Key seen_all[PYHST_MAX_DEVICES];
+  Key key = {{0, (size_t)g->nx, (size_t)g->ny, (size_t)plan.zpad, (size_t)plan.n_lines_alloc, (size_t)nga,
+              (size_t)workspace_generation(WS_XD), (size_t)reinterpret_cast<uintptr_t>(ws)}};
+  Key& seen = seen_all[std::max(0, current_device()) % PYHST_MAX_DEVICES];
+  const size_t seen_groups = seen.k[5];
+  key.k[5] = seen_groups;
+  const bool zeros_in_place = std::memcmp(&seen, &key, sizeof(key)) == 0 && seen_groups >= (size_t)nga;
+  key.k[5] = (size_t)nga;
+  if (zeros_in_place) xd1 = xd0 + (int64_t)seen_groups * group_f4;
   {
     StageScope scope(ST_TRANSPOSE, stream);
-    if (std::memcmp(&seen, &key, sizeof(key)) != 0) {
+    if (!zeros_in_place) {
       PYHST_CUDA_TRY(cudaMemsetAsync(ws, 0, bytes, stream));
       seen = key;
     }
@@ -783,7 +791,7 @@ int launch_forward_project_diag(const float* d_img, float* d_sino, int64_t pitch
   prm.part = nullptr;
   prm.part_pitch = g->n_bins;
   prm.part_stride = 0;
-  static uint64_t configured[12] = {0};
+  static DeviceMask configured[12];
 #define FD_LAUNCH(NGV, NPJV, RBV, TWOV)                                                                             \
   do {                                                                                                              \
     if (first)                                                                                                      \

@@ -892,3 +892,72 @@ def test_patch_gradient_tensor_core_gemm(lib, oracle, m, st, n_atoms):
             assert_parity(X[s].cpu().numpy(), Xw, "patch X, GEMM variant %d" % variant)
             assert_parity(G[s].cpu().numpy(), Gw, "patch G, GEMM variant %d" % variant, rel=PATCH_REL_L2, mabs=2e-4)
     assert not np.array_equal(out[1][0].cpu().numpy(), out[2][0].cpu().numpy())    # the two kernels really differ
+
+
+# ------------------------------------------------------------------------------ workspace handling
+def _dense_scan(S, n, P, B, seed):
+    rng = np.random.default_rng(seed)
+    angles = np.arange(P) * (math.pi / P)
+    axis = (B - 1) / 2.0 + rng.uniform(-1.5, 1.5, size=P)
+    x = rng.normal(size=(S, n, n)).astype(np.float32)
+    return x, angles, axis
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("variant", [0, 2, 5])
+def test_forward_project_smaller_stack_after_larger_one(lib, oracle, variant):
+    """A stack of fewer slice groups than the one before it (the last chunk of a host pipeline) is laid out
+    inside the workspace block that was zeroed for the larger stack and does not clear it again: results must
+    be the same as from a freshly cleared block, bit for bit, for the sheared (diagonal-line) and the
+    line-interleaved (banded) layouts, and whichever of the two the automatic choice takes."""
+    n, P, B = 160, 360, 240
+    big, angles, axis = _dense_scan(12, n, P, B, seed=5)
+    small = _dense_scan(5, n, P, B, seed=6)[0]
+    prev = lib.set_forward_project_variant(variant)
+    try:
+        fp = lambda x: lib.forward_project(_dev(x), angles, axis, B).cpu().numpy()
+        lib.release_cache()
+        ref_small = fp(small)                      # block sized and cleared for 2 slice groups
+        assert_parity(ref_small, oracle.forward_project(small, angles, axis, B), "forward_project, 5 slices")
+        lib.release_cache()
+        ref_two = fp(small[:2])                    # one slice group (the automatic choice may differ per group count)
+        lib.release_cache()
+        ref_big = fp(big)                          # block sized and cleared for 3 slice groups
+        assert np.array_equal(fp(small), ref_small)    # laid out as the 3-group stack, pads found zero
+        assert np.array_equal(fp(big), ref_big)
+        assert np.array_equal(fp(small[:2]), ref_two)
+        assert np.array_equal(fp(big), ref_big)
+    finally:
+        lib.set_forward_project_variant(prev)
+
+
+@pytest.mark.gpu
+def test_forward_project_falls_back_to_banded_kernel_without_room_for_the_sheared_copies(lib, oracle):
+    """Automatic kernel choice: when the block for the two sheared image copies (about 4.8x the stack) cannot be
+    allocated, the call runs on the banded kernel (about 2x) instead of failing with NOMEM."""
+    n, P, B = 512, 360, 512
+    x, angles, axis = _dense_scan(8, n, P, B, seed=7)
+    lib.release_cache()
+    ref = lib.forward_project(_dev(x), angles, axis, B).cpu().numpy()
+    assert lib.last_forward_project_kernel() == 5          # the diagonal-line kernel is the automatic choice here
+    xd_bytes = 2 * 2 * (n + n + 7) * (n + 392) * 16         # pyhst.h: two copies, 2 slice groups
+    lib.release_cache()
+    prev_limit = lib.set_test_workspace_limit(xd_bytes - 1)
+    try:
+        got = lib.forward_project(_dev(x), angles, axis, B).cpu().numpy()
+        assert lib.last_forward_project_kernel() == 2
+        assert_parity(got, ref.astype(np.float64), "forward_project on the banded kernel vs the diagonal-line kernel")
+        rows = [0, 89, 90, 91, 180, 359]
+        want = oracle.forward_project(x[:1], angles[rows], axis[rows], B)
+        assert_parity(got[:1, rows], want, "forward_project fall-back vs oracle")
+        prev = lib.set_forward_project_variant(5)          # forced: no fall-back, the error is reported
+        try:
+            with pytest.raises(lib.PyhstError, match="refused"):
+                lib.forward_project(_dev(x), angles, axis, B)
+        finally:
+            lib.set_forward_project_variant(prev)
+    finally:
+        lib.set_test_workspace_limit(prev_limit)
+        lib.release_cache()
+    assert np.array_equal(lib.forward_project(_dev(x), angles, axis, B).cpu().numpy(), ref)
+    assert lib.last_forward_project_kernel() == 5
