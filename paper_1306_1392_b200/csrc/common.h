@@ -337,8 +337,8 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 
 // (c0, c1) += (a0, a1) * s: one packed FFMA2 (ptxas encodes the broadcast scalar operand directly).  On
-// sm_100a an FFMA2 takes one issue slot and holds the FMA pipe for two cycles, so ALU-pipe / LSU
-// instructions issue in its shadow (profiles/r02_micro.md).
+// sm_100a an FFMA2 occupies both 16-lane FMA pipes and the dispatch port for two cycles -- the cost of two
+// scalar FFMAs; nothing issues in its shadow (profiles/r03_micro.md).
 __device__ __forceinline__ void ffma2_bcast(float& c0, float& c1, float a0, float a1, float s) {
   asm("{\n\t.reg .b64 ra, rs, rc;\n\t"
       "mov.b64 ra, {%2, %3};\n\t"
