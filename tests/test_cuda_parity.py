@@ -756,7 +756,7 @@ def test_ecohe_and_cv_distance_match_oracle(lib, oracle):
 
 
 # ------------------------------------------------------------------------------ N3: overlapping patches
-PATCH_REL_L2 = 2e-5      # two projector calls + two FP32 GEMMs (K <= 256) on top of each other
+PATCH_REL_L2 = REL_L2    # north_star's bar also for Algorithm 1's gradient (measured <= 2.8e-6)
 
 
 @pytest.mark.gpu
@@ -780,7 +780,7 @@ def test_patch_gradient_matches_oracle(lib, oracle, ny, nx, m, st, n_atoms, rho)
         Gw, Xw, fw = oracle.patch_gradient(W[s].astype(np.float64), D.astype(np.float64), data[s], w.angles, w.axis,
                                            nx, ny, m, st, rho)
         assert_parity(X[s].cpu().numpy(), Xw, "patch X slice %d" % s)
-        assert_parity(G[s].cpu().numpy(), Gw, "patch G slice %d" % s, rel=PATCH_REL_L2, mabs=2e-4)
+        assert_parity(G[s].cpu().numpy(), Gw, "patch G slice %d" % s, rel=PATCH_REL_L2, mabs=MAX_ABS)
         f_want += fw
     assert f == pytest.approx(f_want, rel=1e-5)
 
@@ -890,7 +890,7 @@ def test_patch_gradient_tensor_core_gemm(lib, oracle, m, st, n_atoms):
         for variant in (1, 2):
             G, X, f = out[variant]
             assert_parity(X[s].cpu().numpy(), Xw, "patch X, GEMM variant %d" % variant)
-            assert_parity(G[s].cpu().numpy(), Gw, "patch G, GEMM variant %d" % variant, rel=PATCH_REL_L2, mabs=2e-4)
+            assert_parity(G[s].cpu().numpy(), Gw, "patch G, GEMM variant %d" % variant, rel=PATCH_REL_L2, mabs=MAX_ABS)
     assert not np.array_equal(out[1][0].cpu().numpy(), out[2][0].cpu().numpy())    # the two kernels really differ
 
 
