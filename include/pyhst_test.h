@@ -2,8 +2,10 @@
  * pyhst_test.h -- test / bench hooks of libpyhst_b200 (NOT part of the product API of pyhst.h).
  *
  * Process-wide switches that select older or alternative kernels for cross-checks.  They are
- * plain globals read at the start of a call: set them only while no call is in flight.  Every
- * variant computes the operation pyhst.h defines; results agree within FP32 rounding.
+ * atomic integers shared by all devices and threads and read at the start of a call: setting
+ * one while a call is in flight on another thread is not a data race, but which kernel that call
+ * runs is then unspecified -- set them only while no call is in flight.  Every variant computes
+ * the operation pyhst.h defines; results agree within FP32 rounding.
  */
 #ifndef PYHST_TEST_H_
 #define PYHST_TEST_H_

@@ -73,12 +73,14 @@ struct DeviceCtx {
 namespace {
 std::mutex g_map_mu;
 std::map<int, std::unique_ptr<DeviceCtx>> g_ctx;
-int g_bp_variant = 0;
-int g_fp_variant = 0;
-int g_last_fp_kernel = 0;
-int g_halfacq_stitch = 1;
-int g_filter_variant = 0;
-int g_patch_gemm_variant = 0;
+// test / bench hooks of pyhst_test.h: process-wide, read at the start of a call (atomic so that a hook set from one
+// thread while another thread is inside a call is a defined, if unspecified, choice -- not a data race)
+std::atomic<int> g_bp_variant{0};
+std::atomic<int> g_fp_variant{0};
+std::atomic<int> g_last_fp_kernel{0};
+std::atomic<int> g_halfacq_stitch{1};
+std::atomic<int> g_filter_variant{0};
+std::atomic<int> g_patch_gemm_variant{0};
 std::atomic<int64_t> g_ws_limit{0};   // pyhst_test_set_workspace_limit
 
 DeviceCtx* ctx_of(int dev) {
@@ -737,7 +739,7 @@ int pyhst_backproject(const float* d_sino, float* d_img, const pyhst_geom_t* g, 
   const int kern = pick_bp_kernel(g->pixel_size, g->n_slices);
   if (kern < 0)
     return set_error(PYHST_ERR_UNSUPPORTED, "backprojector variant %d does not cover pixel_size %g",
-                     g_bp_variant, g->pixel_size);
+                     g_bp_variant.load(), g->pixel_size);
   if (kern == 1) return launch_backproject_reference(d_sino, pitch, a, stream);
   const QiLayout L = qi_layout(g->n_slices, g->n_angles, g->n_bins, g->pixel_size);
   void* qi = nullptr;
@@ -760,12 +762,13 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
   PYHST_TRY(check_geom(g, &pitch));
   PYHST_TRY(require_sm100(nullptr));
   PYHST_CALL_SCOPE(stream);
+  const int fp_variant = g_fp_variant.load();   // one choice per call
   const GeomPlan* plan = nullptr;
   PYHST_TRY(get_geom_plan(g, 0.0, g->n_bins, stream, &plan));
-  if (g_fp_variant != 1) {
+  if (fp_variant != 1) {
     const FpPlan* fplan = nullptr;
-    PYHST_TRY(get_fp_plan(g, stream, g_fp_variant == 5 ? 2 : (g_fp_variant == 0 ? 1 : 0), &fplan));
-    if (fplan->diag && g_fp_variant == 0) {
+    PYHST_TRY(get_fp_plan(g, stream, fp_variant == 5 ? 2 : (fp_variant == 0 ? 1 : 0), &fplan));
+    if (fplan->diag && fp_variant == 0) {
       // automatic choice: the diagonal-line kernel needs two sheared copies of the stack (about 4.6x its size,
       // see pyhst.h).  If that block cannot be had, the banded kernel (about 2x) still can run: take its plan.
       void* xd = nullptr;
@@ -779,13 +782,13 @@ int pyhst_forward_project(const float* d_img, float* d_sino, const pyhst_geom_t*
         return launch_forward_project_banded(d_img, d_sino, pitch, g, scale, *fplan, 0, stream);
       return PYHST_OK;
     }
-    if (g_fp_variant == 5)
+    if (fp_variant == 5)
       return set_error(PYHST_ERR_UNSUPPORTED, "diagonal-line forward projector does not cover this geometry");
     if (fplan->n_chunks > 0) {
-      g_last_fp_kernel = g_fp_variant == 3 || g_fp_variant == 4 ? g_fp_variant : 2;
-      return launch_forward_project_banded(d_img, d_sino, pitch, g, scale, *fplan, g_fp_variant == 3 ? 1 : (g_fp_variant == 4 ? 2 : 0), stream);
+      g_last_fp_kernel = fp_variant == 3 || fp_variant == 4 ? fp_variant : 2;
+      return launch_forward_project_banded(d_img, d_sino, pitch, g, scale, *fplan, fp_variant == 3 ? 1 : (fp_variant == 4 ? 2 : 0), stream);
     }
-    if (g_fp_variant == 2)
+    if (fp_variant == 2)
       return set_error(PYHST_ERR_UNSUPPORTED, "banded forward projector does not cover pixel_size %g",
                        g->pixel_size);
   }
@@ -873,7 +876,7 @@ static int fbp_device(const float* d_sino_raw, int64_t pitch, float* d_img, cons
   const int kern = pick_bp_kernel(g->pixel_size, ns);
   if (kern < 0)
     return set_error(PYHST_ERR_UNSUPPORTED, "backprojector variant %d does not cover pixel_size %g",
-                     g_bp_variant, g->pixel_size);
+                     g_bp_variant.load(), g->pixel_size);
   if (kern == 1) {
     void* rows = nullptr;
     PYHST_TRY(get_workspace(WS_ROWS, (size_t)ns * P * b_out * 4, &rows));

@@ -88,20 +88,23 @@ int get_spectrum(int filter, int M, cudaStream_t stream, const float** out) {
   double* d_hc = nullptr;
   cufftDoubleComplex* d_Hd = nullptr;
   float* d_H = nullptr;
+  struct Cleanup {   // the temporaries always, the spectrum itself unless it reached the cache
+    double*& hc; cufftDoubleComplex*& Hd; float*& H; bool keep = false; cufftHandle* plan = nullptr;
+    ~Cleanup() { if (plan) cufftDestroy(*plan); cudaFree(hc); cudaFree(Hd); if (!keep) cudaFree(H); }
+  } cleanup{d_hc, d_Hd, d_H};
   PYHST_CUDA_TRY(cudaMalloc(&d_hc, sizeof(double) * M));
   PYHST_CUDA_TRY(cudaMalloc(&d_Hd, sizeof(cufftDoubleComplex) * nk));
   PYHST_CUDA_TRY(cudaMalloc(&d_H, sizeof(float) * nk));
   cufftHandle plan;
   PYHST_CUFFT_TRY(cufftPlan1d(&plan, M, CUFFT_D2Z, 1));
+  cleanup.plan = &plan;
   PYHST_CUFFT_TRY(cufftSetStream(plan, stream));
   ramp_kernel_table<<<(M + 255) / 256, 256, 0, stream>>>(d_hc, M, filter);
   PYHST_CUFFT_TRY(cufftExecD2Z(plan, d_hc, d_Hd));
   spectrum_to_float<<<(nk + 255) / 256, 256, 0, stream>>>(d_Hd, d_H, nk, 1.0 / (double)M);
   PYHST_CUDA_TRY(cudaGetLastError());
   PYHST_CUDA_TRY(cudaStreamSynchronize(stream));  // one-time set-up; temporaries freed below
-  cufftDestroy(plan);
-  cudaFree(d_hc);
-  cudaFree(d_Hd);
+  cleanup.keep = true;   // (the plan and the temporaries go with `cleanup`)
   g_spectra[key].d_H = d_H;
   *out = d_H;
   return PYHST_OK;
