@@ -188,13 +188,33 @@ def test_bench_reference_arm_runs_on_cpu():
     """bench.py --impl reference prints one JSON line with the contract's keys (tiny config 1)."""
     import json
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1",
-                        "--steps", "1"], capture_output=True, text=True, timeout=300)
+                        "--steps", "3", "--warmup", "2"], capture_output=True, text=True, timeout=300)
     assert r.returncode == 0, r.stderr
     line = json.loads(r.stdout.strip().splitlines()[-1])
     for k in ("impl", "metric", "value", "unit", "n_gpus", "steps", "ms_per_step", "higher_is_better",
               "cpu_baseline", "e2e", "config"):
         assert k in line
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
+    # the two arms print the same quantity on the same config (VERDICT round 2, item 5)
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1306_1392_b200 import workloads
+    assert line["metric"] == bench.METRIC and line["unit"] == bench.UNIT and line["metric_version"] == bench.METRIC_VERSION
+    assert line["config"] == bench._config_dict(workloads.config(1), 1)          # exactly the b200 arm's config dict
+    assert (line["steps"], line["warmup"]) == (3, 2)                             # honoured (they fit --ref-seconds)
+    m = line["metrics"]
+    w = workloads.config(1)
+    upd = m["slices_timed_per_step"] * w.nx * w.ny * w.n_angles
+    assert line["value"] == pytest.approx(upd / (m["ms_backproject"] * 1e-3) / 1e9, rel=1e-9)   # BP updates / BP seconds
+    assert line["ms_per_step"] == pytest.approx(m["ms_ramp_filter"] + m["ms_backproject"] + m["ms_forward_project"], rel=1e-6)
+    assert line["e2e"]["value"] == line["value"] and line["cpu_baseline"]["value"] == line["value"]
+    # a budget too small for the request: fewer steps are run and REPORTED, never more than asked
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1",
+                        "--steps", "50", "--warmup", "5", "--ref-seconds", "0.5"], capture_output=True, text=True,
+                       timeout=300)
+    assert r.returncode == 0, r.stderr
+    short = json.loads(r.stdout.strip().splitlines()[-1])
+    assert 1 <= short["steps"] < 50 and 0 <= short["warmup"] <= 5
 
 
 # ------------------------------------------------------------------ diagonal-line forward projector: host tables
